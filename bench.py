@@ -1,0 +1,387 @@
+#!/usr/bin/env python
+"""bench.py -- IntentKV hot path on B200: history tokens scored+pruned per second at C=8k.
+
+One "step" = one pass of the whole hot path over one synthetic Qwen3-8B-shaped session (BASELINE.json
+configs[1]): ikv_memory_update (4 rows) -> ikv_score (LEARNABLE: rule + residual head) -> ikv_select_evict
+(C = 8192) -> 256 decode steps x 36 layers of ikv_decode_attn through the pruned slot map (CUDA graph).
+`value` = live history tokens / time of the pruning pass (memory update + score + select/evict), the metric
+BASELINE.json names; the decode stage is reported beside it (`decode`, `roofline_decode`).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W]            # our arm (N>1: under torchrun, replicas)
+  python bench.py --impl reference ...                           # the CPU oracle timed on the host cores
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "history tokens scored+pruned/sec at C=8k"
+UNIT = "tokens/s"
+NOMINAL_HBM_GBS = 8000.0
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+def oracle_sample(w, sess, layers, kp_host, full_layers=36):
+    """Times the oracle's pruning pass (memory update, partition, rule score, mean keys, residual head, select,
+    rewrite) on the first `layers` layers of the workload, all tokens.  The steps whose cost grows with the layer
+    count (memory update, rule score, mean keys) are scaled by full_layers/layers; the rest are taken as measured.
+    Returns (estimated seconds for the full pass, seconds actually spent, threads)."""
+    import numpy as np
+    from oracle import ikv_oracle as o
+    from paper_2606_09916_b200 import workloads as wl
+    g = o.Geometry(layers, w.shape.Hq, w.shape.Hkv, w.shape.D, w.n_slots, o.BF16, w.dead_slot)
+    M = np.zeros((layers, w.shape.Hq, w.shape.D))
+    rows = sess.mem_rows[:, :layers].contiguous().numpy()
+    wts = o.ResidualWeights(**wl.residual_weights(w.shape.D, w.seed + 5))
+    S = sess.slot_map[:sess.N].numpy()
+    t0 = time.perf_counter()
+    o.memory_update(M, rows[-4:], 0.5)
+    cls, _ = o.partition(S, w.dead_slot, sess.pi, sess.qs, sess.qe)
+    rule = o.rule_score(g, kp_host, M, S, cls)
+    cand = np.nonzero(cls == o.CAND)[0].astype(np.int32)
+    kbar = o.mean_key(g, kp_host, S, cand)
+    qpos = np.array([j for j in range(sess.qs, sess.qe) if S[j] != w.dead_slot], np.int32)
+    Kq = o.mean_key(g, kp_host, S, qpos)
+    t1 = time.perf_counter()
+    s_c = o.residual(rule[cand], kbar, o.mean_memory(M), Kq, wts)
+    scores = np.where(cls == o.FORCED, np.inf, -np.inf).astype(np.float32)
+    scores[cand] = s_c.astype(np.float32)
+    keep, _ = o.select(scores, cls, sess.spec.budget)
+    o.rewrite(S, w.dead_slot, keep, sess.pi, w.n_slots)
+    t2 = time.perf_counter()
+    return (t1 - t0) * full_layers / layers + (t2 - t1), t2 - t0, os.cpu_count()
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores, on a bounded sample per step."""
+    import torch
+    from paper_2606_09916_b200 import workloads as wl
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    layers = args.ref_layers
+    w = wl.cfg1(device="cpu", shape=wl.ModelShape(layers, 32, 8, 128), decode_tokens=0, n_tokens=args.tokens)
+    sess = w.sessions[0]
+    kp = wl.to_numpy_bits(w.k_pool)
+    for _ in range(args.warmup):
+        oracle_sample(w, sess, layers, kp)
+    times = []
+    for _ in range(args.steps):
+        t, _, cores = oracle_sample(w, sess, layers, kp)
+        times.append(t)
+    t_mean = sum(times) / len(times)
+    full_layers = 36
+    value = sess.N / t_mean
+    sample = (f"oracle pruning pass (memory update + learnable score + select + rewrite) on all {sess.N} tokens of "
+              f"the first {layers} of {full_layers} layers per step; layer-dependent steps scaled by "
+              f"{full_layers}/{layers}")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_mean * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[1] Qwen3-8B-shaped single session, 32,768 live tokens, C=8192",
+                       "n_tokens": sess.N, "budget": sess.spec.budget, "mode": "learnable"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2606_09916_b200 import ikv, workloads as wl
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    hbm_peak, peak_src = peaks()
+
+    T, C, DEC = args.tokens, args.budget, args.decode_steps
+    shape = wl.QWEN3_8B
+    w = wl.cfg1(device="cuda", seed=1000 + rank, n_tokens=T, budget=C, decode_tokens=DEC)
+    sess = w.sessions[0]
+    L, Hq, Hkv, D = shape.L, shape.Hq, shape.Hkv, shape.D
+    ctx = ikv.Context(L, Hq, Hkv, D, w.k_pool, w.v_pool, dead_slot=w.dead_slot)
+    ctx.reserve(T + DEC, 1)
+    ctx.residual_load(wl.residual_weights(D, w.seed + 5))
+    sid = sess.spec.session_id
+    ctx.session_open(sid)
+    ups = [u.to(dev).contiguous() for u in sess.updates()]
+    for u in ups[:-1]:
+        ctx.memory_update(sid, u)
+    new_rows = ups[-1]
+    mode = ikv.MODE_LEARNABLE if args.mode == "learnable" else ikv.MODE_MEMORY
+
+    pristine = sess.slot_map.to(dev)
+    S_dev = pristine.clone()
+    valid = torch.empty(T + DEC, dtype=torch.uint8, device=dev)
+    scores = torch.empty(T, device=dev)
+    freed = torch.empty(T, dtype=torch.int32, device=dev)
+    nf = torch.zeros(1, dtype=torch.int32, device=dev)
+    nk = torch.zeros(1, dtype=torch.int32, device=dev)
+    req = ikv.make_request(sid, S_dev, T, sess.pi, sess.qs, sess.qe, C, sess.pi, valid_mask=valid)
+    dq = wl.decode_queries(shape, DEC, w.seed, device="cuda")
+    dout = torch.empty((DEC, L, 1, Hq, D), dtype=torch.bfloat16, device=dev)
+    scale = 1.0 / math.sqrt(D)
+    stream = torch.cuda.Stream(device=dev)
+
+    def prune():
+        ctx.memory_update(sid, new_rows, stream)
+        ctx.score([req], mode, scores, None, stream)
+        ctx.select_evict([req], scores, freed, nf, nk, stream)
+
+    def decode_all():
+        for t in range(DEC):
+            r = ikv.make_request(sid, S_dev, T + t + 1, sess.pi, sess.qs, sess.qe, C, sess.pi)
+            for l in range(L):
+                ctx.decode_attn(l, [r], dq[t, l:l + 1], dout[t, l], scale, stream)
+
+    # un-captured warm-up pass (sizes every lazily grown buffer), then capture the decode loop in a graph
+    with torch.cuda.stream(stream):
+        S_dev.copy_(pristine)
+        prune()
+        r0 = ikv.make_request(sid, S_dev, T + 1, sess.pi, sess.qs, sess.qe, C, sess.pi)
+        ctx.decode_attn(0, [r0], dq[0, 0:1], dout[0, 0], scale, stream)
+    stream.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=stream):
+        decode_all()
+    stream.synchronize()
+
+    n_prune_launch = 6 + (5 if mode == ikv.MODE_LEARNABLE else 0)
+    n_decode_launch = DEC * L * 2
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def one_step(record):
+        with torch.cuda.stream(stream):
+            S_dev.copy_(pristine)           # untimed restore of the slot map (a new turn's map)
+            e0, e1, e2 = ev(), ev(), ev()
+            e0.record(stream)
+            prune()
+            e1.record(stream)
+            graph.replay()
+            e2.record(stream)
+        if record is not None:
+            record.append((e0, e1, e2))
+
+    for _ in range(args.warmup):
+        one_step(None)
+    stream.synchronize()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ctx.profile_enable(True)
+    recs = []
+    t_wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        one_step(recs)
+    stream.synchronize()
+    torch.cuda.synchronize()
+    t_wall = time.perf_counter() - t_wall0
+    prof = ctx.profile_read()
+    ctx.profile_enable(False)
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    prune_ms = [a.elapsed_time(b) for a, b, _ in recs]
+    dec_ms = [b.elapsed_time(c) for _, b, c in recs]
+    step_ms = [a.elapsed_time(c) for a, _, c in recs]
+    tot_prune, tot_dec, tot_step = sum(prune_ms), sum(dec_ms), sum(step_ms)
+    n_kept = int(nk.item())
+
+    # ---- end-to-end through ikv_prune_host with pinned HOST buffers
+    h_map0 = sess.slot_map[:T].clone().pin_memory()
+    h_map = torch.empty_like(h_map0).pin_memory()
+    h_rows = sess.updates()[-1].contiguous().pin_memory()
+    h_valid = torch.empty(T, dtype=torch.uint8).pin_memory()
+    h_freed = torch.empty(T, dtype=torch.int32).pin_memory()
+    req_h = ikv.make_request(sid, None, T, sess.pi, sess.qs, sess.qe, C, sess.pi)
+    e2e_t = []
+    n_freed_h = 0
+    for i in range(args.warmup + args.steps):
+        h_map.copy_(h_map0)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        n_freed_h, n_kept_h = ctx.prune_host(req_h, h_rows, mode, h_map, h_valid, None, h_freed, stream)
+        dt = time.perf_counter() - t0
+        if i >= args.warmup:
+            e2e_t.append(dt)
+    e2e_total = sum(e2e_t)
+    h2d = T * 4 + h_rows.numel() * 4
+    d2h = T * 4 + T + n_freed_h * 4 + 8
+
+    # ---- phase-1 (memory mode) beside the headline
+    p1 = []
+    for _ in range(3 + 5):
+        with torch.cuda.stream(stream):
+            S_dev.copy_(pristine)
+            a, b = ev(), ev()
+            a.record(stream)
+            ctx.memory_update(sid, new_rows, stream)
+            ctx.score([req], ikv.MODE_MEMORY, scores, None, stream)
+            ctx.select_evict([req], scores, freed, nf, nk, stream)
+            b.record(stream)
+        stream.synchronize()
+        p1.append(a.elapsed_time(b))
+    p1_ms = statistics.median(p1[3:])
+
+    # ---- max over ranks
+    tt = torch.tensor([tot_prune, tot_dec, tot_step, e2e_total * 1e3], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    tot_prune, tot_dec, tot_step, e2e_ms_total = tt.tolist()
+
+    if rank == 0:
+        K = args.steps
+        key_bytes = L * Hkv * T * D * shape.elem_bytes                 # algorithmic bytes of the key pass
+        dec_tokens_sum = sum(n_kept + t + 1 for t in range(DEC))        # live tokens read over the decode loop
+        dec_bytes_step = dec_tokens_sum * L * Hkv * D * 2 * shape.elem_bytes
+        value = world * T * K / (tot_prune * 1e-3)
+        logits_ms = prof["score_logits_ms"] / max(1, prof["score_logits_n"])
+        ach = key_bytes / (logits_ms * 1e-3) / 1e9 if logits_ms > 0 else 0.0
+        dec_kernel_ms = tot_dec / K / (DEC * L)                         # split + merge + launch gap per layer call
+        dec_bytes_call = dec_bytes_step / (DEC * L)
+        dec_ach = dec_bytes_call / (dec_kernel_ms * 1e-3) / 1e9
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+            "ms_per_step": tot_step / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16 keys/values, f32 accumulate", "data": "synthetic",
+            "config": {"workload": "configs[1] Qwen3-8B-shaped single session per GPU: 36 layers, 32 Q / 8 KV heads, "
+                                   "head_dim 128, bf16 K/V, 32,768 live tokens in 16-token pages, M=64 memory rows, "
+                                   "1% planted, C=8192, one prune pass then 256 decode steps",
+                       "n_tokens": T, "budget": C, "decode_steps": DEC, "mode": args.mode, "n_kept": n_kept,
+                       "l2": "inputs larger than L2 (2.4 GB of keys per prune, 1.2 GB of K/V per decode step; "
+                             "126 MB L2)", "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
+            "prune_ms": tot_prune / K, "prune_ms_memory_mode": p1_ms,
+            "prune_hbm_gbs": key_bytes / (tot_prune / K * 1e-3) / 1e9,
+            "prune_frac_of_nominal_8TBs": key_bytes / (tot_prune / K * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+            "decode": {"ms_per_decode_step": tot_dec / K / DEC, "kv_gbs": dec_bytes_step / (tot_dec / K * 1e-3) / 1e9,
+                       "tokens_per_s": world * DEC * K / (tot_dec * 1e-3),
+                       "frac_of_nominal_8TBs": dec_bytes_step / (tot_dec / K * 1e-3) / 1e9 / NOMINAL_HBM_GBS},
+            "e2e": {"value": world * T * K / (e2e_ms_total * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h,
+                    "what": "ikv_prune_host: slot map + query rows H2D, memory update + score + select/evict, "
+                            "slot map + valid mask + freed list + counts D2H; the K/V pool is device-resident state"},
+            "gpu_launches": K * (n_prune_launch + n_decode_launch),
+            "roofline": {"kernel": "k_score_logits", "bound": "hbm", "achieved": ach, "peak": hbm_peak,
+                         "unit": "GB/s", "frac": ach / hbm_peak, "frac_of_nominal_8TBs": ach / NOMINAL_HBM_GBS,
+                         "peak_source": peak_src, "traffic": None, "algorithmic_bytes": key_bytes,
+                         "ms": logits_ms},
+            "roofline_decode": {"kernel": "k_decode_split (+k_decode_merge, per-layer launch gap included)",
+                                "bound": "hbm", "achieved": dec_ach, "peak": hbm_peak, "unit": "GB/s",
+                                "frac": dec_ach / hbm_peak, "frac_of_nominal_8TBs": dec_ach / NOMINAL_HBM_GBS,
+                                "algorithmic_bytes": dec_bytes_call, "traffic": None, "ms": dec_kernel_ms},
+            "clocks": clocks, "wall_s_timed_region": t_wall,
+        }
+        if not args.no_cpu_baseline and world >= 1:
+            layers = args.ref_layers
+            wc = wl.cfg1(device="cpu", shape=wl.ModelShape(layers, 32, 8, 128), decode_tokens=0, n_tokens=T, budget=C)
+            tfull, tsec, cores = oracle_sample(wc, wc.sessions[0], layers, wl.to_numpy_bits(wc.k_pool), L)
+            line["cpu_baseline"] = {
+                "value": T / tfull, "unit": UNIT, "cores": cores, "kind": "oracle",
+                "sample": f"oracle pruning pass (learnable mode) on all {T} tokens of {layers} of {L} layers; "
+                          f"layer-dependent steps scaled by {L}/{layers}",
+                "sample_seconds": tsec}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--mode", default="learnable", choices=["learnable", "memory"])
+    ap.add_argument("--tokens", type=int, default=32768)
+    ap.add_argument("--budget", type=int, default=8192)
+    ap.add_argument("--decode-steps", type=int, default=256)
+    ap.add_argument("--ref-layers", type=int, default=6, help="layers in the oracle's bounded sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

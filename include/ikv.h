@@ -1,0 +1,174 @@
+/*
+ * ikv.h -- C-ABI of libikv: IntentKV's pruning pass and slot-map paged decode on one B200 (sm_100a).
+ *
+ * Source of every definition: arxiv 2606.09916 (cited as PAPER.md:<line> of /root/reference/PAPER.md);
+ * readings of silent points are R1..R24 in DESIGN.md section 3.
+ *
+ * Conventions
+ *  - "DEVICE" pointers are CUDA device memory of the current device; "HOST" pointers are ordinary host memory.
+ *  - Ownership: the caller owns K/V pools, slot maps, q / out / scores buffers and the allocator that
+ *    consumes freed slots.  The library owns session memories, its copy of the residual weights, scratch,
+ *    the contents of the dead slot and the derived compact live lists.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Hot calls
+ *    (ikv_memory_update, ikv_score, ikv_select_evict, ikv_decode_attn) only enqueue work on `stream`; they
+ *    never synchronise the host, provided scratch was sized once with ikv_reserve (otherwise a call that
+ *    needs more scratch grows it with cudaMalloc first, which synchronises).
+ *  - Errors: every call returns an ikv_status.  Argument errors are reported before anything is launched.
+ *    CUDA launch errors surface as IKV_ERR_CUDA.  Nothing throws or aborts across the ABI.
+ *    ikv_last_error() returns a human-readable description of the last failure on that context.
+ *  - Pool layout: K and V are [n_layers][n_slots][n_kv_heads][head_dim] (token-major), element type
+ *    kv_dtype; slot = page * page_size + offset.  A request reaches K/V only through its slot map
+ *    S[0:seq_len).
+ */
+#ifndef IKV_H
+#define IKV_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ikv_ctx ikv_ctx; /* opaque, library-owned */
+typedef int32_t ikv_status;
+
+#define IKV_OK 0
+#define IKV_ERR_INVALID_ARG (-1)
+#define IKV_ERR_NO_SESSION (-2)
+#define IKV_ERR_CAPACITY (-3)
+#define IKV_ERR_OOM (-4)
+#define IKV_ERR_CUDA (-5)
+#define IKV_ERR_UNSUPPORTED (-6)
+
+/* kv_dtype / q_dtype */
+#define IKV_F32 0
+#define IKV_BF16 1
+
+/* scorer modes ("three scorer modes") and ablation knobs, OR-ed into `mode` */
+#define IKV_MODE_MEMORY 0    /* rule score against the session QueryMemory M_t (Eq. 3)              */
+#define IKV_MODE_LEARNABLE 1 /* rule + alpha * MLP(phi (+) c) (Eq. 4-6); needs ikv_residual_load    */
+#define IKV_MODE_QUERY 2     /* rule score against normalize(Enc(q_t)) of the latest update only    */
+#define IKV_FLAG_NO_XATTN 0x100    /* "- x-attn": c_j = 0                                            */
+#define IKV_FLAG_NO_RESIDUAL 0x200 /* "- residual": alpha = 0, recovers the rule scorer exactly      */
+
+/* request flags */
+#define IKV_REQ_RESCAN 1 /* ikv_decode_attn: ignore the cached live list, rescan the slot map       */
+
+typedef struct {
+  int32_t n_layers, n_q_heads, n_kv_heads, head_dim; /* L, H_q, H_kv, D; H_q % H_kv == 0; D in {64,128}   */
+  int32_t page_size;                                 /* 16 (R18)                                          */
+  int32_t kv_dtype;                                  /* IKV_BF16 | IKV_F32 (R20)            */
+  int64_t n_slots;                                   /* pool capacity in token slots, dead slot included  */
+  void *k_pool, *v_pool;                             /* DEVICE, caller-owned, [L][n_slots][H_kv][D]       */
+  int32_t dead_slot;                                 /* s+ ; ikv_create writes K=-1e4, V=0 there on every
+                                                        layer                              */
+  float lambda;                                      /* decay of Eq. 2; the paper uses 0.5 */
+  int32_t max_sessions;                              /* LRU capacity; the paper uses 1024  */
+} ikv_config;
+
+/* One request of a batch.  The array of requests lives on the HOST. */
+typedef struct {
+  uint64_t session_id;         /* explicit session key (first priority)                     */
+  int32_t *slot_map;           /* DEVICE, caller-owned, length >= seq_len; rewritten in place by
+                                  ikv_select_evict (Eq. 7)                                                */
+  uint8_t *valid_mask;         /* DEVICE, optional (may be NULL), length >= seq_len (R21)                 */
+  int32_t seq_len;             /* N -- never modified                                                     */
+  int32_t prefix_len;          /* pi: protected system prefix [0,pi)                                      */
+  int32_t q_start, q_end;      /* actionable query span [q_s,q_e); 0 <= pi <= q_s <= q_e <= N             */
+  int32_t budget;              /* C >= 0                                                                  */
+  int32_t radix_protected_len; /* positions below it are never reported as freed (PAPER.md:132 (a))       */
+  const int32_t *xattn_pos;    /* DEVICE, positions forming K^q (Eq. 6); NULL => [q_s,q_e) (R7)           */
+  int32_t n_xattn_pos;
+  int32_t flags;               /* IKV_REQ_*                                                               */
+} ikv_request;
+
+/* Residual head parameters (R9), HOST fp32 arrays, row-major [out][in]:
+ * wq[128][3D+1] bq[128]  wk[128][D] bk[128]  wv[128][D] bv[128]  fc1_w[256][3D+1+128] fc1_b[256]
+ * fc2_w[256] fc2_b[1]; alpha is clipped to [-5,5] at inference. */
+typedef struct {
+  const float *wq, *bq, *wk, *bk, *wv, *bv, *fc1_w, *fc1_b, *fc2_w, *fc2_b;
+  float alpha;
+} ikv_residual_weights;
+
+/* ---- lifecycle ------------------------------------------------------------------------------------- */
+/* Validates the config, initialises the dead slot's K/V rows on every layer, allocates the session slab.
+ * Synchronises.  *out receives the context. */
+ikv_status ikv_create(const ikv_config *cfg, ikv_ctx **out);
+ikv_status ikv_destroy(ikv_ctx *ctx);
+const char *ikv_last_error(const ikv_ctx *ctx);
+
+/* Pre-sizes every scratch buffer so that later hot calls never allocate: `max_tokens` = largest sum of
+ * seq_len over one batch, `max_requests` = largest batch.  Synchronises. */
+ikv_status ikv_reserve(ikv_ctx *ctx, int64_t max_tokens, int32_t max_requests);
+
+/* ---- sessions (explicit session id, LRU store) ------------------------------------------ */
+/* M_0 = 0 (R3).  Opening an existing id resets it.  Beyond max_sessions the least-recently-used session is
+ * evicted. */
+ikv_status ikv_session_open(ikv_ctx *ctx, uint64_t id);
+/* child <- copy of the parent's QueryMemory (a forked trajectory); shares no K/V state. */
+ikv_status ikv_session_fork(ikv_ctx *ctx, uint64_t parent, uint64_t child, void *stream);
+ikv_status ikv_session_close(ikv_ctx *ctx, uint64_t id);
+/* Debug/test access to the state: copies M_t ([L][H_q][D] fp32) to / from HOST memory.  Synchronises. */
+ikv_status ikv_session_get_memory(ikv_ctx *ctx, uint64_t id, float *host_out);
+ikv_status ikv_session_set_memory(ikv_ctx *ctx, uint64_t id, const float *host_in);
+
+/* Copies the residual head to the device (synchronises). */
+ikv_status ikv_residual_load(ikv_ctx *ctx, const ikv_residual_weights *w);
+
+/* ---- hot path ------------------------------------------------------------------------------------------ */
+/* a0, Eq. 2: Enc = mean of the n post-RoPE Q rows; M <- e^{-lambda} M + Enc; each
+ * (layer, head) row <- row / max(||row||_2, 1e-12).  q_rows: DEVICE [n][L][H_q][D], q_dtype IKV_F32 or
+ * IKV_BF16.  Also stores normalize(Enc) for IKV_MODE_QUERY.  The session is created if it does not exist. */
+ikv_status ikv_memory_update(ikv_ctx *ctx, uint64_t id, const void *q_rows, int32_t n, int32_t q_dtype,
+                             void *stream);
+
+/* a1-a5, Eq. 3-6: scores of every position of every request.
+ * scores: DEVICE fp32, requests concatenated (request r starts at sum of seq_len of requests < r), indexed by
+ * logical position: s_j at candidate positions, +INF at forced live positions, -INF at dead positions (R6).
+ * rule_out: optional DEVICE fp32 of the same shape receiving rule_j (Eq. 3) at candidates, 0 elsewhere. */
+ikv_status ikv_score(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req, int32_t mode, float *scores,
+                     float *rule_out, void *stream);
+
+/* a6-a7, Eq. 1 and Eq. 7.  For each request: if N <= C nothing changes
+ * (R15).  Otherwise K* = F u top-C*(candidates by score desc, position asc), C* = max(0, C - |F|) (R13, R14);
+ * S[j] <- s+ for every live j outside K*; valid_mask[j] = (S'[j] != s+); no K/V byte moves.
+ * freed_slots: DEVICE int32, requests concatenated like `scores` (capacity seq_len each); receives, per
+ * request, the slots that pass the prefix-safe test (a)(b)(c) of PAPER.md:132, each once, ordered by first
+ * dropped position (R22).  n_freed / n_kept: DEVICE int32[n_req].
+ * Also refreshes the session's compact live list used by ikv_decode_attn. */
+ikv_status ikv_select_evict(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req, const float *scores,
+                            int32_t *freed_slots, int32_t *n_freed, int32_t *n_kept, void *stream);
+
+/* a8 (R16): paged GQA decode attention of one layer through the slot map, dead entries
+ * skipped:  out[r,h] = sum_{j<seq_len, S_r[j] != s+} softmax_j(q[r,h] . K[layer, h div G, S_r[j]] * sm_scale)
+ *                       V[layer, h div G, S_r[j]].
+ * q, out: DEVICE [n_req][H_q][D]; bf16 for a bf16 pool, fp32 for an fp32 pool.  Positions below the seq_len of
+ * the last ikv_select_evict on the same (session, slot_map) come from the cached compact live list; positions
+ * appended since are read from slot_map.  A caller that edited the slot map itself passes IKV_REQ_RESCAN. */
+ikv_status ikv_decode_attn(ikv_ctx *ctx, int32_t layer, const ikv_request *reqs, int32_t n_req, const void *q,
+                           void *out, float sm_scale, void *stream);
+
+/* The whole pruning pass of one request with HOST buffers (used for end-to-end timing): copies
+ * q_rows_host ([n_rows][L][H_q][D] fp32, may be NULL/0 to skip the memory update) and slot_map_host[seq_len]
+ * to the device, runs ikv_memory_update -> ikv_score(mode) -> ikv_select_evict, copies the new slot map,
+ * valid mask (optional), freed list and counts back to the HOST buffers and synchronises `stream`.
+ * req->slot_map / valid_mask / xattn_pos are ignored (xattn_pos defaults to the span). */
+ikv_status ikv_prune_host(ikv_ctx *ctx, const ikv_request *req, const float *q_rows_host, int32_t n_rows,
+                          int32_t mode, int32_t *slot_map_host, uint8_t *valid_host, float *scores_host,
+                          int32_t *freed_host, int32_t *n_freed_host, int32_t *n_kept_host, void *stream);
+
+/* Kernel-level timing for bench.py's roofline: while enabled, the library brackets its two dominant kernels
+ * (the key pass k_score_logits and the decode kernel k_decode_split) with CUDA events on the caller's stream
+ * (no host synchronisation; not allowed during stream capture).  ikv_profile_read synchronises, sums the
+ * elapsed times recorded since the last read and clears them.
+ * out_ms[0] = key-pass total ms, out_ms[1] = decode-split total ms; out_n[0], out_n[1] = launch counts. */
+ikv_status ikv_profile_enable(ikv_ctx *ctx, int32_t on);
+ikv_status ikv_profile_read(ikv_ctx *ctx, float *out_ms, int32_t *out_n);
+
+/* Library / build identification, e.g. "ikv 0.1 sm_100a". */
+const char *ikv_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IKV_H */

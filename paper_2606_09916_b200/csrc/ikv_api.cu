@@ -1,0 +1,794 @@
+// ikv_api.cu -- C-ABI of libikv (include/ikv.h): host-side session/scratch manager and kernel launches.
+// Everything on the hot path runs in the kernels of score.cuh / residual.cuh / select.cuh / decode.cuh.
+#include <limits.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+#include "../../include/ikv.h"
+#include "common.cuh"
+#include "decode.cuh"
+#include "residual.cuh"
+#include "score.cuh"
+#include "select.cuh"
+
+using namespace ikv;
+
+namespace {
+
+struct Session {
+  uint64_t id = 0;
+  float* d_mem = nullptr;   // M_t      [L][Hq][D]
+  float* d_qenc = nullptr;  // normalize(Enc(q_t)) of the latest update
+  uint64_t tick = 0;
+  bool has_update = false;
+  // compact survivor list for decode
+  int32_t* live_slots = nullptr;
+  int32_t* d_n_live = nullptr;
+  int live_cap = 0;
+  int covered = 0;            // positions [0, covered) are represented by the list
+  int live_ub = 0;            // host upper bound of the list length
+  const int32_t* map_ptr = nullptr;
+};
+
+template <typename T>
+struct DevBuf {
+  T* p = nullptr;
+  size_t n = 0;
+};
+
+}  // namespace
+
+struct ikv_ctx {
+  ikv_config cfg;
+  int G = 1;
+  int64_t layer_stride = 0;  // elements
+  std::unordered_map<uint64_t, Session> sessions;
+  uint64_t tick = 0;
+  std::string err;
+  int n_sm = 148;
+
+  // scratch (per request, sized by ensure_scratch)
+  int64_t cap_tokens = 0;
+  int32_t *cand_pos = nullptr, *cand_slot = nullptr, *d_ncand = nullptr;
+  float* logits = nullptr;
+  float2* partials = nullptr;
+  float *lse = nullptr, *rule_c = nullptr, *kbar = nullptr, *mbar = nullptr;
+  int32_t *xq_slot = nullptr, *d_nxq = nullptr;
+  float *kq = nullptr, *kc = nullptr, *vc = nullptr;
+  int64_t xq_cap = 0;
+  uint32_t* kept_bits = nullptr;
+  int32_t* firstpos = nullptr;
+  uint8_t* keepflag = nullptr;
+  int32_t* tmp_slot = nullptr;
+  float* part_o = nullptr;
+  float2* part_ml = nullptr;
+  int64_t part_cap = 0;  // in (req*Hq*split) units
+  // ikv_prune_host staging
+  int32_t *st_map = nullptr, *st_freed = nullptr, *st_counts = nullptr;
+  uint8_t* st_valid = nullptr;
+  float *st_scores = nullptr, *st_qrows = nullptr;
+  int64_t st_cap = 0, st_qcap = 0;
+
+  // kernel-level profiling (ikv_profile_*)
+  bool prof_on = false;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[2];
+
+  // residual head (transposed on the device)
+  bool has_resid = false;
+  float* resid_blob = nullptr;
+  ResidW rw{};
+};
+
+namespace {
+
+#define IKV_FAIL(ctx, code, ...)                         \
+  do {                                                   \
+    char _b[512];                                        \
+    snprintf(_b, sizeof _b, __VA_ARGS__);                \
+    (ctx)->err = _b;                                     \
+    return (code);                                       \
+  } while (0)
+
+#define CU(ctx, call)                                                                              \
+  do {                                                                                             \
+    cudaError_t _e = (call);                                                                       \
+    if (_e != cudaSuccess) {                                                                       \
+      const bool oom = (_e == cudaErrorMemoryAllocation);                                          \
+      IKV_FAIL(ctx, oom ? IKV_ERR_OOM : IKV_ERR_CUDA, "%s failed: %s (%s:%d)", #call,              \
+               cudaGetErrorString(_e), __FILE__, __LINE__);                                        \
+    }                                                                                              \
+  } while (0)
+
+#define LAUNCH_CHECK(ctx)                                                                          \
+  do {                                                                                             \
+    cudaError_t _e = cudaGetLastError();                                                           \
+    if (_e != cudaSuccess)                                                                         \
+      IKV_FAIL(ctx, IKV_ERR_CUDA, "kernel launch failed: %s (%s:%d)", cudaGetErrorString(_e),      \
+               __FILE__, __LINE__);                                                                \
+  } while (0)
+
+struct ProfScope {  // brackets a launch with events when profiling is on and the stream is not capturing
+  ikv_ctx* c; int which; cudaStream_t st; cudaEvent_t a = nullptr, b = nullptr;
+  ProfScope(ikv_ctx* c_, int which_, cudaStream_t st_) : c(c_), which(which_), st(st_) {
+    if (!c->prof_on) return;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    cudaStreamIsCapturing(st, &cs);
+    if (cs != cudaStreamCaptureStatusNone) return;
+    cudaEventCreate(&a);
+    cudaEventCreate(&b);
+    cudaEventRecord(a, st);
+  }
+  ~ProfScope() {
+    if (!a) return;
+    cudaEventRecord(b, st);
+    c->prof_ev[which].emplace_back(a, b);
+  }
+};
+
+template <typename T>
+ikv_status grow(ikv_ctx* ctx, T** p, size_t count) {
+  if (*p) CU(ctx, cudaFree(*p));
+  *p = nullptr;
+  CU(ctx, cudaMalloc((void**)p, count * sizeof(T)));
+  return IKV_OK;
+}
+
+#define TRY(expr)                      \
+  do {                                 \
+    ikv_status _s = (expr);            \
+    if (_s != IKV_OK) return _s;       \
+  } while (0)
+
+__global__ void k_fill_i32(int32_t* p, int64_t n, int32_t v) {
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+    p[i] = v;
+}
+
+template <typename T>
+__global__ void k_init_dead(T* k_pool, T* v_pool, int64_t layer_stride, int L, int row /* Hkv*D */, int64_t slot) {
+  const int l = blockIdx.x;
+  for (int i = threadIdx.x; i < row; i += blockDim.x) {
+    k_pool[(int64_t)l * layer_stride + slot * row + i] = (T)(-1.0e4f);
+    v_pool[(int64_t)l * layer_stride + slot * row + i] = (T)0.f;
+  }
+}
+
+int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
+
+ikv_status ensure_scratch(ikv_ctx* c, int64_t tokens) {
+  if (tokens <= c->cap_tokens) return IKV_OK;
+  const int L = c->cfg.n_layers, Hq = c->cfg.n_q_heads, D = c->cfg.head_dim;
+  const int64_t cap = round_up(tokens, 1024);
+  const int64_t n_tiles = cap / SCORE_TILE;
+  TRY(grow(c, &c->cand_pos, cap));
+  TRY(grow(c, &c->cand_slot, cap));
+  TRY(grow(c, &c->logits, (size_t)L * Hq * cap));
+  TRY(grow(c, &c->partials, (size_t)L * Hq * n_tiles));
+  TRY(grow(c, &c->rule_c, cap));
+  TRY(grow(c, &c->kbar, (size_t)cap * D));
+  TRY(grow(c, &c->keepflag, cap));
+  TRY(grow(c, &c->tmp_slot, cap));
+  c->cap_tokens = cap;
+  return IKV_OK;
+}
+
+ikv_status ensure_xq(ikv_ctx* c, int64_t n) {
+  if (n <= c->xq_cap) return IKV_OK;
+  const int64_t cap = round_up(n, 256);
+  TRY(grow(c, &c->xq_slot, cap));
+  TRY(grow(c, &c->kq, (size_t)cap * c->cfg.head_dim));
+  TRY(grow(c, &c->kc, (size_t)cap * R_DC));
+  TRY(grow(c, &c->vc, (size_t)cap * R_DC));
+  c->xq_cap = cap;
+  return IKV_OK;
+}
+
+ikv_status ensure_parts(ikv_ctx* c, int64_t units) {
+  if (units <= c->part_cap) return IKV_OK;
+  TRY(grow(c, &c->part_o, (size_t)units * c->cfg.head_dim));
+  TRY(grow(c, &c->part_ml, (size_t)units));
+  c->part_cap = units;
+  return IKV_OK;
+}
+
+ikv_status ensure_staging(ikv_ctx* c, int64_t tokens, int64_t qelems) {
+  if (tokens > c->st_cap) {
+    const int64_t cap = round_up(tokens, 1024);
+    TRY(grow(c, &c->st_map, cap));
+    TRY(grow(c, &c->st_freed, cap));
+    TRY(grow(c, &c->st_valid, cap));
+    TRY(grow(c, &c->st_scores, cap));
+    c->st_cap = cap;
+  }
+  if (qelems > c->st_qcap) {
+    TRY(grow(c, &c->st_qrows, qelems));
+    c->st_qcap = qelems;
+  }
+  return IKV_OK;
+}
+
+ikv_status session_live_reserve(ikv_ctx* c, Session& s, int n) {
+  if (n <= s.live_cap) return IKV_OK;
+  const int cap = (int)round_up((int64_t)n + n / 4 + 1024, 1024);
+  TRY(grow(c, &s.live_slots, cap));
+  s.live_cap = cap;
+  s.covered = 0;
+  s.map_ptr = nullptr;
+  return IKV_OK;
+}
+
+void session_free(Session& s) {
+  cudaFree(s.d_mem);
+  cudaFree(s.d_qenc);
+  cudaFree(s.live_slots);
+  cudaFree(s.d_n_live);
+}
+
+ikv_status session_create(ikv_ctx* c, uint64_t id, Session** out) {
+  auto it = c->sessions.find(id);
+  if (it == c->sessions.end()) {
+    if ((int)c->sessions.size() >= c->cfg.max_sessions) {  // LRU eviction
+      auto victim = c->sessions.begin();
+      for (auto jt = c->sessions.begin(); jt != c->sessions.end(); ++jt)
+        if (jt->second.tick < victim->second.tick) victim = jt;
+      session_free(victim->second);
+      c->sessions.erase(victim);
+    }
+    Session s;
+    s.id = id;
+    const size_t n = (size_t)c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim;
+    CU(c, cudaMalloc((void**)&s.d_mem, n * sizeof(float)));
+    CU(c, cudaMalloc((void**)&s.d_qenc, n * sizeof(float)));
+    CU(c, cudaMalloc((void**)&s.d_n_live, sizeof(int32_t)));
+    it = c->sessions.emplace(id, s).first;
+  }
+  Session& s = it->second;
+  const size_t n = (size_t)c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim;
+  CU(c, cudaMemset(s.d_mem, 0, n * sizeof(float)));  // M_0 = 0 (R3)
+  CU(c, cudaMemset(s.d_qenc, 0, n * sizeof(float)));
+  CU(c, cudaMemset(s.d_n_live, 0, sizeof(int32_t)));
+  s.has_update = false;
+  s.covered = 0;
+  s.map_ptr = nullptr;
+  s.tick = ++c->tick;
+  *out = &s;
+  return IKV_OK;
+}
+
+Session* session_find(ikv_ctx* c, uint64_t id) {
+  auto it = c->sessions.find(id);
+  if (it == c->sessions.end()) return nullptr;
+  it->second.tick = ++c->tick;
+  return &it->second;
+}
+
+ikv_status check_request(ikv_ctx* c, const ikv_request& r) {
+  if (r.seq_len < 0) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "seq_len < 0");
+  if (r.seq_len > 0 && !r.slot_map) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "slot_map is NULL");
+  if (!(0 <= r.prefix_len && r.prefix_len <= r.q_start && r.q_start <= r.q_end && r.q_end <= r.seq_len))
+    IKV_FAIL(c, IKV_ERR_INVALID_ARG, "need 0 <= prefix_len <= q_start <= q_end <= seq_len (got %d %d %d %d)",
+             r.prefix_len, r.q_start, r.q_end, r.seq_len);
+  if (r.budget < 0) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "budget < 0");
+  if (r.radix_protected_len < 0) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "radix_protected_len < 0");
+  if (r.n_xattn_pos < 0 || (r.n_xattn_pos > 0 && !r.xattn_pos))
+    IKV_FAIL(c, IKV_ERR_INVALID_ARG, "bad xattn_pos / n_xattn_pos");
+  return IKV_OK;
+}
+
+// ---- typed launch helpers -------------------------------------------------------------------------------
+template <typename T, int D, int G>
+ikv_status launch_logits(ikv_ctx* c, const Session& s, const float* M, int N, bool kbar, cudaStream_t st) {
+  const int L = c->cfg.n_layers, Hkv = c->cfg.n_kv_heads, Hq = c->cfg.n_q_heads;
+  const int n_tiles = (N + SCORE_TILE - 1) / SCORE_TILE;
+  const int64_t ldc = c->cap_tokens;
+  const size_t smem = (size_t)Hq * (SCORE_TILE + 1) * 4 + SCORE_TILE * 4 + (kbar ? (size_t)SCORE_TILE * D * 4 : 0);
+  const float isd = 1.0f / sqrtf((float)D);
+  ProfScope prof(c, 0, st);
+  if (kbar) {
+    auto fn = k_score_logits<T, D, G, true>;
+    if (smem > 48 * 1024) CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    fn<<<n_tiles, 256, smem, st>>>((const T*)c->cfg.k_pool, c->layer_stride, L, Hkv, M, c->cand_slot, c->d_ncand,
+                                   c->cfg.dead_slot, c->logits, ldc, c->partials, n_tiles, c->kbar, isd);
+  } else {
+    auto fn = k_score_logits<T, D, G, false>;
+    if (smem > 48 * 1024) CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    fn<<<n_tiles, 256, smem, st>>>((const T*)c->cfg.k_pool, c->layer_stride, L, Hkv, M, c->cand_slot, c->d_ncand,
+                                   c->cfg.dead_slot, c->logits, ldc, c->partials, n_tiles, nullptr, isd);
+  }
+  LAUNCH_CHECK(c);
+  (void)s;
+  return IKV_OK;
+}
+
+template <typename T, int D>
+ikv_status dispatch_logits_g(ikv_ctx* c, const Session& s, const float* M, int N, bool kbar, cudaStream_t st) {
+  switch (c->G) {
+    case 1: return launch_logits<T, D, 1>(c, s, M, N, kbar, st);
+    case 2: return launch_logits<T, D, 2>(c, s, M, N, kbar, st);
+    case 4: return launch_logits<T, D, 4>(c, s, M, N, kbar, st);
+    case 5: return launch_logits<T, D, 5>(c, s, M, N, kbar, st);
+    case 8: return launch_logits<T, D, 8>(c, s, M, N, kbar, st);
+  }
+  IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "GQA group size %d not supported (1,2,4,5,8)", c->G);
+}
+
+ikv_status dispatch_logits(ikv_ctx* c, const Session& s, const float* M, int N, bool kbar, cudaStream_t st) {
+  const bool b = c->cfg.kv_dtype == IKV_BF16;
+  if (c->cfg.head_dim == 128) return b ? dispatch_logits_g<bf16, 128>(c, s, M, N, kbar, st)
+                                       : dispatch_logits_g<float, 128>(c, s, M, N, kbar, st);
+  return b ? dispatch_logits_g<bf16, 64>(c, s, M, N, kbar, st) : dispatch_logits_g<float, 64>(c, s, M, N, kbar, st);
+}
+
+template <typename T, int D, int G>
+ikv_status launch_decode(ikv_ctx* c, int layer, const DecBatch& batch, int n_req, int n_split, const void* q,
+                         void* out, float sm_scale, cudaStream_t st) {
+  constexpr int VEC = Elem<T>::VEC;
+  constexpr int NGRP = 4 * (32 / (D / VEC));
+  const int Hkv = c->cfg.n_kv_heads, Hq = c->cfg.n_q_heads;
+  const size_t smem = (size_t)NGRP * G * (D + 2) * 4;
+  auto fn = k_decode_split<T, D, G>;
+  if (smem > 48 * 1024) CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const T* kl = (const T*)c->cfg.k_pool + (int64_t)layer * c->layer_stride;
+  const T* vl = (const T*)c->cfg.v_pool + (int64_t)layer * c->layer_stride;
+  {
+    ProfScope prof(c, 1, st);
+    fn<<<dim3(n_split, Hkv, n_req), 128, smem, st>>>(kl, vl, Hkv, c->cfg.dead_slot, batch, (const T*)q, sm_scale,
+                                                     c->part_o, c->part_ml, n_split);
+  }
+  LAUNCH_CHECK(c);
+  k_decode_merge<T, D><<<dim3(Hq, n_req), D, 0, st>>>(c->part_o, c->part_ml, n_split, (T*)out);
+  LAUNCH_CHECK(c);
+  return IKV_OK;
+}
+
+template <typename T, int D>
+ikv_status dispatch_decode_g(ikv_ctx* c, int layer, const DecBatch& b, int n_req, int n_split, const void* q,
+                             void* out, float sc, cudaStream_t st) {
+  switch (c->G) {
+    case 1: return launch_decode<T, D, 1>(c, layer, b, n_req, n_split, q, out, sc, st);
+    case 2: return launch_decode<T, D, 2>(c, layer, b, n_req, n_split, q, out, sc, st);
+    case 4: return launch_decode<T, D, 4>(c, layer, b, n_req, n_split, q, out, sc, st);
+    case 5: return launch_decode<T, D, 5>(c, layer, b, n_req, n_split, q, out, sc, st);
+    case 8: return launch_decode<T, D, 8>(c, layer, b, n_req, n_split, q, out, sc, st);
+  }
+  IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "GQA group size %d not supported (1,2,4,5,8)", c->G);
+}
+
+ikv_status dispatch_decode(ikv_ctx* c, int layer, const DecBatch& b, int n_req, int n_split, const void* q,
+                           void* out, float sc, cudaStream_t st) {
+  const bool bf = c->cfg.kv_dtype == IKV_BF16;
+  if (c->cfg.head_dim == 128) return bf ? dispatch_decode_g<bf16, 128>(c, layer, b, n_req, n_split, q, out, sc, st)
+                                        : dispatch_decode_g<float, 128>(c, layer, b, n_req, n_split, q, out, sc, st);
+  return bf ? dispatch_decode_g<bf16, 64>(c, layer, b, n_req, n_split, q, out, sc, st)
+            : dispatch_decode_g<float, 64>(c, layer, b, n_req, n_split, q, out, sc, st);
+}
+
+ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, float* rule_out, cudaStream_t st) {
+  const int N = r.seq_len;
+  if (N == 0) return IKV_OK;
+  const int base_mode = mode & 0xff;
+  Session* s = session_find(c, r.session_id);
+  if (!s) IKV_FAIL(c, IKV_ERR_NO_SESSION, "session %llu does not exist", (unsigned long long)r.session_id);
+  const int L = c->cfg.n_layers, Hq = c->cfg.n_q_heads, Hkv = c->cfg.n_kv_heads, D = c->cfg.head_dim;
+  const bool learn = (base_mode == IKV_MODE_LEARNABLE) && !(mode & IKV_FLAG_NO_RESIDUAL);
+  if (base_mode == IKV_MODE_LEARNABLE && !c->has_resid)
+    IKV_FAIL(c, IKV_ERR_INVALID_ARG, "IKV_MODE_LEARNABLE needs ikv_residual_load first");
+  TRY(ensure_scratch(c, N));
+  const float* M = (base_mode == IKV_MODE_QUERY) ? s->d_qenc : s->d_mem;
+
+  k_partition<<<1, 1024, 0, st>>>(r.slot_map, N, c->cfg.dead_slot, r.prefix_len, r.q_start, r.q_end, scores, rule_out,
+                                  c->cand_pos, c->cand_slot, c->d_ncand);
+  LAUNCH_CHECK(c);
+  TRY(dispatch_logits(c, *s, M, N, learn, st));
+  const int n_tiles = (N + SCORE_TILE - 1) / SCORE_TILE;
+  k_score_lse<<<L * Hq, 128, 0, st>>>(c->partials, n_tiles, c->lse);
+  LAUNCH_CHECK(c);
+  k_score_rule<<<(N + 255) / 256, 256, (size_t)L * Hq * 4, st>>>(c->logits, c->cap_tokens, L * Hq, c->lse, c->d_ncand,
+                                                                 c->cand_pos, c->rule_c, scores, learn ? 0 : 1,
+                                                                 rule_out);
+  LAUNCH_CHECK(c);
+  if (learn) {
+    const bool use_x = !(mode & IKV_FLAG_NO_XATTN);
+    const int n_x = r.xattn_pos ? r.n_xattn_pos : (r.q_end - r.q_start);
+    TRY(ensure_xq(c, n_x > 0 ? n_x : 1));
+    k_mean_memory<<<1, D, 0, st>>>(M, L * Hq, D, c->mbar);
+    LAUNCH_CHECK(c);
+    if (use_x && n_x > 0) {
+      k_xattn_compact<<<1, 1024, 0, st>>>(r.slot_map, N, c->cfg.dead_slot, r.xattn_pos, n_x, r.q_start, c->xq_slot,
+                                          c->d_nxq);
+      LAUNCH_CHECK(c);
+      if (c->cfg.kv_dtype == IKV_BF16)
+        k_mean_key_list<bf16><<<n_x, D, 0, st>>>((const bf16*)c->cfg.k_pool, c->layer_stride, L, Hkv, D, c->xq_slot,
+                                                 c->d_nxq, c->kq);
+      else
+        k_mean_key_list<float><<<n_x, D, 0, st>>>((const float*)c->cfg.k_pool, c->layer_stride, L, Hkv, D,
+                                                  c->xq_slot, c->d_nxq, c->kq);
+      LAUNCH_CHECK(c);
+      k_resid_kv<<<n_x, R_DC, 0, st>>>(c->kq, c->d_nxq, D, c->rw, c->kc, c->vc);
+      LAUNCH_CHECK(c);
+    }
+    const int nblk = (N + R_TOK - 1) / R_TOK;
+    const int ux = (use_x && n_x > 0) ? 1 : 0;
+    if (D == 128)
+      k_residual<128><<<nblk, 256, 0, st>>>(c->rule_c, c->kbar, c->mbar, c->kc, c->vc, c->d_nxq, c->d_ncand,
+                                            c->cand_pos, c->rw, ux, scores);
+    else
+      k_residual<64><<<nblk, 256, 0, st>>>(c->rule_c, c->kbar, c->mbar, c->kc, c->vc, c->d_nxq, c->d_ncand,
+                                           c->cand_pos, c->rw, ux, scores);
+    LAUNCH_CHECK(c);
+  }
+  return IKV_OK;
+}
+
+ikv_status select_one(ikv_ctx* c, const ikv_request& r, const float* scores, int32_t* freed, int32_t* n_freed,
+                      int32_t* n_kept, cudaStream_t st) {
+  Session* s = session_find(c, r.session_id);
+  if (!s) IKV_FAIL(c, IKV_ERR_NO_SESSION, "session %llu does not exist", (unsigned long long)r.session_id);
+  const int N = r.seq_len;
+  TRY(ensure_scratch(c, N > 0 ? N : 1));
+  TRY(session_live_reserve(c, *s, N > 0 ? N : 1));
+  SelParams p;
+  p.S = r.slot_map; p.valid = r.valid_mask; p.scores = scores;
+  p.N = N; p.pi = r.prefix_len; p.qs = r.q_start; p.qe = r.q_end; p.C = r.budget; p.radix = r.radix_protected_len;
+  p.dead = c->cfg.dead_slot;
+  p.freed = freed; p.n_freed = n_freed; p.n_kept = n_kept;
+  p.live_slots = s->live_slots; p.n_live = s->d_n_live;
+  p.kept_bits = c->kept_bits; p.firstpos = c->firstpos; p.keepflag = c->keepflag; p.tmp_slot = c->tmp_slot;
+  k_select_evict<<<1, 1024, 0, st>>>(p);
+  LAUNCH_CHECK(c);
+  s->covered = N;
+  s->map_ptr = r.slot_map;
+  s->live_ub = N;
+  if (N > r.budget) {
+    const int forced_ub = r.prefix_len + (r.q_end - r.q_start);
+    s->live_ub = (forced_ub > r.budget ? forced_ub : r.budget);
+    if (s->live_ub > N) s->live_ub = N;
+  }
+  return IKV_OK;
+}
+
+}  // namespace
+
+// ======================================================================================================
+extern "C" {
+
+const char* ikv_version(void) { return "ikv 0.1 (sm_100a)"; }
+
+const char* ikv_last_error(const ikv_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+
+ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
+  if (!cfg || !out) return IKV_ERR_INVALID_ARG;
+  *out = nullptr;
+  ikv_ctx* c = new ikv_ctx();
+  c->cfg = *cfg;
+  auto fail = [&](ikv_status code, const char* msg) {
+    fprintf(stderr, "ikv_create: %s\n", msg);
+    delete c;
+    return code;
+  };
+  if (cfg->n_layers <= 0 || cfg->n_q_heads <= 0 || cfg->n_kv_heads <= 0 || cfg->n_q_heads % cfg->n_kv_heads != 0)
+    return fail(IKV_ERR_INVALID_ARG, "bad layer / head counts");
+  if (cfg->head_dim != 64 && cfg->head_dim != 128) return fail(IKV_ERR_UNSUPPORTED, "head_dim must be 64 or 128");
+  if (cfg->kv_dtype != IKV_BF16 && cfg->kv_dtype != IKV_F32)
+    return fail(IKV_ERR_UNSUPPORTED, "kv_dtype must be IKV_BF16 or IKV_F32 (PAPER.md:263)");
+  if (cfg->page_size <= 0 || cfg->n_slots <= 0 || cfg->n_slots > INT32_MAX || !cfg->k_pool || !cfg->v_pool)
+    return fail(IKV_ERR_INVALID_ARG, "bad pool description");
+  if (cfg->dead_slot < 0 || cfg->dead_slot >= cfg->n_slots) return fail(IKV_ERR_INVALID_ARG, "dead_slot out of range");
+  if (cfg->max_sessions <= 0) return fail(IKV_ERR_INVALID_ARG, "max_sessions must be > 0");
+  if (!(cfg->lambda >= 0.f)) return fail(IKV_ERR_INVALID_ARG, "lambda must be >= 0");
+  c->G = cfg->n_q_heads / cfg->n_kv_heads;
+  if (c->G != 1 && c->G != 2 && c->G != 4 && c->G != 5 && c->G != 8)
+    return fail(IKV_ERR_UNSUPPORTED, "GQA group size must be one of 1,2,4,5,8");
+  c->layer_stride = cfg->n_slots * cfg->n_kv_heads * cfg->head_dim;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return fail(IKV_ERR_CUDA, "no CUDA device");
+  cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
+  const int row = cfg->n_kv_heads * cfg->head_dim;
+  if (cfg->kv_dtype == IKV_BF16)
+    k_init_dead<bf16><<<cfg->n_layers, 256>>>((bf16*)cfg->k_pool, (bf16*)cfg->v_pool, c->layer_stride, cfg->n_layers,
+                                              row, cfg->dead_slot);
+  else
+    k_init_dead<float><<<cfg->n_layers, 256>>>((float*)cfg->k_pool, (float*)cfg->v_pool, c->layer_stride,
+                                               cfg->n_layers, row, cfg->dead_slot);
+  bool ok = cudaGetLastError() == cudaSuccess;
+  const size_t words = (size_t)(cfg->n_slots + 31) / 32;
+  ok = ok && cudaMalloc((void**)&c->kept_bits, words * 4) == cudaSuccess;
+  ok = ok && cudaMemset(c->kept_bits, 0, words * 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&c->firstpos, (size_t)cfg->n_slots * 4) == cudaSuccess;
+  if (ok) {
+    k_fill_i32<<<256, 256>>>(c->firstpos, cfg->n_slots, INT_MAX);
+    ok = cudaGetLastError() == cudaSuccess;
+  }
+  ok = ok && cudaMalloc((void**)&c->d_ncand, 4) == cudaSuccess && cudaMalloc((void**)&c->d_nxq, 4) == cudaSuccess;
+  ok = ok && cudaMemset(c->d_nxq, 0, 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&c->lse, (size_t)cfg->n_layers * cfg->n_q_heads * 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&c->mbar, (size_t)cfg->head_dim * 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&c->st_counts, 16) == cudaSuccess;
+  ok = ok && cudaDeviceSynchronize() == cudaSuccess;
+  if (!ok) {
+    ikv_destroy(c);
+    fprintf(stderr, "ikv_create: CUDA initialisation failed: %s\n", cudaGetErrorString(cudaGetLastError()));
+    return IKV_ERR_CUDA;
+  }
+  *out = c;
+  return IKV_OK;
+}
+
+ikv_status ikv_destroy(ikv_ctx* c) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  cudaDeviceSynchronize();
+  for (auto& kv : c->sessions) session_free(kv.second);
+  void* bufs[] = {c->cand_pos, c->cand_slot, c->d_ncand, c->logits, c->partials, c->lse, c->rule_c, c->kbar, c->mbar,
+                  c->xq_slot, c->d_nxq, c->kq, c->kc, c->vc, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
+                  c->part_o, c->part_ml, c->st_map, c->st_freed, c->st_counts, c->st_valid, c->st_scores,
+                  c->st_qrows, c->resid_blob};
+  for (void* b : bufs) cudaFree(b);
+  const cudaError_t e = cudaGetLastError();
+  delete c;
+  return e == cudaSuccess ? IKV_OK : IKV_ERR_CUDA;
+}
+
+ikv_status ikv_profile_enable(ikv_ctx* c, int32_t on) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  c->prof_on = on != 0;
+  return IKV_OK;
+}
+
+ikv_status ikv_profile_read(ikv_ctx* c, float* out_ms, int32_t* out_n) {
+  if (!c || !out_ms || !out_n) return IKV_ERR_INVALID_ARG;
+  CU(c, cudaDeviceSynchronize());
+  for (int w = 0; w < 2; ++w) {
+    float tot = 0.f;
+    for (auto& pr : c->prof_ev[w]) {
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, pr.first, pr.second);
+      tot += ms;
+      cudaEventDestroy(pr.first);
+      cudaEventDestroy(pr.second);
+    }
+    out_ms[w] = tot;
+    out_n[w] = (int32_t)c->prof_ev[w].size();
+    c->prof_ev[w].clear();
+  }
+  return IKV_OK;
+}
+
+ikv_status ikv_reserve(ikv_ctx* c, int64_t max_tokens, int32_t max_requests) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (max_tokens <= 0 || max_requests <= 0) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_reserve: sizes must be > 0");
+  TRY(ensure_scratch(c, max_tokens));
+  TRY(ensure_xq(c, 1024));
+  TRY(ensure_parts(c, (int64_t)max_requests * c->cfg.n_q_heads * 4 * c->n_sm));
+  TRY(ensure_staging(c, max_tokens, 0));
+  CU(c, cudaDeviceSynchronize());
+  return IKV_OK;
+}
+
+ikv_status ikv_session_open(ikv_ctx* c, uint64_t id) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  Session* s;
+  return session_create(c, id, &s);
+}
+
+ikv_status ikv_session_fork(ikv_ctx* c, uint64_t parent, uint64_t child, void* stream) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (parent == child) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "fork onto itself");
+  if (!session_find(c, parent)) IKV_FAIL(c, IKV_ERR_NO_SESSION, "parent session does not exist");
+  Session* ch;
+  TRY(session_create(c, child, &ch));
+  Session* p = session_find(c, parent);  // re-find: the map may have rehashed
+  const size_t n = (size_t)c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim * sizeof(float);
+  CU(c, cudaMemcpyAsync(ch->d_mem, p->d_mem, n, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  CU(c, cudaMemcpyAsync(ch->d_qenc, p->d_qenc, n, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  ch->has_update = p->has_update;
+  return IKV_OK;
+}
+
+ikv_status ikv_session_close(ikv_ctx* c, uint64_t id) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  auto it = c->sessions.find(id);
+  if (it == c->sessions.end()) IKV_FAIL(c, IKV_ERR_NO_SESSION, "session does not exist");
+  CU(c, cudaDeviceSynchronize());
+  session_free(it->second);
+  c->sessions.erase(it);
+  return IKV_OK;
+}
+
+ikv_status ikv_session_get_memory(ikv_ctx* c, uint64_t id, float* host_out) {
+  if (!c || !host_out) return IKV_ERR_INVALID_ARG;
+  Session* s = session_find(c, id);
+  if (!s) IKV_FAIL(c, IKV_ERR_NO_SESSION, "session does not exist");
+  const size_t n = (size_t)c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim * sizeof(float);
+  CU(c, cudaDeviceSynchronize());
+  CU(c, cudaMemcpy(host_out, s->d_mem, n, cudaMemcpyDeviceToHost));
+  return IKV_OK;
+}
+
+ikv_status ikv_session_set_memory(ikv_ctx* c, uint64_t id, const float* host_in) {
+  if (!c || !host_in) return IKV_ERR_INVALID_ARG;
+  Session* s = session_find(c, id);
+  if (!s) IKV_FAIL(c, IKV_ERR_NO_SESSION, "session does not exist");
+  const size_t n = (size_t)c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim * sizeof(float);
+  CU(c, cudaDeviceSynchronize());
+  CU(c, cudaMemcpy(s->d_mem, host_in, n, cudaMemcpyHostToDevice));
+  return IKV_OK;
+}
+
+ikv_status ikv_residual_load(ikv_ctx* c, const ikv_residual_weights* w) {
+  if (!c || !w) return IKV_ERR_INVALID_ARG;
+  if (!w->wq || !w->bq || !w->wk || !w->bk || !w->wv || !w->bv || !w->fc1_w || !w->fc1_b || !w->fc2_w || !w->fc2_b)
+    IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_residual_load: NULL weight array");
+  const int D = c->cfg.head_dim, P = 3 * D + 1, IN = P + R_DC;
+  // blob layout (floats): wq_t[P][128] bq[128] wk_t[D][128] bk[128] wv_t[D][128] bv[128] fc1_t[IN][256] fc1_b[256]
+  //                       fc2_w[256] fc2_b[1]
+  const size_t sizes[10] = {(size_t)P * R_DC, R_DC, (size_t)D * R_DC, R_DC, (size_t)D * R_DC, R_DC,
+                            (size_t)IN * R_HID, R_HID, R_HID, 1};
+  size_t off[11];
+  off[0] = 0;
+  for (int i = 0; i < 10; ++i) off[i + 1] = off[i] + ((sizes[i] + 3) / 4) * 4;  // keep 16-byte alignment
+  std::vector<float> h(off[10], 0.f);
+  auto transpose = [&](const float* src, int out_n, int in_n, float* dst) {
+    for (int o = 0; o < out_n; ++o)
+      for (int i = 0; i < in_n; ++i) dst[(size_t)i * out_n + o] = src[(size_t)o * in_n + i];
+  };
+  transpose(w->wq, R_DC, P, &h[off[0]]);
+  memcpy(&h[off[1]], w->bq, R_DC * 4);
+  transpose(w->wk, R_DC, D, &h[off[2]]);
+  memcpy(&h[off[3]], w->bk, R_DC * 4);
+  transpose(w->wv, R_DC, D, &h[off[4]]);
+  memcpy(&h[off[5]], w->bv, R_DC * 4);
+  transpose(w->fc1_w, R_HID, IN, &h[off[6]]);
+  memcpy(&h[off[7]], w->fc1_b, R_HID * 4);
+  memcpy(&h[off[8]], w->fc2_w, R_HID * 4);
+  h[off[9]] = w->fc2_b[0];
+  CU(c, cudaDeviceSynchronize());
+  if (!c->resid_blob) CU(c, cudaMalloc((void**)&c->resid_blob, h.size() * 4));
+  CU(c, cudaMemcpy(c->resid_blob, h.data(), h.size() * 4, cudaMemcpyHostToDevice));
+  float* b = c->resid_blob;
+  c->rw.wq_t = b + off[0]; c->rw.bq = b + off[1]; c->rw.wk_t = b + off[2]; c->rw.bk = b + off[3];
+  c->rw.wv_t = b + off[4]; c->rw.bv = b + off[5]; c->rw.fc1_t = b + off[6]; c->rw.fc1_b = b + off[7];
+  c->rw.fc2_w = b + off[8]; c->rw.fc2_b = b + off[9];
+  float a = w->alpha;  // "clipped at inference"
+  c->rw.alpha = a > 5.f ? 5.f : (a < -5.f ? -5.f : a);
+  c->has_resid = true;
+  return IKV_OK;
+}
+
+ikv_status ikv_memory_update(ikv_ctx* c, uint64_t id, const void* q_rows, int32_t n, int32_t q_dtype, void* stream) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (!q_rows || n <= 0) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_memory_update: need n > 0 query rows");
+  if (q_dtype != IKV_F32 && q_dtype != IKV_BF16) IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "q_dtype must be IKV_F32 or IKV_BF16");
+  Session* s = session_find(c, id);
+  if (!s) TRY(session_create(c, id, &s));
+  const int L = c->cfg.n_layers, Hq = c->cfg.n_q_heads, D = c->cfg.head_dim;
+  const float decay = expf(-c->cfg.lambda);
+  const int64_t rs = (int64_t)L * Hq * D;
+  if (q_dtype == IKV_F32)
+    k_memory_update<float><<<L * Hq, D, 0, (cudaStream_t)stream>>>(s->d_mem, s->d_qenc, (const float*)q_rows, n, rs, D,
+                                                                   decay);
+  else
+    k_memory_update<bf16><<<L * Hq, D, 0, (cudaStream_t)stream>>>(s->d_mem, s->d_qenc, (const bf16*)q_rows, n, rs, D,
+                                                                  decay);
+  LAUNCH_CHECK(c);
+  s->has_update = true;
+  return IKV_OK;
+}
+
+ikv_status ikv_score(ikv_ctx* c, const ikv_request* reqs, int32_t n_req, int32_t mode, float* scores, float* rule_out,
+                     void* stream) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (n_req < 0 || (n_req > 0 && (!reqs || !scores))) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_score: NULL argument");
+  const int bm = mode & 0xff;
+  if (bm != IKV_MODE_MEMORY && bm != IKV_MODE_LEARNABLE && bm != IKV_MODE_QUERY)
+    IKV_FAIL(c, IKV_ERR_INVALID_ARG, "unknown scorer mode %d", bm);
+  for (int r = 0; r < n_req; ++r) TRY(check_request(c, reqs[r]));
+  int64_t off = 0;
+  for (int r = 0; r < n_req; ++r) {
+    TRY(score_one(c, reqs[r], mode, scores + off, rule_out ? rule_out + off : nullptr, (cudaStream_t)stream));
+    off += reqs[r].seq_len;
+  }
+  return IKV_OK;
+}
+
+ikv_status ikv_select_evict(ikv_ctx* c, const ikv_request* reqs, int32_t n_req, const float* scores,
+                            int32_t* freed_slots, int32_t* n_freed, int32_t* n_kept, void* stream) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (n_req < 0 || (n_req > 0 && (!reqs || !scores || !freed_slots || !n_freed || !n_kept)))
+    IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_select_evict: NULL argument");
+  for (int r = 0; r < n_req; ++r) TRY(check_request(c, reqs[r]));
+  int64_t off = 0;
+  for (int r = 0; r < n_req; ++r) {
+    TRY(select_one(c, reqs[r], scores + off, freed_slots + off, n_freed + r, n_kept + r, (cudaStream_t)stream));
+    off += reqs[r].seq_len;
+  }
+  return IKV_OK;
+}
+
+ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, int32_t n_req, const void* q, void* out,
+                           float sm_scale, void* stream) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (n_req < 0 || (n_req > 0 && (!reqs || !q || !out))) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_decode_attn: NULL argument");
+  if (layer < 0 || layer >= c->cfg.n_layers) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "layer %d out of range", layer);
+  cudaStream_t st = (cudaStream_t)stream;
+  const int Hq = c->cfg.n_q_heads, Hkv = c->cfg.n_kv_heads, D = c->cfg.head_dim;
+  const size_t esz = c->cfg.kv_dtype == IKV_BF16 ? 2 : 4;
+  for (int r0 = 0; r0 < n_req; r0 += DEC_MAX_REQ) {
+    const int nb = (n_req - r0 < DEC_MAX_REQ) ? n_req - r0 : DEC_MAX_REQ;
+    DecBatch batch;
+    int max_items = 1;
+    for (int i = 0; i < nb; ++i) {
+      const ikv_request& r = reqs[r0 + i];
+      if (r.seq_len < 0 || (r.seq_len > 0 && !r.slot_map)) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "bad request %d", r0 + i);
+      Session* s = session_find(c, r.session_id);
+      if (!s) IKV_FAIL(c, IKV_ERR_NO_SESSION, "session %llu does not exist", (unsigned long long)r.session_id);
+      const bool stale = (r.flags & IKV_REQ_RESCAN) || s->map_ptr != r.slot_map || s->covered > r.seq_len ||
+                         (s->covered == 0 && r.seq_len > 0) || (r.seq_len - s->covered) > 4096;
+      if (stale) {
+        TRY(session_live_reserve(c, *s, r.seq_len > 0 ? r.seq_len : 1));
+        k_build_live<<<1, 1024, 0, st>>>(r.slot_map, r.seq_len, c->cfg.dead_slot, s->live_slots, s->d_n_live);
+        LAUNCH_CHECK(c);
+        s->covered = r.seq_len;
+        s->map_ptr = r.slot_map;
+        s->live_ub = r.seq_len;
+      }
+      batch.r[i].S = r.slot_map;
+      batch.r[i].live_slots = s->live_slots;
+      batch.r[i].n_live = s->d_n_live;
+      batch.r[i].seq_len = r.seq_len;
+      batch.r[i].covered = s->covered;
+      const int items = s->live_ub + (r.seq_len - s->covered);
+      if (items > max_items) max_items = items;
+    }
+    // split-K sizing: ~4 CTAs per SM, at least 64 tokens per split
+    int n_split = (4 * c->n_sm + Hkv * nb - 1) / (Hkv * nb);
+    const int by_len = (max_items + 63) / 64;
+    if (n_split > by_len) n_split = by_len;
+    if (n_split < 1) n_split = 1;
+    TRY(ensure_parts(c, (int64_t)nb * Hq * n_split));
+    TRY(dispatch_decode(c, layer, batch, nb, n_split, (const char*)q + (size_t)r0 * Hq * D * esz,
+                        (char*)out + (size_t)r0 * Hq * D * esz, sm_scale, st));
+  }
+  return IKV_OK;
+}
+
+ikv_status ikv_prune_host(ikv_ctx* c, const ikv_request* req, const float* q_rows_host, int32_t n_rows, int32_t mode,
+                          int32_t* slot_map_host, uint8_t* valid_host, float* scores_host, int32_t* freed_host,
+                          int32_t* n_freed_host, int32_t* n_kept_host, void* stream) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (!req || !slot_map_host || !freed_host || !n_freed_host || !n_kept_host)
+    IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_prune_host: NULL argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int N = req->seq_len;
+  const int64_t qel = (int64_t)(n_rows > 0 ? n_rows : 0) * c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim;
+  TRY(ensure_staging(c, N > 0 ? N : 1, qel));
+  ikv_request r = *req;
+  r.slot_map = c->st_map;
+  r.valid_mask = c->st_valid;
+  r.xattn_pos = nullptr;
+  r.n_xattn_pos = 0;
+  TRY(check_request(c, r));
+  CU(c, cudaMemcpyAsync(c->st_map, slot_map_host, (size_t)N * 4, cudaMemcpyHostToDevice, st));
+  if (q_rows_host && n_rows > 0) {
+    CU(c, cudaMemcpyAsync(c->st_qrows, q_rows_host, (size_t)qel * 4, cudaMemcpyHostToDevice, st));
+    TRY(ikv_memory_update(c, r.session_id, c->st_qrows, n_rows, IKV_F32, stream));
+  }
+  TRY(ikv_score(c, &r, 1, mode, c->st_scores, nullptr, stream));
+  TRY(ikv_select_evict(c, &r, 1, c->st_scores, c->st_freed, c->st_counts, c->st_counts + 1, stream));
+  int32_t counts[2] = {0, 0};
+  CU(c, cudaMemcpyAsync(counts, c->st_counts, 8, cudaMemcpyDeviceToHost, st));
+  CU(c, cudaMemcpyAsync(slot_map_host, c->st_map, (size_t)N * 4, cudaMemcpyDeviceToHost, st));
+  if (valid_host) CU(c, cudaMemcpyAsync(valid_host, c->st_valid, (size_t)N, cudaMemcpyDeviceToHost, st));
+  if (scores_host) CU(c, cudaMemcpyAsync(scores_host, c->st_scores, (size_t)N * 4, cudaMemcpyDeviceToHost, st));
+  CU(c, cudaStreamSynchronize(st));
+  *n_freed_host = counts[0];
+  *n_kept_host = counts[1];
+  if (counts[0] > 0) CU(c, cudaMemcpy(freed_host, c->st_freed, (size_t)counts[0] * 4, cudaMemcpyDeviceToHost));
+  return IKV_OK;
+}
+
+}  // extern "C"
