@@ -14,6 +14,7 @@
 #include "decode.cuh"
 #include "residual.cuh"
 #include "score.cuh"
+#include "score_mma.cuh"
 #include "select.cuh"
 
 using namespace ikv;
@@ -51,6 +52,8 @@ struct ikv_ctx {
   uint64_t tick = 0;
   std::string err;
   int n_sm = 148;
+  int max_smem = 48 * 1024;  // opt-in dynamic shared memory per CTA
+  uint4* frag = nullptr;     // B fragments of M / sqrt(D) for the bf16 key pass
 
   // scratch (per request, sized by ensure_scratch)
   int64_t cap_tokens = 0;
@@ -168,7 +171,7 @@ ikv_status ensure_scratch(ikv_ctx* c, int64_t tokens) {
   TRY(grow(c, &c->cand_pos, cap));
   TRY(grow(c, &c->cand_slot, cap));
   TRY(grow(c, &c->logits, (size_t)L * Hq * cap));
-  TRY(grow(c, &c->partials, (size_t)L * Hq * n_tiles));
+  TRY(grow(c, &c->partials, (size_t)L * Hq * (n_tiles > c->n_sm ? n_tiles : c->n_sm)));
   TRY(grow(c, &c->rule_c, cap));
   TRY(grow(c, &c->kbar, (size_t)cap * D));
   TRY(grow(c, &c->keepflag, cap));
@@ -318,10 +321,9 @@ ikv_status dispatch_logits_g(ikv_ctx* c, const Session& s, const float* M, int N
 }
 
 ikv_status dispatch_logits(ikv_ctx* c, const Session& s, const float* M, int N, bool kbar, cudaStream_t st) {
-  const bool b = c->cfg.kv_dtype == IKV_BF16;
-  if (c->cfg.head_dim == 128) return b ? dispatch_logits_g<bf16, 128>(c, s, M, N, kbar, st)
-                                       : dispatch_logits_g<float, 128>(c, s, M, N, kbar, st);
-  return b ? dispatch_logits_g<bf16, 64>(c, s, M, N, kbar, st) : dispatch_logits_g<float, 64>(c, s, M, N, kbar, st);
+  // plain-FMA kernel: fp32 pools only (the bf16 pools take k_key_pass)
+  if (c->cfg.head_dim == 128) return dispatch_logits_g<float, 128>(c, s, M, N, kbar, st);
+  return dispatch_logits_g<float, 64>(c, s, M, N, kbar, st);
 }
 
 template <typename T, int D, int G>
@@ -368,6 +370,57 @@ ikv_status dispatch_decode(ikv_ctx* c, int layer, const DecBatch& b, int n_req, 
             : dispatch_decode_g<float, 64>(c, layer, b, n_req, n_split, q, out, sc, st);
 }
 
+// bf16 key pass on the tensor pipe (score_mma.cuh).  Returns the number of partial (max, sum) columns.
+template <int D, int G>
+ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, int* n_part, cudaStream_t st) {
+  const int L = c->cfg.n_layers, Hkv = c->cfg.n_kv_heads, Hq = c->cfg.n_q_heads;
+  constexpr int NT = (G <= 4) ? 1 : 2;
+  const int total = L * Hkv * NT * (D / 32) * 32;
+  k_memory_frags<D, G><<<(total + 255) / 256, 256, 0, st>>>(M, L, Hkv, 1.0f / sqrtf((float)D), c->frag);
+  LAUNCH_CHECK(c);
+  int ns = 0;
+  const size_t smem = key_pass_smem(L, Hq, Hkv, D, kbar, c->max_smem, &ns);
+  if (ns < 2) IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "key pass: L*Hq = %d and row of %d bytes do not fit shared memory", L * Hq,
+                       Hkv * D * 2);
+  KeyPassParams p;
+  p.k_pool = (const bf16*)c->cfg.k_pool; p.layer_stride = c->layer_stride; p.L = L; p.Hkv = Hkv; p.frag = c->frag;
+  p.cand_slot = c->cand_slot; p.n_cand = c->d_ncand;
+  p.xq_slot = with_xq ? c->xq_slot : nullptr; p.n_xq = with_xq ? c->d_nxq : nullptr;
+  p.logits = c->logits; p.ldc = c->cap_tokens; p.partials = c->partials; p.kbar = c->kbar; p.kq = c->kq;
+  p.n_stage = ns;
+  const int grid = c->n_sm;
+  ProfScope prof(c, 0, st);
+  if (kbar) {
+    auto fn = k_key_pass<D, G, true>;
+    CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    fn<<<grid, KP_THREADS, smem, st>>>(p);
+  } else {
+    auto fn = k_key_pass<D, G, false>;
+    CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    fn<<<grid, KP_THREADS, smem, st>>>(p);
+  }
+  LAUNCH_CHECK(c);
+  *n_part = grid;
+  return IKV_OK;
+}
+
+template <int D>
+ikv_status dispatch_key_pass_g(ikv_ctx* c, const float* M, bool kbar, bool xq, int* n_part, cudaStream_t st) {
+  switch (c->G) {
+    case 1: return launch_key_pass<D, 1>(c, M, kbar, xq, n_part, st);
+    case 2: return launch_key_pass<D, 2>(c, M, kbar, xq, n_part, st);
+    case 4: return launch_key_pass<D, 4>(c, M, kbar, xq, n_part, st);
+    case 5: return launch_key_pass<D, 5>(c, M, kbar, xq, n_part, st);
+    case 8: return launch_key_pass<D, 8>(c, M, kbar, xq, n_part, st);
+  }
+  IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "GQA group size %d not supported (1,2,4,5,8)", c->G);
+}
+
+ikv_status dispatch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool xq, int* n_part, cudaStream_t st) {
+  return c->cfg.head_dim == 128 ? dispatch_key_pass_g<128>(c, M, kbar, xq, n_part, st)
+                                : dispatch_key_pass_g<64>(c, M, kbar, xq, n_part, st);
+}
+
 ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, float* rule_out, cudaStream_t st) {
   const int N = r.seq_len;
   if (N == 0) return IKV_OK;
@@ -384,31 +437,37 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   k_partition<<<1, 1024, 0, st>>>(r.slot_map, N, c->cfg.dead_slot, r.prefix_len, r.q_start, r.q_end, scores, rule_out,
                                   c->cand_pos, c->cand_slot, c->d_ncand);
   LAUNCH_CHECK(c);
-  TRY(dispatch_logits(c, *s, M, N, learn, st));
-  const int n_tiles = (N + SCORE_TILE - 1) / SCORE_TILE;
-  k_score_lse<<<L * Hq, 128, 0, st>>>(c->partials, n_tiles, c->lse);
-  LAUNCH_CHECK(c);
-  k_score_rule<<<(N + 255) / 256, 256, (size_t)L * Hq * 4, st>>>(c->logits, c->cap_tokens, L * Hq, c->lse, c->d_ncand,
-                                                                 c->cand_pos, c->rule_c, scores, learn ? 0 : 1,
-                                                                 rule_out);
-  LAUNCH_CHECK(c);
+  const bool fast = c->cfg.kv_dtype == IKV_BF16;  // tensor-pipe key pass; fp32 pools take the plain FMA kernel
+  const bool use_x = learn && !(mode & IKV_FLAG_NO_XATTN);
+  const int n_x = use_x ? (r.xattn_pos ? r.n_xattn_pos : (r.q_end - r.q_start)) : 0;
   if (learn) {
-    const bool use_x = !(mode & IKV_FLAG_NO_XATTN);
-    const int n_x = r.xattn_pos ? r.n_xattn_pos : (r.q_end - r.q_start);
     TRY(ensure_xq(c, n_x > 0 ? n_x : 1));
-    k_mean_memory<<<1, D, 0, st>>>(M, L * Hq, D, c->mbar);
-    LAUNCH_CHECK(c);
-    if (use_x && n_x > 0) {
+    if (n_x > 0) {
       k_xattn_compact<<<1, 1024, 0, st>>>(r.slot_map, N, c->cfg.dead_slot, r.xattn_pos, n_x, r.q_start, c->xq_slot,
                                           c->d_nxq);
       LAUNCH_CHECK(c);
-      if (c->cfg.kv_dtype == IKV_BF16)
-        k_mean_key_list<bf16><<<n_x, D, 0, st>>>((const bf16*)c->cfg.k_pool, c->layer_stride, L, Hkv, D, c->xq_slot,
-                                                 c->d_nxq, c->kq);
-      else
-        k_mean_key_list<float><<<n_x, D, 0, st>>>((const float*)c->cfg.k_pool, c->layer_stride, L, Hkv, D,
-                                                  c->xq_slot, c->d_nxq, c->kq);
+    }
+  }
+  int n_part = (N + SCORE_TILE - 1) / SCORE_TILE;
+  if (fast) {
+    TRY(dispatch_key_pass(c, M, learn, n_x > 0, &n_part, st));
+  } else {
+    TRY(dispatch_logits(c, *s, M, N, learn, st));
+    if (n_x > 0) {
+      k_mean_key_list<float><<<n_x, D, 0, st>>>((const float*)c->cfg.k_pool, c->layer_stride, L, Hkv, D, c->xq_slot,
+                                                c->d_nxq, c->kq);
       LAUNCH_CHECK(c);
+    }
+  }
+  k_score_lse<<<L * Hq, 128, 0, st>>>(c->partials, n_part, c->lse);
+  LAUNCH_CHECK(c);
+  k_score_rule4<<<(N + 63) / 64, 256, 0, st>>>(c->logits, c->cap_tokens, L * Hq, c->lse, c->d_ncand, c->cand_pos,
+                                               c->rule_c, scores, learn ? 0 : 1, rule_out);
+  LAUNCH_CHECK(c);
+  if (learn) {
+    k_mean_memory<<<1, D, 0, st>>>(M, L * Hq, D, c->mbar);
+    LAUNCH_CHECK(c);
+    if (n_x > 0) {
       k_resid_kv<<<n_x, R_DC, 0, st>>>(c->kq, c->d_nxq, D, c->rw, c->kc, c->vc);
       LAUNCH_CHECK(c);
     }
@@ -488,6 +547,7 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return fail(IKV_ERR_CUDA, "no CUDA device");
   cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
+  cudaDeviceGetAttribute(&c->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   const int row = cfg->n_kv_heads * cfg->head_dim;
   if (cfg->kv_dtype == IKV_BF16)
     k_init_dead<bf16><<<cfg->n_layers, 256>>>((bf16*)cfg->k_pool, (bf16*)cfg->v_pool, c->layer_stride, cfg->n_layers,
@@ -509,6 +569,9 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
   ok = ok && cudaMalloc((void**)&c->lse, (size_t)cfg->n_layers * cfg->n_q_heads * 4) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&c->mbar, (size_t)cfg->head_dim * 4) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&c->st_counts, 16) == cudaSuccess;
+  // B fragments: [L][Hkv][NT<=2][D/32][32 lanes] uint4
+  ok = ok && cudaMalloc((void**)&c->frag, (size_t)cfg->n_layers * cfg->n_kv_heads * 2 * (cfg->head_dim / 32) * 32 *
+                                              sizeof(uint4)) == cudaSuccess;
   ok = ok && cudaDeviceSynchronize() == cudaSuccess;
   if (!ok) {
     ikv_destroy(c);
@@ -526,7 +589,7 @@ ikv_status ikv_destroy(ikv_ctx* c) {
   void* bufs[] = {c->cand_pos, c->cand_slot, c->d_ncand, c->logits, c->partials, c->lse, c->rule_c, c->kbar, c->mbar,
                   c->xq_slot, c->d_nxq, c->kq, c->kc, c->vc, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
                   c->part_o, c->part_ml, c->st_map, c->st_freed, c->st_counts, c->st_valid, c->st_scores,
-                  c->st_qrows, c->resid_blob};
+                  c->st_qrows, c->resid_blob, c->frag};
   for (void* b : bufs) cudaFree(b);
   const cudaError_t e = cudaGetLastError();
   delete c;
