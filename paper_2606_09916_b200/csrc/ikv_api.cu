@@ -4,6 +4,9 @@
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
+#include <stdlib.h>
+
+#include <type_traits>
 
 #include <string>
 #include <unordered_map>
@@ -12,6 +15,7 @@
 #include "../../include/ikv.h"
 #include "common.cuh"
 #include "decode.cuh"
+#include "decode_mma.cuh"
 #include "residual.cuh"
 #include "score.cuh"
 #include "score_mma.cuh"
@@ -54,6 +58,8 @@ struct ikv_ctx {
   int n_sm = 148;
   int max_smem = 48 * 1024;  // opt-in dynamic shared memory per CTA
   uint4* frag = nullptr;     // B fragments of M / sqrt(D) for the bf16 key pass
+  bool use_pdl = true;       // programmatic dependent launch between decode kernels (IKV_PDL=0 disables)
+  bool attr_done[2][2][9] = {};
 
   // scratch (per request, sized by ensure_scratch)
   int64_t cap_tokens = 0;
@@ -146,6 +152,24 @@ ikv_status grow(ikv_ctx* ctx, T** p, size_t count) {
     ikv_status _s = (expr);            \
     if (_s != IKV_OK) return _s;       \
   } while (0)
+
+// Launch with the programmatic-stream-serialization attribute (PDL): the kernel may start while its predecessor in
+// the stream drains; it orders itself with griddepcontrol.wait.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*fn)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl,
+                       Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, fn, KArgs(args)...);
+}
 
 __global__ void k_fill_i32(int32_t* p, int64_t n, int32_t v) {
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
@@ -329,22 +353,40 @@ ikv_status dispatch_logits(ikv_ctx* c, const Session& s, const float* M, int N, 
 template <typename T, int D, int G>
 ikv_status launch_decode(ikv_ctx* c, int layer, const DecBatch& batch, int n_req, int n_split, const void* q,
                          void* out, float sm_scale, cudaStream_t st) {
-  constexpr int VEC = Elem<T>::VEC;
-  constexpr int NGRP = 4 * (32 / (D / VEC));
   const int Hkv = c->cfg.n_kv_heads, Hq = c->cfg.n_q_heads;
-  const size_t smem = (size_t)NGRP * G * (D + 2) * 4;
-  auto fn = k_decode_split<T, D, G>;
-  if (smem > 48 * 1024) CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const T* kl = (const T*)c->cfg.k_pool + (int64_t)layer * c->layer_stride;
   const T* vl = (const T*)c->cfg.v_pool + (int64_t)layer * c->layer_stride;
-  {
+  if constexpr (std::is_same<T, bf16>::value) {
+    // tensor-pipe split kernel behind a bulk-copy ring (decode_mma.cuh)
+    const int n_hg = (Hkv + DM_CWARPS - 1) / DM_CWARPS;
+    int ns = 0;
+    const size_t smem = decode_mma_smem(Hkv < DM_CWARPS ? Hkv : DM_CWARPS, D, c->max_smem, &ns);
+    if (ns < 2) IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "decode: a stage of %d heads x %d does not fit shared memory", Hkv, D);
+    DecMmaParams p;
+    p.k_layer = kl; p.v_layer = vl; p.Hkv = Hkv; p.dead = c->cfg.dead_slot; p.q = (const bf16*)q; p.sm_scale = sm_scale;
+    p.part_o = c->part_o; p.part_ml = c->part_ml; p.n_split = n_split; p.n_stage = ns;
+    auto fn = k_decode_mma<D, G>;
+    if (!c->attr_done[0][D == 128][G]) {
+      CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      c->attr_done[0][D == 128][G] = true;
+    }
+    {
+      ProfScope prof(c, 1, st);
+      CU(c, launch_pdl(fn, dim3(n_split, n_req, n_hg), dim3(DM_THREADS), smem, st, c->use_pdl, p, batch));
+    }
+  } else {
+    constexpr int VEC = Elem<T>::VEC;
+    constexpr int NGRP = 4 * (32 / (D / VEC));
+    const size_t smem = (size_t)NGRP * G * (D + 2) * 4;
+    auto fn = k_decode_split<T, D, G>;
+    if (smem > 48 * 1024) CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     ProfScope prof(c, 1, st);
     fn<<<dim3(n_split, Hkv, n_req), 128, smem, st>>>(kl, vl, Hkv, c->cfg.dead_slot, batch, (const T*)q, sm_scale,
                                                      c->part_o, c->part_ml, n_split);
+    LAUNCH_CHECK(c);
   }
-  LAUNCH_CHECK(c);
-  k_decode_merge<T, D><<<dim3(Hq, n_req), D, 0, st>>>(c->part_o, c->part_ml, n_split, (T*)out);
-  LAUNCH_CHECK(c);
+  CU(c, launch_pdl(k_decode_merge4<T, D>, dim3(Hq, n_req), dim3(256), 0, st, c->use_pdl, (const float*)c->part_o,
+                   (const float2*)c->part_ml, n_split, (T*)out));
   return IKV_OK;
 }
 
@@ -548,6 +590,7 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
   if (cudaGetDevice(&dev) != cudaSuccess) return fail(IKV_ERR_CUDA, "no CUDA device");
   cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
   cudaDeviceGetAttribute(&c->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (const char* e = getenv("IKV_PDL")) c->use_pdl = atoi(e) != 0;
   const int row = cfg->n_kv_heads * cfg->head_dim;
   if (cfg->kv_dtype == IKV_BF16)
     k_init_dead<bf16><<<cfg->n_layers, 256>>>((bf16*)cfg->k_pool, (bf16*)cfg->v_pool, c->layer_stride, cfg->n_layers,
@@ -807,10 +850,19 @@ ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, i
       const int items = s->live_ub + (r.seq_len - s->covered);
       if (items > max_items) max_items = items;
     }
-    // split-K sizing: ~4 CTAs per SM, at least 64 tokens per split
-    int n_split = (4 * c->n_sm + Hkv * nb - 1) / (Hkv * nb);
-    const int by_len = (max_items + 63) / 64;
-    if (n_split > by_len) n_split = by_len;
+    int n_split;
+    if (c->cfg.kv_dtype == IKV_BF16) {
+      // one CTA (all KV heads of a token range) per SM, at least 16 tokens per split
+      const int n_hg = (Hkv + DM_CWARPS - 1) / DM_CWARPS;
+      n_split = c->n_sm / (nb * n_hg);
+      const int by_len = (max_items + 15) / 16;
+      if (n_split > by_len) n_split = by_len;
+    } else {
+      // ~4 CTAs per SM, at least 64 tokens per split
+      n_split = (4 * c->n_sm + Hkv * nb - 1) / (Hkv * nb);
+      const int by_len = (max_items + 63) / 64;
+      if (n_split > by_len) n_split = by_len;
+    }
     if (n_split < 1) n_split = 1;
     TRY(ensure_parts(c, (int64_t)nb * Hq * n_split));
     TRY(dispatch_decode(c, layer, batch, nb, n_split, (const char*)q + (size_t)r0 * Hq * D * esz,
