@@ -16,7 +16,7 @@
 #include "common.cuh"
 #include "decode.cuh"
 #include "decode_mma.cuh"
-#include "residual.cuh"
+#include "residual_mma.cuh"
 #include "score.cuh"
 #include "score_mma.cuh"
 #include "select.cuh"
@@ -68,8 +68,12 @@ struct ikv_ctx {
   float2* partials = nullptr;
   float *lse = nullptr, *rule_c = nullptr, *kbar = nullptr, *mbar = nullptr;
   int32_t *xq_slot = nullptr, *d_nxq = nullptr;
-  float *kq = nullptr, *kc = nullptr, *vc = nullptr;
+  float* kq = nullptr;
+  uint4 *kc_frag = nullptr, *vc_frag = nullptr;  // B fragments of Kc / Vc (Eq. 6)
   int64_t xq_cap = 0;
+  // folded residual operands of the current call (residual_mma.cuh)
+  float *mpart = nullptr, *bq_eff = nullptr, *b1_eff = nullptr;
+  uint4 *wq_frag = nullptr, *w1k_frag = nullptr;
   uint32_t* kept_bits = nullptr;
   int32_t* firstpos = nullptr;
   uint8_t* keepflag = nullptr;
@@ -209,8 +213,8 @@ ikv_status ensure_xq(ikv_ctx* c, int64_t n) {
   const int64_t cap = round_up(n, 256);
   TRY(grow(c, &c->xq_slot, cap));
   TRY(grow(c, &c->kq, (size_t)cap * c->cfg.head_dim));
-  TRY(grow(c, &c->kc, (size_t)cap * R_DC));
-  TRY(grow(c, &c->vc, (size_t)cap * R_DC));
+  TRY(grow(c, &c->kc_frag, (size_t)cap * 32));  // 4 heads x 2 k-steps x cap/8 tiles x 32 lanes
+  TRY(grow(c, &c->vc_frag, (size_t)cap * 32));  // 4 heads x cap/16 steps x 4 tiles x 32 lanes
   c->xq_cap = cap;
   return IKV_OK;
 }
@@ -490,6 +494,16 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
       LAUNCH_CHECK(c);
     }
   }
+  if (learn) {  // fold mbar into W_Q / fc1 (residual_mma.cuh); independent of the key pass
+    const int LH = L * Hq, nb = (LH + 31) / 32;
+    k_mean_memory_part<<<nb, D, 0, st>>>(M, LH, D, c->mpart);
+    LAUNCH_CHECK(c);
+    FoldOut fo;
+    fo.mbar = c->mbar; fo.wq_frag = c->wq_frag; fo.w1k_frag = c->w1k_frag; fo.bq_eff = c->bq_eff; fo.b1_eff = c->b1_eff;
+    if (D == 128) k_resid_fold<128><<<resid_fold_grid<128>(), 128, 0, st>>>(c->mpart, nb, LH, c->rw, fo);
+    else k_resid_fold<64><<<resid_fold_grid<64>(), 128, 0, st>>>(c->mpart, nb, LH, c->rw, fo);
+    LAUNCH_CHECK(c);
+  }
   int n_part = (N + SCORE_TILE - 1) / SCORE_TILE;
   if (fast) {
     TRY(dispatch_key_pass(c, M, learn, n_x > 0, &n_part, st));
@@ -507,20 +521,20 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
                                                c->rule_c, scores, learn ? 0 : 1, rule_out);
   LAUNCH_CHECK(c);
   if (learn) {
-    k_mean_memory<<<1, D, 0, st>>>(M, L * Hq, D, c->mbar);
-    LAUNCH_CHECK(c);
     if (n_x > 0) {
-      k_resid_kv<<<n_x, R_DC, 0, st>>>(c->kq, c->d_nxq, D, c->rw, c->kc, c->vc);
+      k_resid_kv_frags<<<(n_x + 15) / 16, 128, 0, st>>>(c->kq, c->d_nxq, D, c->rw, (int)(c->xq_cap / 16), c->kc_frag,
+                                                       c->vc_frag);
       LAUNCH_CHECK(c);
     }
-    const int nblk = (N + R_TOK - 1) / R_TOK;
-    const int ux = (use_x && n_x > 0) ? 1 : 0;
-    if (D == 128)
-      k_residual<128><<<nblk, 256, 0, st>>>(c->rule_c, c->kbar, c->mbar, c->kc, c->vc, c->d_nxq, c->d_ncand,
-                                            c->cand_pos, c->rw, ux, scores);
-    else
-      k_residual<64><<<nblk, 256, 0, st>>>(c->rule_c, c->kbar, c->mbar, c->kc, c->vc, c->d_nxq, c->d_ncand,
-                                           c->cand_pos, c->rw, ux, scores);
+    ResidMmaParams rp;
+    rp.rule_c = c->rule_c; rp.kbar = c->kbar; rp.n_cand = c->d_ncand; rp.cand_pos = c->cand_pos; rp.n_xq = c->d_nxq;
+    rp.wq_frag = c->wq_frag; rp.w1k_frag = c->w1k_frag; rp.kc_frag = c->kc_frag; rp.vc_frag = c->vc_frag;
+    rp.bq_eff = c->bq_eff; rp.b1_eff = c->b1_eff; rp.nks = (int)(c->xq_cap / 16);
+    rp.use_xattn = (use_x && n_x > 0) ? 1 : 0;
+    rp.scores = scores;
+    const int nblk = (N + R_WARPS * 16 - 1) / (R_WARPS * 16);
+    if (D == 128) k_residual_mma<128><<<nblk, R_WARPS * 32, 0, st>>>(rp, c->rw);
+    else k_residual_mma<64><<<nblk, R_WARPS * 32, 0, st>>>(rp, c->rw);
     LAUNCH_CHECK(c);
   }
   return IKV_OK;
@@ -612,6 +626,14 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
   ok = ok && cudaMalloc((void**)&c->lse, (size_t)cfg->n_layers * cfg->n_q_heads * 4) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&c->mbar, (size_t)cfg->head_dim * 4) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&c->st_counts, 16) == cudaSuccess;
+  {
+    const int LH = cfg->n_layers * cfg->n_q_heads, KS = cfg->head_dim / 16;
+    ok = ok && cudaMalloc((void**)&c->mpart, (size_t)((LH + 31) / 32) * cfg->head_dim * 4) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->bq_eff, R_DC * 4) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->b1_eff, R_HID * 4) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->wq_frag, (size_t)KS * 16 * 32 * sizeof(uint4)) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->w1k_frag, (size_t)4 * KS * 8 * 32 * sizeof(uint4)) == cudaSuccess;
+  }
   // B fragments: [L][Hkv][NT<=2][D/32][32 lanes] uint4
   ok = ok && cudaMalloc((void**)&c->frag, (size_t)cfg->n_layers * cfg->n_kv_heads * 2 * (cfg->head_dim / 32) * 32 *
                                               sizeof(uint4)) == cudaSuccess;
@@ -630,7 +652,8 @@ ikv_status ikv_destroy(ikv_ctx* c) {
   cudaDeviceSynchronize();
   for (auto& kv : c->sessions) session_free(kv.second);
   void* bufs[] = {c->cand_pos, c->cand_slot, c->d_ncand, c->logits, c->partials, c->lse, c->rule_c, c->kbar, c->mbar,
-                  c->xq_slot, c->d_nxq, c->kq, c->kc, c->vc, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
+                  c->xq_slot, c->d_nxq, c->kq, c->kc_frag, c->vc_frag, c->mpart, c->bq_eff, c->b1_eff, c->wq_frag,
+                  c->w1k_frag, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
                   c->part_o, c->part_ml, c->st_map, c->st_freed, c->st_counts, c->st_valid, c->st_scores,
                   c->st_qrows, c->resid_blob, c->frag};
   for (void* b : bufs) cudaFree(b);
@@ -730,35 +753,64 @@ ikv_status ikv_residual_load(ikv_ctx* c, const ikv_residual_weights* w) {
   if (!w->wq || !w->bq || !w->wk || !w->bk || !w->wv || !w->bv || !w->fc1_w || !w->fc1_b || !w->fc2_w || !w->fc2_b)
     IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_residual_load: NULL weight array");
   const int D = c->cfg.head_dim, P = 3 * D + 1, IN = P + R_DC;
-  // blob layout (floats): wq_t[P][128] bq[128] wk_t[D][128] bk[128] wv_t[D][128] bv[128] fc1_t[IN][256] fc1_b[256]
-  //                       fc2_w[256] fc2_b[1]
-  const size_t sizes[10] = {(size_t)P * R_DC, R_DC, (size_t)D * R_DC, R_DC, (size_t)D * R_DC, R_DC,
-                            (size_t)IN * R_HID, R_HID, R_HID, 1};
-  size_t off[11];
+  // blob layout (floats): wq[128][P] bq[128] wk_t[D][128] bk[128] wv_t[D][128] bv[128] fc1_w[256][IN] fc1_b[256]
+  //                       fc2_w[256] fc2_b[1] w1c_frag[4][8][8][32] (uint4: B fragments of fc1's c columns)
+  const size_t n_frag = (size_t)4 * 8 * 8 * 32;
+  const size_t sizes[11] = {(size_t)R_DC * P, R_DC, (size_t)D * R_DC, R_DC, (size_t)D * R_DC, R_DC,
+                            (size_t)R_HID * IN, R_HID, R_HID, 1, n_frag * 4};
+  size_t off[12];
   off[0] = 0;
-  for (int i = 0; i < 10; ++i) off[i + 1] = off[i] + ((sizes[i] + 3) / 4) * 4;  // keep 16-byte alignment
-  std::vector<float> h(off[10], 0.f);
+  for (int i = 0; i < 11; ++i) off[i + 1] = off[i] + ((sizes[i] + 3) / 4) * 4;  // keep 16-byte alignment
+  std::vector<float> h(off[11], 0.f);
   auto transpose = [&](const float* src, int out_n, int in_n, float* dst) {
     for (int o = 0; o < out_n; ++o)
       for (int i = 0; i < in_n; ++i) dst[(size_t)i * out_n + o] = src[(size_t)o * in_n + i];
   };
-  transpose(w->wq, R_DC, P, &h[off[0]]);
+  memcpy(&h[off[0]], w->wq, sizes[0] * 4);
   memcpy(&h[off[1]], w->bq, R_DC * 4);
   transpose(w->wk, R_DC, D, &h[off[2]]);
   memcpy(&h[off[3]], w->bk, R_DC * 4);
   transpose(w->wv, R_DC, D, &h[off[4]]);
   memcpy(&h[off[5]], w->bv, R_DC * 4);
-  transpose(w->fc1_w, R_HID, IN, &h[off[6]]);
+  memcpy(&h[off[6]], w->fc1_w, sizes[6] * 4);
   memcpy(&h[off[7]], w->fc1_b, R_HID * 4);
   memcpy(&h[off[8]], w->fc2_w, R_HID * 4);
   h[off[9]] = w->fc2_b[0];
+  {  // static B fragments (bf16 hi | lo) of fc1's c columns; k order is natural (the A side comes from accumulators)
+    auto bf16_rn = [](float x) -> uint32_t {
+      uint32_t u;
+      memcpy(&u, &x, 4);
+      if ((u & 0x7fffffffu) > 0x7f800000u) return (u >> 16) | 0x40u;  // NaN stays NaN
+      return (u + 0x7fffu + ((u >> 16) & 1u)) >> 16;
+    };
+    auto up = [](uint32_t b) { uint32_t u = b << 16; float f; memcpy(&f, &u, 4); return f; };
+    uint32_t* fr = reinterpret_cast<uint32_t*>(&h[off[10]]);
+    for (int ch = 0; ch < 4; ++ch)
+      for (int s8 = 0; s8 < 8; ++s8)
+        for (int t = 0; t < 8; ++t)
+          for (int lane = 0; lane < 32; ++lane) {
+            const int r = lane >> 2, q = lane & 3;
+            const int n = ch * 64 + t * 8 + r;
+            const int ks[4] = {2 * q, 2 * q + 1, 2 * q + 8, 2 * q + 9};
+            uint32_t hi[4], lo[4];
+            for (int e = 0; e < 4; ++e) {
+              const float v = w->fc1_w[(size_t)n * IN + P + s8 * 16 + ks[e]];
+              hi[e] = bf16_rn(v);
+              lo[e] = bf16_rn(v - up(hi[e]));
+            }
+            uint32_t* o = fr + ((((size_t)ch * 8 + s8) * 8 + t) * 32 + lane) * 4;
+            o[0] = hi[0] | (hi[1] << 16); o[1] = hi[2] | (hi[3] << 16);
+            o[2] = lo[0] | (lo[1] << 16); o[3] = lo[2] | (lo[3] << 16);
+          }
+  }
   CU(c, cudaDeviceSynchronize());
   if (!c->resid_blob) CU(c, cudaMalloc((void**)&c->resid_blob, h.size() * 4));
   CU(c, cudaMemcpy(c->resid_blob, h.data(), h.size() * 4, cudaMemcpyHostToDevice));
   float* b = c->resid_blob;
-  c->rw.wq_t = b + off[0]; c->rw.bq = b + off[1]; c->rw.wk_t = b + off[2]; c->rw.bk = b + off[3];
-  c->rw.wv_t = b + off[4]; c->rw.bv = b + off[5]; c->rw.fc1_t = b + off[6]; c->rw.fc1_b = b + off[7];
+  c->rw.wq = b + off[0]; c->rw.bq = b + off[1]; c->rw.wk_t = b + off[2]; c->rw.bk = b + off[3];
+  c->rw.wv_t = b + off[4]; c->rw.bv = b + off[5]; c->rw.fc1_w = b + off[6]; c->rw.fc1_b = b + off[7];
   c->rw.fc2_w = b + off[8]; c->rw.fc2_b = b + off[9];
+  c->rw.w1c_frag = reinterpret_cast<const uint4*>(b + off[10]);
   float a = w->alpha;  // "clipped at inference"
   c->rw.alpha = a > 5.f ? 5.f : (a < -5.f ? -5.f : a);
   c->has_resid = true;

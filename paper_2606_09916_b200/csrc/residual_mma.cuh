@@ -1,0 +1,378 @@
+// residual_mma.cuh -- residual head of Eq. 4-6 on the tensor pipe, fp32-grade.
+// Topology per DESIGN.md R9-R12.  "FP32 residual head": every GEMM operand is split into a bf16 hi
+// and a bf16 lo part and each product is taken as hi*hi + lo*hi + hi*lo with fp32 accumulation (mma.sync
+// m16n8k16), which carries ~16 mantissa bits per operand; softmax, GELU and all vectors stay fp32.
+//
+// Folding of the constant inputs: phi_j = [kbar_j | mbar | kbar_j (.) mbar | rule_j] and mbar is the same for every
+// token of the call, so   W phi_j + b = (W_k + W_km diag(mbar)) kbar_j + rule_j w_r + (b + W_m mbar).
+// k_resid_fold builds the folded matrices of W_Q and fc1 once per call, directly in B-fragment order.
+//
+// One warp scores 16 candidates end to end in registers:
+//   Q   = Wq' kbar + rule wq_r + bq'                          (16 x 128, K = D)
+//   c_h = softmax(Q_h Kc_h^T / sqrt(32)) Vc_h,  h = 0..3       (online softmax over chunks of 64 query keys)
+//   hid = W1k' kbar + W1c c + rule w1_r + b1'                 (16 x 256, K = D + 128), in 4 chunks of 64 units
+//   z   = fc2_w . GELU_erf(hid) + fc2_b;   s = rule + alpha z
+// Accumulator (C) fragments are turned into A fragments of the next product in registers.
+#pragma once
+#include "common.cuh"
+#include "pipe.cuh"
+
+namespace ikv {
+
+constexpr int R_DC = 128;   // d_c
+constexpr int R_HC = 4;     // H_c
+constexpr int R_DH = 32;    // d_c / H_c
+constexpr int R_HID = 256;  // hidden width
+constexpr int R_WARPS = 4;  // 16-candidate tiles per CTA
+
+// Device copy of the residual head.  Raw matrices are row-major [out][in] as loaded (R9).
+struct ResidW {
+  const float *wq, *bq;        // [128][3D+1], [128]
+  const float *wk_t, *bk;      // [D][128] (transposed), [128]
+  const float *wv_t, *bv;      // [D][128] (transposed), [128]
+  const float *fc1_w, *fc1_b;  // [256][3D+1+128], [256]
+  const float *fc2_w, *fc2_b;  // [256], [1]
+  const uint4* w1c_frag;       // static: fc1 columns of c, [4 chunks][8 k-steps][8 n-tiles][32 lanes]
+  float alpha;                 // already clipped to [-5,5]
+};
+
+__device__ __forceinline__ uint32_t pack_bf16_rn(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+// (x, y) -> packed bf16 hi parts and packed bf16 lo parts (x = hi + lo up to ~2^-17 |x|)
+__device__ __forceinline__ void split_bf16(float x, float y, uint32_t& hi, uint32_t& lo) {
+  hi = pack_bf16_rn(x, y);
+  lo = pack_bf16_rn(x - bf16lo(hi), y - bf16hi(hi));
+}
+// acc += A * B with A = (ah + al), B = (b.x,b.y hi | b.z,b.w lo), dropping lo*lo
+__device__ __forceinline__ void mma3(float (&acc)[4], const uint32_t (&ah)[4], const uint32_t (&al)[4], const uint4& b) {
+  mma_bf16_16816(acc, ah[0], ah[1], ah[2], ah[3], b.x, b.y);
+  mma_bf16_16816(acc, al[0], al[1], al[2], al[3], b.x, b.y);
+  mma_bf16_16816(acc, ah[0], ah[1], ah[2], ah[3], b.z, b.w);
+}
+
+// k index of the kbar A fragments: lane q loads kbar[row][16 s + 4 q .. + 3] as one float4, so mma k index kappa of
+// k-step s stands for column 16 s + kperm(kappa).
+__host__ __device__ __forceinline__ int kperm(int kappa) {
+  return (kappa < 8) ? 4 * (kappa >> 1) + (kappa & 1) : 4 * ((kappa - 8) >> 1) + 2 + (kappa & 1);
+}
+
+// One B fragment (hi | lo) of lane (r, q) from a functor B(k_local 0..15, n_local 0..7).
+template <typename F>
+__device__ __forceinline__ uint4 make_bfrag(int lane, F B) {
+  const int r = lane >> 2, q = lane & 3;
+  const float v0 = B(2 * q, r), v1 = B(2 * q + 1, r), v2 = B(2 * q + 8, r), v3 = B(2 * q + 9, r);
+  uint4 o;
+  split_bf16(v0, v1, o.x, o.z);
+  split_bf16(v2, v3, o.y, o.w);
+  return o;
+}
+
+// mbar partial sums: grid = ceil(LH / 32), block = D.  part[b][d] = sum of rows 32 b .. 32 b + 31 of M (Eq. 5 mbar).
+__global__ void k_mean_memory_part(const float* __restrict__ M, int LH, int D, float* __restrict__ part) {
+  const int d = threadIdx.x, r0 = blockIdx.x * 32;
+  float acc = 0.f;
+  for (int i = r0; i < min(LH, r0 + 32); ++i) acc += M[(int64_t)i * D + d];
+  part[blockIdx.x * D + d] = acc;
+}
+
+struct FoldOut {
+  float* mbar;      // [D]
+  uint4* wq_frag;   // [D/16][16][32]
+  uint4* w1k_frag;  // [4][D/16][8][32]
+  float* bq_eff;    // [128]
+  float* b1_eff;    // [256]
+};
+
+// Folds mbar into W_Q and fc1 (see the header of this file).  block = 128 threads; grid covers
+// D/16*16*32 + 4*D/16*8*32 fragment items and 384 bias items.
+template <int D>
+__global__ __launch_bounds__(128) void k_resid_fold(const float* __restrict__ part, int n_part, int LH, ResidW w,
+                                                    FoldOut o) {
+  constexpr int KS = D / 16, P = 3 * D + 1, IN = P + R_DC;
+  constexpr int N_WQ = KS * 16 * 32, N_W1 = 4 * KS * 8 * 32, N_B = R_DC + R_HID;
+  __shared__ float mb[D];
+  for (int d = threadIdx.x; d < D; d += 128) {
+    float acc = 0.f;
+    for (int b = 0; b < n_part; ++b) acc += part[b * D + d];
+    mb[d] = acc / (float)LH;
+  }
+  __syncthreads();
+  int idx = blockIdx.x * 128 + threadIdx.x;
+  if (blockIdx.x == 0)
+    for (int d = threadIdx.x; d < D; d += 128) o.mbar[d] = mb[d];
+  if (idx < N_WQ) {
+    const int lane = idx & 31, t = (idx >> 5) & 15, s = idx >> 9;
+    o.wq_frag[idx] = make_bfrag(lane, [&](int kl, int nl) {
+      const int n = t * 8 + nl, k = s * 16 + kperm(kl);
+      const float* row = w.wq + (int64_t)n * P;
+      return fmaf(row[2 * D + k], mb[k], row[k]);
+    });
+    return;
+  }
+  idx -= N_WQ;
+  if (idx < N_W1) {
+    const int lane = idx & 31, t = (idx >> 5) & 7;
+    const int s = (idx >> 8) % KS, ch = (idx >> 8) / KS;
+    o.w1k_frag[idx] = make_bfrag(lane, [&](int kl, int nl) {
+      const int n = ch * 64 + t * 8 + nl, k = s * 16 + kperm(kl);
+      const float* row = w.fc1_w + (int64_t)n * IN;
+      return fmaf(row[2 * D + k], mb[k], row[k]);
+    });
+    return;
+  }
+  idx -= N_W1;
+  if (idx < N_B) {
+    const bool isq = idx < R_DC;
+    const int n = isq ? idx : idx - R_DC;
+    const float* row = isq ? (w.wq + (int64_t)n * P + D) : (w.fc1_w + (int64_t)n * IN + D);
+    float acc = isq ? w.bq[n] : w.fc1_b[n];
+    for (int d = 0; d < D; ++d) acc = fmaf(row[d], mb[d], acc);
+    (isq ? o.bq_eff : o.b1_eff)[n] = acc;
+  }
+}
+template <int D>
+inline int resid_fold_grid() {
+  return ((D / 16) * 16 * 32 + 4 * (D / 16) * 8 * 32 + R_DC + R_HID + 127) / 128;
+}
+
+// Kc = W_K K^q + b_K, Vc = W_V K^q + b_V (Eq. 6) for 16 query keys per CTA (block = 128, thread = output
+// channel), written as B fragments:
+//   kc_frag[((hc*2 + u)*nkt + t)*32 + lane] : S = Q_h Kc_h^T, k = head dim 16 u + kappa, n = key 8 t + r, scaled
+//                                             by log2(e)/sqrt(32) so that the softmax runs on exp2
+//   vc_frag[((hc*nks + v)*4 + nt)*32 + lane]: O = P Vc_h,     k = key 16 v + kappa, n = head dim 8 nt + r
+// nkt = 2 nks = capacity in 8-key tiles.  Keys >= n_xq are zero.
+__global__ __launch_bounds__(128) void k_resid_kv_frags(const float* __restrict__ kq, const int32_t* __restrict__ n_xq,
+                                                        int D, ResidW w, int nks, uint4* __restrict__ kc_frag,
+                                                        uint4* __restrict__ vc_frag) {
+  __shared__ float x[16][128];
+  __shared__ float kc[16][R_DC + 1], vc[16][R_DC + 1];
+  const int nq = *n_xq, v = blockIdx.x, k0 = v * 16, o = threadIdx.x;
+  if (k0 >= nq) return;
+  for (int i = threadIdx.x; i < 16 * D; i += 128) {
+    const int key = i / D, d = i % D;
+    x[key][d] = (k0 + key < nq) ? kq[(int64_t)(k0 + key) * D + d] : 0.f;
+  }
+  __syncthreads();
+  float ak[16], av[16];
+  const float bk = w.bk[o], bv = w.bv[o];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) { ak[i] = bk; av[i] = bv; }
+  for (int d = 0; d < D; ++d) {
+    const float wk = w.wk_t[d * R_DC + o], wv = w.wv_t[d * R_DC + o];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+      ak[i] = fmaf(wk, x[i][d], ak[i]);
+      av[i] = fmaf(wv, x[i][d], av[i]);
+    }
+  }
+  const float sc = 1.4426950408889634f * 0.17677669529663689f;  // log2(e) / sqrt(32)  (R10)
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    const bool ok = k0 + i < nq;
+    kc[i][o] = ok ? ak[i] * sc : 0.f;
+    vc[i][o] = ok ? av[i] : 0.f;
+  }
+  __syncthreads();
+  const int nkt = 2 * nks;
+  for (int it = threadIdx.x; it < 512; it += 128) {
+    const int lane = it & 31, a = (it >> 5) & 3, hc = it >> 7;
+    {  // Kc: a = (u, tile-in-pair)
+      const int u = a >> 1, tl = a & 1;
+      kc_frag[((int64_t)(hc * 2 + u) * nkt + 2 * v + tl) * 32 + lane] =
+          make_bfrag(lane, [&](int kl, int nl) { return kc[tl * 8 + nl][hc * R_DH + u * 16 + kl]; });
+    }
+    {  // Vc: a = nt
+      vc_frag[((int64_t)(hc * nks + v) * 4 + a) * 32 + lane] =
+          make_bfrag(lane, [&](int kl, int nl) { return vc[kl][hc * R_DH + a * 8 + nl]; });
+    }
+  }
+}
+
+struct ResidMmaParams {
+  const float* rule_c;       // [n_cand]
+  const float* kbar;         // [n_cand][D]
+  const int32_t* n_cand;
+  const int32_t* cand_pos;
+  const int32_t* n_xq;
+  const uint4 *wq_frag, *w1k_frag, *kc_frag, *vc_frag;
+  const float *bq_eff, *b1_eff;
+  int nks;                   // capacity of the key fragments in 16-key steps
+  int use_xattn;
+  float* scores;             // by position
+};
+
+__device__ __forceinline__ float gelu_erf(float x) { return 0.5f * x * (1.f + erff(x * 0.70710678118654752f)); }
+__device__ __forceinline__ float ex2f(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+template <int D>
+__global__ __launch_bounds__(R_WARPS * 32) void k_residual_mma(const ResidMmaParams p, const ResidW w) {
+  constexpr int KS = D / 16;
+  const int nc = *p.n_cand;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, r = lane >> 2, q = lane & 3;
+  const int t0 = (blockIdx.x * R_WARPS + warp) * 16;
+  if (t0 >= nc) return;
+  const int row0 = min(t0 + r, nc - 1), row1 = min(t0 + r + 8, nc - 1);
+  const float rule0 = p.rule_c[row0], rule1 = p.rule_c[row1];
+  const int nq = p.use_xattn ? *p.n_xq : 0;
+  const int P = 3 * D + 1, IN = P + R_DC;
+
+  // A fragments of kbar (hi | lo); k order per kperm()
+  uint32_t akh[KS][4], akl[KS][4];
+#pragma unroll
+  for (int s = 0; s < KS; ++s) {
+    const float4 x0 = __ldg(reinterpret_cast<const float4*>(p.kbar + (int64_t)row0 * D + s * 16 + 4 * q));
+    const float4 x1 = __ldg(reinterpret_cast<const float4*>(p.kbar + (int64_t)row1 * D + s * 16 + 4 * q));
+    split_bf16(x0.x, x0.y, akh[s][0], akl[s][0]);
+    split_bf16(x1.x, x1.y, akh[s][1], akl[s][1]);
+    split_bf16(x0.z, x0.w, akh[s][2], akl[s][2]);
+    split_bf16(x1.z, x1.w, akh[s][3], akl[s][3]);
+  }
+
+  // A fragments of c (Eq. 6), 8 k-steps; zero when there is no live query key (R7)
+  uint32_t ach[8][4], acl[8][4];
+  if (nq > 0) {
+    // ---- Q = Wq' kbar + rule wq_r + bq'
+    float accq[16][4];
+#pragma unroll
+    for (int t = 0; t < 16; ++t) { accq[t][0] = accq[t][1] = accq[t][2] = accq[t][3] = 0.f; }
+#pragma unroll
+    for (int s = 0; s < KS; ++s)
+#pragma unroll
+      for (int t = 0; t < 16; ++t) mma3(accq[t], akh[s], akl[s], __ldg(p.wq_frag + (s * 16 + t) * 32 + lane));
+#pragma unroll
+    for (int t = 0; t < 16; ++t) {
+      const int n = t * 8 + 2 * q;
+      const float2 b = *reinterpret_cast<const float2*>(p.bq_eff + n);
+      const float wr0 = __ldg(w.wq + (int64_t)n * P + 3 * D), wr1 = __ldg(w.wq + (int64_t)(n + 1) * P + 3 * D);
+      accq[t][0] += fmaf(rule0, wr0, b.x); accq[t][1] += fmaf(rule0, wr1, b.y);
+      accq[t][2] += fmaf(rule1, wr0, b.x); accq[t][3] += fmaf(rule1, wr1, b.y);
+    }
+    const int nkt = 2 * p.nks;
+    // ---- 4-head cross attention, online softmax in the exp2 domain over chunks of 64 query keys
+#pragma unroll
+    for (int hc = 0; hc < R_HC; ++hc) {
+      uint32_t qh[2][4], ql[2][4];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int ta = hc * 4 + 2 * u, tb = ta + 1;
+        split_bf16(accq[ta][0], accq[ta][1], qh[u][0], ql[u][0]);
+        split_bf16(accq[ta][2], accq[ta][3], qh[u][1], ql[u][1]);
+        split_bf16(accq[tb][0], accq[tb][1], qh[u][2], ql[u][2]);
+        split_bf16(accq[tb][2], accq[tb][3], qh[u][3], ql[u][3]);
+      }
+      float m0 = -CUDART_INF_F, m1 = -CUDART_INF_F, l0 = 0.f, l1 = 0.f;
+      float o[4][4];
+#pragma unroll
+      for (int nt = 0; nt < 4; ++nt) { o[nt][0] = o[nt][1] = o[nt][2] = o[nt][3] = 0.f; }
+      for (int kc0 = 0; kc0 < nq; kc0 += 64) {
+        const int ntn = min(8, (nq - kc0 + 7) >> 3);
+        float sc[8][4];
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {
+          sc[t][0] = sc[t][1] = sc[t][2] = sc[t][3] = 0.f;
+          if (t < ntn) {
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+              mma3(sc[t], qh[u], ql[u], __ldg(p.kc_frag + ((int64_t)(hc * 2 + u) * nkt + (kc0 >> 3) + t) * 32 + lane));
+          }
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const bool ok = t < ntn && (kc0 + t * 8 + 2 * q + e) < nq;
+            if (!ok) { sc[t][e] = -CUDART_INF_F; sc[t][2 + e] = -CUDART_INF_F; }
+          }
+        }
+        float x0 = -CUDART_INF_F, x1 = -CUDART_INF_F;
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {
+          x0 = fmaxf(x0, fmaxf(sc[t][0], sc[t][1]));
+          x1 = fmaxf(x1, fmaxf(sc[t][2], sc[t][3]));
+        }
+        x0 = fmaxf(x0, __shfl_xor_sync(0xffffffffu, x0, 1)); x0 = fmaxf(x0, __shfl_xor_sync(0xffffffffu, x0, 2));
+        x1 = fmaxf(x1, __shfl_xor_sync(0xffffffffu, x1, 1)); x1 = fmaxf(x1, __shfl_xor_sync(0xffffffffu, x1, 2));
+        const float n0 = fmaxf(m0, x0), n1 = fmaxf(m1, x1);  // finite: every chunk holds at least one live key
+        const float c0 = ex2f(m0 - n0), c1 = ex2f(m1 - n1);
+        m0 = n0; m1 = n1;
+        l0 *= c0; l1 *= c1;
+#pragma unroll
+        for (int nt = 0; nt < 4; ++nt) { o[nt][0] *= c0; o[nt][1] *= c0; o[nt][2] *= c1; o[nt][3] *= c1; }
+#pragma unroll
+        for (int t = 0; t < 8; ++t) {
+          sc[t][0] = ex2f(sc[t][0] - n0); sc[t][1] = ex2f(sc[t][1] - n0);
+          sc[t][2] = ex2f(sc[t][2] - n1); sc[t][3] = ex2f(sc[t][3] - n1);
+          l0 += sc[t][0] + sc[t][1];
+          l1 += sc[t][2] + sc[t][3];
+        }
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
+          if (2 * v < ntn) {
+            uint32_t ph[4], pl[4];
+            split_bf16(sc[2 * v][0], sc[2 * v][1], ph[0], pl[0]);
+            split_bf16(sc[2 * v][2], sc[2 * v][3], ph[1], pl[1]);
+            split_bf16(sc[2 * v + 1][0], sc[2 * v + 1][1], ph[2], pl[2]);
+            split_bf16(sc[2 * v + 1][2], sc[2 * v + 1][3], ph[3], pl[3]);
+#pragma unroll
+            for (int nt = 0; nt < 4; ++nt)
+              mma3(o[nt], ph, pl, __ldg(p.vc_frag + ((int64_t)(hc * p.nks + (kc0 >> 4) + v) * 4 + nt) * 32 + lane));
+          }
+        }
+      }
+      l0 += __shfl_xor_sync(0xffffffffu, l0, 1); l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
+      l1 += __shfl_xor_sync(0xffffffffu, l1, 1); l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
+      const float i0 = 1.f / l0, i1 = 1.f / l1;
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int ks = hc * 2 + u, na = 2 * u, nb = 2 * u + 1;
+        split_bf16(o[na][0] * i0, o[na][1] * i0, ach[ks][0], acl[ks][0]);
+        split_bf16(o[na][2] * i1, o[na][3] * i1, ach[ks][1], acl[ks][1]);
+        split_bf16(o[nb][0] * i0, o[nb][1] * i0, ach[ks][2], acl[ks][2]);
+        split_bf16(o[nb][2] * i1, o[nb][3] * i1, ach[ks][3], acl[ks][3]);
+      }
+    }
+  }
+
+  // ---- fc1 -> GELU -> fc2, 4 chunks of 64 hidden units
+  float z0 = 0.f, z1 = 0.f;
+#pragma unroll 1
+  for (int ch = 0; ch < 4; ++ch) {
+    float acc[8][4];
+#pragma unroll
+    for (int t = 0; t < 8; ++t) { acc[t][0] = acc[t][1] = acc[t][2] = acc[t][3] = 0.f; }
+#pragma unroll
+    for (int s = 0; s < KS; ++s)
+#pragma unroll
+      for (int t = 0; t < 8; ++t) mma3(acc[t], akh[s], akl[s], __ldg(p.w1k_frag + ((ch * KS + s) * 8 + t) * 32 + lane));
+    if (nq > 0) {
+#pragma unroll
+      for (int s = 0; s < 8; ++s)
+#pragma unroll
+        for (int t = 0; t < 8; ++t) mma3(acc[t], ach[s], acl[s], __ldg(w.w1c_frag + ((ch * 8 + s) * 8 + t) * 32 + lane));
+    }
+#pragma unroll
+    for (int t = 0; t < 8; ++t) {
+      const int n = ch * 64 + t * 8 + 2 * q;
+      const float2 b = *reinterpret_cast<const float2*>(p.b1_eff + n);
+      const float2 w2 = __ldg(reinterpret_cast<const float2*>(w.fc2_w + n));
+      const float wr0 = __ldg(w.fc1_w + (int64_t)n * IN + 3 * D), wr1 = __ldg(w.fc1_w + (int64_t)(n + 1) * IN + 3 * D);
+      z0 = fmaf(w2.x, gelu_erf(acc[t][0] + fmaf(rule0, wr0, b.x)), z0);
+      z0 = fmaf(w2.y, gelu_erf(acc[t][1] + fmaf(rule0, wr1, b.y)), z0);
+      z1 = fmaf(w2.x, gelu_erf(acc[t][2] + fmaf(rule1, wr0, b.x)), z1);
+      z1 = fmaf(w2.y, gelu_erf(acc[t][3] + fmaf(rule1, wr1, b.y)), z1);
+    }
+  }
+  z0 += __shfl_xor_sync(0xffffffffu, z0, 1); z0 += __shfl_xor_sync(0xffffffffu, z0, 2);
+  z1 += __shfl_xor_sync(0xffffffffu, z1, 1); z1 += __shfl_xor_sync(0xffffffffu, z1, 2);
+  if (q == 0) {
+    const float b2 = w.fc2_b[0];
+    if (t0 + r < nc) p.scores[p.cand_pos[t0 + r]] = rule0 + w.alpha * (z0 + b2);
+    if (t0 + r + 8 < nc) p.scores[p.cand_pos[t0 + r + 8]] = rule1 + w.alpha * (z1 + b2);
+  }
+}
+
+}  // namespace ikv
