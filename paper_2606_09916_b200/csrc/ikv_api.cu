@@ -20,6 +20,7 @@
 #include "score.cuh"
 #include "score_mma.cuh"
 #include "select.cuh"
+#include "select_cluster.cuh"
 
 using namespace ikv;
 
@@ -480,8 +481,13 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   TRY(ensure_scratch(c, N));
   const float* M = (base_mode == IKV_MODE_QUERY) ? s->d_qenc : s->d_mem;
 
-  k_partition<<<1, 1024, 0, st>>>(r.slot_map, N, c->cfg.dead_slot, r.prefix_len, r.q_start, r.q_end, scores, rule_out,
-                                  c->cand_pos, c->cand_slot, c->d_ncand);
+#define IKV_PART_ARGS r.slot_map, N, c->cfg.dead_slot, r.prefix_len, r.q_start, r.q_end, scores, rule_out, \
+                      c->cand_pos, c->cand_slot, c->d_ncand
+  if (N <= CL_CTAS * 1024 * 4) k_partition_cl<4><<<CL_CTAS, 1024, 0, st>>>(IKV_PART_ARGS);
+  else if (N <= CL_CTAS * 1024 * 8) k_partition_cl<8><<<CL_CTAS, 1024, 0, st>>>(IKV_PART_ARGS);
+  else if (N <= CL_MAX_N) k_partition_cl<16><<<CL_CTAS, 1024, 0, st>>>(IKV_PART_ARGS);
+  else k_partition<<<1, 1024, 0, st>>>(IKV_PART_ARGS);
+#undef IKV_PART_ARGS
   LAUNCH_CHECK(c);
   const bool fast = c->cfg.kv_dtype == IKV_BF16;  // tensor-pipe key pass; fp32 pools take the plain FMA kernel
   const bool use_x = learn && !(mode & IKV_FLAG_NO_XATTN);
@@ -554,7 +560,10 @@ ikv_status select_one(ikv_ctx* c, const ikv_request& r, const float* scores, int
   p.freed = freed; p.n_freed = n_freed; p.n_kept = n_kept;
   p.live_slots = s->live_slots; p.n_live = s->d_n_live;
   p.kept_bits = c->kept_bits; p.firstpos = c->firstpos; p.keepflag = c->keepflag; p.tmp_slot = c->tmp_slot;
-  k_select_evict<<<1, 1024, 0, st>>>(p);
+  if (N <= CL_CTAS * 1024 * 4) k_select_evict_cl<4><<<CL_CTAS, 1024, 0, st>>>(p);
+  else if (N <= CL_CTAS * 1024 * 8) k_select_evict_cl<8><<<CL_CTAS, 1024, 0, st>>>(p);
+  else if (N <= CL_MAX_N) k_select_evict_cl<16><<<CL_CTAS, 1024, 0, st>>>(p);
+  else k_select_evict<<<1, 1024, 0, st>>>(p);
   LAUNCH_CHECK(c);
   s->covered = N;
   s->map_ptr = r.slot_map;

@@ -1,0 +1,317 @@
+// select_cluster.cuh -- a1 / a6 / a7 as thread-block-cluster kernels (sm_100a): partition,
+// budgeted top-k (Eq. 1) and slot-map eviction with prefix-safe free (Eq. 7, PAPER.md:121-132,
+// 491-493).  One cluster of CL_CTAS CTAs x 1024 threads per request; every thread keeps MAXI consecutive positions in
+// registers (blocked layout, so order-preserving compaction is one block scan plus a rank offset exchanged through
+// distributed shared memory).  Requests longer than CL_CTAS * 1024 * 16 positions take the single-CTA kernels of
+// select.cuh / score.cuh.  Semantics are identical to k_select_evict / k_partition (R13-R15, R21, R22).
+#pragma once
+#include <cooperative_groups.h>
+#include "common.cuh"
+#include "select.cuh"
+
+namespace ikv {
+
+namespace cg = cooperative_groups;
+
+constexpr int CL_CTAS = 8;
+constexpr int CL_MAX_ITEMS = 16;
+constexpr int CL_MAX_N = CL_CTAS * 1024 * CL_MAX_ITEMS;
+
+// sum over the cluster of one int per CTA, and the exclusive prefix of this CTA's rank
+__device__ __forceinline__ void cluster_offsets(cg::cluster_group& cl, int* sh_val, int crank, int* before, int* total) {
+  int b = 0, t = 0;
+#pragma unroll
+  for (int rk = 0; rk < CL_CTAS; ++rk) {
+    const int v = *cl.map_shared_rank(sh_val, rk);
+    if (rk < crank) b += v;
+    t += v;
+  }
+  *before = b;
+  *total = t;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a1 partition: score fillers (R6), zeroed rule_out, candidates compacted in ascending position.
+// ---------------------------------------------------------------------------------------------------------------
+template <int MAXI>
+__global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_partition_cl(
+    const int32_t* __restrict__ S, int N, int32_t dead, int pi, int qs, int qe, float* __restrict__ scores,
+    float* __restrict__ rule_out, int32_t* __restrict__ cand_pos, int32_t* __restrict__ cand_slot,
+    int32_t* __restrict__ n_cand) {
+  cg::cluster_group cl = cg::this_cluster();
+  const int crank = (int)cl.block_rank();
+  __shared__ int warp_tot[32];
+  __shared__ int sh_tot;
+  const int tid = threadIdx.x;
+  const int base = (crank * 1024 + tid) * MAXI;
+  int slot[MAXI];
+  int cnt = 0;
+  uint32_t cmask = 0;
+  const bool vec = (MAXI % 4 == 0) && ((reinterpret_cast<uintptr_t>(S) & 15) == 0) && (base + MAXI <= N);
+  if (vec) {
+#pragma unroll
+    for (int i = 0; i < MAXI; i += 4) {
+      const int4 v = *reinterpret_cast<const int4*>(S + base + i);
+      slot[i] = v.x; slot[i + 1] = v.y; slot[i + 2] = v.z; slot[i + 3] = v.w;
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < MAXI; ++i) slot[i] = (base + i < N) ? S[base + i] : dead;
+  }
+#pragma unroll
+  for (int i = 0; i < MAXI; ++i) {
+    const int j = base + i;
+    if (j < N) {
+      const int cls = classify(slot[i], j, dead, pi, qs, qe);
+      if (cls == CLS_CAND) { cmask |= 1u << i; ++cnt; }
+      else scores[j] = (cls == CLS_FORCED) ? CUDART_INF_F : -CUDART_INF_F;
+      if (rule_out) rule_out[j] = 0.f;
+    }
+  }
+  int tot;
+  const int ex = block_excl_scan_1024(cnt, warp_tot, &tot);
+  if (tid == 0) sh_tot = tot;
+  cl.sync();
+  int before, total;
+  cluster_offsets(cl, &sh_tot, crank, &before, &total);
+  int o = before + ex;
+#pragma unroll
+  for (int i = 0; i < MAXI; ++i)
+    if ((cmask >> i) & 1u) {
+      cand_pos[o] = base + i;
+      cand_slot[o] = slot[i];
+      ++o;
+    }
+  if (crank == 0 && tid == 0) *n_cand = total;
+  cl.sync();  // keep sh_tot alive until every rank has read it
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// a6 + a7 select and evict.  Phases (cluster barriers between them):
+//   counts |F|, |A|  ->  4 x 8-bit radix-select passes (per-CTA histograms summed through DSMEM, every CTA resolves
+//   the digit redundantly)  ->  rank of threshold ties in position order  ->  keep flags, kept-slot bitmap and
+//   first-dropped-position table (global scratch)  ->  freed test (a)(b)(c)  ->  ordered writes  ->  scratch restore.
+// ---------------------------------------------------------------------------------------------------------------
+template <int MAXI>
+__global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select_evict_cl(SelParams p) {
+  cg::cluster_group cl = cg::this_cluster();
+  const int crank = (int)cl.block_rank();
+  __shared__ int hist[2][256];
+  __shared__ int comb[256];
+  __shared__ int warp_tot[32];
+  __shared__ int sh_cnt[2];   // |F|, |A| of this CTA
+  __shared__ int sh_eq;       // threshold ties of this CTA
+  __shared__ int sh_kf[2];    // kept, freed of this CTA
+  __shared__ uint32_t sh_prefix;
+  __shared__ int sh_remaining;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int N = p.N;
+  const int base = (crank * 1024 + tid) * MAXI;
+
+  int slot[MAXI];
+  uint32_t key[MAXI];
+  uint32_t cand_m = 0, forced_m = 0;  // bit i: item i is a candidate / forced
+  {
+    const bool vec = (MAXI % 4 == 0) && (base + MAXI <= N) &&
+                     (((reinterpret_cast<uintptr_t>(p.S) | reinterpret_cast<uintptr_t>(p.scores)) & 15) == 0);
+    float sc[MAXI];
+    if (vec) {
+#pragma unroll
+      for (int i = 0; i < MAXI; i += 4) {
+        const int4 v = *reinterpret_cast<const int4*>(p.S + base + i);
+        const float4 f = *reinterpret_cast<const float4*>(p.scores + base + i);
+        slot[i] = v.x; slot[i + 1] = v.y; slot[i + 2] = v.z; slot[i + 3] = v.w;
+        sc[i] = f.x; sc[i + 1] = f.y; sc[i + 2] = f.z; sc[i + 3] = f.w;
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < MAXI; ++i) {
+        const bool in = base + i < N;
+        slot[i] = in ? p.S[base + i] : p.dead;
+        sc[i] = in ? p.scores[base + i] : 0.f;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < MAXI; ++i) {
+      const int j = base + i;
+      key[i] = 0u;
+      if (j < N) {
+        const int cls = classify(slot[i], j, p.dead, p.pi, p.qs, p.qe);
+        if (cls == CLS_CAND) { cand_m |= 1u << i; key[i] = score_key(sc[i]); }
+        else if (cls == CLS_FORCED) forced_m |= 1u << i;
+      }
+    }
+  }
+
+  // ---- |F| and |A|
+  if (tid < 2) sh_cnt[tid] = 0;
+  if (tid < 256) { hist[0][tid] = 0; hist[1][tid] = 0; }
+  __syncthreads();
+  {
+    const int nf = warp_sum_i(__popc(forced_m)), nc = warp_sum_i(__popc(cand_m));
+    if (lane == 0) { atomicAdd(&sh_cnt[0], nf); atomicAdd(&sh_cnt[1], nc); }
+  }
+  cl.sync();
+  int nF = 0, nC = 0;
+#pragma unroll
+  for (int rk = 0; rk < CL_CTAS; ++rk) {
+    nF += *cl.map_shared_rank(&sh_cnt[0], rk);
+    nC += *cl.map_shared_rank(&sh_cnt[1], rk);
+  }
+  int cstar = (N <= p.C) ? nC : max(0, p.C - nF);  // R15, R14
+  cstar = min(cstar, nC);
+  const bool keep_all = (cstar == nC), keep_none = (cstar == 0);
+
+  // ---- radix select of the cstar-th largest key, MSB first
+  uint32_t thr = 0;
+  int need_eq = 0;
+  if (!keep_all && !keep_none) {
+    uint32_t prefix = 0u;
+    int remaining = cstar;
+    for (int pass = 3; pass >= 0; --pass) {
+      const int shift = pass * 8;
+      const uint32_t mask = (pass == 3) ? 0u : (0xffffffffu << (shift + 8));
+      int* h = hist[pass & 1];
+#pragma unroll
+      for (int i = 0; i < MAXI; ++i) {
+        const bool on = ((cand_m >> i) & 1u) && ((key[i] & mask) == prefix);
+        const uint32_t digit = (key[i] >> shift) & 255u;
+        const uint32_t act = __ballot_sync(0xffffffffu, on);
+        if (on) {
+          const uint32_t peers = __match_any_sync(act, digit);
+          if (lane == (__ffs(peers) - 1)) atomicAdd(&h[digit], __popc(peers));
+        }
+      }
+      cl.sync();
+      if (tid < 256) {
+        int v = 0;
+#pragma unroll
+        for (int rk = 0; rk < CL_CTAS; ++rk) v += *cl.map_shared_rank(&h[tid], rk);
+        comb[tid] = v;
+        hist[(pass & 1) ^ 1][tid] = 0;  // next pass's buffer: last read before the barrier above
+      }
+      __syncthreads();
+      if (tid < 32) {
+        // lane l covers digits 255 - 8 l .. 248 - 8 l (descending)
+        int s = 0;
+#pragma unroll
+        for (int e = 0; e < 8; ++e) s += comb[255 - (lane * 8 + e)];
+        int inc = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const int n = __shfl_up_sync(0xffffffffu, inc, o);
+          if (lane >= o) inc += n;
+        }
+        const int excl = inc - s;
+        const uint32_t hit = __ballot_sync(0xffffffffu, inc >= remaining);
+        const int src = hit ? (__ffs(hit) - 1) : 31;
+        if (lane == src) {
+          int cum = excl, d = 255 - lane * 8;
+          for (int e = 0; e < 7; ++e, --d) {
+            if (cum + comb[d] >= remaining) break;
+            cum += comb[d];
+          }
+          sh_remaining = remaining - cum;
+          sh_prefix = prefix | ((uint32_t)d << shift);
+        }
+      }
+      __syncthreads();
+      prefix = sh_prefix;
+      remaining = sh_remaining;
+      __syncthreads();
+    }
+    thr = prefix;
+    need_eq = remaining;  // ties at the threshold survive lowest positions first (R13)
+  }
+
+  // ---- ties in position order
+  uint32_t eq_m = 0;
+  if (!keep_all && !keep_none) {
+#pragma unroll
+    for (int i = 0; i < MAXI; ++i)
+      if (((cand_m >> i) & 1u) && key[i] == thr) eq_m |= 1u << i;
+  }
+  int eq_before = 0;
+  {
+    int tot;
+    const int ex = block_excl_scan_1024(__popc(eq_m), warp_tot, &tot);
+    if (tid == 0) sh_eq = tot;
+    cl.sync();
+    int before, total;
+    cluster_offsets(cl, &sh_eq, crank, &before, &total);
+    eq_before = before + ex;
+  }
+
+  // ---- keep flags, kept-slot bitmap, first dropped position per slot
+  uint32_t keep_m = forced_m, drop_m = 0;  // drop_m: live and not kept (newly dropped)
+  {
+    int e = eq_before;
+#pragma unroll
+    for (int i = 0; i < MAXI; ++i) {
+      if ((cand_m >> i) & 1u) {
+        bool keep = keep_all;
+        if (!keep_all && !keep_none) {
+          if (key[i] > thr) keep = true;
+          else if ((eq_m >> i) & 1u) { keep = e < need_eq; ++e; }
+        }
+        if (keep) keep_m |= 1u << i; else drop_m |= 1u << i;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < MAXI; ++i) {
+      const int j = base + i;
+      if ((keep_m >> i) & 1u) atomicOr(&p.kept_bits[slot[i] >> 5], 1u << (slot[i] & 31));
+      else if (((drop_m >> i) & 1u) && j >= p.radix) atomicMin(&p.firstpos[slot[i]], j);
+    }
+  }
+  __threadfence();
+  cl.sync();
+
+  // ---- freed test (PAPER.md:132 (a)(b)(c)), ordered compaction of survivors and freed slots
+  uint32_t freed_m = 0;
+#pragma unroll
+  for (int i = 0; i < MAXI; ++i) {
+    const int j = base + i;
+    if (((drop_m >> i) & 1u) && j >= p.radix) {
+      const uint32_t bits = __ldcg(&p.kept_bits[slot[i] >> 5]);
+      const int fp = __ldcg(&p.firstpos[slot[i]]);
+      if (!((bits >> (slot[i] & 31)) & 1u) && fp == j) freed_m |= 1u << i;
+    }
+  }
+  int live_o, freed_o, n_kept_all, n_freed_all;
+  {
+    int tot;
+    const int ex = block_excl_scan_1024(__popc(keep_m) | (__popc(freed_m) << 16), warp_tot, &tot);
+    if (tid == 0) { sh_kf[0] = tot & 0xffff; sh_kf[1] = tot >> 16; }
+    cl.sync();  // also: every rank has finished reading kept_bits / firstpos
+    int b0, b1;
+    cluster_offsets(cl, &sh_kf[0], crank, &b0, &n_kept_all);
+    cluster_offsets(cl, &sh_kf[1], crank, &b1, &n_freed_all);
+    live_o = b0 + (ex & 0xffff);
+    freed_o = b1 + (ex >> 16);
+  }
+#pragma unroll
+  for (int i = 0; i < MAXI; ++i) {
+    const int j = base + i;
+    if (j < N) {
+      const bool keep = (keep_m >> i) & 1u;
+      if (keep) {
+        p.live_slots[live_o++] = slot[i];
+        p.kept_bits[slot[i] >> 5] = 0u;  // restore the scratch invariant
+      } else if ((drop_m >> i) & 1u) {
+        p.S[j] = p.dead;
+        if (j >= p.radix) p.firstpos[slot[i]] = INT_MAX;
+        if ((freed_m >> i) & 1u) p.freed[freed_o++] = slot[i];
+      }
+      if (p.valid) p.valid[j] = keep ? 1 : 0;
+    }
+  }
+  if (crank == 0 && tid == 0) {
+    *p.n_kept = n_kept_all;
+    *p.n_freed = n_freed_all;
+    *p.n_live = n_kept_all;
+  }
+  cl.sync();  // shared memory stays mapped until every rank has read it
+}
+
+}  // namespace ikv

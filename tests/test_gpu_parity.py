@@ -229,6 +229,26 @@ def test_select_evict_edge_cases(ikv, oracle, case):
     _select_case(ikv, oracle, ctx, w, s, S, sc, budget, radix, seq_len)
 
 
+@pytest.mark.parametrize("n_tokens", [33000, 70001, 131072, 140003])
+def test_score_select_large_maps(ikv, oracle, n_tokens):
+    """Long slot maps: every register-blocking variant of the cluster kernels (4 / 8 / 16 positions per thread) and
+    the single-CTA kernels beyond 131,072 positions; ragged tails; heavy ties; dead positions."""
+    w = build("bf16_d64_g2", SHAPES[2][1], n_tokens=n_tokens, budget=8192)
+    ctx, s, M, kp, _ = run_memory(ikv, oracle, w)
+    rng = np.random.default_rng(n_tokens)
+    S = s.slot_map[:s.N].numpy().copy()
+    S[rng.choice(s.N, s.N // 5, replace=False)] = w.dead_slot
+    S_dev = torch.from_numpy(S.copy()).cuda()
+    scores = torch.empty(s.N, device="cuda")
+    req = gc.request(ikv, s, S_dev, budget=8192)
+    ctx.score([req], ikv.MODE_MEMORY, scores)
+    want = oracle.score(gc.oracle_geom(oracle, w), kp, M, S, s.pi, s.qs, s.qe)
+    gc.assert_scores_close(scores.cpu().numpy(), want, f"N={n_tokens}")
+    sc = np.round(rng.standard_normal(s.N) * 8).astype(np.float32) / 8      # ties across CTA boundaries
+    S[s.N - 3] = S[s.pi + 7]                                                # an alias far away in another CTA
+    _select_case(ikv, oracle, ctx, w, s, S, sc, 8192, radix=s.pi + 1000)
+
+
 def test_end_to_end_prune_kept_set(ikv, oracle):
     """GPU scores -> GPU select vs oracle scores -> oracle select: the kept sets may differ only at tokens whose
     oracle score lies within the score tolerance of the C*-th threshold (north_star)."""
