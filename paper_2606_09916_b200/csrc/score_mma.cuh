@@ -20,9 +20,10 @@
 
 namespace ikv {
 
-constexpr int KP_TOK = 16;       // tokens per stage = M of the mma
-constexpr int KP_CWARPS = 8;     // consumer warps
-constexpr int KP_THREADS = (KP_CWARPS + 1) * 32;
+constexpr int KP_TOK = 32;       // tokens per stage = two m16 tiles of the mma
+constexpr int KP_LWARPS = 4;     // logit warps
+constexpr int KP_KWARPS = 8;     // mean-key warps
+constexpr int KP_THREADS = (KP_LWARPS + KP_KWARPS + 1) * 32;
 constexpr int KP_ROWPAD = 64;    // bytes added to each staged token row (bank spread for the 16-byte reads)
 
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
@@ -90,10 +91,15 @@ struct KeyPassParams {
   int n_stage;
 };
 
+// Warp roles of k_key_pass (one persistent CTA per SM):
+//   warp 0..3   logit warps: warp w owns KV heads w, w+4, ...; both 16-token halves of the stage share the B fragments,
+//               which are prefetched one (layer, head) ahead so that their L2 latency never sits behind the stage wait.
+//   warp 4..11  mean-key warps (KBAR): warp (dq, th) owns the d-quarter dq of the token half th; every lane sums its
+//               16-byte chunks over all KV heads and layers in fp32 registers -- no cross-warp reduction.
+//   warp 12     producer.
 template <int D, int G, bool KBAR>
 __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams p) {
   constexpr int KS = D / 16, NI = D / 32, NT = (G <= 4) ? 1 : 2;
-  constexpr int RSTR = D + 4;  // row stride (floats) of the k_bar reduction buffer
   const int L = p.L, Hkv = p.Hkv, Hq = Hkv * G;
   const int row_bytes = Hkv * D * 2;
   const int row_stride = row_bytes + KP_ROWPAD;
@@ -101,11 +107,10 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
   const int NS = p.n_stage;
 
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  unsigned char* stage_base = smem_raw;                                     // [NS][16][row_stride]
+  unsigned char* stage_base = smem_raw;                                     // [NS][KP_TOK][row_stride]
   float2* stats = (float2*)(stage_base + (size_t)NS * stage_bytes);          // [L*Hq]
   uint64_t* full = (uint64_t*)(stats + (size_t)L * Hq);                      // [NS]
   uint64_t* empty = full + NS;                                               // [NS]
-  float* red = (float*)(empty + NS);                                         // [KP_CWARPS][16][RSTR] if KBAR
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int nc = *p.n_cand;
@@ -115,14 +120,15 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
 
   for (int i = threadIdx.x; i < L * Hq; i += KP_THREADS) stats[i] = make_float2(-CUDART_INF_F, 0.f);
   if (threadIdx.x == 0) {
-    for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], KP_CWARPS); }
+    for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], KP_LWARPS + (KBAR ? KP_KWARPS : 0)); }
     mbar_fence_init();
   }
   __syncthreads();
 
-  if (warp == KP_CWARPS) {
+  if (warp == KP_LWARPS + KP_KWARPS) {
     // ------------------------------------------------------------------ producer
-    int it = 0;
+    int s = 0;
+    uint32_t ph = 0;
     for (int tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
       const bool is_x = tile >= tiles_c;
       const int t0 = (is_x ? tile - tiles_c : tile) * KP_TOK;
@@ -130,9 +136,7 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
       int64_t slot = 0;
       if (lane < nvalid) slot = is_x ? p.xq_slot[t0 + lane] : p.cand_slot[t0 + lane];
       const bf16* src = p.k_pool + slot * (int64_t)(Hkv * D);
-      for (int l = 0; l < L; ++l, ++it) {
-        const int s = it % NS;
-        const uint32_t ph = (uint32_t)(it / NS) & 1u;
+      for (int l = 0; l < L; ++l) {
         if (lane == 0) {
           mbar_wait(&empty[s], ph ^ 1u);
           mbar_arrive_expect_tx(&full[s], (uint32_t)(nvalid * row_bytes));
@@ -141,101 +145,103 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
         if (lane < nvalid)
           bulk_g2s(stage_base + (size_t)s * stage_bytes + lane * row_stride, src + (int64_t)l * p.layer_stride,
                    (uint32_t)row_bytes, &full[s]);
+        if (++s == NS) { s = 0; ph ^= 1u; }
       }
     }
-  } else {
-    // ------------------------------------------------------------------ consumers
+  } else if (warp < KP_LWARPS) {
+    // ------------------------------------------------------------------ logit warps
     const int r = lane >> 2, q = lane & 3;
     const uint32_t stage_u32 = smem_u32(stage_base);
-    int it = 0;
+    const int nhw = (Hkv - warp + KP_LWARPS - 1) / KP_LWARPS;  // heads of this warp (may be 0)
+    uint4 bf[NT][KS / 2], bn[NT][KS / 2];
+    auto load_frags = [&](uint4 (&dst)[NT][KS / 2], int l, int kvh) {
+      const uint4* fp = p.frag + ((int64_t)(l * Hkv + kvh) * NT) * (KS / 2) * 32 + lane;
+#pragma unroll
+      for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+        for (int v = 0; v < KS / 2; ++v) dst[nt][v] = __ldg(fp + (nt * (KS / 2) + v) * 32);
+    };
+    if (nhw > 0) load_frags(bn, 0, warp);
+    int s = 0;
+    uint32_t ph = 0;
     for (int tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
       const bool is_x = tile >= tiles_c;
       const int t0 = (is_x ? tile - tiles_c : tile) * KP_TOK;
       const int nvalid = min(KP_TOK, (is_x ? nx : nc) - t0);
-      float kb[KBAR ? 2 : 1][KBAR ? NI : 1][8];
-      if (KBAR) {
-#pragma unroll
-        for (int a = 0; a < 2; ++a)
-#pragma unroll
-          for (int i = 0; i < NI; ++i)
-#pragma unroll
-            for (int e = 0; e < 8; ++e) kb[a][i][e] = 0.f;
-      }
-      for (int l = 0; l < L; ++l, ++it) {
-        const int s = it % NS;
-        const uint32_t ph = (uint32_t)(it / NS) & 1u;
+      for (int l = 0; l < L; ++l) {
         mbar_wait(&full[s], ph);
-        const uint32_t sb = stage_u32 + (uint32_t)(s * stage_bytes);
-        for (int kvh = warp; kvh < Hkv; kvh += KP_CWARPS) {
-          // B fragments of this (layer, head)
-          const uint4* fp = p.frag + ((int64_t)(l * Hkv + kvh) * NT) * (KS / 2) * 32 + lane;
-          uint4 bf[NT][KS / 2];
+        if (!is_x) {
+          const uint32_t sb = stage_u32 + (uint32_t)(s * stage_bytes);
+          for (int hi = 0; hi < nhw; ++hi) {
+            const int kvh = warp + hi * KP_LWARPS;
 #pragma unroll
-          for (int nt = 0; nt < NT; ++nt)
+            for (int nt = 0; nt < NT; ++nt)
 #pragma unroll
-            for (int v = 0; v < KS / 2; ++v) bf[nt][v] = __ldg(fp + (nt * (KS / 2) + v) * 32);
-          uint4 ka[NI], kc[NI];
-          const uint32_t a_lo = sb + (uint32_t)(r * row_stride + kvh * D * 2 + q * 16);
-          const uint32_t a_hi = a_lo + (uint32_t)(8 * row_stride);
-#pragma unroll
-          for (int i = 0; i < NI; ++i) {
-            ka[i] = lds128(a_lo + i * 64);
-            kc[i] = lds128(a_hi + i * 64);
-          }
-          float c[NT][4];
-#pragma unroll
-          for (int nt = 0; nt < NT; ++nt) { c[nt][0] = c[nt][1] = c[nt][2] = c[nt][3] = 0.f; }
-#pragma unroll
-          for (int i = 0; i < NI; ++i)
-#pragma unroll
-            for (int nt = 0; nt < NT; ++nt) {
-              mma_bf16_16816(c[nt], ka[i].x, kc[i].x, ka[i].y, kc[i].y, bf[nt][i].x, bf[nt][i].y);
-              mma_bf16_16816(c[nt], ka[i].z, kc[i].z, ka[i].w, kc[i].w, bf[nt][i].z, bf[nt][i].w);
+              for (int v = 0; v < KS / 2; ++v) bf[nt][v] = bn[nt][v];
+            {  // prefetch the fragments of the next (layer, head) of this warp; layers wrap to the next tile
+              int nh = hi + 1, nl = l;
+              if (nh == nhw) { nh = 0; nl = (l + 1 == L) ? 0 : l + 1; }
+              load_frags(bn, nl, warp + nh * KP_LWARPS);
             }
-          if (KBAR) {
+            float c[2][NT][4];
 #pragma unroll
-            for (int i = 0; i < NI; ++i) {
-              const uint32_t ua[4] = {ka[i].x, ka[i].y, ka[i].z, ka[i].w};
-              const uint32_t uc[4] = {kc[i].x, kc[i].y, kc[i].z, kc[i].w};
+            for (int mt = 0; mt < 2; ++mt) {
+              uint4 ka[NI], kc[NI];
+              const uint32_t a_lo = sb + (uint32_t)((mt * 16 + r) * row_stride + kvh * D * 2 + q * 16);
+              const uint32_t a_hi = a_lo + (uint32_t)(8 * row_stride);
 #pragma unroll
-              for (int e = 0; e < 4; ++e) {
-                kb[0][i][2 * e] += bf16lo(ua[e]);
-                kb[0][i][2 * e + 1] += bf16hi(ua[e]);
-                kb[1][i][2 * e] += bf16lo(uc[e]);
-                kb[1][i][2 * e + 1] += bf16hi(uc[e]);
+              for (int i = 0; i < NI; ++i) {
+                ka[i] = lds128(a_lo + i * 64);
+                kc[i] = lds128(a_hi + i * 64);
+              }
+#pragma unroll
+              for (int nt = 0; nt < NT; ++nt) { c[mt][nt][0] = c[mt][nt][1] = c[mt][nt][2] = c[mt][nt][3] = 0.f; }
+#pragma unroll
+              for (int i = 0; i < NI; ++i)
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                  mma_bf16_16816(c[mt][nt], ka[i].x, kc[i].x, ka[i].y, kc[i].y, bf[nt][i].x, bf[nt][i].y);
+                  mma_bf16_16816(c[mt][nt], ka[i].z, kc[i].z, ka[i].w, kc[i].w, bf[nt][i].z, bf[nt][i].w);
+                }
+            }
+            // logits of this thread: NH heads x 4 tokens (r, r+8, r+16, r+24)
+            constexpr int NH = (NT == 1) ? 1 : 2;
+            float x[NH][4];
+            int g0;
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) {
+              if (NT == 1) {
+                x[0][2 * mt] = c[mt][0][0] + c[mt][0][1];
+                x[0][2 * mt + 1] = c[mt][0][2] + c[mt][0][3];
+              } else {
+                x[0][2 * mt] = c[mt][0][0] + c[mt][NT - 1][0];
+                x[NH - 1][2 * mt] = c[mt][0][1] + c[mt][NT - 1][1];
+                x[0][2 * mt + 1] = c[mt][0][2] + c[mt][NT - 1][2];
+                x[NH - 1][2 * mt + 1] = c[mt][0][3] + c[mt][NT - 1][3];
               }
             }
-          }
-          if (!is_x) {
-            // logits of this thread: NH heads x 2 tokens (r, r+8)
-            constexpr int NH = (NT == 1) ? 1 : 2;
-            float x[NH][2];
-            int g0;
-            if (NT == 1) {
-              g0 = q;
-              x[0][0] = c[0][0] + c[0][1];
-              x[0][1] = c[0][2] + c[0][3];
-            } else {
-              g0 = 2 * q;
-              x[0][0] = c[0][0] + c[NT - 1][0];
-              x[NH - 1][0] = c[0][1] + c[NT - 1][1];
-              x[0][1] = c[0][2] + c[NT - 1][2];
-              x[NH - 1][1] = c[0][3] + c[NT - 1][3];
-            }
-            const bool v0 = r < nvalid, v1 = (r + 8) < nvalid;
+            g0 = (NT == 1) ? q : 2 * q;
+            bool tv[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) tv[e] = (r + 8 * e) < nvalid;
 #pragma unroll
             for (int hh = 0; hh < NH; ++hh) {
               const int g = g0 + hh;
               const bool gv = g < G;
               const int lh = l * Hq + kvh * G + (gv ? g : 0);
-              float* lrow = p.logits + (int64_t)lh * p.ldc + t0;
-              if (gv && v0) lrow[r] = x[hh][0];
-              if (gv && v1) lrow[r + 8] = x[hh][1];
-              float mx = fmaxf(v0 ? x[hh][0] : -CUDART_INF_F, v1 ? x[hh][1] : -CUDART_INF_F);
+              float* lrow = p.logits + (int64_t)lh * p.ldc + t0 + r;
+              float mx = -CUDART_INF_F;
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                if (gv && tv[e]) lrow[8 * e] = x[hh][e];
+                mx = fmaxf(mx, tv[e] ? x[hh][e] : -CUDART_INF_F);
+              }
               mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 4));
               mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 8));
               mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 16));
-              float se = (v0 ? __expf(x[hh][0] - mx) : 0.f) + (v1 ? __expf(x[hh][1] - mx) : 0.f);
+              float se = 0.f;
+#pragma unroll
+              for (int e = 0; e < 4; ++e) se += tv[e] ? __expf(x[hh][e] - mx) : 0.f;
               se += __shfl_xor_sync(0xffffffffu, se, 4);
               se += __shfl_xor_sync(0xffffffffu, se, 8);
               se += __shfl_xor_sync(0xffffffffu, se, 16);
@@ -249,31 +255,58 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[s]);
+        if (++s == NS) { s = 0; ph ^= 1u; }
       }
-      if (KBAR) {
-        // reduce the per-head-warp partial sums of this tile and write the mean key
-        const int nw = min(KP_CWARPS, Hkv);
-        if (warp < nw) {
-          float* dst = red + ((size_t)warp * KP_TOK) * RSTR;
+    }
+  } else if (KBAR) {
+    // ------------------------------------------------------------------ mean-key warps (Eq. 5)
+    constexpr int CH = D / 32;                 // 16-byte chunks per token in a d-quarter
+    constexpr int TPL = 32 / CH;               // tokens per warp load
+    constexpr int ROWS = KP_TOK / (KP_KWARPS / 4);
+    constexpr int NG = ROWS / TPL;             // token groups per warp
+    const int kw = warp - KP_LWARPS, dq = kw & 3, th = kw >> 2;
+    const int tl = lane / CH, ch = lane % CH;
+    const uint32_t stage_u32 = smem_u32(stage_base);
+    const uint32_t lane_off = (uint32_t)((th * ROWS + tl) * row_stride + dq * (D / 4) * 2 + ch * 16);
+    const float inv = 1.f / (float)(L * Hkv);
+    int s = 0;
+    uint32_t ph = 0;
+    for (int tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
+      const bool is_x = tile >= tiles_c;
+      const int t0 = (is_x ? tile - tiles_c : tile) * KP_TOK;
+      const int nvalid = min(KP_TOK, (is_x ? nx : nc) - t0);
+      float kb[NG][8];
 #pragma unroll
-          for (int a = 0; a < 2; ++a)
+      for (int gI = 0; gI < NG; ++gI)
 #pragma unroll
-            for (int i = 0; i < NI; ++i) {
-              float4* d4 = reinterpret_cast<float4*>(dst + (size_t)(r + 8 * a) * RSTR + 8 * (q + 4 * i));
-              d4[0] = make_float4(kb[a][i][0], kb[a][i][1], kb[a][i][2], kb[a][i][3]);
-              d4[1] = make_float4(kb[a][i][4], kb[a][i][5], kb[a][i][6], kb[a][i][7]);
-            }
+        for (int e = 0; e < 8; ++e) kb[gI][e] = 0.f;
+      for (int l = 0; l < L; ++l) {
+        mbar_wait(&full[s], ph);
+        const uint32_t sb = stage_u32 + (uint32_t)(s * stage_bytes) + lane_off;
+#pragma unroll 4
+        for (int kvh = 0; kvh < Hkv; ++kvh) {
+#pragma unroll
+          for (int gI = 0; gI < NG; ++gI) {
+            const uint4 u = lds128(sb + (uint32_t)(gI * TPL * row_stride + kvh * D * 2));
+            kb[gI][0] += bf16lo(u.x); kb[gI][1] += bf16hi(u.x);
+            kb[gI][2] += bf16lo(u.y); kb[gI][3] += bf16hi(u.y);
+            kb[gI][4] += bf16lo(u.z); kb[gI][5] += bf16hi(u.z);
+            kb[gI][6] += bf16lo(u.w); kb[gI][7] += bf16hi(u.w);
+          }
         }
-        bar_sync(1, KP_CWARPS * 32);
-        const float inv = 1.f / (float)(L * Hkv);
-        float* outp = is_x ? p.kq : p.kbar;
-        for (int o = threadIdx.x; o < nvalid * D; o += KP_CWARPS * 32) {
-          const int tok = o / D, d = o % D;
-          float acc = 0.f;
-          for (int w = 0; w < nw; ++w) acc += red[((size_t)w * KP_TOK + tok) * RSTR + d];
-          outp[(int64_t)(t0 + tok) * D + d] = acc * inv;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[s]);
+        if (++s == NS) { s = 0; ph ^= 1u; }
+      }
+      float* outp = is_x ? p.kq : p.kbar;
+#pragma unroll
+      for (int gI = 0; gI < NG; ++gI) {
+        const int tok = th * ROWS + gI * TPL + tl;
+        if (tok < nvalid) {
+          float4* d4 = reinterpret_cast<float4*>(outp + (int64_t)(t0 + tok) * D + dq * (D / 4) + ch * 8);
+          d4[0] = make_float4(kb[gI][0] * inv, kb[gI][1] * inv, kb[gI][2] * inv, kb[gI][3] * inv);
+          d4[1] = make_float4(kb[gI][4] * inv, kb[gI][5] * inv, kb[gI][6] * inv, kb[gI][7] * inv);
         }
-        bar_sync(1, KP_CWARPS * 32);
       }
     }
   }
@@ -283,8 +316,9 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
 
 // shared memory of k_key_pass; returns 0 if not even two stages fit
 inline size_t key_pass_smem(int L, int Hq, int Hkv, int D, bool kbar, int max_smem, int* n_stage) {
+  (void)kbar;
   const size_t stage = (size_t)KP_TOK * (Hkv * D * 2 + KP_ROWPAD);
-  const size_t fixed = (size_t)L * Hq * 8 + 2 * 8 * 8 + (kbar ? (size_t)KP_CWARPS * KP_TOK * (D + 4) * 4 : 0) + 128;
+  const size_t fixed = (size_t)L * Hq * 8 + 2 * 8 * 8 + 128;
   if (fixed + 2 * stage > (size_t)max_smem) { *n_stage = 0; return 0; }
   int ns = (int)(((size_t)max_smem - fixed) / stage);
   if (ns > 8) ns = 8;
