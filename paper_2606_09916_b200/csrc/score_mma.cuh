@@ -153,15 +153,23 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
     const int r = lane >> 2, q = lane & 3;
     const uint32_t stage_u32 = smem_u32(stage_base);
     const int nhw = (Hkv - warp + KP_LWARPS - 1) / KP_LWARPS;  // heads of this warp (may be 0)
-    uint4 bf[NT][KS / 2], bn[NT][KS / 2];
-    auto load_frags = [&](uint4 (&dst)[NT][KS / 2], int l, int kvh) {
-      const uint4* fp = p.frag + ((int64_t)(l * Hkv + kvh) * NT) * (KS / 2) * 32 + lane;
+    constexpr int HP = (NT == 1) ? 2 : 1;                      // heads per prefetch chunk
+    const int nchunk = (nhw + HP - 1) / HP;
+    uint4 bf[HP][NT][KS / 2], bn[HP][NT][KS / 2];
+    auto load_chunk = [&](uint4 (&dst)[HP][NT][KS / 2], int l, int ck) {
 #pragma unroll
-      for (int nt = 0; nt < NT; ++nt)
+      for (int h = 0; h < HP; ++h) {
+        const int hi = ck * HP + h;
+        if (hi < nhw) {
+          const uint4* fp = p.frag + ((int64_t)(l * Hkv + warp + hi * KP_LWARPS) * NT) * (KS / 2) * 32 + lane;
 #pragma unroll
-        for (int v = 0; v < KS / 2; ++v) dst[nt][v] = __ldg(fp + (nt * (KS / 2) + v) * 32);
+          for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+            for (int v = 0; v < KS / 2; ++v) dst[h][nt][v] = __ldg(fp + (nt * (KS / 2) + v) * 32);
+        }
+      }
     };
-    if (nhw > 0) load_frags(bn, 0, warp);
+    if (nhw > 0) load_chunk(bn, 0, 0);
     int s = 0;
     uint32_t ph = 0;
     for (int tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
@@ -172,17 +180,23 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
         mbar_wait(&full[s], ph);
         if (!is_x) {
           const uint32_t sb = stage_u32 + (uint32_t)(s * stage_bytes);
-          for (int hi = 0; hi < nhw; ++hi) {
-            const int kvh = warp + hi * KP_LWARPS;
+          for (int ck = 0; ck < nchunk; ++ck) {
 #pragma unroll
-            for (int nt = 0; nt < NT; ++nt)
+            for (int h = 0; h < HP; ++h)
 #pragma unroll
-              for (int v = 0; v < KS / 2; ++v) bf[nt][v] = bn[nt][v];
-            {  // prefetch the fragments of the next (layer, head) of this warp; layers wrap to the next tile
-              int nh = hi + 1, nl = l;
-              if (nh == nhw) { nh = 0; nl = (l + 1 == L) ? 0 : l + 1; }
-              load_frags(bn, nl, warp + nh * KP_LWARPS);
+              for (int nt = 0; nt < NT; ++nt)
+#pragma unroll
+                for (int v = 0; v < KS / 2; ++v) bf[h][nt][v] = bn[h][nt][v];
+            {  // prefetch the fragments of this warp's next chunk: one whole stage ahead when Hkv <= 8
+              int nk = ck + 1, nl = l;
+              if (nk == nchunk) { nk = 0; nl = (l + 1 == L) ? 0 : l + 1; }
+              load_chunk(bn, nl, nk);
             }
+#pragma unroll
+            for (int h = 0; h < HP; ++h) {
+            const int hi = ck * HP + h;
+            if (hi >= nhw) break;
+            const int kvh = warp + hi * KP_LWARPS;
             float c[2][NT][4];
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt) {
@@ -200,8 +214,8 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
               for (int i = 0; i < NI; ++i)
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) {
-                  mma_bf16_16816(c[mt][nt], ka[i].x, kc[i].x, ka[i].y, kc[i].y, bf[nt][i].x, bf[nt][i].y);
-                  mma_bf16_16816(c[mt][nt], ka[i].z, kc[i].z, ka[i].w, kc[i].w, bf[nt][i].z, bf[nt][i].w);
+                  mma_bf16_16816(c[mt][nt], ka[i].x, kc[i].x, ka[i].y, kc[i].y, bf[h][nt][i].x, bf[h][nt][i].y);
+                  mma_bf16_16816(c[mt][nt], ka[i].z, kc[i].z, ka[i].w, kc[i].w, bf[h][nt][i].z, bf[h][nt][i].w);
                 }
             }
             // logits of this thread: NH heads x 4 tokens (r, r+8, r+16, r+24)
@@ -250,6 +264,7 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
                 const float mn = fmaxf(st.x, mx);
                 stats[lh] = make_float2(mn, st.y * __expf(st.x - mn) + se * __expf(mx - mn));
               }
+            }
             }
           }
         }
