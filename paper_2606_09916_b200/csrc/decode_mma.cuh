@@ -226,60 +226,62 @@ inline size_t decode_mma_smem(int nh, int D, int max_smem, int* n_stage) {
   return fixed + (size_t)ns * stage;
 }
 
-// grid = (H_q, n_req), block = 256.  Warp w combines splits w, w+8, ...; lanes cover D in float4 (two splits per
-// step when D = 64); the 8 warp results are combined through shared memory.
+// grid = (H_q, n_req), block = DMG_THREADS.  Two phases with no serial dependency between splits:
+//   1. m* = max_s m_s; w_s = exp(m_s - m*) (0 for empty splits) into shared memory; den = sum_s w_s l_s
+//   2. thread (g, d) sums w_s o_s[d] over the splits s = g mod (threads / D) with independent loads; the groups
+//      are combined through shared memory.
+constexpr int DMG_THREADS = 512;
+constexpr int DMG_MAX_SPLIT = 1024;
 template <typename T, int D>
-__global__ __launch_bounds__(256) void k_decode_merge4(const float* __restrict__ part_o,
-                                                       const float2* __restrict__ part_ml, int n_split,
-                                                       T* __restrict__ out) {
-  constexpr int LPS = D / 4;       // lanes per split
-  constexpr int SPW = 32 / LPS;    // splits per warp step
-  __shared__ float4 s_o[8 * SPW][LPS];
-  __shared__ float2 s_ml[8 * SPW];
+__global__ __launch_bounds__(DMG_THREADS) void k_decode_merge4(const float* __restrict__ part_o,
+                                                               const float2* __restrict__ part_ml, int n_split,
+                                                               T* __restrict__ out) {
+  constexpr int NG = DMG_THREADS / D;
+  __shared__ float ws[DMG_MAX_SPLIT];
+  __shared__ float red[DMG_THREADS / 32];
+  __shared__ float acc_s[NG][D];
   pdl_launch_dependents();
   pdl_wait();
   const int64_t ph = ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * n_split;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int sub = lane / LPS, dl = lane % LPS;
-  float m = -CUDART_INF_F, l = 0.f;
-  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll 4
-  for (int s = warp * SPW + sub; s < n_split; s += 8 * SPW) {
-    const float2 ml = part_ml[ph + s];
-    const float4 v = *reinterpret_cast<const float4*>(part_o + (ph + s) * D + dl * 4);
-    if (ml.y > 0.f) {
-      const float mn = fmaxf(m, ml.x);
-      const float c0 = __expf(m - mn), c1 = __expf(ml.x - mn);
-      acc.x = acc.x * c0 + v.x * c1; acc.y = acc.y * c0 + v.y * c1;
-      acc.z = acc.z * c0 + v.z * c1; acc.w = acc.w * c0 + v.w * c1;
-      l = l * c0 + ml.y * c1;
-      m = mn;
-    }
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  float2 ml[DMG_MAX_SPLIT / DMG_THREADS];
+  float mx = -CUDART_INF_F;
+#pragma unroll
+  for (int i = 0; i < DMG_MAX_SPLIT / DMG_THREADS; ++i) {
+    const int sp = tid + i * DMG_THREADS;
+    ml[i] = (sp < n_split) ? part_ml[ph + sp] : make_float2(-CUDART_INF_F, 0.f);
+    if (ml[i].y > 0.f) mx = fmaxf(mx, ml[i].x);
   }
-  s_o[warp * SPW + sub][dl] = acc;
-  if (dl == 0) s_ml[warp * SPW + sub] = make_float2(m, l);
+  mx = warp_max(mx);
+  if (lane == 0) red[warp] = mx;
   __syncthreads();
-  if (threadIdx.x < LPS) {
-    float mx = -CUDART_INF_F;
+  mx = warp_max(lane < DMG_THREADS / 32 ? red[lane] : -CUDART_INF_F);
+  __syncthreads();
+  float den = 0.f;
 #pragma unroll
-    for (int i = 0; i < 8 * SPW; ++i) mx = fmaxf(mx, s_ml[i].x);
-    float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
-    float den = 0.f;
-    if (mx > -CUDART_INF_F) {
+  for (int i = 0; i < DMG_MAX_SPLIT / DMG_THREADS; ++i) {
+    const int sp = tid + i * DMG_THREADS;
+    const float w = (ml[i].y > 0.f) ? __expf(ml[i].x - mx) : 0.f;
+    if (sp < n_split) ws[sp] = w;
+    den = fmaf(w, ml[i].y, den);
+  }
+  den = warp_sum(den);
+  if (lane == 0) red[warp] = den;
+  __syncthreads();
+  den = warp_sum(lane < DMG_THREADS / 32 ? red[lane] : 0.f);
+  const int g = tid / D, d = tid % D;
+  float acc = 0.f;
+  const float* po = part_o + ph * D + d;
+#pragma unroll 8
+  for (int sp = g; sp < n_split; sp += NG) acc = fmaf(ws[sp], po[(int64_t)sp * D], acc);
+  acc_s[g][d] = acc;
+  __syncthreads();
+  if (tid < D) {
+    float a = 0.f;
 #pragma unroll
-      for (int i = 0; i < 8 * SPW; ++i) {
-        const float2 ml = s_ml[i];
-        if (ml.y > 0.f) {
-          const float w = __expf(ml.x - mx);
-          const float4 v = s_o[i][threadIdx.x];
-          a.x += w * v.x; a.y += w * v.y; a.z += w * v.z; a.w += w * v.w;
-          den += w * ml.y;
-        }
-      }
-    }
+    for (int i = 0; i < NG; ++i) a += acc_s[i][tid];
     const float inv = (den > 0.f) ? 1.f / den : 0.f;
-    T* op = out + ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * D + threadIdx.x * 4;
-    op[0] = (T)(a.x * inv); op[1] = (T)(a.y * inv); op[2] = (T)(a.z * inv); op[3] = (T)(a.w * inv);
+    out[((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * D + tid] = (T)(a * inv);
   }
 }
 

@@ -390,7 +390,7 @@ ikv_status launch_decode(ikv_ctx* c, int layer, const DecBatch& batch, int n_req
                                                      c->part_o, c->part_ml, n_split);
     LAUNCH_CHECK(c);
   }
-  CU(c, launch_pdl(k_decode_merge4<T, D>, dim3(Hq, n_req), dim3(256), 0, st, c->use_pdl, (const float*)c->part_o,
+  CU(c, launch_pdl(k_decode_merge4<T, D>, dim3(Hq, n_req), dim3(DMG_THREADS), 0, st, c->use_pdl, (const float*)c->part_o,
                    (const float2*)c->part_ml, n_split, (T*)out));
   return IKV_OK;
 }
@@ -925,6 +925,7 @@ ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, i
       if (n_split > by_len) n_split = by_len;
     }
     if (n_split < 1) n_split = 1;
+    if (n_split > DMG_MAX_SPLIT) n_split = DMG_MAX_SPLIT;
     TRY(ensure_parts(c, (int64_t)nb * Hq * n_split));
     TRY(dispatch_decode(c, layer, batch, nb, n_split, (const char*)q + (size_t)r0 * Hq * D * esz,
                         (char*)out + (size_t)r0 * Hq * D * esz, sm_scale, st));

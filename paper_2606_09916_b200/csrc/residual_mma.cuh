@@ -160,8 +160,9 @@ __global__ __launch_bounds__(128) void k_resid_kv_frags(const float* __restrict_
   const float bk = w.bk[o], bv = w.bv[o];
 #pragma unroll
   for (int i = 0; i < 16; ++i) { ak[i] = bk; av[i] = bv; }
+#pragma unroll 8
   for (int d = 0; d < D; ++d) {
-    const float wk = w.wk_t[d * R_DC + o], wv = w.wv_t[d * R_DC + o];
+    const float wk = __ldg(w.wk_t + d * R_DC + o), wv = __ldg(w.wv_t + d * R_DC + o);
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
       ak[i] = fmaf(wk, x[i][d], ak[i]);
