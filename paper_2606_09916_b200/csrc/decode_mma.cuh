@@ -83,10 +83,13 @@ __global__ __launch_bounds__(DM_THREADS, 1) void k_decode_mma(const DecMmaParams
   __syncthreads();
   pdl_launch_dependents();
 
-  // The slot lists are written only by kernels that never trigger their dependents early, so they are complete
-  // here; q and the partial buffers are touched after pdl_wait() only.
+  // Programmatic dependent launch: this grid may start while the previous decode call (its split and merge grids,
+  // the only kernels of the library that trigger their dependents early) is still running.  Everything READ here --
+  // slot lists, K/V pools, q -- was produced by kernels that never trigger early, so it is complete at this point;
+  // everything WRITTEN here (the partial buffers, which the previous merge may still be reading) is written only
+  // after pdl_wait(), which the consumers execute just before their stores.
   const DecReq rq = batch.r[req];
-  const int n_cached = *rq.n_live;
+  const int n_cached = rq.n_items;  // the list is padded with the dead slot up to n_items: no device-side length read
   const int total = n_cached + (rq.seq_len - rq.covered);
   const int n_gran = (total + DM_GRAN - 1) / DM_GRAN;
   const int begin = (int)(((int64_t)n_gran * split) / p.n_split) * DM_GRAN;
@@ -95,14 +98,23 @@ __global__ __launch_bounds__(DM_THREADS, 1) void k_decode_mma(const DecMmaParams
 
   if (warp == DM_CWARPS) {
     // ------------------------------------------------------------------ producer
+    // slots of 32 tokens (two tiles) per load, fetched two tiles ahead of their bulk copies
+    auto slot_of = [&](int i) -> int {
+      if (i >= end) return p.dead;
+      return (i < n_cached) ? __ldg(rq.live_slots + i) : __ldg(rq.S + rq.covered + (i - n_cached));
+    };
+    int cur = slot_of(begin + lane), nxt = slot_of(begin + 32 + lane);
     for (int t = 0; t < n_tiles; ++t) {
       const int s = t % NS;
       const uint32_t ph = (uint32_t)(t / NS) & 1u;
+      if (t > 0 && (t & 1) == 0) {
+        cur = nxt;
+        nxt = slot_of(begin + (t + 2) * DM_TOK + lane);
+      }
       const int i = begin + t * DM_TOK + lane;
-      int slot = p.dead;
-      if (lane < DM_TOK && i < end) slot = (i < n_cached) ? rq.live_slots[i] : rq.S[rq.covered + (i - n_cached)];
+      const int slot = __shfl_sync(0xffffffffu, cur, (t & 1) * DM_TOK + (lane & (DM_TOK - 1)));
       const bool in_range = lane < DM_TOK && i < end;
-      const bool copy = in_range || (lane < DM_TOK && t < NS);  // first use of a stage: pad with the (finite) dead row
+      const bool copy = in_range;  // rows past the end are never copied; the consumers zero their V slices
       const uint32_t vmask = __ballot_sync(0xffffffffu, in_range && slot != p.dead);
       const uint32_t cmask = __ballot_sync(0xffffffffu, copy);
       unsigned char* sb = stage_base + (size_t)s * stage_bytes;
@@ -123,7 +135,6 @@ __global__ __launch_bounds__(DM_THREADS, 1) void k_decode_mma(const DecMmaParams
     const int r = lane >> 2, q4 = lane & 3;
     const int kvh = h0 + warp;
     const bool active = warp < nh;
-    pdl_wait();
     // A fragments of q (rows g = r < G; rows >= G are zero)
     uint32_t qa[KS][2];
 #pragma unroll
@@ -154,6 +165,16 @@ __global__ __launch_bounds__(DM_THREADS, 1) void k_decode_mma(const DecMmaParams
       if (active) {
         const uint32_t sb = stage_u32 + (uint32_t)(s * stage_bytes);
         const uint32_t vmask = *reinterpret_cast<const uint32_t*>(stage_base + (size_t)s * stage_bytes + 2 * kv_bytes);
+        if (vmask != 0xffffu) {
+          // ragged tile: V rows of masked tokens may hold stale or uninitialised bytes (0 x NaN = NaN): zero this
+          // head's slice of them (D * 2 bytes = D / 8 lanes x 16 bytes per row, two rows per pass when D = 128)
+          constexpr int LPRV = D / 8;
+          for (int tok = lane / LPRV; tok < DM_TOK; tok += 32 / LPRV)
+            if (!((vmask >> tok) & 1u))
+              *reinterpret_cast<uint4*>(stage_base + (size_t)s * stage_bytes + kv_bytes + (size_t)tok * row_stride +
+                                        warp * D * 2 + (lane % LPRV) * 16) = make_uint4(0u, 0u, 0u, 0u);
+          __syncwarp();
+        }
         // S^T tiles: [g][tokens 0-7], [g][tokens 8-15]
         float sacc[2][4];
 #pragma unroll
@@ -202,6 +223,7 @@ __global__ __launch_bounds__(DM_THREADS, 1) void k_decode_mma(const DecMmaParams
       __syncwarp();
       if (lane == 0) mbar_arrive(&empty[s]);
     }
+    pdl_wait();
     if (active) {
       lsum += __shfl_xor_sync(0xffffffffu, lsum, 1);
       lsum += __shfl_xor_sync(0xffffffffu, lsum, 2);

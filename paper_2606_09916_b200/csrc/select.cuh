@@ -171,6 +171,7 @@ __global__ __launch_bounds__(1024) void k_select_evict(SelParams p) {
       if (ds >= 0) p.firstpos[ds] = INT_MAX;
     }
   }
+  for (int i = live_base + tid; i < N; i += 1024) p.live_slots[i] = p.dead;  // padded for decode (host-side bound)
   if (tid == 0) {
     *p.n_kept = live_base;
     *p.n_freed = freed_base;
@@ -191,6 +192,7 @@ __global__ __launch_bounds__(1024) void k_build_live(const int32_t* __restrict__
     if (slot != dead) live_slots[base + ex] = slot;
     base += tot;
   }
+  for (int i = base + threadIdx.x; i < N; i += 1024) live_slots[i] = dead;  // padded for decode (host-side bound)
   if (threadIdx.x == 0) *n_live = base;
 }
 

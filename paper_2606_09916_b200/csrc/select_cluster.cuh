@@ -306,6 +306,8 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select
       if (p.valid) p.valid[j] = keep ? 1 : 0;
     }
   }
+  // pad the survivor list with the dead slot up to N: decode sizes its splits from a host-side bound
+  for (int i = n_kept_all + crank * 1024 + tid; i < N; i += CL_CTAS * 1024) p.live_slots[i] = p.dead;
   if (crank == 0 && tid == 0) {
     *p.n_kept = n_kept_all;
     *p.n_freed = n_freed_all;
