@@ -94,6 +94,7 @@ struct ikv_ctx {
 
   // residual head (transposed on the device)
   bool has_resid = false;
+  bool resid_attr_done = false;
   float* resid_blob = nullptr;
   ResidW rw{};
 };
@@ -538,9 +539,14 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     rp.bq_eff = c->bq_eff; rp.b1_eff = c->b1_eff; rp.nks = (int)(c->xq_cap / 16);
     rp.use_xattn = (use_x && n_x > 0) ? 1 : 0;
     rp.scores = scores;
-    const int nblk = (N + R_WARPS * 16 - 1) / (R_WARPS * 16);
-    if (D == 128) k_residual_mma<128><<<nblk, R_WARPS * 32, 0, st>>>(rp, c->rw);
-    else k_residual_mma<64><<<nblk, R_WARPS * 32, 0, st>>>(rp, c->rw);
+    const int nblk = (N + R_CWARPS * 16 - 1) / (R_CWARPS * 16);
+    if (!c->resid_attr_done) {
+      CU(c, cudaFuncSetAttribute(k_residual_mma<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, RS_SMEM));
+      CU(c, cudaFuncSetAttribute(k_residual_mma<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, RS_SMEM));
+      c->resid_attr_done = true;
+    }
+    if (D == 128) k_residual_mma<128><<<nblk, R_THREADS, RS_SMEM, st>>>(rp, c->rw);
+    else k_residual_mma<64><<<nblk, R_THREADS, RS_SMEM, st>>>(rp, c->rw);
     LAUNCH_CHECK(c);
   }
   return IKV_OK;

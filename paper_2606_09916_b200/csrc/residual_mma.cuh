@@ -212,17 +212,86 @@ __device__ __forceinline__ float ex2f(float x) {
   return y;
 }
 
+// ---- k_residual_mma: CTA = R_CWARPS consumer warps (one 16-candidate tile each) + 1 producer warp.
+// All B fragments are laid out in global memory in the order they are consumed, so the producer streams them as bulk
+// copies (TMA unit) through a ring of RS_BYTES stages and every consumer warp reads them with conflict-free 16-byte
+// shared loads: no fragment load waits on L2 and no fragment is fetched more than once per CTA.
+// Stage sequence (identical in producer and consumers):
+//   nq > 0:  KS stages  W_Q' k-step s (16 n-tiles)
+//            per head, per chunk of 64 query keys: 1 stage Kc (2 k-steps x ntn tiles), 1 stage Vc (nv steps x 4 tiles)
+//   4 x [ KS/2 stages fc1' kbar columns (2 k-steps x 8 tiles), nq > 0: 4 stages fc1 c columns (2 k-steps x 8 tiles) ]
+constexpr int R_CWARPS = 7;
+constexpr int R_THREADS = (R_CWARPS + 1) * 32;
+constexpr int RS_BYTES = 8192;
+constexpr int RS_STAGES = 8;
+constexpr int RS_SMEM = RS_STAGES * RS_BYTES + 2 * 8 * RS_STAGES;
+
 template <int D>
-__global__ __launch_bounds__(R_WARPS * 32) void k_residual_mma(const ResidMmaParams p, const ResidW w) {
+__global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaParams p, const ResidW w) {
   constexpr int KS = D / 16;
+  extern __shared__ __align__(128) unsigned char ring[];  // [RS_STAGES][RS_BYTES], then the barriers
+  uint64_t* full = reinterpret_cast<uint64_t*>(ring + RS_STAGES * RS_BYTES);
+  uint64_t* empty = full + RS_STAGES;
   const int nc = *p.n_cand;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, r = lane >> 2, q = lane & 3;
-  const int t0 = (blockIdx.x * R_WARPS + warp) * 16;
-  if (t0 >= nc) return;
+  if (blockIdx.x * R_CWARPS * 16 >= nc) return;
+  const int nq = p.use_xattn ? *p.n_xq : 0;
+  const int nkt = 2 * p.nks;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < RS_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], R_CWARPS); }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  if (warp == R_CWARPS) {
+    // ------------------------------------------------------------------ producer
+    if (lane == 0) {
+      int s = 0;
+      uint32_t ph = 0;
+      auto push = [&](const uint4* src0, uint32_t bytes0, const uint4* src1, uint32_t bytes1) {
+        mbar_wait(&empty[s], ph ^ 1u);
+        mbar_arrive_expect_tx(&full[s], bytes0 + bytes1);
+        bulk_g2s(ring + s * RS_BYTES, src0, bytes0, &full[s]);
+        if (bytes1) bulk_g2s(ring + s * RS_BYTES + bytes0, src1, bytes1, &full[s]);
+        if (++s == RS_STAGES) { s = 0; ph ^= 1u; }
+      };
+      if (nq > 0) {
+        for (int ks = 0; ks < KS; ++ks) push(p.wq_frag + ks * 16 * 32, 16 * 512, nullptr, 0);
+        for (int hc = 0; hc < R_HC; ++hc)
+          for (int kc0 = 0; kc0 < nq; kc0 += 64) {
+            const int ntn = min(8, (nq - kc0 + 7) >> 3), nv = (ntn + 1) >> 1;
+            push(p.kc_frag + ((int64_t)(hc * 2) * nkt + (kc0 >> 3)) * 32, ntn * 512,
+                 p.kc_frag + ((int64_t)(hc * 2 + 1) * nkt + (kc0 >> 3)) * 32, ntn * 512);
+            push(p.vc_frag + ((int64_t)(hc * p.nks + (kc0 >> 4)) * 4) * 32, nv * 4 * 512, nullptr, 0);
+          }
+      }
+      for (int ch = 0; ch < 4; ++ch) {
+        for (int ks = 0; ks < KS; ks += 2) push(p.w1k_frag + ((ch * KS + ks) * 8) * 32, 16 * 512, nullptr, 0);
+        if (nq > 0)
+          for (int ks = 0; ks < 8; ks += 2) push(w.w1c_frag + ((ch * 8 + ks) * 8) * 32, 16 * 512, nullptr, 0);
+      }
+    }
+    return;
+  }
+
+  // -------------------------------------------------------------------- consumers
+  const int t0 = (blockIdx.x * R_CWARPS + warp) * 16;
+  const bool live = t0 < nc;  // warps past the end still walk the ring
   const int row0 = min(t0 + r, nc - 1), row1 = min(t0 + r + 8, nc - 1);
   const float rule0 = p.rule_c[row0], rule1 = p.rule_c[row1];
-  const int nq = p.use_xattn ? *p.n_xq : 0;
   const int P = 3 * D + 1, IN = P + R_DC;
+  const uint32_t ring_u32 = smem_u32(ring) + lane * 16;
+  int rs = 0;
+  uint32_t rph = 0;
+  auto stage_wait = [&]() -> uint32_t {
+    mbar_wait(&full[rs], rph);
+    return ring_u32 + rs * RS_BYTES;
+  };
+  auto stage_done = [&]() {
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty[rs]);
+    if (++rs == RS_STAGES) { rs = 0; rph ^= 1u; }
+  };
 
   // A fragments of kbar (hi | lo); k order per kperm()
   uint32_t akh[KS][4], akl[KS][4];
@@ -236,7 +305,7 @@ __global__ __launch_bounds__(R_WARPS * 32) void k_residual_mma(const ResidMmaPar
     split_bf16(x1.z, x1.w, akh[s][3], akl[s][3]);
   }
 
-  // A fragments of c (Eq. 6), 8 k-steps; zero when there is no live query key (R7)
+  // A fragments of c (Eq. 6), 8 k-steps; unused when there is no live query key (R7)
   uint32_t ach[8][4], acl[8][4];
   if (nq > 0) {
     // ---- Q = Wq' kbar + rule wq_r + bq'
@@ -244,9 +313,12 @@ __global__ __launch_bounds__(R_WARPS * 32) void k_residual_mma(const ResidMmaPar
 #pragma unroll
     for (int t = 0; t < 16; ++t) { accq[t][0] = accq[t][1] = accq[t][2] = accq[t][3] = 0.f; }
 #pragma unroll
-    for (int s = 0; s < KS; ++s)
+    for (int s = 0; s < KS; ++s) {
+      const uint32_t sb = stage_wait();
 #pragma unroll
-      for (int t = 0; t < 16; ++t) mma3(accq[t], akh[s], akl[s], __ldg(p.wq_frag + (s * 16 + t) * 32 + lane));
+      for (int t = 0; t < 16; ++t) mma3(accq[t], akh[s], akl[s], lds128(sb + t * 512));
+      stage_done();
+    }
 #pragma unroll
     for (int t = 0; t < 16; ++t) {
       const int n = t * 8 + 2 * q;
@@ -255,7 +327,6 @@ __global__ __launch_bounds__(R_WARPS * 32) void k_residual_mma(const ResidMmaPar
       accq[t][0] += fmaf(rule0, wr0, b.x); accq[t][1] += fmaf(rule0, wr1, b.y);
       accq[t][2] += fmaf(rule1, wr0, b.x); accq[t][3] += fmaf(rule1, wr1, b.y);
     }
-    const int nkt = 2 * p.nks;
     // ---- 4-head cross attention, online softmax in the exp2 domain over chunks of 64 query keys
 #pragma unroll
     for (int hc = 0; hc < R_HC; ++hc) {
@@ -275,19 +346,22 @@ __global__ __launch_bounds__(R_WARPS * 32) void k_residual_mma(const ResidMmaPar
       for (int kc0 = 0; kc0 < nq; kc0 += 64) {
         const int ntn = min(8, (nq - kc0 + 7) >> 3);
         float sc[8][4];
+        {
+          const uint32_t sb = stage_wait();  // [u][ntn tiles]
 #pragma unroll
-        for (int t = 0; t < 8; ++t) {
-          sc[t][0] = sc[t][1] = sc[t][2] = sc[t][3] = 0.f;
-          if (t < ntn) {
+          for (int t = 0; t < 8; ++t) {
+            sc[t][0] = sc[t][1] = sc[t][2] = sc[t][3] = 0.f;
+            if (t < ntn) {
 #pragma unroll
-            for (int u = 0; u < 2; ++u)
-              mma3(sc[t], qh[u], ql[u], __ldg(p.kc_frag + ((int64_t)(hc * 2 + u) * nkt + (kc0 >> 3) + t) * 32 + lane));
+              for (int u = 0; u < 2; ++u) mma3(sc[t], qh[u], ql[u], lds128(sb + (u * ntn + t) * 512));
+            }
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+              const bool ok = t < ntn && (kc0 + t * 8 + 2 * q + e) < nq;
+              if (!ok) { sc[t][e] = -CUDART_INF_F; sc[t][2 + e] = -CUDART_INF_F; }
+            }
           }
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            const bool ok = t < ntn && (kc0 + t * 8 + 2 * q + e) < nq;
-            if (!ok) { sc[t][e] = -CUDART_INF_F; sc[t][2 + e] = -CUDART_INF_F; }
-          }
+          stage_done();
         }
         float x0 = -CUDART_INF_F, x1 = -CUDART_INF_F;
 #pragma unroll
@@ -310,18 +384,21 @@ __global__ __launch_bounds__(R_WARPS * 32) void k_residual_mma(const ResidMmaPar
           l0 += sc[t][0] + sc[t][1];
           l1 += sc[t][2] + sc[t][3];
         }
+        {
+          const uint32_t sb = stage_wait();  // [nv key steps][4 tiles]
 #pragma unroll
-        for (int v = 0; v < 4; ++v) {
-          if (2 * v < ntn) {
-            uint32_t ph[4], pl[4];
-            split_bf16(sc[2 * v][0], sc[2 * v][1], ph[0], pl[0]);
-            split_bf16(sc[2 * v][2], sc[2 * v][3], ph[1], pl[1]);
-            split_bf16(sc[2 * v + 1][0], sc[2 * v + 1][1], ph[2], pl[2]);
-            split_bf16(sc[2 * v + 1][2], sc[2 * v + 1][3], ph[3], pl[3]);
+          for (int v = 0; v < 4; ++v) {
+            if (2 * v < ntn) {
+              uint32_t ph[4], pl[4];
+              split_bf16(sc[2 * v][0], sc[2 * v][1], ph[0], pl[0]);
+              split_bf16(sc[2 * v][2], sc[2 * v][3], ph[1], pl[1]);
+              split_bf16(sc[2 * v + 1][0], sc[2 * v + 1][1], ph[2], pl[2]);
+              split_bf16(sc[2 * v + 1][2], sc[2 * v + 1][3], ph[3], pl[3]);
 #pragma unroll
-            for (int nt = 0; nt < 4; ++nt)
-              mma3(o[nt], ph, pl, __ldg(p.vc_frag + ((int64_t)(hc * p.nks + (kc0 >> 4) + v) * 4 + nt) * 32 + lane));
+              for (int nt = 0; nt < 4; ++nt) mma3(o[nt], ph, pl, lds128(sb + (v * 4 + nt) * 512));
+            }
           }
+          stage_done();
         }
       }
       l0 += __shfl_xor_sync(0xffffffffu, l0, 1); l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
@@ -346,14 +423,24 @@ __global__ __launch_bounds__(R_WARPS * 32) void k_residual_mma(const ResidMmaPar
 #pragma unroll
     for (int t = 0; t < 8; ++t) { acc[t][0] = acc[t][1] = acc[t][2] = acc[t][3] = 0.f; }
 #pragma unroll
-    for (int s = 0; s < KS; ++s)
+    for (int s = 0; s < KS; s += 2) {
+      const uint32_t sb = stage_wait();
 #pragma unroll
-      for (int t = 0; t < 8; ++t) mma3(acc[t], akh[s], akl[s], __ldg(p.w1k_frag + ((ch * KS + s) * 8 + t) * 32 + lane));
+      for (int t = 0; t < 8; ++t) mma3(acc[t], akh[s], akl[s], lds128(sb + t * 512));
+#pragma unroll
+      for (int t = 0; t < 8; ++t) mma3(acc[t], akh[s + 1], akl[s + 1], lds128(sb + (8 + t) * 512));
+      stage_done();
+    }
     if (nq > 0) {
 #pragma unroll
-      for (int s = 0; s < 8; ++s)
+      for (int s = 0; s < 8; s += 2) {
+        const uint32_t sb = stage_wait();
 #pragma unroll
-        for (int t = 0; t < 8; ++t) mma3(acc[t], ach[s], acl[s], __ldg(w.w1c_frag + ((ch * 8 + s) * 8 + t) * 32 + lane));
+        for (int t = 0; t < 8; ++t) mma3(acc[t], ach[s], acl[s], lds128(sb + t * 512));
+#pragma unroll
+        for (int t = 0; t < 8; ++t) mma3(acc[t], ach[s + 1], acl[s + 1], lds128(sb + (8 + t) * 512));
+        stage_done();
+      }
     }
 #pragma unroll
     for (int t = 0; t < 8; ++t) {
@@ -369,7 +456,7 @@ __global__ __launch_bounds__(R_WARPS * 32) void k_residual_mma(const ResidMmaPar
   }
   z0 += __shfl_xor_sync(0xffffffffu, z0, 1); z0 += __shfl_xor_sync(0xffffffffu, z0, 2);
   z1 += __shfl_xor_sync(0xffffffffu, z1, 1); z1 += __shfl_xor_sync(0xffffffffu, z1, 2);
-  if (q == 0) {
+  if (q == 0 && live) {
     const float b2 = w.fc2_b[0];
     if (t0 + r < nc) p.scores[p.cand_pos[t0 + r]] = rule0 + w.alpha * (z0 + b2);
     if (t0 + r + 8 < nc) p.scores[p.cand_pos[t0 + r + 8]] = rule1 + w.alpha * (z1 + b2);
