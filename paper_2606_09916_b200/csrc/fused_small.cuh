@@ -1,0 +1,46 @@
+// fused_small.cuh -- the small per-call kernels around the key pass, fused into two launches (each launch costs
+// ~1.2 us of stream latency on B200, and several of these bodies are latency-bound on their own):
+//   k_mem_prep : B fragments of M / sqrt(D) for the key pass  |  partial sums of mbar (Eq. 5)
+//   k_post_key : lse[l,h] from the per-CTA partials (Eq. 3)   |  folded W_Q / fc1 operands  |  Kc / Vc fragments (Eq. 6)
+// Blocks of 128 threads; the block index selects the body.
+#pragma once
+#include "residual_mma.cuh"
+#include "score.cuh"
+#include "score_mma.cuh"
+
+namespace ikv {
+
+template <int D, int G>
+__global__ __launch_bounds__(128) void k_mem_prep(const float* __restrict__ M, int L, int Hkv, float inv_sqrt_d,
+                                                  uint4* __restrict__ frag, int n_frag_blocks, int LH,
+                                                  float* __restrict__ mpart) {
+  const int bid = blockIdx.x;
+  if (bid < n_frag_blocks) {
+    memory_frags_item<D, G>(bid * 128 + threadIdx.x, M, L, Hkv, inv_sqrt_d, frag);
+    return;
+  }
+  mean_memory_part_block(bid - n_frag_blocks, M, LH, D, mpart);
+}
+template <int D, int G>
+inline int mem_prep_frag_blocks(int L, int Hkv) {
+  constexpr int NT = (G <= 4) ? 1 : 2;
+  return (L * Hkv * NT * (D / 32) * 32 + 127) / 128;
+}
+
+struct PostKeyParams {
+  const float2* partials; int n_part; float* lse; int n_lse;          // lse rows
+  const float* mpart; int n_mpart; int LH; FoldOut fold; int n_fold;  // fold blocks (0: not a learnable call)
+  const float* kq; const int32_t* n_xq; int nks; uint4 *kc_frag, *vc_frag; int n_kv;  // Kc / Vc blocks
+};
+
+template <int D>
+__global__ __launch_bounds__(128) void k_post_key(const PostKeyParams p, const ResidW w) {
+  int bid = blockIdx.x;
+  if (bid < p.n_lse) { score_lse_block(bid, p.partials, p.n_part, p.lse); return; }
+  bid -= p.n_lse;
+  if (bid < p.n_fold) { resid_fold_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.fold); return; }
+  bid -= p.n_fold;
+  resid_kv_frags_block(bid, p.kq, p.n_xq, D, w, p.nks, p.kc_frag, p.vc_frag);
+}
+
+}  // namespace ikv

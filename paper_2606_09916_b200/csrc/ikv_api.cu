@@ -21,6 +21,7 @@
 #include "score_mma.cuh"
 #include "select.cuh"
 #include "select_cluster.cuh"
+#include "fused_small.cuh"
 
 using namespace ikv;
 
@@ -420,11 +421,11 @@ ikv_status dispatch_decode(ikv_ctx* c, int layer, const DecBatch& b, int n_req, 
 
 // bf16 key pass on the tensor pipe (score_mma.cuh).  Returns the number of partial (max, sum) columns.
 template <int D, int G>
-ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, int* n_part, cudaStream_t st) {
+ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, int n_mpart, int* n_part,
+                           cudaStream_t st) {
   const int L = c->cfg.n_layers, Hkv = c->cfg.n_kv_heads, Hq = c->cfg.n_q_heads;
-  constexpr int NT = (G <= 4) ? 1 : 2;
-  const int total = L * Hkv * NT * (D / 32) * 32;
-  k_memory_frags<D, G><<<(total + 255) / 256, 256, 0, st>>>(M, L, Hkv, 1.0f / sqrtf((float)D), c->frag);
+  const int n_fb = mem_prep_frag_blocks<D, G>(L, Hkv);
+  k_mem_prep<D, G><<<n_fb + n_mpart, 128, 0, st>>>(M, L, Hkv, 1.0f / sqrtf((float)D), c->frag, n_fb, L * Hq, c->mpart);
   LAUNCH_CHECK(c);
   int ns = 0;
   const size_t smem = key_pass_smem(L, Hq, Hkv, D, kbar, c->max_smem, &ns);
@@ -453,20 +454,22 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
 }
 
 template <int D>
-ikv_status dispatch_key_pass_g(ikv_ctx* c, const float* M, bool kbar, bool xq, int* n_part, cudaStream_t st) {
+ikv_status dispatch_key_pass_g(ikv_ctx* c, const float* M, bool kbar, bool xq, int n_mpart, int* n_part,
+                               cudaStream_t st) {
   switch (c->G) {
-    case 1: return launch_key_pass<D, 1>(c, M, kbar, xq, n_part, st);
-    case 2: return launch_key_pass<D, 2>(c, M, kbar, xq, n_part, st);
-    case 4: return launch_key_pass<D, 4>(c, M, kbar, xq, n_part, st);
-    case 5: return launch_key_pass<D, 5>(c, M, kbar, xq, n_part, st);
-    case 8: return launch_key_pass<D, 8>(c, M, kbar, xq, n_part, st);
+    case 1: return launch_key_pass<D, 1>(c, M, kbar, xq, n_mpart, n_part, st);
+    case 2: return launch_key_pass<D, 2>(c, M, kbar, xq, n_mpart, n_part, st);
+    case 4: return launch_key_pass<D, 4>(c, M, kbar, xq, n_mpart, n_part, st);
+    case 5: return launch_key_pass<D, 5>(c, M, kbar, xq, n_mpart, n_part, st);
+    case 8: return launch_key_pass<D, 8>(c, M, kbar, xq, n_mpart, n_part, st);
   }
   IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "GQA group size %d not supported (1,2,4,5,8)", c->G);
 }
 
-ikv_status dispatch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool xq, int* n_part, cudaStream_t st) {
-  return c->cfg.head_dim == 128 ? dispatch_key_pass_g<128>(c, M, kbar, xq, n_part, st)
-                                : dispatch_key_pass_g<64>(c, M, kbar, xq, n_part, st);
+ikv_status dispatch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool xq, int n_mpart, int* n_part,
+                             cudaStream_t st) {
+  return c->cfg.head_dim == 128 ? dispatch_key_pass_g<128>(c, M, kbar, xq, n_mpart, n_part, st)
+                                : dispatch_key_pass_g<64>(c, M, kbar, xq, n_mpart, n_part, st);
 }
 
 ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, float* rule_out, cudaStream_t st) {
@@ -482,39 +485,39 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   TRY(ensure_scratch(c, N));
   const float* M = (base_mode == IKV_MODE_QUERY) ? s->d_qenc : s->d_mem;
 
-#define IKV_PART_ARGS r.slot_map, N, c->cfg.dead_slot, r.prefix_len, r.q_start, r.q_end, scores, rule_out, \
-                      c->cand_pos, c->cand_slot, c->d_ncand
-  if (N <= CL_CTAS * 1024 * 4) k_partition_cl<4><<<CL_CTAS, 1024, 0, st>>>(IKV_PART_ARGS);
-  else if (N <= CL_CTAS * 1024 * 8) k_partition_cl<8><<<CL_CTAS, 1024, 0, st>>>(IKV_PART_ARGS);
-  else if (N <= CL_MAX_N) k_partition_cl<16><<<CL_CTAS, 1024, 0, st>>>(IKV_PART_ARGS);
-  else k_partition<<<1, 1024, 0, st>>>(IKV_PART_ARGS);
-#undef IKV_PART_ARGS
-  LAUNCH_CHECK(c);
   const bool fast = c->cfg.kv_dtype == IKV_BF16;  // tensor-pipe key pass; fp32 pools take the plain FMA kernel
   const bool use_x = learn && !(mode & IKV_FLAG_NO_XATTN);
   const int n_x = use_x ? (r.xattn_pos ? r.n_xattn_pos : (r.q_end - r.q_start)) : 0;
-  if (learn) {
-    TRY(ensure_xq(c, n_x > 0 ? n_x : 1));
-    if (n_x > 0) {
-      k_xattn_compact<<<1, 1024, 0, st>>>(r.slot_map, N, c->cfg.dead_slot, r.xattn_pos, n_x, r.q_start, c->xq_slot,
-                                          c->d_nxq);
-      LAUNCH_CHECK(c);
+  if (learn) TRY(ensure_xq(c, n_x > 0 ? n_x : 1));
+  {
+    // a1 (+ the compaction of the live cross-attention positions as a second cluster of the same launch)
+    const int grid = CL_CTAS * (n_x > 0 ? 2 : 1);
+#define IKV_PART_ARGS r.slot_map, N, c->cfg.dead_slot, r.prefix_len, r.q_start, r.q_end, scores, rule_out, \
+                      c->cand_pos, c->cand_slot, c->d_ncand
+#define IKV_X_ARGS r.xattn_pos, n_x, c->xq_slot, c->d_nxq
+    if (N <= CL_CTAS * 1024 * 4) k_partition_cl<4><<<grid, 1024, 0, st>>>(IKV_PART_ARGS, IKV_X_ARGS);
+    else if (N <= CL_CTAS * 1024 * 8) k_partition_cl<8><<<grid, 1024, 0, st>>>(IKV_PART_ARGS, IKV_X_ARGS);
+    else if (N <= CL_MAX_N) k_partition_cl<16><<<grid, 1024, 0, st>>>(IKV_PART_ARGS, IKV_X_ARGS);
+    else {
+      k_partition<<<1, 1024, 0, st>>>(IKV_PART_ARGS);
+      if (n_x > 0)
+        k_xattn_compact<<<1, 1024, 0, st>>>(r.slot_map, N, c->cfg.dead_slot, r.xattn_pos, n_x, r.q_start, c->xq_slot,
+                                            c->d_nxq);
     }
-  }
-  if (learn) {  // fold mbar into W_Q / fc1 (residual_mma.cuh); independent of the key pass
-    const int LH = L * Hq, nb = (LH + 31) / 32;
-    k_mean_memory_part<<<nb, D, 0, st>>>(M, LH, D, c->mpart);
-    LAUNCH_CHECK(c);
-    FoldOut fo;
-    fo.mbar = c->mbar; fo.wq_frag = c->wq_frag; fo.w1k_frag = c->w1k_frag; fo.bq_eff = c->bq_eff; fo.b1_eff = c->b1_eff;
-    if (D == 128) k_resid_fold<128><<<resid_fold_grid<128>(), 128, 0, st>>>(c->mpart, nb, LH, c->rw, fo);
-    else k_resid_fold<64><<<resid_fold_grid<64>(), 128, 0, st>>>(c->mpart, nb, LH, c->rw, fo);
+#undef IKV_PART_ARGS
+#undef IKV_X_ARGS
     LAUNCH_CHECK(c);
   }
+  const int LH = L * Hq, n_mpart = learn ? (LH + 31) / 32 : 0;  // mbar partial sums ride along with the fragments
   int n_part = (N + SCORE_TILE - 1) / SCORE_TILE;
   if (fast) {
-    TRY(dispatch_key_pass(c, M, learn, n_x > 0, &n_part, st));
+    TRY(dispatch_key_pass(c, M, learn, n_x > 0, n_mpart, &n_part, st));
   } else {
+    if (n_mpart > 0) {
+      if (D == 128) k_mem_prep<128, 1><<<n_mpart, 128, 0, st>>>(M, L, Hkv, 0.f, nullptr, 0, LH, c->mpart);
+      else k_mem_prep<64, 1><<<n_mpart, 128, 0, st>>>(M, L, Hkv, 0.f, nullptr, 0, LH, c->mpart);
+      LAUNCH_CHECK(c);
+    }
     TRY(dispatch_logits(c, *s, M, N, learn, st));
     if (n_x > 0) {
       k_mean_key_list<float><<<n_x, D, 0, st>>>((const float*)c->cfg.k_pool, c->layer_stride, L, Hkv, D, c->xq_slot,
@@ -522,17 +525,25 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
       LAUNCH_CHECK(c);
     }
   }
-  k_score_lse<<<L * Hq, 128, 0, st>>>(c->partials, n_part, c->lse);
-  LAUNCH_CHECK(c);
+  {
+    // lse rows, and for a learnable call the folded residual operands and the Kc / Vc fragments, in one launch
+    PostKeyParams pk;
+    pk.partials = c->partials; pk.n_part = n_part; pk.lse = c->lse; pk.n_lse = LH;
+    pk.mpart = c->mpart; pk.n_mpart = n_mpart; pk.LH = LH;
+    pk.fold.mbar = c->mbar; pk.fold.wq_frag = c->wq_frag; pk.fold.w1k_frag = c->w1k_frag;
+    pk.fold.bq_eff = c->bq_eff; pk.fold.b1_eff = c->b1_eff;
+    pk.n_fold = learn ? (D == 128 ? resid_fold_grid<128>() : resid_fold_grid<64>()) : 0;
+    pk.kq = c->kq; pk.n_xq = c->d_nxq; pk.nks = (int)(c->xq_cap / 16); pk.kc_frag = c->kc_frag; pk.vc_frag = c->vc_frag;
+    pk.n_kv = (learn && n_x > 0) ? 4 * ((n_x + 15) / 16) : 0;
+    const int grid = pk.n_lse + pk.n_fold + pk.n_kv;
+    if (D == 128) k_post_key<128><<<grid, 128, 0, st>>>(pk, c->rw);
+    else k_post_key<64><<<grid, 128, 0, st>>>(pk, c->rw);
+    LAUNCH_CHECK(c);
+  }
   k_score_rule4<<<(N + 63) / 64, 256, 0, st>>>(c->logits, c->cap_tokens, L * Hq, c->lse, c->d_ncand, c->cand_pos,
                                                c->rule_c, scores, learn ? 0 : 1, rule_out);
   LAUNCH_CHECK(c);
   if (learn) {
-    if (n_x > 0) {
-      k_resid_kv_frags<<<(n_x + 15) / 16, 128, 0, st>>>(c->kq, c->d_nxq, D, c->rw, (int)(c->xq_cap / 16), c->kc_frag,
-                                                       c->vc_frag);
-      LAUNCH_CHECK(c);
-    }
     ResidMmaParams rp;
     rp.rule_c = c->rule_c; rp.kbar = c->kbar; rp.n_cand = c->d_ncand; rp.cand_pos = c->cand_pos; rp.n_xq = c->d_nxq;
     rp.wq_frag = c->wq_frag; rp.w1k_frag = c->w1k_frag; rp.kc_frag = c->kc_frag; rp.vc_frag = c->vc_frag;

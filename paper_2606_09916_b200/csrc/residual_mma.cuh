@@ -70,12 +70,15 @@ __device__ __forceinline__ uint4 make_bfrag(int lane, F B) {
   return o;
 }
 
-// mbar partial sums: grid = ceil(LH / 32), block = D.  part[b][d] = sum of rows 32 b .. 32 b + 31 of M (Eq. 5 mbar).
-__global__ void k_mean_memory_part(const float* __restrict__ M, int LH, int D, float* __restrict__ part) {
-  const int d = threadIdx.x, r0 = blockIdx.x * 32;
+// mbar partial sums (Eq. 5 mbar): block b of >= D threads; part[b][d] = sum of rows 32 b .. 32 b + 31 of M.
+__device__ __forceinline__ void mean_memory_part_block(int b, const float* __restrict__ M, int LH, int D,
+                                                       float* __restrict__ part) {
+  const int d = threadIdx.x, r0 = b * 32;
+  if (d >= D) return;
   float acc = 0.f;
+#pragma unroll 8
   for (int i = r0; i < min(LH, r0 + 32); ++i) acc += M[(int64_t)i * D + d];
-  part[blockIdx.x * D + d] = acc;
+  part[b * D + d] = acc;
 }
 
 struct FoldOut {
@@ -86,11 +89,11 @@ struct FoldOut {
   float* b1_eff;    // [256]
 };
 
-// Folds mbar into W_Q and fc1 (see the header of this file).  block = 128 threads; grid covers
+// Folds mbar into W_Q and fc1 (see the header of this file).  Blocks of 128 threads; resid_fold_grid() blocks cover
 // D/16*16*32 + 4*D/16*8*32 fragment items and 384 bias items.
 template <int D>
-__global__ __launch_bounds__(128) void k_resid_fold(const float* __restrict__ part, int n_part, int LH, ResidW w,
-                                                    FoldOut o) {
+__device__ __forceinline__ void resid_fold_block(int bid, const float* __restrict__ part, int n_part, int LH,
+                                                 const ResidW& w, const FoldOut& o) {
   constexpr int KS = D / 16, P = 3 * D + 1, IN = P + R_DC;
   constexpr int N_WQ = KS * 16 * 32, N_W1 = 4 * KS * 8 * 32, N_B = R_DC + R_HID;
   __shared__ float mb[D];
@@ -100,8 +103,8 @@ __global__ __launch_bounds__(128) void k_resid_fold(const float* __restrict__ pa
     mb[d] = acc / (float)LH;
   }
   __syncthreads();
-  int idx = blockIdx.x * 128 + threadIdx.x;
-  if (blockIdx.x == 0)
+  int idx = bid * 128 + threadIdx.x;
+  if (bid == 0)
     for (int d = threadIdx.x; d < D; d += 128) o.mbar[d] = mb[d];
   if (idx < N_WQ) {
     const int lane = idx & 31, t = (idx >> 5) & 15, s = idx >> 9;
@@ -138,58 +141,56 @@ inline int resid_fold_grid() {
   return ((D / 16) * 16 * 32 + 4 * (D / 16) * 8 * 32 + R_DC + R_HID + 127) / 128;
 }
 
-// Kc = W_K K^q + b_K, Vc = W_V K^q + b_V (Eq. 6) for 16 query keys per CTA (block = 128, thread = output
-// channel), written as B fragments:
+// Kc = W_K K^q + b_K, Vc = W_V K^q + b_V (Eq. 6): block `bid` = (16-key step v, cross-attention head hc), 128 threads
+// = 32 channels of the head x 4 groups of 4 keys.  Written as B fragments:
 //   kc_frag[((hc*2 + u)*nkt + t)*32 + lane] : S = Q_h Kc_h^T, k = head dim 16 u + kappa, n = key 8 t + r, scaled
 //                                             by log2(e)/sqrt(32) so that the softmax runs on exp2
 //   vc_frag[((hc*nks + v)*4 + nt)*32 + lane]: O = P Vc_h,     k = key 16 v + kappa, n = head dim 8 nt + r
 // nkt = 2 nks = capacity in 8-key tiles.  Keys >= n_xq are zero.
-__global__ __launch_bounds__(128) void k_resid_kv_frags(const float* __restrict__ kq, const int32_t* __restrict__ n_xq,
-                                                        int D, ResidW w, int nks, uint4* __restrict__ kc_frag,
-                                                        uint4* __restrict__ vc_frag) {
+__device__ __forceinline__ void resid_kv_frags_block(int bid, const float* __restrict__ kq,
+                                                     const int32_t* __restrict__ n_xq, int D, const ResidW& w, int nks,
+                                                     uint4* __restrict__ kc_frag, uint4* __restrict__ vc_frag) {
   __shared__ float x[16][128];
-  __shared__ float kc[16][R_DC + 1], vc[16][R_DC + 1];
-  const int nq = *n_xq, v = blockIdx.x, k0 = v * 16, o = threadIdx.x;
+  __shared__ float kc[16][R_DH + 1], vc[16][R_DH + 1];
+  const int nq = *n_xq, v = bid >> 2, hc = bid & 3, k0 = v * 16;
   if (k0 >= nq) return;
   for (int i = threadIdx.x; i < 16 * D; i += 128) {
     const int key = i / D, d = i % D;
     x[key][d] = (k0 + key < nq) ? kq[(int64_t)(k0 + key) * D + d] : 0.f;
   }
   __syncthreads();
-  float ak[16], av[16];
+  const int ch = threadIdx.x & 31, kg = threadIdx.x >> 5, o = hc * R_DH + ch;
+  float ak[4], av[4];
   const float bk = w.bk[o], bv = w.bv[o];
 #pragma unroll
-  for (int i = 0; i < 16; ++i) { ak[i] = bk; av[i] = bv; }
-#pragma unroll 8
+  for (int i = 0; i < 4; ++i) { ak[i] = bk; av[i] = bv; }
+#pragma unroll 16
   for (int d = 0; d < D; ++d) {
     const float wk = __ldg(w.wk_t + d * R_DC + o), wv = __ldg(w.wv_t + d * R_DC + o);
 #pragma unroll
-    for (int i = 0; i < 16; ++i) {
-      ak[i] = fmaf(wk, x[i][d], ak[i]);
-      av[i] = fmaf(wv, x[i][d], av[i]);
+    for (int i = 0; i < 4; ++i) {
+      ak[i] = fmaf(wk, x[kg * 4 + i][d], ak[i]);
+      av[i] = fmaf(wv, x[kg * 4 + i][d], av[i]);
     }
   }
   const float sc = 1.4426950408889634f * 0.17677669529663689f;  // log2(e) / sqrt(32)  (R10)
 #pragma unroll
-  for (int i = 0; i < 16; ++i) {
-    const bool ok = k0 + i < nq;
-    kc[i][o] = ok ? ak[i] * sc : 0.f;
-    vc[i][o] = ok ? av[i] : 0.f;
+  for (int i = 0; i < 4; ++i) {
+    const int key = kg * 4 + i;
+    const bool ok = k0 + key < nq;
+    kc[key][ch] = ok ? ak[i] * sc : 0.f;
+    vc[key][ch] = ok ? av[i] : 0.f;
   }
   __syncthreads();
-  const int nkt = 2 * nks;
-  for (int it = threadIdx.x; it < 512; it += 128) {
-    const int lane = it & 31, a = (it >> 5) & 3, hc = it >> 7;
-    {  // Kc: a = (u, tile-in-pair)
-      const int u = a >> 1, tl = a & 1;
-      kc_frag[((int64_t)(hc * 2 + u) * nkt + 2 * v + tl) * 32 + lane] =
-          make_bfrag(lane, [&](int kl, int nl) { return kc[tl * 8 + nl][hc * R_DH + u * 16 + kl]; });
-    }
-    {  // Vc: a = nt
-      vc_frag[((int64_t)(hc * nks + v) * 4 + a) * 32 + lane] =
-          make_bfrag(lane, [&](int kl, int nl) { return vc[kl][hc * R_DH + a * 8 + nl]; });
-    }
+  const int nkt = 2 * nks, lane = threadIdx.x & 31, a = threadIdx.x >> 5;
+  {  // Kc: a = (u, tile-in-pair)
+    const int u = a >> 1, tl = a & 1;
+    kc_frag[((int64_t)(hc * 2 + u) * nkt + 2 * v + tl) * 32 + lane] =
+        make_bfrag(lane, [&](int kl, int nl) { return kc[tl * 8 + nl][u * 16 + kl]; });
   }
+  // Vc: a = nt
+  vc_frag[((int64_t)(hc * nks + v) * 4 + a) * 32 + lane] =
+      make_bfrag(lane, [&](int kl, int nl) { return vc[kl][a * 8 + nl]; });
 }
 
 struct ResidMmaParams {

@@ -172,10 +172,11 @@ __global__ __launch_bounds__(256) void k_score_logits(
   }
 }
 
-// lse[l,h] = log sum_c exp(x[l,h,c]) from the per-tile partials.  grid = L*Hq, block = 128.
-__global__ void k_score_lse(const float2* __restrict__ partials, int n_tiles, float* __restrict__ lse) {
+// lse[l,h] = log sum_c exp(x[l,h,c]) from the per-CTA partials.  One block of 128 threads per (l,h) row `row`.
+__device__ __forceinline__ void score_lse_block(int row, const float2* __restrict__ partials, int n_tiles,
+                                                float* __restrict__ lse) {
   __shared__ float red[4];
-  const float2* p = partials + (int64_t)blockIdx.x * n_tiles;
+  const float2* p = partials + (int64_t)row * n_tiles;
   float mx = -CUDART_INF_F;
   for (int i = threadIdx.x; i < n_tiles; i += 128) mx = fmaxf(mx, p[i].x);
   mx = warp_max(mx);
@@ -191,7 +192,7 @@ __global__ void k_score_lse(const float2* __restrict__ partials, int n_tiles, fl
   s = warp_sum(s);
   if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
   __syncthreads();
-  if (threadIdx.x == 0) lse[blockIdx.x] = mx + logf(red[0] + red[1] + red[2] + red[3]);
+  if (threadIdx.x == 0) lse[row] = mx + logf(red[0] + red[1] + red[2] + red[3]);
 }
 
 // a3  rule_c = sum_{l,h} exp(x[l,h,c] - lse[l,h])   (Eq. 3).  One thread per candidate.
@@ -212,13 +213,6 @@ __global__ void k_score_rule(const float* __restrict__ logits, int64_t ldc, int 
   const int pos = cand_pos[c];
   if (scatter_scores) scores[pos] = r;
   if (rule_out) rule_out[pos] = r;
-}
-
-// m_bar[d] = mean_{l,h} M[l,h,d].  grid = 1, block = D.
-__global__ void k_mean_memory(const float* __restrict__ M, int LH, int D, float* __restrict__ mbar) {
-  float acc = 0.f;
-  for (int lh = 0; lh < LH; ++lh) acc += M[(int64_t)lh * D + threadIdx.x];
-  mbar[threadIdx.x] = acc / (float)LH;
 }
 
 // live cross-attention positions ("positions evicted in a prior round are excluded"):

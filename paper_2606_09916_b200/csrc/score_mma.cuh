@@ -38,9 +38,9 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
 // k-step s = 2i+j uses d = 8(q+4i) + 4j + {0,1} (b0) and + {2,3} (b1).  Column n = r:
 //   G <= 4 (NT = 1): n = 2g -> hi(M[l, kvh*G+g]), n = 2g+1 -> lo;      G > 4 (NT = 2): tile 0 hi, tile 1 lo, n = g.
 template <int D, int G>
-__global__ void k_memory_frags(const float* __restrict__ M, int L, int Hkv, float inv_sqrt_d, uint4* __restrict__ frag) {
+__device__ __forceinline__ void memory_frags_item(int idx, const float* __restrict__ M, int L, int Hkv, float inv_sqrt_d,
+                                                  uint4* __restrict__ frag) {
   constexpr int KS = D / 16, NT = (G <= 4) ? 1 : 2;
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const int total = L * Hkv * NT * (KS / 2) * 32;
   if (idx >= total) return;
   const int lane = idx & 31;

@@ -37,12 +37,32 @@ template <int MAXI>
 __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_partition_cl(
     const int32_t* __restrict__ S, int N, int32_t dead, int pi, int qs, int qe, float* __restrict__ scores,
     float* __restrict__ rule_out, int32_t* __restrict__ cand_pos, int32_t* __restrict__ cand_slot,
-    int32_t* __restrict__ n_cand) {
+    int32_t* __restrict__ n_cand, const int32_t* __restrict__ xattn_pos, int n_x, int32_t* __restrict__ xq_slot,
+    int32_t* __restrict__ n_xq) {
   cg::cluster_group cl = cg::this_cluster();
   const int crank = (int)cl.block_rank();
   __shared__ int warp_tot[32];
   __shared__ int sh_tot;
   const int tid = threadIdx.x;
+  if (blockIdx.x >= CL_CTAS) {
+    // second cluster (launched when n_x > 0): rank 0 compacts the live cross-attention positions
+    if (crank != 0) return;
+    int xb = 0;
+    for (int i0 = 0; i0 < n_x; i0 += 1024) {
+      const int i = i0 + tid;
+      int sl = dead;
+      if (i < n_x) {
+        const int pos = xattn_pos ? xattn_pos[i] : qs + i;
+        if (pos >= 0 && pos < N) sl = S[pos];
+      }
+      int tot;
+      const int ex = block_excl_scan_1024(sl != dead ? 1 : 0, warp_tot, &tot);
+      if (sl != dead) xq_slot[xb + ex] = sl;
+      xb += tot;
+    }
+    if (tid == 0) *n_xq = xb;
+    return;
+  }
   const int base = (crank * 1024 + tid) * MAXI;
   int slot[MAXI];
   int cnt = 0;
