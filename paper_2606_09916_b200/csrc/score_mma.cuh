@@ -21,8 +21,8 @@
 namespace ikv {
 
 constexpr int KP_TOK = 32;       // tokens per stage = two m16 tiles of the mma
-constexpr int KP_LWARPS = 4;     // logit warps
-constexpr int KP_KWARPS = 8;     // mean-key warps
+constexpr int KP_LWARPS = 8;     // logit warps
+constexpr int KP_KWARPS = 4;     // mean-key warps
 constexpr int KP_THREADS = (KP_LWARPS + KP_KWARPS + 1) * 32;
 constexpr int KP_ROWPAD = 64;    // bytes added to each staged token row (bank spread for the 16-byte reads)
 
