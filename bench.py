@@ -219,7 +219,8 @@ def run_ours(args):
         decode_all()
     stream.synchronize()
 
-    n_prune_launch = 6 + (5 if mode == ikv.MODE_LEARNABLE else 0)
+    # memory_update, partition(+xattn compaction), mem_prep, key_pass, post_key, rule4, select_evict (+ residual_mma)
+    n_prune_launch = 7 + (1 if mode == ikv.MODE_LEARNABLE else 0)
     n_decode_launch = DEC * L * 2
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -338,11 +339,11 @@ def run_ours(args):
                     "what": "ikv_prune_host: slot map + query rows H2D, memory update + score + select/evict, "
                             "slot map + valid mask + freed list + counts D2H; the K/V pool is device-resident state"},
             "gpu_launches": K * (n_prune_launch + n_decode_launch),
-            "roofline": {"kernel": "k_score_logits", "bound": "hbm", "achieved": ach, "peak": hbm_peak,
+            "roofline": {"kernel": "k_key_pass", "bound": "hbm", "achieved": ach, "peak": hbm_peak,
                          "unit": "GB/s", "frac": ach / hbm_peak, "frac_of_nominal_8TBs": ach / NOMINAL_HBM_GBS,
                          "peak_source": peak_src, "traffic": None, "algorithmic_bytes": key_bytes,
                          "ms": logits_ms},
-            "roofline_decode": {"kernel": "k_decode_split (+k_decode_merge, per-layer launch gap included)",
+            "roofline_decode": {"kernel": "k_decode_mma (+k_decode_merge4, per-layer launch gap included)",
                                 "bound": "hbm", "achieved": dec_ach, "peak": hbm_peak, "unit": "GB/s",
                                 "frac": dec_ach / hbm_peak, "frac_of_nominal_8TBs": dec_ach / NOMINAL_HBM_GBS,
                                 "algorithmic_bytes": dec_bytes_call, "traffic": None, "ms": dec_kernel_ms},

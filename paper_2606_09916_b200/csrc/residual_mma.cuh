@@ -90,7 +90,7 @@ struct FoldOut {
 };
 
 // Folds mbar into W_Q and fc1 (see the header of this file).  Blocks of 128 threads; resid_fold_grid() blocks cover
-// D/16*16*32 + 4*D/16*8*32 fragment items and 384 bias items.
+// D/16*16*32 + 4*D/16*8*32 fragment items and 384 bias warps.
 template <int D>
 __device__ __forceinline__ void resid_fold_block(int bid, const float* __restrict__ part, int n_part, int LH,
                                                  const ResidW& w, const FoldOut& o) {
@@ -127,18 +127,22 @@ __device__ __forceinline__ void resid_fold_block(int bid, const float* __restric
     return;
   }
   idx -= N_W1;
-  if (idx < N_B) {
-    const bool isq = idx < R_DC;
-    const int n = isq ? idx : idx - R_DC;
+  // folded biases: one warp per output unit (lanes stride the D columns of W_m, one round of coalesced loads)
+  const int unit = idx >> 5, lane = threadIdx.x & 31;
+  if (unit < N_B) {
+    const bool isq = unit < R_DC;
+    const int n = isq ? unit : unit - R_DC;
     const float* row = isq ? (w.wq + (int64_t)n * P + D) : (w.fc1_w + (int64_t)n * IN + D);
-    float acc = isq ? w.bq[n] : w.fc1_b[n];
-    for (int d = 0; d < D; ++d) acc = fmaf(row[d], mb[d], acc);
-    (isq ? o.bq_eff : o.b1_eff)[n] = acc;
+    float acc = 0.f;
+#pragma unroll
+    for (int d = lane; d < D; d += 32) acc = fmaf(__ldg(row + d), mb[d], acc);
+    acc = warp_sum(acc);
+    if (lane == 0) (isq ? o.bq_eff : o.b1_eff)[n] = acc + (isq ? w.bq[n] : w.fc1_b[n]);
   }
 }
 template <int D>
 inline int resid_fold_grid() {
-  return ((D / 16) * 16 * 32 + 4 * (D / 16) * 8 * 32 + R_DC + R_HID + 127) / 128;
+  return ((D / 16) * 16 * 32 + 4 * (D / 16) * 8 * 32 + (R_DC + R_HID) * 32 + 127) / 128;
 }
 
 // Kc = W_K K^q + b_K, Vc = W_V K^q + b_V (Eq. 6): block `bid` = (16-key step v, cross-attention head hc), 128 threads
@@ -159,27 +163,36 @@ __device__ __forceinline__ void resid_kv_frags_block(int bid, const float* __res
     x[key][d] = (k0 + key < nq) ? kq[(int64_t)(k0 + key) * D + d] : 0.f;
   }
   __syncthreads();
-  const int ch = threadIdx.x & 31, kg = threadIdx.x >> 5, o = hc * R_DH + ch;
-  float ak[4], av[4];
-  const float bk = w.bk[o], bv = w.bv[o];
+  // thread (ch, dg): channel ch of the head, quarter dg of the D columns, all 16 keys; quarters summed through smem
+  __shared__ float part[2][4][16][R_DH + 1];
+  const int ch = threadIdx.x & 31, dg = threadIdx.x >> 5, o = hc * R_DH + ch;
+  float ak[16], av[16];
 #pragma unroll
-  for (int i = 0; i < 4; ++i) { ak[i] = bk; av[i] = bv; }
+  for (int i = 0; i < 16; ++i) { ak[i] = 0.f; av[i] = 0.f; }
+  const int dq = D / 4;
 #pragma unroll 16
-  for (int d = 0; d < D; ++d) {
+  for (int dd = 0; dd < dq; ++dd) {
+    const int d = dg * dq + dd;
     const float wk = __ldg(w.wk_t + d * R_DC + o), wv = __ldg(w.wv_t + d * R_DC + o);
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      ak[i] = fmaf(wk, x[kg * 4 + i][d], ak[i]);
-      av[i] = fmaf(wv, x[kg * 4 + i][d], av[i]);
+    for (int i = 0; i < 16; ++i) {
+      ak[i] = fmaf(wk, x[i][d], ak[i]);
+      av[i] = fmaf(wv, x[i][d], av[i]);
     }
   }
+#pragma unroll
+  for (int i = 0; i < 16; ++i) { part[0][dg][i][ch] = ak[i]; part[1][dg][i][ch] = av[i]; }
+  __syncthreads();
   const float sc = 1.4426950408889634f * 0.17677669529663689f;  // log2(e) / sqrt(32)  (R10)
+  const float bk = w.bk[o], bv = w.bv[o];
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
-    const int key = kg * 4 + i;
+    const int key = dg * 4 + i;
     const bool ok = k0 + key < nq;
-    kc[key][ch] = ok ? ak[i] * sc : 0.f;
-    vc[key][ch] = ok ? av[i] : 0.f;
+    const float sk = bk + ((part[0][0][key][ch] + part[0][1][key][ch]) + (part[0][2][key][ch] + part[0][3][key][ch]));
+    const float sv = bv + ((part[1][0][key][ch] + part[1][1][key][ch]) + (part[1][2][key][ch] + part[1][3][key][ch]));
+    kc[key][ch] = ok ? sk * sc : 0.f;
+    vc[key][ch] = ok ? sv : 0.f;
   }
   __syncthreads();
   const int nkt = 2 * nks, lane = threadIdx.x & 31, a = threadIdx.x >> 5;
