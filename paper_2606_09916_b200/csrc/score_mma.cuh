@@ -1,18 +1,19 @@
 // score_mma.cuh -- the bf16 key pass of the rule scorer (Eq. 3) and the mean key of Eq. 5
-// as ONE persistent streaming kernel for sm_100a.
+// as ONE persistent streaming kernel for sm_100a (one CTA per SM, three warp roles).
 //
-//   producer warp : per (16-token tile, layer) one 1-D bulk copy (TMA unit, UBLKCP) per token row
-//                   [H_kv][D] bf16 (2 KB at Qwen3-8B shape) through the slot map into a ring of shared-memory
-//                   stages, completion on an mbarrier (full[stage]); waits on empty[stage] before reuse.
-//   consumer warps: warp w owns KV head(s) w, w+8, ...; the 16 x D key tile is the A operand of
-//                   mma.sync.m16n8k16 (bf16 in, fp32 accumulate); the B operand holds the G memory rows of the
-//                   group, each split into a bf16 hi and a bf16 lo part (two columns), so that
-//                   hi + lo carries ~16 mantissa bits of M / sqrt(D) and keys are exact => fp32-grade logits.
-//                   The contraction has only G (<= 8) useful columns: it is not a tcgen05 tile (R1);
-//                   the tensor pipe is used here to keep the FMA pipe free, the kernel is HBM-bound.
-//   Per (layer, head): logits -> scratch [L*Hq][ldc] (fp32), running (max, sum exp) per CTA in shared memory,
-//   key bytes -> fp32 k_bar accumulators in registers (Eq. 5), reduced over the 8 head-warps per tile.
-//   Tiles [0, ceil(n_cand/16)) are the candidates; the tiles after them are the live cross-attention positions
+//   producer warp  : per (32-token tile, layer) one 1-D bulk copy (TMA unit, UBLKCP) per token row
+//                    [H_kv][D] bf16 (2 KB at Qwen3-8B shape) through the slot map into a ring of shared-memory
+//                    stages, completion on an mbarrier (full[stage]); waits on empty[stage] before reuse.
+//   logit warps    : warp w owns KV head(s) w, w+8, ...; the two 16 x D key tiles of the stage are the A operands of
+//                    mma.sync.m16n8k16 (bf16 in, fp32 accumulate); the B operand holds the G memory rows of the
+//                    group, each split into a bf16 hi and a bf16 lo part (two columns), so that hi + lo carries
+//                    ~16 mantissa bits of M / sqrt(D) and keys are exact => fp32-grade logits.  The B fragments are
+//                    prefetched one whole stage ahead.  The contraction has only G (<= 8) useful columns: it is
+//                    not a tcgen05 tile (R1); the tensor pipe keeps the FMA pipe free, the kernel is
+//                    HBM-bound.  Logits -> scratch [L*Hq][ldc] (fp32); running (max, sum exp) per (l,h) per CTA.
+//   mean-key warps : warp dq owns one quarter of D; every lane sums its 16-byte chunks over all KV heads and layers
+//                    in fp32 registers (Eq. 5) and writes k_bar once per tile -- no cross-warp reduction.
+//   Tiles [0, ceil(n_cand/32)) are the candidates; the tiles after them are the live cross-attention positions
 //   (K^q of Eq. 6, R7/R8) for which only the mean key is produced.
 #pragma once
 #include "common.cuh"
@@ -91,12 +92,8 @@ struct KeyPassParams {
   int n_stage;
 };
 
-// Warp roles of k_key_pass (one persistent CTA per SM):
-//   warp 0..3   logit warps: warp w owns KV heads w, w+4, ...; both 16-token halves of the stage share the B fragments,
-//               which are prefetched one (layer, head) ahead so that their L2 latency never sits behind the stage wait.
-//   warp 4..11  mean-key warps (KBAR): warp (dq, th) owns the d-quarter dq of the token half th; every lane sums its
-//               16-byte chunks over all KV heads and layers in fp32 registers -- no cross-warp reduction.
-//   warp 12     producer.
+// Warp roles of k_key_pass: warps [0, KP_LWARPS) logit warps, [KP_LWARPS, KP_LWARPS + KP_KWARPS) mean-key warps
+// (KBAR only; warp (dq, th) owns the d-quarter dq of the token part th), last warp producer.
 template <int D, int G, bool KBAR>
 __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams p) {
   constexpr int KS = D / 16, NI = D / 32, NT = (G <= 4) ? 1 : 2;
