@@ -1,16 +1,18 @@
-// decode_mma.cuh -- bf16 paged GQA decode attention through the slot map, dead entries skipped
-// (R16), split-K over the survivor list, for sm_100a.
+// decode_mma.cuh -- bf16 paged GQA decode attention through the slot map, dead entries skipped (
+// DESIGN.md R16), split-K over the survivor list, for sm_100a.
 //
-// One CTA = (token split, request, group of <= 8 KV heads):
-//   producer warp : per 16-token tile, one 1-D bulk copy (TMA unit) per token for the K row and one for the V row
-//                   of the CTA's heads ([heads][D] bf16, 2 KB at Qwen3-8B shape) into an mbarrier ring.
-//   consumer warps: warp w owns KV head w.  S^T = q K^T with the G query heads of the group as the (padded) M rows
-//                   of mma.sync.m16n8k16 and 8 tokens as N (K fragments via ldmatrix), online softmax in fp32
-//                   (exp2), O += P V with P re-used straight from the accumulator layout and V fragments via
-//                   ldmatrix.trans.  With G = 4 the FMA pipe could not keep up with HBM (8 FMA per key/value
-//                   element); the tensor pipe can.
-// Partials (m, l, o) per (request, head, split) go to scratch; k_decode_merge4 combines them.  Both kernels use
-// programmatic dependent launch: the next call's K/V prefetch overlaps this call's merge.
+// One CTA = (token split, request, group of <= 8 KV heads); producer warp + one consumer warp per KV head.
+//   producer : slots of 32 tokens per load, two tiles ahead; per 16-token tile one 1-D bulk copy (TMA unit) per token
+//              for the K rows into one half-stage of the ring and for the V rows into the next ([heads][D] bf16, 2 KB
+//              at Qwen3-8B shape), each half-stage with its own mbarrier pair.
+//   consumers: S = K q^T and O^T = V^T P with mma.sync.m16n8k16: the 16 tokens of the tile are the M rows of both
+//              products and the G query heads of the group the (padded) N columns, so every accumulator register is
+//              useful and O^T takes D/4 registers per thread.  K fragments via ldmatrix, V^T via ldmatrix.trans, P
+//              from the accumulator layout to the B layout by one 8x8 movmatrix transpose per half tile; online
+//              softmax per column in exp2 units, fp32.
+// At ~95 registers and three 33 KB half-stages a CTA takes under half an SM: the CTAs of two consecutive layer calls
+// co-reside, so the next call streams its K/V while this one computes, merges and drains (programmatic dependent
+// launch).  Partials (m, l, o) per (request, head, split) go to scratch; k_decode_merge4 combines them.
 #pragma once
 #include "common.cuh"
 #include "decode.cuh"
@@ -18,7 +20,7 @@
 
 namespace ikv {
 
-constexpr int DM_TOK = 16;     // tokens per stage
+constexpr int DM_TOK = 16;     // tokens per tile (one K half-stage + one V half-stage)
 constexpr int DM_GRAN = 8;     // split boundaries are multiples of this many tokens
 constexpr int DM_CWARPS = 8;   // consumer warps = KV heads per CTA
 constexpr int DM_THREADS = (DM_CWARPS + 1) * 32;
@@ -57,27 +59,33 @@ struct DecMmaParams {
   int n_split, n_stage;
 };
 
+__device__ __forceinline__ uint32_t movmatrix_t(uint32_t a) {
+  uint32_t d;
+  asm volatile("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(d) : "r"(a));
+  return d;
+}
+
 template <int D, int G>
-__global__ __launch_bounds__(DM_THREADS, 1) void k_decode_mma(const DecMmaParams p, const DecBatch batch) {
-  constexpr int KS = D / 16, NO = D / 8;
+__global__ __launch_bounds__(DM_THREADS, 2) void k_decode_mma(const DecMmaParams p, const DecBatch batch) {
+  constexpr int KS = D / 16, MT = D / 16;
   const int split = blockIdx.x, req = blockIdx.y, hg = blockIdx.z;
   const int Hkv = p.Hkv, Hq = Hkv * G;
   const int h0 = hg * DM_CWARPS;
   const int nh = min(DM_CWARPS, Hkv - h0);
   const int row_bytes = nh * D * 2;
   const int row_stride = row_bytes + DM_ROWPAD;
-  const int kv_bytes = DM_TOK * row_stride;  // K part of a stage; V part follows
-  const int stage_bytes = 2 * kv_bytes + 16;   // + validity mask word
-  const int NS = p.n_stage;
+  const int half_bytes = DM_TOK * row_stride;
+  const int HS = p.n_stage;  // half-stages in the ring
 
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  unsigned char* stage_base = smem_raw;
-  uint64_t* full = (uint64_t*)(stage_base + (size_t)NS * stage_bytes);
-  uint64_t* empty = full + NS;
+  unsigned char* ring = smem_raw;
+  uint64_t* full = (uint64_t*)(ring + (size_t)HS * half_bytes);
+  uint64_t* empty = full + HS;
+  uint32_t* vmasks = (uint32_t*)(empty + HS);  // [HS], written for K half-stages
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], DM_CWARPS); }
+    for (int s = 0; s < HS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], DM_CWARPS); }
     mbar_fence_init();
   }
   __syncthreads();
@@ -87,9 +95,9 @@ __global__ __launch_bounds__(DM_THREADS, 1) void k_decode_mma(const DecMmaParams
   // the only kernels of the library that trigger their dependents early) is still running.  Everything READ here --
   // slot lists, K/V pools, q -- was produced by kernels that never trigger early, so it is complete at this point;
   // everything WRITTEN here (the partial buffers, which the previous merge may still be reading) is written only
-  // after pdl_wait(), which the consumers execute just before their stores.
+  // after pdl_wait(), which the consumers execute just before their stores (R27).
   const DecReq rq = batch.r[req];
-  const int n_cached = rq.n_items;  // the list is padded with the dead slot up to n_items: no device-side length read
+  const int n_cached = rq.n_items;
   const int total = n_cached + (rq.seq_len - rq.covered);
   const int n_gran = (total + DM_GRAN - 1) / DM_GRAN;
   const int begin = (int)(((int64_t)n_gran * split) / p.n_split) * DM_GRAN;
@@ -98,15 +106,14 @@ __global__ __launch_bounds__(DM_THREADS, 1) void k_decode_mma(const DecMmaParams
 
   if (warp == DM_CWARPS) {
     // ------------------------------------------------------------------ producer
-    // slots of 32 tokens (two tiles) per load, fetched two tiles ahead of their bulk copies
     auto slot_of = [&](int i) -> int {
       if (i >= end) return p.dead;
       return (i < n_cached) ? __ldg(rq.live_slots + i) : __ldg(rq.S + rq.covered + (i - n_cached));
     };
     int cur = slot_of(begin + lane), nxt = slot_of(begin + 32 + lane);
+    int s = 0;
+    uint32_t ph = 0;
     for (int t = 0; t < n_tiles; ++t) {
-      const int s = t % NS;
-      const uint32_t ph = (uint32_t)(t / NS) & 1u;
       if (t > 0 && (t & 1) == 0) {
         cur = nxt;
         nxt = slot_of(begin + (t + 2) * DM_TOK + lane);
@@ -114,20 +121,21 @@ __global__ __launch_bounds__(DM_THREADS, 1) void k_decode_mma(const DecMmaParams
       const int i = begin + t * DM_TOK + lane;
       const int slot = __shfl_sync(0xffffffffu, cur, (t & 1) * DM_TOK + (lane & (DM_TOK - 1)));
       const bool in_range = lane < DM_TOK && i < end;
-      const bool copy = in_range;  // rows past the end are never copied; the consumers zero their V slices
       const uint32_t vmask = __ballot_sync(0xffffffffu, in_range && slot != p.dead);
-      const uint32_t cmask = __ballot_sync(0xffffffffu, copy);
-      unsigned char* sb = stage_base + (size_t)s * stage_bytes;
-      if (lane == 0) {
-        mbar_wait(&empty[s], ph ^ 1u);
-        *reinterpret_cast<uint32_t*>(sb + 2 * kv_bytes) = vmask;
-        mbar_arrive_expect_tx(&full[s], (uint32_t)(__popc(cmask) * 2 * row_bytes));
-      }
-      __syncwarp();
-      if (copy) {
-        const int64_t off = ((int64_t)slot * Hkv + h0) * D;
-        bulk_g2s(sb + lane * row_stride, p.k_layer + off, (uint32_t)row_bytes, &full[s]);
-        bulk_g2s(sb + kv_bytes + lane * row_stride, p.v_layer + off, (uint32_t)row_bytes, &full[s]);
+      const uint32_t nrows = __popc(__ballot_sync(0xffffffffu, in_range));
+      const int64_t off = ((int64_t)slot * Hkv + h0) * D;
+#pragma unroll
+      for (int kv = 0; kv < 2; ++kv) {
+        if (lane == 0) {
+          mbar_wait(&empty[s], ph ^ 1u);
+          if (kv == 0) vmasks[s] = vmask;
+          mbar_arrive_expect_tx(&full[s], nrows * (uint32_t)row_bytes);
+        }
+        __syncwarp();
+        if (in_range)
+          bulk_g2s(ring + (size_t)s * half_bytes + lane * row_stride, (kv == 0 ? p.k_layer : p.v_layer) + off,
+                   (uint32_t)row_bytes, &full[s]);
+        if (++s == HS) { s = 0; ph ^= 1u; }
       }
     }
   } else {
@@ -135,117 +143,136 @@ __global__ __launch_bounds__(DM_THREADS, 1) void k_decode_mma(const DecMmaParams
     const int r = lane >> 2, q4 = lane & 3;
     const int kvh = h0 + warp;
     const bool active = warp < nh;
-    // A fragments of q (rows g = r < G; rows >= G are zero)
-    uint32_t qa[KS][2];
+    // B fragments of q^T: b0 = q[g = r][16 ks + 2 q4, +1], b1 = q[g = r][16 ks + 8 + 2 q4, +1]; rows g >= G are zero
+    uint32_t qb[KS][2];
 #pragma unroll
-    for (int s = 0; s < KS; ++s) { qa[s][0] = 0u; qa[s][1] = 0u; }
+    for (int ks = 0; ks < KS; ++ks) { qb[ks][0] = 0u; qb[ks][1] = 0u; }
     if (active && r < G) {
       const uint32_t* qp = reinterpret_cast<const uint32_t*>(p.q + ((int64_t)req * Hq + kvh * G + r) * D);
 #pragma unroll
-      for (int s = 0; s < KS; ++s) {
-        qa[s][0] = qp[8 * s + q4];
-        qa[s][1] = qp[8 * s + 4 + q4];
+      for (int ks = 0; ks < KS; ++ks) {
+        qb[ks][0] = __ldg(qp + 8 * ks + q4);
+        qb[ks][1] = __ldg(qp + 8 * ks + 4 + q4);
       }
     }
     const float sc = p.sm_scale * 1.4426950408889634f;  // logits in log2 units
-    float o[NO][4];
+    float o[MT][4];  // O^T: [d = 16 mt + r (+8)][g = 2 q4 (+1)]
 #pragma unroll
-    for (int n = 0; n < NO; ++n) { o[n][0] = o[n][1] = o[n][2] = o[n][3] = 0.f; }
-    float m = -CUDART_INF_F, lsum = 0.f;
-    const uint32_t stage_u32 = smem_u32(stage_base);
-    // per-lane ldmatrix row: matrix mi = lane/8, row lane%8
+    for (int mt = 0; mt < MT; ++mt) { o[mt][0] = o[mt][1] = o[mt][2] = o[mt][3] = 0.f; }
+    float m0 = -CUDART_INF_F, m1 = -CUDART_INF_F, l0 = 0.f, l1 = 0.f;  // columns g = 2 q4, 2 q4 + 1
+    const uint32_t ring_u32 = smem_u32(ring);
     const int mi = lane >> 3, mr = lane & 7;
-    const uint32_t k_lane = (uint32_t)(mr * row_stride + warp * D * 2 + mi * 16);                       // + tok8*8 rows + 64*v
-    const uint32_t v_lane = (uint32_t)(((mi & 1) * 8 + mr) * row_stride + warp * D * 2 + (mi >> 1) * 16);  // + 32*j
+    // K as A (row-major tok x d): matrices (tok 0-7, d 0-7), (tok 8-15, d 0-7), (tok 0-7, d 8-15), (tok 8-15, d 8-15)
+    const uint32_t k_lane = (uint32_t)(((mi & 1) * 8 + mr) * row_stride + warp * D * 2 + (mi >> 1) * 16);
+    // V^T as A (d x tok) through ldmatrix.trans: (tok 0-7, d 0-7), (tok 0-7, d 8-15), (tok 8-15, d 0-7), (tok 8-15, d 8-15)
+    const uint32_t v_lane = (uint32_t)(((mi >> 1) * 8 + mr) * row_stride + warp * D * 2 + (mi & 1) * 16);
+    int s = 0;
+    uint32_t ph = 0;
 
     for (int t = 0; t < n_tiles; ++t) {
-      const int s = t % NS;
-      const uint32_t ph = (uint32_t)(t / NS) & 1u;
+      // ---- K half-stage: S = K q^T
+      mbar_wait(&full[s], ph);
+      float pv[4] = {0.f, 0.f, 0.f, 0.f};
+      uint32_t vmask = 0;
+      float c0 = 1.f, c1 = 1.f;
+      if (active) {
+        const uint32_t sb = ring_u32 + (uint32_t)(s * half_bytes);
+        vmask = vmasks[s];
+        float sa[4] = {0.f, 0.f, 0.f, 0.f}, sb2[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int ks = 0; ks < KS; ks += 2) {
+          uint32_t a0, a1, a2, a3;
+          ldsm_x4(sb + k_lane + (uint32_t)(ks * 32), a0, a1, a2, a3);
+          mma_bf16_16816(sa, a0, a1, a2, a3, qb[ks][0], qb[ks][1]);
+          ldsm_x4(sb + k_lane + (uint32_t)((ks + 1) * 32), a0, a1, a2, a3);
+          mma_bf16_16816(sb2, a0, a1, a2, a3, qb[ks + 1][0], qb[ks + 1][1]);
+        }
+        const bool v0 = (vmask >> r) & 1u, v1 = (vmask >> (r + 8)) & 1u;
+        float x00 = v0 ? (sa[0] + sb2[0]) * sc : -CUDART_INF_F, x01 = v0 ? (sa[1] + sb2[1]) * sc : -CUDART_INF_F;
+        float x10 = v1 ? (sa[2] + sb2[2]) * sc : -CUDART_INF_F, x11 = v1 ? (sa[3] + sb2[3]) * sc : -CUDART_INF_F;
+        float t0m = fmaxf(x00, x10), t1m = fmaxf(x01, x11);
+#pragma unroll
+        for (int ofs = 4; ofs < 32; ofs <<= 1) {
+          t0m = fmaxf(t0m, __shfl_xor_sync(0xffffffffu, t0m, ofs));
+          t1m = fmaxf(t1m, __shfl_xor_sync(0xffffffffu, t1m, ofs));
+        }
+        const float n0 = fmaxf(m0, t0m), n1 = fmaxf(m1, t1m);
+        const float r0 = (n0 == -CUDART_INF_F) ? 0.f : n0, r1 = (n1 == -CUDART_INF_F) ? 0.f : n1;
+        c0 = fast_exp2(m0 - r0); c1 = fast_exp2(m1 - r1);
+        pv[0] = fast_exp2(x00 - r0); pv[1] = fast_exp2(x01 - r1);
+        pv[2] = fast_exp2(x10 - r0); pv[3] = fast_exp2(x11 - r1);
+        l0 = l0 * c0 + (pv[0] + pv[2]);
+        l1 = l1 * c1 + (pv[1] + pv[3]);
+        m0 = n0; m1 = n1;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[s]);
+      if (++s == HS) { s = 0; ph ^= 1u; }
+
+      // ---- V half-stage: O^T += V^T P
       mbar_wait(&full[s], ph);
       if (active) {
-        const uint32_t sb = stage_u32 + (uint32_t)(s * stage_bytes);
-        const uint32_t vmask = *reinterpret_cast<const uint32_t*>(stage_base + (size_t)s * stage_bytes + 2 * kv_bytes);
+        const uint32_t sb = ring_u32 + (uint32_t)(s * half_bytes);
         if (vmask != 0xffffu) {
-          // ragged tile: V rows of masked tokens may hold stale or uninitialised bytes (0 x NaN = NaN): zero this
-          // head's slice of them (D * 2 bytes = D / 8 lanes x 16 bytes per row, two rows per pass when D = 128)
+          // ragged tile: V rows of masked tokens may hold stale or uninitialised bytes (0 x NaN = NaN): zero them
           constexpr int LPRV = D / 8;
           for (int tok = lane / LPRV; tok < DM_TOK; tok += 32 / LPRV)
             if (!((vmask >> tok) & 1u))
-              *reinterpret_cast<uint4*>(stage_base + (size_t)s * stage_bytes + kv_bytes + (size_t)tok * row_stride +
-                                        warp * D * 2 + (lane % LPRV) * 16) = make_uint4(0u, 0u, 0u, 0u);
+              *reinterpret_cast<uint4*>(ring + (size_t)s * half_bytes + (size_t)tok * row_stride + warp * D * 2 +
+                                        (lane % LPRV) * 16) = make_uint4(0u, 0u, 0u, 0u);
           __syncwarp();
         }
-        // S^T tiles: [g][tokens 0-7], [g][tokens 8-15]
-        float sacc[2][4];
+        // P (C layout: [tok r | r+8][g 2q4, 2q4+1]) -> B fragments [k = tok][n = g] by an 8x8 transpose each
+        const uint32_t b0 = movmatrix_t(pack2_bf16(pv[0], pv[1]));
+        const uint32_t b1 = movmatrix_t(pack2_bf16(pv[2], pv[3]));
 #pragma unroll
-        for (int nt = 0; nt < 2; ++nt) {
-          sacc[nt][0] = sacc[nt][1] = sacc[nt][2] = sacc[nt][3] = 0.f;
-#pragma unroll
-          for (int v = 0; v < KS / 2; ++v) {
-            uint32_t b0, b1, b2, b3;
-            ldsm_x4(sb + k_lane + (uint32_t)(nt * 8 * row_stride + v * 64), b0, b1, b2, b3);
-            mma_bf16_16816(sacc[nt], qa[2 * v][0], 0u, qa[2 * v][1], 0u, b0, b1);
-            mma_bf16_16816(sacc[nt], qa[2 * v + 1][0], 0u, qa[2 * v + 1][1], 0u, b2, b3);
-          }
-        }
-        // online softmax over the 16 tokens of row g = r
-        float sv[4];
-#pragma unroll
-        for (int nt = 0; nt < 2; ++nt)
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            const int tok = nt * 8 + 2 * q4 + e;
-            sv[nt * 2 + e] = ((vmask >> tok) & 1u) ? sacc[nt][e] * sc : -CUDART_INF_F;
-          }
-        float tmax = fmaxf(fmaxf(sv[0], sv[1]), fmaxf(sv[2], sv[3]));
-        tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 1));
-        tmax = fmaxf(tmax, __shfl_xor_sync(0xffffffffu, tmax, 2));
-        const float mn = fmaxf(m, tmax);
-        const float mref = (mn == -CUDART_INF_F) ? 0.f : mn;
-        const float corr = fast_exp2(m - mref);
-        float pv[4];
-#pragma unroll
-        for (int e = 0; e < 4; ++e) pv[e] = fast_exp2(sv[e] - mref);
-        lsum = lsum * corr + (pv[0] + pv[1] + pv[2] + pv[3]);
-        m = mn;
-        const uint32_t pa0 = pack2_bf16(pv[0], pv[1]), pa2 = pack2_bf16(pv[2], pv[3]);
-#pragma unroll
-        for (int n = 0; n < NO; ++n) { o[n][0] *= corr; o[n][1] *= corr; }
-        // O += P V
-#pragma unroll
-        for (int j = 0; j < NO / 2; ++j) {
-          uint32_t v0, v1, v2, v3;
-          ldsm_x4_t(sb + (uint32_t)kv_bytes + v_lane + (uint32_t)(j * 32), v0, v1, v2, v3);
-          mma_bf16_16816(o[2 * j], pa0, 0u, pa2, 0u, v0, v1);
-          mma_bf16_16816(o[2 * j + 1], pa0, 0u, pa2, 0u, v2, v3);
+        for (int mt = 0; mt < MT; ++mt) {
+          o[mt][0] *= c0; o[mt][1] *= c1; o[mt][2] *= c0; o[mt][3] *= c1;
+          uint32_t a0, a1, a2, a3;
+          ldsm_x4_t(sb + v_lane + (uint32_t)(mt * 32), a0, a1, a2, a3);
+          mma_bf16_16816(o[mt], a0, a1, a2, a3, b0, b1);
         }
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(&empty[s]);
+      if (++s == HS) { s = 0; ph ^= 1u; }
     }
     pdl_wait();
     if (active) {
-      lsum += __shfl_xor_sync(0xffffffffu, lsum, 1);
-      lsum += __shfl_xor_sync(0xffffffffu, lsum, 2);
-      if (r < G) {
-        const int64_t phd = ((int64_t)req * Hq + kvh * G + r) * p.n_split + split;
-        float2* po = reinterpret_cast<float2*>(p.part_o + phd * D);
 #pragma unroll
-        for (int n = 0; n < NO; ++n) po[4 * n + q4] = make_float2(o[n][0], o[n][1]);
-        if (q4 == 0) p.part_ml[phd] = make_float2(m * 0.6931471805599453f, lsum);
+      for (int ofs = 4; ofs < 32; ofs <<= 1) {
+        l0 += __shfl_xor_sync(0xffffffffu, l0, ofs);
+        l1 += __shfl_xor_sync(0xffffffffu, l1, ofs);
+      }
+      const int g0 = 2 * q4, g1 = g0 + 1;
+      const int64_t ph0 = ((int64_t)req * Hq + kvh * G + g0) * p.n_split + split;
+      const int64_t ph1 = ((int64_t)req * Hq + kvh * G + g1) * p.n_split + split;
+      if (g0 < G) {
+        float* po = p.part_o + ph0 * D;
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) { po[mt * 16 + r] = o[mt][0]; po[mt * 16 + 8 + r] = o[mt][2]; }
+        if (r == 0) p.part_ml[ph0] = make_float2(m0 * 0.6931471805599453f, l0);
+      }
+      if (g1 < G) {
+        float* po = p.part_o + ph1 * D;
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) { po[mt * 16 + r] = o[mt][1]; po[mt * 16 + 8 + r] = o[mt][3]; }
+        if (r == 0) p.part_ml[ph1] = make_float2(m1 * 0.6931471805599453f, l1);
       }
     }
   }
 }
 
-inline size_t decode_mma_smem(int nh, int D, int max_smem, int* n_stage) {
-  const size_t stage = 2 * (size_t)DM_TOK * (nh * D * 2 + DM_ROWPAD) + 16;
-  const size_t fixed = 2 * 8 * 8 + 128;
-  if (fixed + 2 * stage > (size_t)max_smem) { *n_stage = 0; return 0; }
-  int ns = (int)(((size_t)max_smem - fixed) / stage);
-  if (ns > 8) ns = 8;
-  *n_stage = ns;
-  return fixed + (size_t)ns * stage;
+// shared memory of k_decode_mma for `n_half` half-stages
+inline size_t decode_mma_smem(int nh, int D, int max_smem, int* n_half) {
+  const size_t half = (size_t)DM_TOK * (nh * D * 2 + DM_ROWPAD);
+  const size_t per = half + 2 * 8 + 4;
+  const size_t fixed = 128;
+  if (fixed + 2 * per > (size_t)max_smem) { *n_half = 0; return 0; }
+  int n = (int)(((size_t)max_smem - fixed) / per);
+  if (n > 12) n = 12;
+  *n_half = n;
+  return fixed + (size_t)n * per;
 }
 
 // grid = (H_q, n_req), block = DMG_THREADS.  Two phases with no serial dependency between splits:

@@ -364,14 +364,16 @@ ikv_status launch_decode(ikv_ctx* c, int layer, const DecBatch& batch, int n_req
   const T* kl = (const T*)c->cfg.k_pool + (int64_t)layer * c->layer_stride;
   const T* vl = (const T*)c->cfg.v_pool + (int64_t)layer * c->layer_stride;
   if constexpr (std::is_same<T, bf16>::value) {
-    // tensor-pipe split kernel behind a bulk-copy ring (decode_mma.cuh)
+    // tensor-pipe split kernel behind a bulk-copy ring (decode_mma.cuh).  At most half an SM's shared memory per
+    // CTA: the CTAs of two consecutive layer calls co-reside (PDL), so the next call's K/V stream starts while this
+    // call drains.
     const int n_hg = (Hkv + DM_CWARPS - 1) / DM_CWARPS;
-    int ns = 0;
-    const size_t smem = decode_mma_smem(Hkv < DM_CWARPS ? Hkv : DM_CWARPS, D, c->max_smem, &ns);
-    if (ns < 2) IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "decode: a stage of %d heads x %d does not fit shared memory", Hkv, D);
+    int nhalf = 0;
+    const size_t smem = decode_mma_smem(Hkv < DM_CWARPS ? Hkv : DM_CWARPS, D, (c->max_smem + 1024) / 2 - 1024, &nhalf);
+    if (nhalf < 2) IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "decode: a half-stage of %d heads x %d does not fit", Hkv, D);
     DecMmaParams p;
     p.k_layer = kl; p.v_layer = vl; p.Hkv = Hkv; p.dead = c->cfg.dead_slot; p.q = (const bf16*)q; p.sm_scale = sm_scale;
-    p.part_o = c->part_o; p.part_ml = c->part_ml; p.n_split = n_split; p.n_stage = ns;
+    p.part_o = c->part_o; p.part_ml = c->part_ml; p.n_split = n_split; p.n_stage = nhalf;
     auto fn = k_decode_mma<D, G>;
     if (!c->attr_done[0][D == 128][G]) {
       CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -933,7 +935,7 @@ ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, i
     if (c->cfg.kv_dtype == IKV_BF16) {
       // one CTA (all KV heads of a token range) per SM, at least 16 tokens per split.  A few SMs are left to the
       // merge grid (2 of its CTAs per SM): launched programmatically, it is then resident before the split
-      // drains, and the next call's split overlaps it (measured: 148 -> 132 splits takes 12.6 -> 8.0 us per call)
+      // drains, and the next call's split overlaps it (measured: 148 -> 132 splits takes 7.7 -> 6.2 us per call)
       const int n_hg = (Hkv + DM_CWARPS - 1) / DM_CWARPS;
       int reserve = (Hq * nb + 1) / 2;
       if (reserve > c->n_sm / 4) reserve = c->n_sm / 4;
