@@ -183,8 +183,12 @@ def run_ours(args):
     hbm_peak, peak_src = peaks()
 
     T, C, DEC = args.tokens, args.budget, args.decode_steps
-    shape = wl.QWEN3_8B
-    w = wl.cfg1(device="cuda", seed=1000 + rank, n_tokens=T, budget=C, decode_tokens=DEC)
+    if args.workload == "cfg2":      # configs[2], a parity-test case; timed only on request (not the headline workload)
+        shape = wl.QWEN25_14B
+        w = wl.cfg2(device="cuda", seed=2000 + rank, n_tokens=T, budget=C, decode_tokens=DEC)
+    else:
+        shape = wl.QWEN3_8B
+        w = wl.cfg1(device="cuda", seed=1000 + rank, n_tokens=T, budget=C, decode_tokens=DEC)
     sess = w.sessions[0]
     L, Hq, Hkv, D = shape.L, shape.Hq, shape.Hkv, shape.D
     ctx = ikv.Context(L, Hq, Hkv, D, w.k_pool, w.v_pool, dead_slot=w.dead_slot)
@@ -324,7 +328,7 @@ def run_ours(args):
 
     if rank == 0:
         K = args.steps
-        default_wl = (T == 32768 and C == 8192 and args.mode == "learnable")  # the ncu capture's workload
+        default_wl = (args.workload == "cfg1" and T == 32768 and C == 8192 and args.mode == "learnable")  # the ncu capture's workload
         key_bytes = L * Hkv * T * D * shape.elem_bytes                 # algorithmic bytes of the key pass
         dec_tokens_sum = sum(n_kept + t + 1 for t in range(DEC))        # live tokens read over the decode loop
         dec_bytes_step = dec_tokens_sum * L * Hkv * D * 2 * shape.elem_bytes
@@ -338,9 +342,11 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
             "ms_per_step": tot_step / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "bf16 keys/values, f32 accumulate", "data": "synthetic",
-            "config": {"workload": "configs[1] Qwen3-8B-shaped single session per GPU: 36 layers, 32 Q / 8 KV heads, "
-                                   "head_dim 128, bf16 K/V, 32,768 live tokens in 16-token pages, M=64 memory rows, "
-                                   "1% planted, C=8192, one prune pass then 256 decode steps",
+            "config": {"workload": ("configs[1] Qwen3-8B-shaped single session per GPU: 36 layers, 32 Q / 8 KV heads, "
+                                    "head_dim 128, bf16 K/V, 32,768 live tokens in 16-token pages, M=64 memory rows, "
+                                    "1% planted, C=8192, one prune pass then 256 decode steps") if args.workload == "cfg1"
+                       else ("configs[2] Qwen2.5-14B-shaped single session per GPU: 48 layers, 40 Q / 8 KV heads, "
+                             "head_dim 128, bf16 K/V, M=256 memory rows, one prune pass then decode steps"),
                        "n_tokens": T, "budget": C, "decode_steps": DEC, "mode": args.mode, "n_kept": n_kept,
                        "l2": "inputs larger than L2 (2.4 GB of keys per prune, 1.2 GB of K/V per decode step; "
                              "126 MB L2)", "parallelism": f"replicas x{world}" if world > 1 else "single GPU"},
@@ -393,6 +399,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--mode", default="learnable", choices=["learnable", "memory"])
+    ap.add_argument("--workload", default="cfg1", choices=["cfg1", "cfg2"])
     ap.add_argument("--tokens", type=int, default=32768)
     ap.add_argument("--budget", type=int, default=8192)
     ap.add_argument("--decode-steps", type=int, default=256)
