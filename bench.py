@@ -53,6 +53,22 @@ def ncu_traffic(kernel):
     return sum(vals) / len(vals) if vals else None
 
 
+def max_over_ranks(times_ms, world, device):
+    """Replicas-only multi-GPU (DESIGN.md section 2, 8(e)): no data-path collective; the only exchange is this MAX of
+    the device-timed milliseconds, so that `value` = units of all ranks / slowest rank's time."""
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return tt.tolist()
+
+
+def whole_job_value(units_per_rank, world, steps, total_ms):
+    """Weak scaling: every rank processes `units_per_rank` per step; total_ms is the max-over-ranks time of `steps`."""
+    return world * units_per_rank * steps / (total_ms * 1e-3)
+
+
 class ClockSampler:
     """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -321,10 +337,7 @@ def run_ours(args):
     p1_ms = statistics.median(p1[3:])
 
     # ---- max over ranks
-    tt = torch.tensor([tot_prune, tot_dec, tot_step, e2e_total * 1e3], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    tot_prune, tot_dec, tot_step, e2e_ms_total = tt.tolist()
+    tot_prune, tot_dec, tot_step, e2e_ms_total = max_over_ranks([tot_prune, tot_dec, tot_step, e2e_total * 1e3], world, dev)
 
     if rank == 0:
         K = args.steps
@@ -332,7 +345,7 @@ def run_ours(args):
         key_bytes = L * Hkv * T * D * shape.elem_bytes                 # algorithmic bytes of the key pass
         dec_tokens_sum = sum(n_kept + t + 1 for t in range(DEC))        # live tokens read over the decode loop
         dec_bytes_step = dec_tokens_sum * L * Hkv * D * 2 * shape.elem_bytes
-        value = world * T * K / (tot_prune * 1e-3)
+        value = whole_job_value(T, world, K, tot_prune)
         logits_ms = prof["score_logits_ms"] / max(1, prof["score_logits_n"])
         ach = key_bytes / (logits_ms * 1e-3) / 1e9 if logits_ms > 0 else 0.0
         dec_kernel_ms = tot_dec / K / (DEC * L)                         # split + merge + launch gap per layer call
