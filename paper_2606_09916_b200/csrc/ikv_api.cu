@@ -444,11 +444,11 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
   if (kbar) {
     auto fn = k_key_pass<D, G, true>;
     CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    fn<<<grid, KP_THREADS, smem, st>>>(p);
+    fn<<<grid, kp_threads(G, true), smem, st>>>(p);
   } else {
     auto fn = k_key_pass<D, G, false>;
     CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    fn<<<grid, KP_THREADS, smem, st>>>(p);
+    fn<<<grid, kp_threads(G, false), smem, st>>>(p);
   }
   LAUNCH_CHECK(c);
   *n_part = grid;

@@ -24,7 +24,12 @@ namespace ikv {
 constexpr int KP_TOK = 32;       // tokens per stage = two m16 tiles of the mma
 constexpr int KP_LWARPS = 8;     // logit warps
 constexpr int KP_KWARPS = 4;     // mean-key warps
-constexpr int KP_THREADS = (KP_LWARPS + KP_KWARPS + 1) * 32;
+// G <= 4: a producer warp of its own (13 warps, 128 registers per thread).  G > 4 with mean keys: the two-tile B
+// fragments need more registers than a 13-warp CTA leaves, so the first mean-key warp also produces (12 warps, 170
+// registers); measured at configs[2]: 2.38 -> 1.98 ms.  (At G = 4 the shared producer costs 20 %: it refills a slot only
+// between its own stages.)
+__host__ __device__ constexpr bool kp_merged(int G, bool kbar) { return kbar && G > 4; }
+__host__ __device__ constexpr int kp_threads(int G, bool kbar) { return (KP_LWARPS + KP_KWARPS + (kp_merged(G, kbar) ? 0 : 1)) * 32; }
 constexpr int KP_ROWPAD = 64;    // bytes added to each staged token row (bank spread for the 16-byte reads)
 
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
@@ -93,10 +98,13 @@ struct KeyPassParams {
 };
 
 // Warp roles of k_key_pass: warps [0, KP_LWARPS) logit warps, [KP_LWARPS, KP_LWARPS + KP_KWARPS) mean-key warps
-// (KBAR only; warp (dq, th) owns the d-quarter dq of the token part th), last warp producer.
+// (KBAR only; warp (dq, th) owns the d-quarter dq of the token part th).  Producer: a warp of its own, or the first
+// mean-key warp (kp_merged).
 template <int D, int G, bool KBAR>
-__global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams p) {
+__global__ __launch_bounds__(kp_threads(G, KBAR), 1) void k_key_pass(const KeyPassParams p) {
   constexpr int KS = D / 16, NI = D / 32, NT = (G <= 4) ? 1 : 2;
+  constexpr bool MERGED = kp_merged(G, KBAR);
+  constexpr int KP_THREADS = kp_threads(G, KBAR);
   const int L = p.L, Hkv = p.Hkv, Hq = Hkv * G;
   const int row_bytes = Hkv * D * 2;
   const int row_stride = row_bytes + KP_ROWPAD;
@@ -122,8 +130,8 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
   }
   __syncthreads();
 
-  if (warp == KP_LWARPS + KP_KWARPS) {
-    // ------------------------------------------------------------------ producer
+  if (!MERGED && warp == KP_LWARPS + KP_KWARPS) {
+    // ------------------------------------------------------------------ producer (a warp of its own)
     int s = 0;
     uint32_t ph = 0;
     for (int tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
@@ -270,17 +278,61 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
         if (++s == NS) { s = 0; ph ^= 1u; }
       }
     }
-  } else if (KBAR) {
-    // ------------------------------------------------------------------ mean-key warps (Eq. 5)
+  } else if (KBAR && warp < KP_LWARPS + KP_KWARPS) {
+    // ------------------------------------------------------------------ mean-key warps (Eq. 5).  MERGED: the first one
+    // also produces: it tops the ring up (non-blocking test of the slot's empty barrier) before every stage it consumes,
+    // and blocks on a slot only when nothing it issued is left for it to consume.
     constexpr int CH = D / 32;                 // 16-byte chunks per token in a d-quarter
     constexpr int TPL = 32 / CH;               // tokens per warp load
     constexpr int ROWS = KP_TOK / (KP_KWARPS / 4);
     constexpr int NG = ROWS / TPL;             // token groups per warp
     const int kw = warp - KP_LWARPS, dq = kw & 3, th = kw >> 2;
+    const bool prod = MERGED && (kw == 0);
     const int tl = lane / CH, ch = lane % CH;
     const uint32_t stage_u32 = smem_u32(stage_base);
     const uint32_t lane_off = (uint32_t)((th * ROWS + tl) * row_stride + dq * (D / 4) * 2 + ch * 16);
     const float inv = 1.f / (float)(L * Hkv);
+    // producer state
+    const int my_tiles = (tiles > (int)blockIdx.x) ? (tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    const int total_stages = my_tiles * L;
+    int issued = 0, consumed = 0, p_tile = blockIdx.x, p_l = 0, p_s = 0;
+    uint32_t p_ph = 0;
+    auto slot_of_tile = [&](int tile) -> int64_t {
+      if (tile >= tiles) return 0;
+      const bool tx = tile >= tiles_c;
+      const int t0 = (tx ? tile - tiles_c : tile) * KP_TOK;
+      const int nv = min(KP_TOK, (tx ? nx : nc) - t0);
+      return (lane < nv) ? (int64_t)(tx ? p.xq_slot[t0 + lane] : p.cand_slot[t0 + lane]) : 0;
+    };
+    int64_t p_slot = 0, p_slot_next = 0;
+    if (prod) { p_slot = slot_of_tile(p_tile); p_slot_next = slot_of_tile(p_tile + gridDim.x); }
+    auto try_issue = [&](bool block) -> bool {
+      if (issued >= total_stages || issued - consumed >= NS) return false;
+      uint32_t ok = 1u;
+      if (lane == 0) {
+        if (block) mbar_wait(&empty[p_s], p_ph ^ 1u);
+        else ok = mbar_test_wait(&empty[p_s], p_ph ^ 1u) ? 1u : 0u;
+      }
+      ok = __shfl_sync(0xffffffffu, ok, 0);
+      if (!ok) return false;
+      const bool tx = p_tile >= tiles_c;
+      const int t0 = (tx ? p_tile - tiles_c : p_tile) * KP_TOK;
+      const int nv = min(KP_TOK, (tx ? nx : nc) - t0);
+      if (lane == 0) mbar_arrive_expect_tx(&full[p_s], (uint32_t)(nv * row_bytes));
+      __syncwarp();
+      if (lane < nv)
+        bulk_g2s(stage_base + (size_t)p_s * stage_bytes + lane * row_stride,
+                 p.k_pool + p_slot * (int64_t)(Hkv * D) + (int64_t)p_l * p.layer_stride, (uint32_t)row_bytes, &full[p_s]);
+      if (++p_l == L) {
+        p_l = 0;
+        p_tile += gridDim.x;
+        p_slot = p_slot_next;
+        p_slot_next = slot_of_tile(p_tile + gridDim.x);
+      }
+      if (++p_s == NS) { p_s = 0; p_ph ^= 1u; }
+      ++issued;
+      return true;
+    };
     int s = 0;
     uint32_t ph = 0;
     for (int tile = blockIdx.x; tile < tiles; tile += gridDim.x) {
@@ -293,6 +345,11 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
 #pragma unroll
         for (int e = 0; e < 8; ++e) kb[gI][e] = 0.f;
       for (int l = 0; l < L; ++l) {
+        if (prod) {
+          while (try_issue(false)) {
+          }
+          if (issued == consumed) try_issue(true);
+        }
         mbar_wait(&full[s], ph);
         const uint32_t sb = stage_u32 + (uint32_t)(s * stage_bytes) + lane_off;
 #pragma unroll 4
@@ -309,6 +366,7 @@ __global__ __launch_bounds__(KP_THREADS, 1) void k_key_pass(const KeyPassParams 
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[s]);
         if (++s == NS) { s = 0; ph ^= 1u; }
+        ++consumed;
       }
       float* outp = is_x ? p.kq : p.kbar;
 #pragma unroll
