@@ -12,6 +12,7 @@ struct DecReq {
   const int32_t* live_slots;  // compact survivor list covering positions [0, covered)
   const int32_t* n_live;      // its length (device scalar)
   int seq_len, covered;
+  int n_split;                // splits of this request (<= the launch's n_split, which is the scratch stride)
   int n_items;                // host-side upper bound of the list length; entries past *n_live hold the dead slot
 };
 struct DecBatch {

@@ -99,9 +99,10 @@ __global__ __launch_bounds__(DM_THREADS, 2) void k_decode_mma(const DecMmaParams
   const DecReq rq = batch.r[req];
   const int n_cached = rq.n_items;
   const int total = n_cached + (rq.seq_len - rq.covered);
+  if (split >= rq.n_split) return;  // requests of a batch get splits in proportion to their length
   const int n_gran = (total + DM_GRAN - 1) / DM_GRAN;
-  const int begin = (int)(((int64_t)n_gran * split) / p.n_split) * DM_GRAN;
-  const int end = min(total, (int)(((int64_t)n_gran * (split + 1)) / p.n_split) * DM_GRAN);
+  const int begin = (int)(((int64_t)n_gran * split) / rq.n_split) * DM_GRAN;
+  const int end = min(total, (int)(((int64_t)n_gran * (split + 1)) / rq.n_split) * DM_GRAN);
   const int n_tiles = (end > begin) ? (end - begin + DM_TOK - 1) / DM_TOK : 0;
 
   if (warp == DM_CWARPS) {
@@ -283,15 +284,16 @@ constexpr int DMG_THREADS = 512;
 constexpr int DMG_MAX_SPLIT = 1024;
 template <typename T, int D>
 __global__ __launch_bounds__(DMG_THREADS) void k_decode_merge4(const float* __restrict__ part_o,
-                                                               const float2* __restrict__ part_ml, int n_split,
-                                                               T* __restrict__ out) {
+                                                               const float2* __restrict__ part_ml, int stride,
+                                                               const DecBatch batch, T* __restrict__ out) {
   constexpr int NG = DMG_THREADS / D;
   __shared__ float ws[DMG_MAX_SPLIT];
   __shared__ float red[DMG_THREADS / 32];
   __shared__ float acc_s[NG][D];
   pdl_launch_dependents();
   pdl_wait();
-  const int64_t ph = ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * n_split;
+  const int64_t ph = ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * stride;
+  const int n_split = batch.r[blockIdx.y].n_split;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   float2 ml[DMG_MAX_SPLIT / DMG_THREADS];
   float mx = -CUDART_INF_F;

@@ -395,7 +395,7 @@ ikv_status launch_decode(ikv_ctx* c, int layer, const DecBatch& batch, int n_req
     LAUNCH_CHECK(c);
   }
   CU(c, launch_pdl(k_decode_merge4<T, D>, dim3(Hq, n_req), dim3(DMG_THREADS), 0, st, c->use_pdl, (const float*)c->part_o,
-                   (const float2*)c->part_ml, n_split, (T*)out));
+                   (const float2*)c->part_ml, n_split, batch, (T*)out));
   return IKV_OK;
 }
 
@@ -907,6 +907,7 @@ ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, i
     const int nb = (n_req - r0 < DEC_MAX_REQ) ? n_req - r0 : DEC_MAX_REQ;
     DecBatch batch;
     int max_items = 1;
+    int items_of[DEC_MAX_REQ];
     for (int i = 0; i < nb; ++i) {
       const ikv_request& r = reqs[r0 + i];
       if (r.seq_len < 0 || (r.seq_len > 0 && !r.slot_map)) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "bad request %d", r0 + i);
@@ -929,27 +930,40 @@ ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, i
       batch.r[i].covered = s->covered;
       batch.r[i].n_items = s->live_ub;
       const int items = s->live_ub + (r.seq_len - s->covered);
+      items_of[i] = items;
       if (items > max_items) max_items = items;
     }
     int n_split;
     if (c->cfg.kv_dtype == IKV_BF16) {
-      // one CTA (all KV heads of a token range) per SM, at least 16 tokens per split.  A few SMs are left to the
-      // merge grid (2 of its CTAs per SM): launched programmatically, it is then resident before the split
-      // drains, and the next call's split overlaps it (measured: 148 -> 132 splits takes 7.7 -> 6.2 us per call)
+      // One request: one CTA (all KV heads of a token range) per SM, minus a few SMs left to the merge grid (2 of its
+      // CTAs per SM): launched programmatically, it is then resident before the split drains, and the next call's
+      // split overlaps it (measured: 148 -> 132 splits takes 7.7 -> 6.2 us per call).  A batch: two CTAs per SM, and
+      // every request gets splits in proportion to its length (at least 16 tokens per split).
       const int n_hg = (Hkv + DM_CWARPS - 1) / DM_CWARPS;
       int reserve = (Hq * nb + 1) / 2;
       if (reserve > c->n_sm / 4) reserve = c->n_sm / 4;
-      n_split = (c->n_sm - reserve) / (nb * n_hg);
-      const int by_len = (max_items + 15) / 16;
-      if (n_split > by_len) n_split = by_len;
+      const int cap = ((nb == 1 ? 1 : 2) * c->n_sm - reserve) / n_hg;
+      int64_t tot_items = 0;
+      for (int i = 0; i < nb; ++i) tot_items += items_of[i] > 0 ? items_of[i] : 1;
+      n_split = 1;
+      for (int i = 0; i < nb; ++i) {
+        int ns = (int)(((int64_t)(items_of[i] > 0 ? items_of[i] : 1) * cap) / tot_items);  // its share of the CTAs
+        const int by_len = (items_of[i] + 15) / 16;
+        if (ns > by_len) ns = by_len;
+        if (ns < 1) ns = 1;
+        if (ns > DMG_MAX_SPLIT) ns = DMG_MAX_SPLIT;
+        batch.r[i].n_split = ns;
+        if (ns > n_split) n_split = ns;
+      }
     } else {
       // ~4 CTAs per SM, at least 64 tokens per split
       n_split = (4 * c->n_sm + Hkv * nb - 1) / (Hkv * nb);
       const int by_len = (max_items + 63) / 64;
       if (n_split > by_len) n_split = by_len;
+      if (n_split < 1) n_split = 1;
+      if (n_split > DMG_MAX_SPLIT) n_split = DMG_MAX_SPLIT;
+      for (int i = 0; i < nb; ++i) batch.r[i].n_split = n_split;
     }
-    if (n_split < 1) n_split = 1;
-    if (n_split > DMG_MAX_SPLIT) n_split = DMG_MAX_SPLIT;
     TRY(ensure_parts(c, (int64_t)nb * Hq * n_split));
     TRY(dispatch_decode(c, layer, batch, nb, n_split, (const char*)q + (size_t)r0 * Hq * D * esz,
                         (char*)out + (size_t)r0 * Hq * D * esz, sm_scale, st));
