@@ -175,7 +175,9 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_mean * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "configs[1] Qwen3-8B-shaped single session, 32,768 live tokens, C=8192",
+            "config": {"workload": "configs[1] Qwen3-8B-shaped single session per GPU: 36 layers, 32 Q / 8 KV heads, "
+                                   "head_dim 128, bf16 K/V, 32,768 live tokens in 16-token pages, M=64 memory rows, "
+                                   "1% planted, C=8192, one prune pass then 256 decode steps",
                        "n_tokens": sess.N, "budget": sess.spec.budget, "mode": "learnable"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
