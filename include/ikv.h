@@ -158,7 +158,7 @@ ikv_status ikv_prune_host(ikv_ctx *ctx, const ikv_request *req, const float *q_r
                           int32_t *freed_host, int32_t *n_freed_host, int32_t *n_kept_host, void *stream);
 
 /* Kernel-level timing for bench.py's roofline: while enabled, the library brackets its two dominant kernels
- * (the key pass k_score_logits and the decode kernel k_decode_split) with CUDA events on the caller's stream
+ * (the key pass k_key_pass / k_score_logits and the decode split kernel k_decode_mma / k_decode_split) with CUDA events on the caller's stream
  * (no host synchronisation; not allowed during stream capture).  ikv_profile_read synchronises, sums the
  * elapsed times recorded since the last read and clears them.
  * out_ms[0] = key-pass total ms, out_ms[1] = decode-split total ms; out_n[0], out_n[1] = launch counts. */

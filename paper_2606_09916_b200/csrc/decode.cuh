@@ -143,25 +143,4 @@ __global__ __launch_bounds__(128) void k_decode_split(const T* __restrict__ k_la
   }
 }
 
-// grid = (H_q, n_req), block = D.  out = sum_s w_s o_s / sum_s w_s l_s, w_s = exp(m_s - max m).
-template <typename T, int D>
-__global__ void k_decode_merge(const float* __restrict__ part_o, const float2* __restrict__ part_ml, int n_split,
-                               T* __restrict__ out) {
-  const int64_t ph = ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * n_split;
-  const int d = threadIdx.x;
-  float mx = -CUDART_INF_F;
-  for (int s = 0; s < n_split; ++s) mx = fmaxf(mx, part_ml[ph + s].x);
-  float acc = 0.f, den = 0.f;
-  if (mx > -CUDART_INF_F) {
-    for (int s = 0; s < n_split; ++s) {
-      const float2 ml = part_ml[ph + s];
-      const float w = __expf(ml.x - mx);
-      acc = fmaf(w, part_o[(ph + s) * D + d], acc);
-      den = fmaf(w, ml.y, den);
-    }
-  }
-  const float r = (den > 0.f) ? acc / den : 0.f;
-  out[((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * D + d] = (T)r;
-}
-
 }  // namespace ikv

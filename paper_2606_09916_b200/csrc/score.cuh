@@ -195,26 +195,6 @@ __device__ __forceinline__ void score_lse_block(int row, const float2* __restric
   if (threadIdx.x == 0) lse[row] = mx + logf(red[0] + red[1] + red[2] + red[3]);
 }
 
-// a3  rule_c = sum_{l,h} exp(x[l,h,c] - lse[l,h])   (Eq. 3).  One thread per candidate.
-// Writes rule_c[c]; scatters to scores[pos] (when `scatter_scores`) and rule_out[pos].
-__global__ void k_score_rule(const float* __restrict__ logits, int64_t ldc, int LH, const float* __restrict__ lse,
-                             const int32_t* __restrict__ n_cand_p, const int32_t* __restrict__ cand_pos,
-                             float* __restrict__ rule_c, float* __restrict__ scores, int scatter_scores,
-                             float* __restrict__ rule_out) {
-  extern __shared__ float s_lse[];
-  for (int i = threadIdx.x; i < LH; i += blockDim.x) s_lse[i] = lse[i];
-  __syncthreads();
-  const int c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= *n_cand_p) return;
-  float r = 0.f;
-#pragma unroll 8
-  for (int lh = 0; lh < LH; ++lh) r += expf(logits[(int64_t)lh * ldc + c] - s_lse[lh]);
-  rule_c[c] = r;
-  const int pos = cand_pos[c];
-  if (scatter_scores) scores[pos] = r;
-  if (rule_out) rule_out[pos] = r;
-}
-
 // live cross-attention positions ("positions evicted in a prior round are excluded"):
 // compacts the slots of the live entries of xattn_pos (or of [qs,qe) when xattn_pos == NULL).  1 CTA of 1024.
 __global__ __launch_bounds__(1024) void k_xattn_compact(const int32_t* __restrict__ S, int N, int32_t dead,

@@ -349,6 +349,66 @@ def test_decode_batched_and_empty(ikv, oracle):
     assert torch.count_nonzero(out[-1]) == 0
 
 
+def test_decode_padded_list_and_long_append(ikv, oracle):
+    """Survivor list shorter than its host-side bound (live < C < N: the padding entries must be masked), then more
+    than 4096 positions appended after the select (the library rescans the map instead of walking the tail)."""
+    shape = wl.ModelShape(2, 8, 2, 128, "bf16")
+    w = wl.make_workload(shape, [wl.SessionSpec(5, n_tokens=3000, n_mem_rows=4, budget=2000, prefix_len=16, span_len=16,
+                                                decode_tokens=5000)], 23)
+    kp, vp = gc.to_cuda(w)
+    ctx = gc.make_ctx(w)
+    g = gc.oracle_geom(oracle, w)
+    s = w.sessions[0]
+    ctx.session_open(5)
+    S = s.slot_map.clone()
+    rng = np.random.default_rng(2)
+    S[torch.from_numpy(rng.choice(3000, 1800, replace=False))] = w.dead_slot      # live 1200 < C 2000 < N 3000
+    S_dev = S.cuda()
+    scores = torch.randn(3000, generator=torch.Generator().manual_seed(9)).cuda()
+    freed = torch.empty(3000, dtype=torch.int32, device="cuda")
+    nf = torch.zeros(1, dtype=torch.int32, device="cuda")
+    nk = torch.zeros(1, dtype=torch.int32, device="cuda")
+    req = ikv.make_request(5, S_dev, 3000, 16, 2984, 3000, 2000, 16)
+    ctx.select_evict([req], scores, freed, nf, nk)
+    assert nk.item() == 1200
+    scale = 1 / math.sqrt(128)
+    gen = torch.Generator().manual_seed(4)
+    for seq_len in (3000, 3001, 3000 + 4096, 3000 + 4097, 8000):
+        q = torch.randn((1, 8, 128), generator=gen).to(torch.bfloat16)
+        out = torch.empty((1, 8, 128), dtype=torch.bfloat16, device="cuda")
+        r = ikv.make_request(5, S_dev, seq_len, 16, 2984, 3000, 2000, 16)
+        ctx.decode_attn(0, [r], q.cuda(), out, scale)
+        want = oracle.decode(g, kp, vp, 0, S_dev.cpu().numpy()[:seq_len], q[0].float().numpy(), scale)
+        gc.assert_decode_close(out[0].float().cpu().numpy(), want, True, f"seq_len {seq_len}")
+
+
+def test_decode_many_unequal_requests(ikv, oracle):
+    """40 requests (more than one launch holds) of very different lengths: splits are handed out in proportion."""
+    shape = wl.ModelShape(1, 8, 2, 128, "bf16")
+    lens = [17 + (i * 977) % 9000 for i in range(40)]
+    specs = [wl.SessionSpec(200 + i, n, 4, 100, prefix_len=4, span_len=4) for i, n in enumerate(lens)]
+    w = wl.make_workload(shape, specs, 29)
+    kp, vp = gc.to_cuda(w)
+    ctx = gc.make_ctx(w, max_sessions=64)
+    g = gc.oracle_geom(oracle, w)
+    maps, reqs = [], []
+    for i, s in enumerate(w.sessions):
+        ctx.session_open(s.spec.session_id)
+        m = s.slot_map[:s.N].clone()
+        if i % 3 == 0:
+            m[1::2] = w.dead_slot
+        maps.append(m.cuda())
+        reqs.append(ikv.make_request(s.spec.session_id, maps[-1], s.N, 0, 0, 0, 100))
+    q = torch.randn((40, 8, 128), generator=torch.Generator().manual_seed(6)).to(torch.bfloat16)
+    out = torch.empty((40, 8, 128), dtype=torch.bfloat16, device="cuda")
+    scale = 1 / math.sqrt(128)
+    ctx.decode_attn(0, reqs, q.cuda(), out, scale)
+    torch.cuda.synchronize()
+    for i in range(40):
+        want = oracle.decode(g, kp, vp, 0, maps[i].cpu().numpy(), q[i].float().numpy(), scale)
+        gc.assert_decode_close(out[i].float().cpu().numpy(), want, True, f"request {i} len {lens[i]}")
+
+
 # ------------------------------------------------------------------------------------------- batches, host path, errors
 def test_batched_score_select(ikv, oracle):
     shape = wl.ModelShape(2, 8, 2, 128, "bf16")
