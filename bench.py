@@ -321,7 +321,7 @@ def run_ours(args):
             e2e_t.append(dt)
     e2e_total = sum(e2e_t)
     h2d = T * 4 + h_rows.numel() * 4
-    d2h = T * 4 + T + n_freed_h * 4 + 8
+    d2h = 16 + ((T + 1023) // 1024 * 1024) * 8 + T     # one copy: counts | slot map | freed list (capacity) | valid mask
 
     # ---- phase-1 (memory mode) beside the headline
     p1 = []

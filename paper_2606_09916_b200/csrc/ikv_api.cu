@@ -88,6 +88,8 @@ struct ikv_ctx {
   uint8_t* st_valid = nullptr;
   float *st_scores = nullptr, *st_qrows = nullptr;
   int64_t st_cap = 0, st_qcap = 0;
+  unsigned char* st_out = nullptr;   // device: [counts 16 B][slot map cap*4][freed cap*4][valid cap], one D2H copy
+  unsigned char* st_host = nullptr;  // pinned host mirror of st_out
 
   // kernel-level profiling (ikv_profile_*)
   bool prof_on = false;
@@ -233,9 +235,16 @@ ikv_status ensure_parts(ikv_ctx* c, int64_t units) {
 ikv_status ensure_staging(ikv_ctx* c, int64_t tokens, int64_t qelems) {
   if (tokens > c->st_cap) {
     const int64_t cap = round_up(tokens, 1024);
-    TRY(grow(c, &c->st_map, cap));
-    TRY(grow(c, &c->st_freed, cap));
-    TRY(grow(c, &c->st_valid, cap));
+    const size_t bytes = 16 + (size_t)cap * 9;
+    if (c->st_out) CU(c, cudaFree(c->st_out));
+    if (c->st_host) CU(c, cudaFreeHost(c->st_host));
+    c->st_out = nullptr; c->st_host = nullptr;
+    CU(c, cudaMalloc((void**)&c->st_out, bytes));
+    CU(c, cudaMallocHost((void**)&c->st_host, bytes));
+    c->st_counts = reinterpret_cast<int32_t*>(c->st_out);
+    c->st_map = reinterpret_cast<int32_t*>(c->st_out + 16);
+    c->st_freed = c->st_map + cap;
+    c->st_valid = reinterpret_cast<uint8_t*>(c->st_freed + cap);
     TRY(grow(c, &c->st_scores, cap));
     c->st_cap = cap;
   }
@@ -653,7 +662,6 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
   ok = ok && cudaMemset(c->d_nxq, 0, 4) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&c->lse, (size_t)cfg->n_layers * cfg->n_q_heads * 4) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&c->mbar, (size_t)cfg->head_dim * 4) == cudaSuccess;
-  ok = ok && cudaMalloc((void**)&c->st_counts, 16) == cudaSuccess;
   {
     const int LH = cfg->n_layers * cfg->n_q_heads, KS = cfg->head_dim / 16;
     ok = ok && cudaMalloc((void**)&c->mpart, (size_t)((LH + 31) / 32) * cfg->head_dim * 4) == cudaSuccess;
@@ -682,9 +690,10 @@ ikv_status ikv_destroy(ikv_ctx* c) {
   void* bufs[] = {c->cand_pos, c->cand_slot, c->d_ncand, c->logits, c->partials, c->lse, c->rule_c, c->kbar, c->mbar,
                   c->xq_slot, c->d_nxq, c->kq, c->kc_frag, c->vc_frag, c->mpart, c->bq_eff, c->b1_eff, c->wq_frag,
                   c->w1k_frag, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
-                  c->part_o, c->part_ml, c->st_map, c->st_freed, c->st_counts, c->st_valid, c->st_scores,
+                  c->part_o, c->part_ml, c->st_out, c->st_scores,
                   c->st_qrows, c->resid_blob, c->frag};
   for (void* b : bufs) cudaFree(b);
+  if (c->st_host) cudaFreeHost(c->st_host);
   const cudaError_t e = cudaGetLastError();
   delete c;
   return e == cudaSuccess ? IKV_OK : IKV_ERR_CUDA;
@@ -994,15 +1003,20 @@ ikv_status ikv_prune_host(ikv_ctx* c, const ikv_request* req, const float* q_row
   }
   TRY(ikv_score(c, &r, 1, mode, c->st_scores, nullptr, stream));
   TRY(ikv_select_evict(c, &r, 1, c->st_scores, c->st_freed, c->st_counts, c->st_counts + 1, stream));
-  int32_t counts[2] = {0, 0};
-  CU(c, cudaMemcpyAsync(counts, c->st_counts, 8, cudaMemcpyDeviceToHost, st));
-  CU(c, cudaMemcpyAsync(slot_map_host, c->st_map, (size_t)N * 4, cudaMemcpyDeviceToHost, st));
-  if (valid_host) CU(c, cudaMemcpyAsync(valid_host, c->st_valid, (size_t)N, cudaMemcpyDeviceToHost, st));
+  // one device-to-host copy of [counts | slot map | freed list | valid mask] into the pinned mirror, then host copies
+  const size_t out_bytes = 16 + (size_t)c->st_cap * 8 + (size_t)N;
+  CU(c, cudaMemcpyAsync(c->st_host, c->st_out, out_bytes, cudaMemcpyDeviceToHost, st));
   if (scores_host) CU(c, cudaMemcpyAsync(scores_host, c->st_scores, (size_t)N * 4, cudaMemcpyDeviceToHost, st));
   CU(c, cudaStreamSynchronize(st));
-  *n_freed_host = counts[0];
-  *n_kept_host = counts[1];
-  if (counts[0] > 0) CU(c, cudaMemcpy(freed_host, c->st_freed, (size_t)counts[0] * 4, cudaMemcpyDeviceToHost));
+  const int32_t* h_counts = reinterpret_cast<const int32_t*>(c->st_host);
+  const int32_t* h_map = reinterpret_cast<const int32_t*>(c->st_host + 16);
+  const int32_t* h_freed = h_map + c->st_cap;
+  const uint8_t* h_valid = reinterpret_cast<const uint8_t*>(h_freed + c->st_cap);
+  *n_freed_host = h_counts[0];
+  *n_kept_host = h_counts[1];
+  memcpy(slot_map_host, h_map, (size_t)N * 4);
+  if (valid_host) memcpy(valid_host, h_valid, (size_t)N);
+  if (h_counts[0] > 0) memcpy(freed_host, h_freed, (size_t)h_counts[0] * 4);
   return IKV_OK;
 }
 
