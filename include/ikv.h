@@ -144,7 +144,13 @@ ikv_status ikv_select_evict(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req
  *                       V[layer, h div G, S_r[j]].
  * q, out: DEVICE [n_req][H_q][D]; bf16 for a bf16 pool, fp32 for an fp32 pool.  Positions below the seq_len of
  * the last ikv_select_evict on the same (session, slot_map) come from the cached compact live list; positions
- * appended since are read from slot_map.  A caller that edited the slot map itself passes IKV_REQ_RESCAN. */
+ * appended since are read from slot_map.  A caller that edited the slot map itself passes IKV_REQ_RESCAN.
+ * Stream ordering (R27): the kernels of this call are launched with programmatic stream serialization and
+ * read q, the slot maps and the K/V pools as soon as they start; they order only their WRITES after the preceding
+ * kernel of the stream.  This is ordinary stream order as long as the producer of those inputs is a normally
+ * completing kernel or copy (anything but this library's own decode kernels, which write none of them); a caller whose
+ * own producer kernel triggers its dependents early (griddepcontrol.launch_dependents) must not do so before its
+ * writes, or sets IKV_PDL=0 in the environment.  Up to 32 requests go into one launch; larger batches are chunked. */
 ikv_status ikv_decode_attn(ikv_ctx *ctx, int32_t layer, const ikv_request *reqs, int32_t n_req, const void *q,
                            void *out, float sm_scale, void *stream);
 
