@@ -256,7 +256,7 @@ def run_ours(args):
         decode_all()
     stream.synchronize()
 
-    # memory_update, partition(+xattn compaction), mem_prep, key_pass, post_key, rule4, select_evict (+ residual_mma)
+    # memory_update, partition(+xattn compaction), mem_prep, key_pass, post_key(lse), rule_fused, select_evict (+ residual_mma)
     n_prune_launch = 7 + (1 if mode == ikv.MODE_LEARNABLE else 0)
     n_decode_launch = DEC * L * 2
 

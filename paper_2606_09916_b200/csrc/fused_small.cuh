@@ -43,4 +43,27 @@ __global__ __launch_bounds__(128) void k_post_key(const PostKeyParams p, const R
   resid_kv_frags_block(bid, p.kq, p.n_xq, D, w, p.nks, p.kc_frag, p.vc_frag);
 }
 
+struct RuleParams {
+  const float* logits; int64_t ldc; int LH; const float* lse; const int32_t* n_cand; const int32_t* cand_pos;
+  float* rule_c; float* scores; int scatter_scores; float* rule_out; int n_rule;  // rule blocks (256 threads)
+};
+
+// rule_c of Eq. 3 (HBM-bound, 256-thread blocks) and, for a learnable call, the folded W_Q / fc1 operands and the
+// Kc / Vc fragments (latency-bound 128-thread bodies, warps 4-7 of their blocks exit) in one launch: the residual
+// kernel needs all three, and the small bodies hide under the rule blocks' stream of the logits.
+template <int D>
+__global__ __launch_bounds__(256) void k_rule_fused(const RuleParams r, const PostKeyParams p, const ResidW w) {
+  int bid = blockIdx.x;
+  if (bid < r.n_rule) {
+    score_rule4_block(bid, r.n_rule, r.logits, r.ldc, r.LH, r.lse, r.n_cand, r.cand_pos, r.rule_c, r.scores,
+                      r.scatter_scores, r.rule_out);
+    return;
+  }
+  if (threadIdx.x >= 128) return;
+  bid -= r.n_rule;
+  if (bid < p.n_fold) { resid_fold_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.fold); return; }
+  bid -= p.n_fold;
+  resid_kv_frags_block(bid, p.kq, p.n_xq, D, w, p.nks, p.kc_frag, p.vc_frag);
+}
+
 }  // namespace ikv

@@ -537,23 +537,29 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     }
   }
   {
-    // lse rows, and for a learnable call the folded residual operands and the Kc / Vc fragments, in one launch
+    // launch 1: lse rows.  launch 2: rule_c (Eq. 3) and, for a learnable call, the folded residual operands and the
+    // Kc / Vc fragments, whose latency-bound bodies hide under the rule blocks' stream of the logits.
     PostKeyParams pk;
     pk.partials = c->partials; pk.n_part = n_part; pk.lse = c->lse; pk.n_lse = LH;
     pk.mpart = c->mpart; pk.n_mpart = n_mpart; pk.LH = LH;
     pk.fold.mbar = c->mbar; pk.fold.wq_frag = c->wq_frag; pk.fold.w1k_frag = c->w1k_frag;
     pk.fold.bq_eff = c->bq_eff; pk.fold.b1_eff = c->b1_eff;
-    pk.n_fold = learn ? (D == 128 ? resid_fold_grid<128>() : resid_fold_grid<64>()) : 0;
     pk.kq = c->kq; pk.n_xq = c->d_nxq; pk.nks = (int)(c->xq_cap / 16); pk.kc_frag = c->kc_frag; pk.vc_frag = c->vc_frag;
+    pk.n_fold = 0; pk.n_kv = 0;
+    if (D == 128) k_post_key<128><<<pk.n_lse, 128, 0, st>>>(pk, c->rw);
+    else k_post_key<64><<<pk.n_lse, 128, 0, st>>>(pk, c->rw);
+    LAUNCH_CHECK(c);
+    pk.n_fold = learn ? (D == 128 ? resid_fold_grid<128>() : resid_fold_grid<64>()) : 0;
     pk.n_kv = (learn && n_x > 0) ? 4 * ((n_x + 15) / 16) : 0;
-    const int grid = pk.n_lse + pk.n_fold + pk.n_kv;
-    if (D == 128) k_post_key<128><<<grid, 128, 0, st>>>(pk, c->rw);
-    else k_post_key<64><<<grid, 128, 0, st>>>(pk, c->rw);
+    RuleParams rp;
+    rp.logits = c->logits; rp.ldc = c->cap_tokens; rp.LH = LH; rp.lse = c->lse; rp.n_cand = c->d_ncand;
+    rp.cand_pos = c->cand_pos; rp.rule_c = c->rule_c; rp.scores = scores; rp.scatter_scores = learn ? 0 : 1;
+    rp.rule_out = rule_out; rp.n_rule = (N + 63) / 64;
+    const int grid = rp.n_rule + pk.n_fold + pk.n_kv;
+    if (D == 128) k_rule_fused<128><<<grid, 256, 0, st>>>(rp, pk, c->rw);
+    else k_rule_fused<64><<<grid, 256, 0, st>>>(rp, pk, c->rw);
     LAUNCH_CHECK(c);
   }
-  k_score_rule4<<<(N + 63) / 64, 256, 0, st>>>(c->logits, c->cap_tokens, L * Hq, c->lse, c->d_ncand, c->cand_pos,
-                                               c->rule_c, scores, learn ? 0 : 1, rule_out);
-  LAUNCH_CHECK(c);
   if (learn) {
     ResidMmaParams rp;
     rp.rule_c = c->rule_c; rp.kbar = c->kbar; rp.n_cand = c->d_ncand; rp.cand_pos = c->cand_pos; rp.n_xq = c->d_nxq;

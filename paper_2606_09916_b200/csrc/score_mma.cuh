@@ -397,24 +397,26 @@ inline size_t key_pass_smem(int L, int Hq, int Hkv, int D, bool kbar, int max_sm
 }
 
 // ---------------------------------------------------------------------------------------------
-// a3  rule_c = sum_{l,h} exp(x[l,h,c] - lse[l,h])   (Eq. 3).  One CTA of 256 threads per 64 candidates:
+// a3  rule_c = sum_{l,h} exp(x[l,h,c] - lse[l,h])   (Eq. 3).  One block of 256 threads per 64 candidates (launched
+// from k_rule_fused, fused_small.cuh):
 // thread (cq = tid % 16 -> 4 candidates, lg = tid / 16 -> rows lg, lg+16, ...), 16-byte loads.
 // ---------------------------------------------------------------------------------------------
-__global__ __launch_bounds__(256) void k_score_rule4(const float* __restrict__ logits, int64_t ldc, int LH,
-                                                     const float* __restrict__ lse,
-                                                     const int32_t* __restrict__ n_cand_p,
-                                                     const int32_t* __restrict__ cand_pos, float* __restrict__ rule_c,
-                                                     float* __restrict__ scores, int scatter_scores,
-                                                     float* __restrict__ rule_out) {
+__device__ __forceinline__ void score_rule4_block(int bid, int n_blocks, const float* __restrict__ logits, int64_t ldc,
+                                                  int LH, const float* __restrict__ lse,
+                                                  const int32_t* __restrict__ n_cand_p,
+                                                  const int32_t* __restrict__ cand_pos, float* __restrict__ rule_c,
+                                                  float* __restrict__ scores, int scatter_scores,
+                                                  float* __restrict__ rule_out) {
   __shared__ float4 part[16][16];
   const int nc = *n_cand_p;
-  const int c0 = blockIdx.x * 64;
+  // newest tiles first: the key pass wrote the logits in tile order, so the tail of the scratch is still in L2
+  const int c0 = (n_blocks - 1 - bid) * 64;
   if (c0 >= nc) return;
   const int cq = threadIdx.x & 15, lg = threadIdx.x >> 4;
   const int c = c0 + cq * 4;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   if (c < nc) {  // rows are padded to a multiple of 4 (ldc % 4 == 0); lanes past n_cand read scratch, never stored
-#pragma unroll 6
+#pragma unroll 12
     for (int lh = lg; lh < LH; lh += 16) {
       const float4 v = *reinterpret_cast<const float4*>(logits + (int64_t)lh * ldc + c);
       const float e = __ldg(lse + lh);
