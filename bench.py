@@ -305,7 +305,7 @@ def run_ours(args):
     # ---- end-to-end through ikv_prune_host with pinned HOST buffers
     h_map0 = sess.slot_map[:T].clone().pin_memory()
     h_map = torch.empty_like(h_map0).pin_memory()
-    h_rows = sess.updates()[-1].contiguous().pin_memory()
+    h_rows = sess.updates()[-1].to(torch.bfloat16).contiguous().pin_memory()   # post-RoPE Q rows in the model's dtype
     h_valid = torch.empty(T, dtype=torch.uint8).pin_memory()
     h_freed = torch.empty(T, dtype=torch.int32).pin_memory()
     req_h = ikv.make_request(sid, None, T, sess.pi, sess.qs, sess.qe, C, sess.pi)
@@ -320,7 +320,7 @@ def run_ours(args):
         if i >= args.warmup:
             e2e_t.append(dt)
     e2e_total = sum(e2e_t)
-    h2d = T * 4 + h_rows.numel() * 4
+    h2d = T * 4 + h_rows.numel() * h_rows.element_size()
     d2h = 16 + ((T + 1023) // 1024 * 1024) * 8 + T     # one copy: counts | slot map | freed list (capacity) | valid mask
 
     # ---- phase-1 (memory mode) beside the headline
@@ -373,7 +373,7 @@ def run_ours(args):
                        "frac_of_nominal_8TBs": dec_bytes_step / (tot_dec / K * 1e-3) / 1e9 / NOMINAL_HBM_GBS},
             "e2e": {"value": world * T * K / (e2e_ms_total * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h,
-                    "what": "ikv_prune_host: slot map + query rows H2D, memory update + score + select/evict, "
+                    "what": "ikv_prune_host: slot map + bf16 query rows H2D, memory update + score + select/evict, "
                             "slot map + valid mask + freed list + counts D2H; the K/V pool is device-resident state"},
             "gpu_launches": K * (n_prune_launch + n_decode_launch),
             "roofline": {"kernel": "k_key_pass", "bound": "hbm", "achieved": ach, "peak": hbm_peak,

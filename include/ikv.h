@@ -155,13 +155,14 @@ ikv_status ikv_decode_attn(ikv_ctx *ctx, int32_t layer, const ikv_request *reqs,
                            void *out, float sm_scale, void *stream);
 
 /* The whole pruning pass of one request with HOST buffers (used for end-to-end timing): copies
- * q_rows_host ([n_rows][L][H_q][D] fp32, may be NULL/0 to skip the memory update) and slot_map_host[seq_len]
- * to the device, runs ikv_memory_update -> ikv_score(mode) -> ikv_select_evict, copies the new slot map,
- * valid mask (optional), freed list and counts back to the HOST buffers and synchronises `stream`.
+ * q_rows_host ([n_rows][L][H_q][D], q_dtype IKV_F32 or IKV_BF16; may be NULL/0 to skip the memory update) and
+ * slot_map_host[seq_len] to the device, runs ikv_memory_update -> ikv_score(mode) -> ikv_select_evict, brings the new
+ * slot map, valid mask (optional), freed list and counts back in one device-to-host copy and synchronises `stream`.
  * req->slot_map / valid_mask / xattn_pos are ignored (xattn_pos defaults to the span). */
-ikv_status ikv_prune_host(ikv_ctx *ctx, const ikv_request *req, const float *q_rows_host, int32_t n_rows,
-                          int32_t mode, int32_t *slot_map_host, uint8_t *valid_host, float *scores_host,
-                          int32_t *freed_host, int32_t *n_freed_host, int32_t *n_kept_host, void *stream);
+ikv_status ikv_prune_host(ikv_ctx *ctx, const ikv_request *req, const void *q_rows_host, int32_t n_rows,
+                          int32_t q_dtype, int32_t mode, int32_t *slot_map_host, uint8_t *valid_host,
+                          float *scores_host, int32_t *freed_host, int32_t *n_freed_host, int32_t *n_kept_host,
+                          void *stream);
 
 /* Kernel-level timing for bench.py's roofline: while enabled, the library brackets its two dominant kernels
  * (the key pass k_key_pass / k_score_logits and the decode split kernel k_decode_mma / k_decode_split) with CUDA events on the caller's stream

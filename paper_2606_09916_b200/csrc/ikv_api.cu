@@ -986,7 +986,8 @@ ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, i
   return IKV_OK;
 }
 
-ikv_status ikv_prune_host(ikv_ctx* c, const ikv_request* req, const float* q_rows_host, int32_t n_rows, int32_t mode,
+ikv_status ikv_prune_host(ikv_ctx* c, const ikv_request* req, const void* q_rows_host, int32_t n_rows, int32_t q_dtype,
+                          int32_t mode,
                           int32_t* slot_map_host, uint8_t* valid_host, float* scores_host, int32_t* freed_host,
                           int32_t* n_freed_host, int32_t* n_kept_host, void* stream) {
   if (!c) return IKV_ERR_INVALID_ARG;
@@ -994,6 +995,8 @@ ikv_status ikv_prune_host(ikv_ctx* c, const ikv_request* req, const float* q_row
     IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_prune_host: NULL argument");
   cudaStream_t st = (cudaStream_t)stream;
   const int N = req->seq_len;
+  if (q_dtype != IKV_F32 && q_dtype != IKV_BF16) IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "q_dtype must be IKV_F32 or IKV_BF16");
+  const size_t qes = (q_dtype == IKV_F32) ? 4 : 2;
   const int64_t qel = (int64_t)(n_rows > 0 ? n_rows : 0) * c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim;
   TRY(ensure_staging(c, N > 0 ? N : 1, qel));
   ikv_request r = *req;
@@ -1004,8 +1007,8 @@ ikv_status ikv_prune_host(ikv_ctx* c, const ikv_request* req, const float* q_row
   TRY(check_request(c, r));
   CU(c, cudaMemcpyAsync(c->st_map, slot_map_host, (size_t)N * 4, cudaMemcpyHostToDevice, st));
   if (q_rows_host && n_rows > 0) {
-    CU(c, cudaMemcpyAsync(c->st_qrows, q_rows_host, (size_t)qel * 4, cudaMemcpyHostToDevice, st));
-    TRY(ikv_memory_update(c, r.session_id, c->st_qrows, n_rows, IKV_F32, stream));
+    CU(c, cudaMemcpyAsync(c->st_qrows, q_rows_host, (size_t)qel * qes, cudaMemcpyHostToDevice, st));
+    TRY(ikv_memory_update(c, r.session_id, c->st_qrows, n_rows, q_dtype, stream));
   }
   TRY(ikv_score(c, &r, 1, mode, c->st_scores, nullptr, stream));
   TRY(ikv_select_evict(c, &r, 1, c->st_scores, c->st_freed, c->st_counts, c->st_counts + 1, stream));

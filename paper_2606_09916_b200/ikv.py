@@ -72,7 +72,7 @@ _lib.ikv_decode_attn.argtypes = [C.c_void_p, C.c_int32, C.POINTER(Request), C.c_
                                  C.c_float, C.c_void_p]
 _lib.ikv_profile_enable.argtypes = [C.c_void_p, C.c_int32]
 _lib.ikv_profile_read.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
-_lib.ikv_prune_host.argtypes = [C.c_void_p, C.POINTER(Request), C.c_void_p, C.c_int32, C.c_int32, C.c_void_p,
+_lib.ikv_prune_host.argtypes = [C.c_void_p, C.POINTER(Request), C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p,
                                 C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 
 
@@ -208,7 +208,8 @@ class Context:
         """HOST-buffer variant. Tensors are CPU tensors (pinned or not). Returns (n_freed, n_kept)."""
         nf, nk = C.c_int32(0), C.c_int32(0)
         n_rows = 0 if q_rows_host is None else q_rows_host.shape[0]
-        self._chk(_lib.ikv_prune_host(self._h, C.byref(req), _ptr(q_rows_host), n_rows, mode, _ptr(slot_map_host),
+        q_dtype = BF16 if (q_rows_host is not None and q_rows_host.dtype == torch.bfloat16) else F32
+        self._chk(_lib.ikv_prune_host(self._h, C.byref(req), _ptr(q_rows_host), n_rows, q_dtype, mode, _ptr(slot_map_host),
                                       _ptr(valid_host), _ptr(scores_host), _ptr(freed_host), C.byref(nf),
                                       C.byref(nk), _stream(stream)))
         return nf.value, nk.value

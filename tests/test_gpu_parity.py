@@ -447,7 +447,8 @@ def test_batched_score_select(ikv, oracle):
         off += s.N
 
 
-def test_prune_host_path(ikv, oracle):
+@pytest.mark.parametrize("row_dtype", ["f32", "bf16"])
+def test_prune_host_path(ikv, oracle, row_dtype):
     w = build("bf16_d128_g4", SHAPES[1][1], n_tokens=2500, budget=700)
     kp, vp = gc.to_cuda(w)
     ctx = gc.make_ctx(w)
@@ -462,8 +463,14 @@ def test_prune_host_path(ikv, oracle):
     sc = torch.empty(s.N, dtype=torch.float32).pin_memory()
     freed = torch.empty(s.N, dtype=torch.int32).pin_memory()
     req = ikv.make_request(s.spec.session_id, None, s.N, s.pi, s.qs, s.qe, 700, s.pi)
-    n_freed, n_kept = ctx.prune_host(req, ups[-1].contiguous(), ikv.MODE_MEMORY, S_host, valid, sc, freed)
-    M = gc.fold_memory_oracle(oracle, s)
+    last = ups[-1].contiguous()
+    if row_dtype == "bf16":                                  # query rows in the model's dtype: half the H2D bytes
+        last = last.to(torch.bfloat16)
+    n_freed, n_kept = ctx.prune_host(req, last, ikv.MODE_MEMORY, S_host, valid, sc, freed)
+    M = np.zeros((w.shape.L, w.shape.Hq, w.shape.D))
+    for rows in ups[:-1]:
+        oracle.memory_update(M, rows.numpy(), 0.5)
+    oracle.memory_update(M, last.float().numpy(), 0.5)
     g = gc.oracle_geom(oracle, w)
     want = oracle.score(g, kp, M, S.numpy(), s.pi, s.qs, s.qe)
     gc.assert_scores_close(sc.numpy(), want, "prune_host scores")
