@@ -27,6 +27,7 @@ SHAPES = [
     ("bf16_d128_g8", wl.ModelShape(2, 16, 2, 128, "bf16")),
     ("f32_d128_g4", wl.ModelShape(2, 8, 2, 128, "f32")),
     ("bf16_d128_h12", wl.ModelShape(2, 24, 12, 128, "bf16")),   # more KV heads than warps
+    ("bf16_d128_g5_h8", wl.ModelShape(2, 40, 8, 128, "bf16")),  # configs[2] head layout: one KV head per logit warp
 ]
 
 
@@ -109,7 +110,8 @@ def test_query_mode_and_fresh_session(ikv, oracle):
 
 
 # ------------------------------------------------------------------------------------------- a4-a5
-@pytest.mark.parametrize("name,shape", [SHAPES[0], SHAPES[1], SHAPES[2], SHAPES[3]], ids=["tiny", "d128g4", "d64g2", "d128g5"])
+@pytest.mark.parametrize("name,shape", [SHAPES[0], SHAPES[1], SHAPES[2], SHAPES[3], SHAPES[8], SHAPES[5]],
+                         ids=["tiny", "d128g4", "d64g2", "d128g5", "d128g5h8", "d128g8"])
 def test_learnable_score_matches_oracle(ikv, oracle, name, shape):
     w = build(name, shape)
     ctx, s, M, kp, _ = run_memory(ikv, oracle, w)
