@@ -580,8 +580,9 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   return IKV_OK;
 }
 
-ikv_status select_one(ikv_ctx* c, const ikv_request& r, const float* scores, int32_t* freed, int32_t* n_freed,
-                      int32_t* n_kept, cudaStream_t st) {
+// Fills the kernel parameters of one request and updates the session's decode bookkeeping.
+ikv_status select_prepare(ikv_ctx* c, const ikv_request& r, const float* scores, int32_t* freed, int32_t* n_freed,
+                          int32_t* n_kept, SelParams* out) {
   Session* s = session_find(c, r.session_id);
   if (!s) IKV_FAIL(c, IKV_ERR_NO_SESSION, "session %llu does not exist", (unsigned long long)r.session_id);
   const int N = r.seq_len;
@@ -594,11 +595,7 @@ ikv_status select_one(ikv_ctx* c, const ikv_request& r, const float* scores, int
   p.freed = freed; p.n_freed = n_freed; p.n_kept = n_kept;
   p.live_slots = s->live_slots; p.n_live = s->d_n_live;
   p.kept_bits = c->kept_bits; p.firstpos = c->firstpos; p.keepflag = c->keepflag; p.tmp_slot = c->tmp_slot;
-  if (N <= CL_CTAS * 1024 * 4) k_select_evict_cl<4><<<CL_CTAS, 1024, 0, st>>>(p);
-  else if (N <= CL_CTAS * 1024 * 8) k_select_evict_cl<8><<<CL_CTAS, 1024, 0, st>>>(p);
-  else if (N <= CL_MAX_N) k_select_evict_cl<16><<<CL_CTAS, 1024, 0, st>>>(p);
-  else k_select_evict<<<1, 1024, 0, st>>>(p);
-  LAUNCH_CHECK(c);
+  *out = p;
   s->covered = N;
   s->map_ptr = r.slot_map;
   s->live_ub = N;
@@ -607,6 +604,16 @@ ikv_status select_one(ikv_ctx* c, const ikv_request& r, const float* scores, int
     s->live_ub = (forced_ub > r.budget ? forced_ub : r.budget);
     if (s->live_ub > N) s->live_ub = N;
   }
+  return IKV_OK;
+}
+
+// One launch for up to SEL_MAX_REQ requests (one cluster each); longer maps take the single-CTA kernel one by one.
+ikv_status select_launch(ikv_ctx* c, const SelBatch& b, int n, int max_n, cudaStream_t st) {
+  if (n == 0) return IKV_OK;
+  if (max_n <= CL_CTAS * 1024 * 4) k_select_evict_cl<4><<<n * CL_CTAS, 1024, 0, st>>>(b);
+  else if (max_n <= CL_CTAS * 1024 * 8) k_select_evict_cl<8><<<n * CL_CTAS, 1024, 0, st>>>(b);
+  else k_select_evict_cl<16><<<n * CL_CTAS, 1024, 0, st>>>(b);
+  LAUNCH_CHECK(c);
   return IKV_OK;
 }
 
@@ -903,10 +910,27 @@ ikv_status ikv_select_evict(ikv_ctx* c, const ikv_request* reqs, int32_t n_req, 
     IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_select_evict: NULL argument");
   for (int r = 0; r < n_req; ++r) TRY(check_request(c, reqs[r]));
   int64_t off = 0;
+  SelBatch batch;
+  int nb = 0, max_n = 0;
   for (int r = 0; r < n_req; ++r) {
-    TRY(select_one(c, reqs[r], scores + off, freed_slots + off, n_freed + r, n_kept + r, (cudaStream_t)stream));
+    SelParams p;
+    TRY(select_prepare(c, reqs[r], scores + off, freed_slots + off, n_freed + r, n_kept + r, &p));
     off += reqs[r].seq_len;
+    if (p.N > CL_MAX_N) {  // beyond the cluster kernel's register blocking: single-CTA kernel, in stream order
+      TRY(select_launch(c, batch, nb, max_n, (cudaStream_t)stream));
+      nb = 0; max_n = 0;
+      k_select_evict<<<1, 1024, 0, (cudaStream_t)stream>>>(p);
+      LAUNCH_CHECK(c);
+      continue;
+    }
+    batch.p[nb++] = p;
+    if (p.N > max_n) max_n = p.N;
+    if (nb == SEL_MAX_REQ) {
+      TRY(select_launch(c, batch, nb, max_n, (cudaStream_t)stream));
+      nb = 0; max_n = 0;
+    }
   }
+  TRY(select_launch(c, batch, nb, max_n, (cudaStream_t)stream));
   return IKV_OK;
 }
 

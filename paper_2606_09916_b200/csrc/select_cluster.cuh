@@ -16,6 +16,10 @@ namespace cg = cooperative_groups;
 constexpr int CL_CTAS = 8;
 constexpr int CL_MAX_ITEMS = 16;
 constexpr int CL_MAX_N = CL_CTAS * 1024 * CL_MAX_ITEMS;
+constexpr int SEL_MAX_REQ = 16;  // requests per launch of k_select_evict_cl (parameters travel by value)
+struct SelBatch {
+  SelParams p[SEL_MAX_REQ];
+};
 
 // sum over the cluster of one int per CTA, and the exclusive prefix of this CTA's rank
 __device__ __forceinline__ void cluster_offsets(cg::cluster_group& cl, int* sh_val, int crank, int* before, int* total) {
@@ -113,7 +117,11 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_partit
 //   first-dropped-position table (global scratch)  ->  freed test (a)(b)(c)  ->  ordered writes  ->  scratch restore.
 // ---------------------------------------------------------------------------------------------------------------
 template <int MAXI>
-__global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select_evict_cl(SelParams p) {
+__global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select_evict_cl(const SelBatch batch) {
+  // one cluster per request of the batch.  Requests run concurrently on the shared kept-slot bitmap and
+  // first-dropped-position table: they may share slots only below their radix_protected_len (forks, R19), where neither
+  // structure is consulted, and every request clears exactly the bits it set.
+  const SelParams p = batch.p[blockIdx.x / CL_CTAS];
   cg::cluster_group cl = cg::this_cluster();
   const int crank = (int)cl.block_rank();
   __shared__ int hist[2][256];
@@ -317,7 +325,7 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select
       const bool keep = (keep_m >> i) & 1u;
       if (keep) {
         p.live_slots[live_o++] = slot[i];
-        p.kept_bits[slot[i] >> 5] = 0u;  // restore the scratch invariant
+        atomicAnd(&p.kept_bits[slot[i] >> 5], ~(1u << (slot[i] & 31)));  // restore the scratch invariant
       } else if ((drop_m >> i) & 1u) {
         p.S[j] = p.dead;
         if (j >= p.radix) p.firstpos[slot[i]] = INT_MAX;

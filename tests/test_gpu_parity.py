@@ -449,6 +449,48 @@ def test_batched_score_select(ikv, oracle):
         off += s.N
 
 
+def test_batched_select_many_requests(ikv, oracle):
+    """20 requests in one ikv_select_evict call (two launches of one cluster per request) on pages interleaved in one
+    pool: mixed lengths (one beyond 32,768 positions), heavy ties, dead positions; every request bit-exact."""
+    shape = wl.ModelShape(1, 2, 1, 64, "bf16")
+    lens = [300 + (i * 1237) % 5000 for i in range(19)] + [40000]
+    specs = [wl.SessionSpec(300 + i, n, 4, 128 + 64 * (i % 5), prefix_len=8, span_len=8) for i, n in enumerate(lens)]
+    w = wl.make_workload(shape, specs, 41)
+    gc.to_cuda(w)
+    ctx = gc.make_ctx(w, max_sessions=64)
+    rng = np.random.default_rng(12)
+    tot = sum(lens)
+    maps_h, maps, reqs, sc_parts = [], [], [], []
+    for s in w.sessions:
+        ctx.session_open(s.spec.session_id)
+        S = s.slot_map[:s.N].numpy().copy()
+        S[rng.choice(s.N, s.N // 6, replace=False)] = w.dead_slot
+        maps_h.append(S)
+        maps.append(torch.from_numpy(S.copy()).cuda())
+        reqs.append(gc.request(ikv, s, maps[-1], radix=s.pi + 50))
+        sc_parts.append((np.round(rng.standard_normal(s.N) * 4) / 4).astype(np.float32))
+    scores = torch.from_numpy(np.concatenate(sc_parts)).cuda()
+    freed = torch.empty(tot, dtype=torch.int32, device="cuda")
+    nf = torch.zeros(20, dtype=torch.int32, device="cuda")
+    nk = torch.zeros(20, dtype=torch.int32, device="cuda")
+    ctx.select_evict(reqs, scores, freed, nf, nk)
+    torch.cuda.synchronize()
+    off = 0
+    for i, s in enumerate(w.sessions):
+        cls, _ = oracle.partition(maps_h[i], 0, s.pi, s.qs, s.qe)
+        keep, n_kept = oracle.select(sc_parts[i], cls, s.spec.budget)
+        S2, _, freed_o = oracle.rewrite(maps_h[i], 0, keep, s.pi + 50, w.n_slots)
+        assert nk[i].item() == n_kept and nf[i].item() == len(freed_o), f"request {i}"
+        assert np.array_equal(maps[i].cpu().numpy(), S2), f"request {i}"
+        assert np.array_equal(freed.cpu().numpy()[off:off + len(freed_o)], freed_o), f"request {i}"
+        off += s.N
+    # the shared scratch is back to its invariant: a second call on the pruned maps changes nothing
+    before = [m.clone() for m in maps]
+    ctx.select_evict(reqs, scores, freed, nf, nk)
+    torch.cuda.synchronize()
+    assert all(torch.equal(a, b) for a, b in zip(before, maps)) and int(nf.sum().item()) == 0
+
+
 @pytest.mark.parametrize("row_dtype", ["f32", "bf16"])
 def test_prune_host_path(ikv, oracle, row_dtype):
     w = build("bf16_d128_g4", SHAPES[1][1], n_tokens=2500, budget=700)
