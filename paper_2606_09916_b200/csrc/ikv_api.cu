@@ -201,6 +201,7 @@ ikv_status ensure_scratch(ikv_ctx* c, int64_t tokens) {
   const int L = c->cfg.n_layers, Hq = c->cfg.n_q_heads, D = c->cfg.head_dim;
   const int64_t cap = round_up(tokens, 1024);
   const int64_t n_tiles = cap / SCORE_TILE;
+  c->cap_tokens = 0;  // a failed growth must not leave the old capacity standing over freed buffers
   TRY(grow(c, &c->cand_pos, cap));
   TRY(grow(c, &c->cand_slot, cap));
   TRY(grow(c, &c->logits, (size_t)L * Hq * cap));
@@ -216,6 +217,7 @@ ikv_status ensure_scratch(ikv_ctx* c, int64_t tokens) {
 ikv_status ensure_xq(ikv_ctx* c, int64_t n) {
   if (n <= c->xq_cap) return IKV_OK;
   const int64_t cap = round_up(n, 256);
+  c->xq_cap = 0;
   TRY(grow(c, &c->xq_slot, cap));
   TRY(grow(c, &c->kq, (size_t)cap * c->cfg.head_dim));
   TRY(grow(c, &c->kc_frag, (size_t)cap * 32));  // 4 heads x 2 k-steps x cap/8 tiles x 32 lanes
@@ -226,6 +228,7 @@ ikv_status ensure_xq(ikv_ctx* c, int64_t n) {
 
 ikv_status ensure_parts(ikv_ctx* c, int64_t units) {
   if (units <= c->part_cap) return IKV_OK;
+  c->part_cap = 0;
   TRY(grow(c, &c->part_o, (size_t)units * c->cfg.head_dim));
   TRY(grow(c, &c->part_ml, (size_t)units));
   c->part_cap = units;
@@ -236,6 +239,7 @@ ikv_status ensure_staging(ikv_ctx* c, int64_t tokens, int64_t qelems) {
   if (tokens > c->st_cap) {
     const int64_t cap = round_up(tokens, 1024);
     const size_t bytes = 16 + (size_t)cap * 9;
+    c->st_cap = 0;
     if (c->st_out) CU(c, cudaFree(c->st_out));
     if (c->st_host) CU(c, cudaFreeHost(c->st_host));
     c->st_out = nullptr; c->st_host = nullptr;
@@ -249,6 +253,7 @@ ikv_status ensure_staging(ikv_ctx* c, int64_t tokens, int64_t qelems) {
     c->st_cap = cap;
   }
   if (qelems > c->st_qcap) {
+    c->st_qcap = 0;
     TRY(grow(c, &c->st_qrows, qelems));
     c->st_qcap = qelems;
   }
@@ -258,6 +263,7 @@ ikv_status ensure_staging(ikv_ctx* c, int64_t tokens, int64_t qelems) {
 ikv_status session_live_reserve(ikv_ctx* c, Session& s, int n) {
   if (n <= s.live_cap) return IKV_OK;
   const int cap = (int)round_up((int64_t)n + n / 4 + 1024, 1024);
+  s.live_cap = 0;
   TRY(grow(c, &s.live_slots, cap));
   s.live_cap = cap;
   s.covered = 0;
