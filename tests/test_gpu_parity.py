@@ -351,6 +351,37 @@ def test_decode_batched_and_empty(ikv, oracle):
     assert torch.count_nonzero(out[-1]) == 0
 
 
+def test_decode_back_to_back_calls(ikv, oracle):
+    """Programmatic dependent launch (R27): 48 layer calls enqueued back to back without any host
+    synchronisation share the split-K scratch; each must still see only its own partials."""
+    shape = wl.ModelShape(3, 8, 2, 128, "bf16")
+    w = wl.small(seed=5, shape=shape, n_tokens=6000, budget=6000)
+    kp, vp = gc.to_cuda(w)
+    ctx = gc.make_ctx(w)
+    g = gc.oracle_geom(oracle, w)
+    s = w.sessions[0]
+    ctx.session_open(s.spec.session_id)
+    S = s.slot_map[:s.N].clone()
+    S[::5] = w.dead_slot
+    S_dev = S.cuda()
+    n_calls = 48
+    q = torch.randn((n_calls, 1, 8, 128), generator=torch.Generator().manual_seed(8)).to(torch.bfloat16)
+    q_dev = q.cuda()
+    out = torch.zeros((n_calls, 1, 8, 128), dtype=torch.bfloat16, device="cuda")
+    scale = 1 / math.sqrt(128)
+    # 32 calls of one length (an unbroken chain of programmatically launched kernels), then shrinking lengths (each of
+    # those forces a rescan kernel in between)
+    lens = [s.N] * 32 + [s.N - (i % 7) * 100 for i in range(n_calls - 32)]
+    torch.cuda.synchronize()
+    for i in range(n_calls):
+        r = gc.request(ikv, s, S_dev, seq_len=lens[i], flags=ikv.REQ_RESCAN if i == 0 else 0)
+        ctx.decode_attn(i % 3, [r], q_dev[i], out[i], scale)
+    torch.cuda.synchronize()
+    for i in range(n_calls):
+        want = oracle.decode(g, kp, vp, i % 3, S.numpy()[:lens[i]], q[i, 0].float().numpy(), scale)
+        gc.assert_decode_close(out[i, 0].float().cpu().numpy(), want, True, f"call {i}")
+
+
 def test_decode_padded_list_and_long_append(ikv, oracle):
     """Survivor list shorter than its host-side bound (live < C < N: the padding entries must be masked), then more
     than 4096 positions appended after the select (the library rescans the map instead of walking the tail)."""
