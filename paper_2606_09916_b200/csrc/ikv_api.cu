@@ -75,7 +75,8 @@ struct ikv_ctx {
   int64_t xq_cap = 0;
   // folded residual operands of the current call (residual_mma.cuh)
   float *mpart = nullptr, *bq_eff = nullptr, *b1_eff = nullptr;
-  uint4 *wq_frag = nullptr, *w1k_frag = nullptr;
+  uint4* wq_frag = nullptr;
+  unsigned char* w1_can = nullptr;  // fc1' chunks for tcgen05 (residual_mma.cuh)
   uint32_t* kept_bits = nullptr;
   int32_t* firstpos = nullptr;
   uint8_t* keepflag = nullptr;
@@ -548,7 +549,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     PostKeyParams pk;
     pk.partials = c->partials; pk.n_part = n_part; pk.lse = c->lse; pk.n_lse = LH;
     pk.mpart = c->mpart; pk.n_mpart = n_mpart; pk.LH = LH;
-    pk.fold.mbar = c->mbar; pk.fold.wq_frag = c->wq_frag; pk.fold.w1k_frag = c->w1k_frag;
+    pk.fold.mbar = c->mbar; pk.fold.wq_frag = c->wq_frag; pk.fold.w1_can = c->w1_can;
     pk.fold.bq_eff = c->bq_eff; pk.fold.b1_eff = c->b1_eff;
     pk.kq = c->kq; pk.n_xq = c->d_nxq; pk.nks = (int)(c->xq_cap / 16); pk.kc_frag = c->kc_frag; pk.vc_frag = c->vc_frag;
     pk.n_fold = 0; pk.n_kv = 0;
@@ -569,18 +570,18 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   if (learn) {
     ResidMmaParams rp;
     rp.rule_c = c->rule_c; rp.kbar = c->kbar; rp.n_cand = c->d_ncand; rp.cand_pos = c->cand_pos; rp.n_xq = c->d_nxq;
-    rp.wq_frag = c->wq_frag; rp.w1k_frag = c->w1k_frag; rp.kc_frag = c->kc_frag; rp.vc_frag = c->vc_frag;
+    rp.wq_frag = c->wq_frag; rp.w1_can = c->w1_can; rp.kc_frag = c->kc_frag; rp.vc_frag = c->vc_frag;
     rp.bq_eff = c->bq_eff; rp.b1_eff = c->b1_eff; rp.nks = (int)(c->xq_cap / 16);
     rp.use_xattn = (use_x && n_x > 0) ? 1 : 0;
     rp.scores = scores;
     const int nblk = (N + R_CWARPS * 16 - 1) / (R_CWARPS * 16);
     if (!c->resid_attr_done) {
-      CU(c, cudaFuncSetAttribute(k_residual_mma<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, RS_SMEM));
-      CU(c, cudaFuncSetAttribute(k_residual_mma<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, RS_SMEM));
+      CU(c, cudaFuncSetAttribute(k_residual_mma<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, resid_smem<128>()));
+      CU(c, cudaFuncSetAttribute(k_residual_mma<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, resid_smem<64>()));
       c->resid_attr_done = true;
     }
-    if (D == 128) k_residual_mma<128><<<nblk, R_THREADS, RS_SMEM, st>>>(rp, c->rw);
-    else k_residual_mma<64><<<nblk, R_THREADS, RS_SMEM, st>>>(rp, c->rw);
+    if (D == 128) k_residual_mma<128><<<nblk, R_THREADS, resid_smem<128>(), st>>>(rp, c->rw);
+    else k_residual_mma<64><<<nblk, R_THREADS, resid_smem<64>(), st>>>(rp, c->rw);
     LAUNCH_CHECK(c);
   }
   return IKV_OK;
@@ -687,7 +688,7 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
     ok = ok && cudaMalloc((void**)&c->bq_eff, R_DC * 4) == cudaSuccess;
     ok = ok && cudaMalloc((void**)&c->b1_eff, R_HID * 4) == cudaSuccess;
     ok = ok && cudaMalloc((void**)&c->wq_frag, (size_t)KS * 16 * 32 * sizeof(uint4)) == cudaSuccess;
-    ok = ok && cudaMalloc((void**)&c->w1k_frag, (size_t)4 * KS * 8 * 32 * sizeof(uint4)) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->w1_can, (size_t)2 * (cfg->head_dim / 64 + 2) * W1C_CHUNK) == cudaSuccess;
   }
   // B fragments: [L][Hkv][NT<=2][D/32][32 lanes] uint4
   ok = ok && cudaMalloc((void**)&c->frag, (size_t)cfg->n_layers * cfg->n_kv_heads * 2 * (cfg->head_dim / 32) * 32 *
@@ -708,7 +709,7 @@ ikv_status ikv_destroy(ikv_ctx* c) {
   for (auto& kv : c->sessions) session_free(kv.second);
   void* bufs[] = {c->cand_pos, c->cand_slot, c->d_ncand, c->logits, c->partials, c->lse, c->rule_c, c->kbar, c->mbar,
                   c->xq_slot, c->d_nxq, c->kq, c->kc_frag, c->vc_frag, c->mpart, c->bq_eff, c->b1_eff, c->wq_frag,
-                  c->w1k_frag, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
+                  c->w1_can, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
                   c->part_o, c->part_ml, c->st_out, c->st_scores,
                   c->st_qrows, c->resid_blob, c->frag};
   for (void* b : bufs) cudaFree(b);
@@ -858,6 +859,28 @@ ikv_status ikv_residual_load(ikv_ctx* c, const ikv_residual_weights* w) {
             o[0] = hi[0] | (hi[1] << 16); o[1] = hi[2] | (hi[3] << 16);
             o[2] = lo[0] | (lo[1] << 16); o[3] = lo[2] | (lo[3] << 16);
           }
+  }
+  {  // fc1's c columns as tcgen05 B-operand chunks (k >= D of w1_can; the kbar chunks are folded per call)
+    auto bf16_rn = [](float x) -> uint32_t {
+      uint32_t u;
+      memcpy(&u, &x, 4);
+      if ((u & 0x7fffffffu) > 0x7f800000u) return (u >> 16) | 0x40u;
+      return (u + 0x7fffu + ((u >> 16) & 1u)) >> 16;
+    };
+    auto up = [](uint32_t b) { uint32_t u = b << 16; float f; memcpy(&f, &u, 4); return f; };
+    const size_t bytes = (size_t)2 * (D / 64 + 2) * W1C_CHUNK;
+    std::vector<unsigned char> can(bytes, 0);
+    for (int n = 0; n < R_HID; ++n)
+      for (int kc = 0; kc < R_DC; ++kc) {
+        const float v = w->fc1_w[(size_t)n * IN + P + kc];
+        const uint32_t hi = bf16_rn(v), lo = bf16_rn(v - up(hi));
+        const size_t o = (D == 128) ? w1_can_offset<128>(n, D + kc) : w1_can_offset<64>(n, D + kc);
+        const uint16_t h16 = (uint16_t)hi, l16 = (uint16_t)lo;
+        memcpy(&can[o], &h16, 2);
+        memcpy(&can[o + W1C_PART], &l16, 2);
+      }
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(c->w1_can, can.data(), bytes, cudaMemcpyHostToDevice));
   }
   CU(c, cudaDeviceSynchronize());
   if (!c->resid_blob) CU(c, cudaMalloc((void**)&c->resid_blob, h.size() * 4));

@@ -81,21 +81,33 @@ __device__ __forceinline__ void mean_memory_part_block(int b, const float* __res
   part[b * D + d] = acc;
 }
 
+// fc1' as the B operand of tcgen05.mma (kind::f16, K-major, no swizzle): chunks of 128 hidden units x 64 k, each as a hi
+// and a lo bf16 part of W1C_PART bytes in the canonical layout (8 x 16-byte core matrices, 128 B contiguous; core
+// matrix (n/8, k/8) at ((n/8) * 8 + k/8) * 128).  k < D: folded kbar columns (natural order); k >= D: the c columns.
+constexpr int W1C_PART = 128 * 64 * 2;      // bytes of one part of one chunk
+constexpr int W1C_CHUNK = 2 * W1C_PART;     // hi | lo
+template <int D>
+__host__ __device__ inline size_t w1_can_offset(int n, int k) {
+  constexpr int NKC = D / 64 + 2;
+  const int nh = n >> 7, nl = n & 127, kc = k >> 6, kl = k & 63;
+  return (size_t)(nh * NKC + kc) * W1C_CHUNK + (size_t)((nl >> 3) * 8 + (kl >> 3)) * 128 + (nl & 7) * 16 + (kl & 7) * 2;
+}
+
 struct FoldOut {
   float* mbar;      // [D]
   uint4* wq_frag;   // [D/16][16][32]
-  uint4* w1k_frag;  // [4][D/16][8][32]
+  unsigned char* w1_can;  // fc1' for tcgen05: [2 N halves][D/64 + 2 K chunks][hi | lo][128 x 64 bf16, canonical K-major]
   float* bq_eff;    // [128]
   float* b1_eff;    // [256]
 };
 
 // Folds mbar into W_Q and fc1 (see the header of this file).  Blocks of 128 threads; resid_fold_grid() blocks cover
-// D/16*16*32 + 4*D/16*8*32 fragment items and 384 bias warps.
+// D/16*16*32 W_Q fragment items, 256*D/8 canonical fc1 rows and 384 bias warps.
 template <int D>
 __device__ __forceinline__ void resid_fold_block(int bid, const float* __restrict__ part, int n_part, int LH,
                                                  const ResidW& w, const FoldOut& o) {
   constexpr int KS = D / 16, P = 3 * D + 1, IN = P + R_DC;
-  constexpr int N_WQ = KS * 16 * 32, N_W1 = 4 * KS * 8 * 32, N_B = R_DC + R_HID;
+  constexpr int N_WQ = KS * 16 * 32, N_W1 = R_HID * (D / 8), N_B = R_DC + R_HID;
   __shared__ float mb[D];
   for (int d = threadIdx.x; d < D; d += 128) {
     float acc = 0.f;
@@ -117,13 +129,18 @@ __device__ __forceinline__ void resid_fold_block(int bid, const float* __restric
   }
   idx -= N_WQ;
   if (idx < N_W1) {
-    const int lane = idx & 31, t = (idx >> 5) & 7;
-    const int s = (idx >> 8) % KS, ch = (idx >> 8) / KS;
-    o.w1k_frag[idx] = make_bfrag(lane, [&](int kl, int nl) {
-      const int n = ch * 64 + t * 8 + nl, k = s * 16 + kperm(kl);
-      const float* row = w.fc1_w + (int64_t)n * IN;
-      return fmaf(row[2 * D + k], mb[k], row[k]);
-    });
+    // one 16-byte core-matrix row (8 consecutive k) of the folded fc1 kbar columns, hi and lo parts
+    const int n = idx / (D / 8), kg = idx % (D / 8), k0 = kg * 8;
+    const float* row = w.fc1_w + (int64_t)n * IN;
+    uint32_t hi[4], lo[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const int k = k0 + 2 * e;
+      split_bf16(fmaf(row[2 * D + k], mb[k], row[k]), fmaf(row[2 * D + k + 1], mb[k + 1], row[k + 1]), hi[e], lo[e]);
+    }
+    unsigned char* dst = o.w1_can + w1_can_offset<D>(n, k0);
+    *reinterpret_cast<uint4*>(dst) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+    *reinterpret_cast<uint4*>(dst + W1C_PART) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
     return;
   }
   idx -= N_W1;
@@ -142,7 +159,7 @@ __device__ __forceinline__ void resid_fold_block(int bid, const float* __restric
 }
 template <int D>
 inline int resid_fold_grid() {
-  return ((D / 16) * 16 * 32 + 4 * (D / 16) * 8 * 32 + (R_DC + R_HID) * 32 + 127) / 128;
+  return ((D / 16) * 16 * 32 + R_HID * (D / 8) + (R_DC + R_HID) * 32 + 127) / 128;
 }
 
 // Kc = W_K K^q + b_K, Vc = W_V K^q + b_V (Eq. 6): block `bid` = (16-key step v, cross-attention head hc), 128 threads
@@ -212,7 +229,8 @@ struct ResidMmaParams {
   const int32_t* n_cand;
   const int32_t* cand_pos;
   const int32_t* n_xq;
-  const uint4 *wq_frag, *w1k_frag, *kc_frag, *vc_frag;
+  const uint4 *wq_frag, *kc_frag, *vc_frag;
+  const unsigned char* w1_can;  // fc1' chunks (tcgen05 B operand)
   const float *bq_eff, *b1_eff;
   int nks;                   // capacity of the key fragments in 16-key steps
   int use_xattn;
@@ -226,39 +244,94 @@ __device__ __forceinline__ float ex2f(float x) {
   return y;
 }
 
-// ---- k_residual_mma: CTA = R_CWARPS consumer warps (one 16-candidate tile each) + 1 producer warp.
-// All B fragments are laid out in global memory in the order they are consumed, so the producer streams them as bulk
-// copies (TMA unit) through a ring of RS_BYTES stages and every consumer warp reads them with conflict-free 16-byte
-// shared loads: no fragment load waits on L2 and no fragment is fetched more than once per CTA.
-// Stage sequence (identical in producer and consumers):
-//   nq > 0:  KS stages  W_Q' k-step s (16 n-tiles)
-//            per head, per chunk of 64 query keys: 1 stage Kc (2 k-steps x ntn tiles), 1 stage Vc (nv steps x 4 tiles)
-//   4 x [ KS/2 stages fc1' kbar columns (2 k-steps x 8 tiles), nq > 0: 4 stages fc1 c columns (2 k-steps x 8 tiles) ]
+// ---- k_residual_mma: CTA = R_CWARPS consumer warps (one 16-candidate tile each) + 1 producer / MMA-issuer warp.
+// Q projection and cross-attention run per warp in registers on mma.sync; their B fragments are laid out in global
+// memory in consumption order and streamed by the producer as bulk copies (TMA unit) through a ring of RS_BYTES stages.
+// fc1 -- the dense contraction of the head, (tokens x (D+128)) x ((D+128) x 256) -- runs on tcgen05: the consumer warps
+// write their [kbar | c] rows, split into bf16 hi and lo parts, into shared memory in the canonical K-major layout (A
+// operand, M = 128 rows per CTA of which 16 R_CWARPS are used), the producer streams the folded fc1 chunks (B operand,
+// 128 hidden units x 64 k, hi | lo) into the dead ring and one thread issues hi*hi + lo*hi + hi*lo as tcgen05.mma
+// kind::f16 into two 128-column accumulators in TMEM; warps 0-3 read them back with tcgen05.ld (one token row per
+// thread) for the epilogue: + b1' + rule w_r, erf-GELU, fc2 dot, s = rule + alpha z.
+// Ring stage sequence (identical in producer and consumers), nq > 0 only:
+//   KS stages W_Q' k-step s (16 n-tiles); per head, per chunk of 64 query keys: 1 stage Kc, 1 stage Vc.
 constexpr int R_CWARPS = 7;
 constexpr int R_THREADS = (R_CWARPS + 1) * 32;
 constexpr int RS_BYTES = 8192;
 constexpr int RS_STAGES = 8;
-constexpr int RS_SMEM = RS_STAGES * RS_BYTES + 2 * 8 * RS_STAGES;
+constexpr int R_TMEM_COLS = 256;
+template <int D>
+constexpr int resid_smem() {
+  // ring / fc1 chunk buffers | A hi | A lo | epilogue vectors (b1', w_r, fc2) | barriers + tmem base
+  return RS_STAGES * RS_BYTES + 2 * 128 * (D + R_DC) * 2 + 3 * R_HID * 4 + 256;
+}
+
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+  // shared-memory matrix descriptor, SWIZZLE_NONE: start address, leading (K) and stride (M/N) byte offsets between
+  // core matrices, all >> 4; version 1 (sm_100)
+  return (uint64_t)((saddr >> 4) & 0x3fff) | ((uint64_t)((lbo >> 4) & 0x3fff) << 16) |
+         ((uint64_t)((sbo >> 4) & 0x3fff) << 32) | ((uint64_t)1 << 46);
+}
+__device__ __forceinline__ void umma_bf16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}" ::"r"(tmem_d),
+      "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 
 template <int D>
 __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaParams p, const ResidW w) {
   constexpr int KS = D / 16;
-  extern __shared__ __align__(128) unsigned char ring[];  // [RS_STAGES][RS_BYTES], then the barriers
-  uint64_t* full = reinterpret_cast<uint64_t*>(ring + RS_STAGES * RS_BYTES);
+  constexpr int KA = D + R_DC;                 // K of fc1 = row length of the A operand
+  constexpr int A_PART = 128 * KA * 2;         // bytes of A hi (and of A lo)
+  constexpr int A_SBO = (KA / 8) * 128;        // byte distance between 8-row groups of A
+  constexpr int NKC = D / 64 + 2;              // 64-wide K chunks of fc1: kbar chunks, then the two c chunks
+  extern __shared__ __align__(128) unsigned char ring[];  // [RS_STAGES][RS_BYTES] = two fc1 chunk buffers later
+  unsigned char* a_hi = ring + RS_STAGES * RS_BYTES;
+  unsigned char* a_lo = a_hi + A_PART;
+  float* ep_b1 = reinterpret_cast<float*>(a_lo + A_PART);  // [256] b1', then w_r, then fc2_w
+  float* ep_wr = ep_b1 + R_HID;
+  float* ep_w2 = ep_wr + R_HID;
+  uint64_t* full = reinterpret_cast<uint64_t*>(ep_w2 + R_HID);
   uint64_t* empty = full + RS_STAGES;
+  uint64_t* a_ready = empty + RS_STAGES;       // all consumer warps have written their A rows
+  uint64_t* bfull = a_ready + 1;               // [2] fc1 chunk landed
+  uint64_t* bempty = bfull + 2;                // [2] its MMAs have completed
+  uint64_t* tfull = bempty + 2;                // [2] accumulator half complete
+  uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(tfull + 2);
   const int nc = *p.n_cand;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, r = lane >> 2, q = lane & 3;
   if (blockIdx.x * R_CWARPS * 16 >= nc) return;
   const int nq = p.use_xattn ? *p.n_xq : 0;
   const int nkt = 2 * p.nks;
+  const int P = 3 * D + 1, IN = P + R_DC;
   if (threadIdx.x == 0) {
     for (int s = 0; s < RS_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], R_CWARPS); }
+    mbar_init(a_ready, R_CWARPS);
+    for (int i = 0; i < 2; ++i) { mbar_init(&bfull[i], 1); mbar_init(&bempty[i], 1); mbar_init(&tfull[i], 1); }
     mbar_fence_init();
   }
+  for (int n = threadIdx.x; n < R_HID; n += R_THREADS) {
+    ep_b1[n] = p.b1_eff[n];
+    ep_wr[n] = __ldg(w.fc1_w + (int64_t)n * IN + 3 * D);
+    ep_w2[n] = __ldg(w.fc2_w + n);
+  }
+  if (warp == R_CWARPS) {  // the producer warp owns the tensor-memory allocation
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_base_p)), "n"(R_TMEM_COLS));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tmem = *tmem_base_p;
+  const int n_kc = (nq > 0) ? NKC : D / 64;    // without live query keys c = 0: its chunks are skipped
 
   if (warp == R_CWARPS) {
-    // ------------------------------------------------------------------ producer
+    // ------------------------------------------------------------------ producer, then MMA issuer
     if (lane == 0) {
       int s = 0;
       uint32_t ph = 0;
@@ -279,12 +352,49 @@ __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaPar
             push(p.vc_frag + ((int64_t)(hc * p.nks + (kc0 >> 4)) * 4) * 32, nv * 4 * 512, nullptr, 0);
           }
       }
-      for (int ch = 0; ch < 4; ++ch) {
-        for (int ks = 0; ks < KS; ks += 2) push(p.w1k_frag + ((ch * KS + ks) * 8) * 32, 16 * 512, nullptr, 0);
-        if (nq > 0)
-          for (int ks = 0; ks < 8; ks += 2) push(w.w1c_frag + ((ch * 8 + ks) * 8) * 32, 16 * 512, nullptr, 0);
+      // ---- fc1 on tcgen05: wait for the A rows (which also means the ring is dead), stream the chunks, issue
+      mbar_wait(a_ready, 0u);
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      const int n_chunks = 2 * n_kc;
+      auto chunk_src = [&](int i) { return p.w1_can + (size_t)((i / n_kc) * NKC + (i % n_kc)) * W1C_CHUNK; };
+      auto load_chunk = [&](int i) {
+        const int b = i & 1;
+        mbar_arrive_expect_tx(&bfull[b], (uint32_t)W1C_CHUNK);
+        bulk_g2s(ring + b * W1C_CHUNK, chunk_src(i), (uint32_t)W1C_CHUNK, &bfull[b]);
+      };
+      // instruction descriptor: D fp32, A and B bf16, both K-major, N = 128, M = 128
+      const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+      load_chunk(0);
+      if (n_chunks > 1) load_chunk(1);
+      for (int i = 0; i < n_chunks; ++i) {
+        const int b = i & 1, nh = i / n_kc, kc = i % n_kc;
+        mbar_wait(&bfull[b], (uint32_t)(i >> 1) & 1u);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t bb = smem_u32(ring + b * W1C_CHUNK);
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks) {
+          const uint32_t a_off = (uint32_t)((kc * 8 + ks * 2) * 128);
+          const uint64_t dah = umma_desc(smem_u32(a_hi) + a_off, 128, A_SBO);
+          const uint64_t dal = umma_desc(smem_u32(a_lo) + a_off, 128, A_SBO);
+          const uint64_t dbh = umma_desc(bb + ks * 256, 128, 1024);
+          const uint64_t dbl = umma_desc(bb + W1C_PART + ks * 256, 128, 1024);
+          const uint32_t td = tmem + (uint32_t)(nh * 128);
+          umma_bf16(td, dah, dbh, idesc, (kc | ks) ? 1u : 0u);
+          umma_bf16(td, dal, dbh, idesc, 1u);
+          umma_bf16(td, dah, dbl, idesc, 1u);
+        }
+        umma_commit(&bempty[b]);
+        if (kc == n_kc - 1) umma_commit(&tfull[nh]);
+        if (i + 2 < n_chunks) {
+          mbar_wait(&bempty[b], (uint32_t)(i >> 1) & 1u);  // the MMAs reading this buffer are done
+          load_chunk(i + 2);
+        }
       }
     }
+    __syncwarp();
+    __syncthreads();  // epilogue finished (the consumer warps arrive below)
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(R_TMEM_COLS));
     return;
   }
 
@@ -293,7 +403,6 @@ __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaPar
   const bool live = t0 < nc;  // warps past the end still walk the ring
   const int row0 = min(t0 + r, nc - 1), row1 = min(t0 + r + 8, nc - 1);
   const float rule0 = p.rule_c[row0], rule1 = p.rule_c[row1];
-  const int P = 3 * D + 1, IN = P + R_DC;
   const uint32_t ring_u32 = smem_u32(ring) + lane * 16;
   int rs = 0;
   uint32_t rph = 0;
@@ -319,8 +428,17 @@ __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaPar
     split_bf16(x1.z, x1.w, akh[s][3], akl[s][3]);
   }
 
-  // A fragments of c (Eq. 6), 8 k-steps; unused when there is no live query key (R7)
-  uint32_t ach[8][4], acl[8][4];
+  // the same values as rows of the fc1 A operand (canonical K-major layout, natural k order)
+  const uint32_t a_row0 = (uint32_t)((warp * 2) * A_SBO + r * 16), a_row1 = a_row0 + (uint32_t)A_SBO;
+#pragma unroll
+  for (int s = 0; s < KS; ++s) {
+    const uint32_t ko = (uint32_t)((2 * s + (q >> 1)) * 128 + (q & 1) * 8);
+    *reinterpret_cast<uint2*>(a_hi + a_row0 + ko) = make_uint2(akh[s][0], akh[s][2]);
+    *reinterpret_cast<uint2*>(a_hi + a_row1 + ko) = make_uint2(akh[s][1], akh[s][3]);
+    *reinterpret_cast<uint2*>(a_lo + a_row0 + ko) = make_uint2(akl[s][0], akl[s][2]);
+    *reinterpret_cast<uint2*>(a_lo + a_row1 + ko) = make_uint2(akl[s][1], akl[s][3]);
+  }
+
   if (nq > 0) {
     // ---- Q = Wq' kbar + rule wq_r + bq'
     float accq[16][4];
@@ -418,63 +536,58 @@ __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaPar
       l0 += __shfl_xor_sync(0xffffffffu, l0, 1); l0 += __shfl_xor_sync(0xffffffffu, l0, 2);
       l1 += __shfl_xor_sync(0xffffffffu, l1, 1); l1 += __shfl_xor_sync(0xffffffffu, l1, 2);
       const float i0 = 1.f / l0, i1 = 1.f / l1;
+      // c_h (Eq. 6) -> columns D + 32 hc .. of the fc1 A operand, hi and lo parts
 #pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        const int ks = hc * 2 + u, na = 2 * u, nb = 2 * u + 1;
-        split_bf16(o[na][0] * i0, o[na][1] * i0, ach[ks][0], acl[ks][0]);
-        split_bf16(o[na][2] * i1, o[na][3] * i1, ach[ks][1], acl[ks][1]);
-        split_bf16(o[nb][0] * i0, o[nb][1] * i0, ach[ks][2], acl[ks][2]);
-        split_bf16(o[nb][2] * i1, o[nb][3] * i1, ach[ks][3], acl[ks][3]);
+      for (int nt = 0; nt < 4; ++nt) {
+        const uint32_t ko = (uint32_t)((D / 8 + hc * 4 + nt) * 128 + q * 4);
+        uint32_t h0, l0b, h1, l1b;
+        split_bf16(o[nt][0] * i0, o[nt][1] * i0, h0, l0b);
+        split_bf16(o[nt][2] * i1, o[nt][3] * i1, h1, l1b);
+        *reinterpret_cast<uint32_t*>(a_hi + a_row0 + ko) = h0;
+        *reinterpret_cast<uint32_t*>(a_lo + a_row0 + ko) = l0b;
+        *reinterpret_cast<uint32_t*>(a_hi + a_row1 + ko) = h1;
+        *reinterpret_cast<uint32_t*>(a_lo + a_row1 + ko) = l1b;
       }
     }
   }
 
-  // ---- fc1 -> GELU -> fc2, 4 chunks of 64 hidden units
-  float z0 = 0.f, z1 = 0.f;
+  // ---- fc1 on tcgen05 (issued by the producer warp): publish the A rows to the async proxy, then the epilogue
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  __syncwarp();
+  if (lane == 0) mbar_arrive(a_ready);
+  if (warp < 4) {
+    // thread = token row m of the CTA tile = TMEM lane m: hid = acc + b1' + rule w_r -> erf-GELU -> fc2 dot
+    const int m = warp * 32 + lane;
+    const int tok = blockIdx.x * R_CWARPS * 16 + m;
+    const bool valid = (m < R_CWARPS * 16) && (tok < nc);
+    const float rule = valid ? p.rule_c[tok] : 0.f;
+    float z = 0.f;
 #pragma unroll 1
-  for (int ch = 0; ch < 4; ++ch) {
-    float acc[8][4];
+    for (int nh = 0; nh < 2; ++nh) {
+      mbar_wait(&tfull[nh], 0u);
+      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll 1
+      for (int c0 = 0; c0 < 128; c0 += 16) {
+        uint32_t v[16];
+        const uint32_t taddr = tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(nh * 128 + c0);
+        asm volatile(
+            "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+            : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+              "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+            : "r"(taddr));
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-    for (int t = 0; t < 8; ++t) { acc[t][0] = acc[t][1] = acc[t][2] = acc[t][3] = 0.f; }
-#pragma unroll
-    for (int s = 0; s < KS; s += 2) {
-      const uint32_t sb = stage_wait();
-#pragma unroll
-      for (int t = 0; t < 8; ++t) mma3(acc[t], akh[s], akl[s], lds128(sb + t * 512));
-#pragma unroll
-      for (int t = 0; t < 8; ++t) mma3(acc[t], akh[s + 1], akl[s + 1], lds128(sb + (8 + t) * 512));
-      stage_done();
-    }
-    if (nq > 0) {
-#pragma unroll
-      for (int s = 0; s < 8; s += 2) {
-        const uint32_t sb = stage_wait();
-#pragma unroll
-        for (int t = 0; t < 8; ++t) mma3(acc[t], ach[s], acl[s], lds128(sb + t * 512));
-#pragma unroll
-        for (int t = 0; t < 8; ++t) mma3(acc[t], ach[s + 1], acl[s + 1], lds128(sb + (8 + t) * 512));
-        stage_done();
+        for (int j = 0; j < 16; ++j) {
+          const int n = nh * 128 + c0 + j;
+          z = fmaf(ep_w2[n], gelu_erf(__uint_as_float(v[j]) + fmaf(rule, ep_wr[n], ep_b1[n])), z);
+        }
       }
     }
-#pragma unroll
-    for (int t = 0; t < 8; ++t) {
-      const int n = ch * 64 + t * 8 + 2 * q;
-      const float2 b = *reinterpret_cast<const float2*>(p.b1_eff + n);
-      const float2 w2 = __ldg(reinterpret_cast<const float2*>(w.fc2_w + n));
-      const float wr0 = __ldg(w.fc1_w + (int64_t)n * IN + 3 * D), wr1 = __ldg(w.fc1_w + (int64_t)(n + 1) * IN + 3 * D);
-      z0 = fmaf(w2.x, gelu_erf(acc[t][0] + fmaf(rule0, wr0, b.x)), z0);
-      z0 = fmaf(w2.y, gelu_erf(acc[t][1] + fmaf(rule0, wr1, b.y)), z0);
-      z1 = fmaf(w2.x, gelu_erf(acc[t][2] + fmaf(rule1, wr0, b.x)), z1);
-      z1 = fmaf(w2.y, gelu_erf(acc[t][3] + fmaf(rule1, wr1, b.y)), z1);
-    }
+    if (valid) p.scores[p.cand_pos[tok]] = rule + w.alpha * (z + w.fc2_b[0]);
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   }
-  z0 += __shfl_xor_sync(0xffffffffu, z0, 1); z0 += __shfl_xor_sync(0xffffffffu, z0, 2);
-  z1 += __shfl_xor_sync(0xffffffffu, z1, 1); z1 += __shfl_xor_sync(0xffffffffu, z1, 2);
-  if (q == 0 && live) {
-    const float b2 = w.fc2_b[0];
-    if (t0 + r < nc) p.scores[p.cand_pos[t0 + r]] = rule0 + w.alpha * (z0 + b2);
-    if (t0 + r + 8 < nc) p.scores[p.cand_pos[t0 + r + 8]] = rule1 + w.alpha * (z1 + b2);
-  }
+  (void)live; (void)rule0; (void)rule1;
+  __syncthreads();  // the producer warp frees the tensor memory after this
 }
 
 }  // namespace ikv
