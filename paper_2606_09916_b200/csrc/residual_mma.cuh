@@ -256,14 +256,15 @@ __device__ __forceinline__ float ex2f(float x) {
 // Ring stage sequence (identical in producer and consumers), nq > 0 only:
 //   KS stages W_Q' k-step s (16 n-tiles); per head, per chunk of 64 query keys: 1 stage Kc, 1 stage Vc.
 constexpr int R_CWARPS = 7;
-constexpr int R_THREADS = (R_CWARPS + 1) * 32;
+constexpr int R_THREADS = (R_CWARPS + 2) * 32;  // + ring producer warp + fc1 loader / MMA issuer warp
 constexpr int RS_BYTES = 8192;
-constexpr int RS_STAGES = 8;
+constexpr int RS_STAGES = 4;
 constexpr int R_TMEM_COLS = 256;
 template <int D>
 constexpr int resid_smem() {
-  // ring / fc1 chunk buffers | A hi | A lo | epilogue vectors (b1', w_r, fc2) | barriers + tmem base
-  return RS_STAGES * RS_BYTES + 2 * 128 * (D + R_DC) * 2 + 3 * R_HID * 4 + 256;
+  // ring | two fc1 chunk buffers | A hi | A lo (16 R_CWARPS rows each) | epilogue vectors (b1', w_r, fc2), z halves |
+  // barriers + tmem base
+  return RS_STAGES * RS_BYTES + 2 * W1C_CHUNK + 2 * (R_CWARPS * 16) * (D + R_DC) * 2 + 3 * R_HID * 4 + 2 * 128 * 4 + 256;
 }
 
 __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
@@ -284,22 +285,26 @@ __device__ __forceinline__ void umma_commit(uint64_t* bar) {
 }
 
 template <int D>
-__global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaParams p, const ResidW w) {
+__global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaParams p, const ResidW w) {  // 9 warps
   constexpr int KS = D / 16;
   constexpr int KA = D + R_DC;                 // K of fc1 = row length of the A operand
-  constexpr int A_PART = 128 * KA * 2;         // bytes of A hi (and of A lo)
+  constexpr int A_PART = R_CWARPS * 16 * KA * 2;  // bytes of A hi (and of A lo); the MMA's rows 112..127 read past it
   constexpr int A_SBO = (KA / 8) * 128;        // byte distance between 8-row groups of A
-  constexpr int NKC = D / 64 + 2;              // 64-wide K chunks of fc1: kbar chunks, then the two c chunks
-  extern __shared__ __align__(128) unsigned char ring[];  // [RS_STAGES][RS_BYTES] = two fc1 chunk buffers later
-  unsigned char* a_hi = ring + RS_STAGES * RS_BYTES;
+  constexpr int KCK = D / 64;                  // 64-wide K chunks of the kbar columns
+  constexpr int NKC = KCK + 2;                 // ... then the two c chunks
+  // A first: the MMA's unused rows 112..127 of a_lo then fall into the chunk buffers, inside the allocation
+  extern __shared__ __align__(128) unsigned char a_hi[];
   unsigned char* a_lo = a_hi + A_PART;
-  float* ep_b1 = reinterpret_cast<float*>(a_lo + A_PART);  // [256] b1', then w_r, then fc2_w
+  unsigned char* bbuf = a_lo + A_PART;                     // two fc1 chunk buffers
+  unsigned char* ring = bbuf + 2 * W1C_CHUNK;              // [RS_STAGES][RS_BYTES]
+  float* ep_b1 = reinterpret_cast<float*>(ring + RS_STAGES * RS_BYTES);  // [256] b1', then w_r, then fc2_w
   float* ep_wr = ep_b1 + R_HID;
   float* ep_w2 = ep_wr + R_HID;
-  uint64_t* full = reinterpret_cast<uint64_t*>(ep_w2 + R_HID);
+  float* ep_z = ep_w2 + R_HID;                 // [2][128] fc2 partial dots of the two accumulator halves
+  uint64_t* full = reinterpret_cast<uint64_t*>(ep_z + 2 * 128);
   uint64_t* empty = full + RS_STAGES;
-  uint64_t* a_ready = empty + RS_STAGES;       // all consumer warps have written their A rows
-  uint64_t* bfull = a_ready + 1;               // [2] fc1 chunk landed
+  uint64_t* a_ready = empty + RS_STAGES;       // [2]: kbar columns of A written / c columns written (all consumer warps)
+  uint64_t* bfull = a_ready + 2;               // [2] fc1 chunk landed
   uint64_t* bempty = bfull + 2;                // [2] its MMAs have completed
   uint64_t* tfull = bempty + 2;                // [2] accumulator half complete
   uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(tfull + 2);
@@ -311,7 +316,8 @@ __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaPar
   const int P = 3 * D + 1, IN = P + R_DC;
   if (threadIdx.x == 0) {
     for (int s = 0; s < RS_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], R_CWARPS); }
-    mbar_init(a_ready, R_CWARPS);
+    mbar_init(&a_ready[0], R_CWARPS);
+    mbar_init(&a_ready[1], R_CWARPS);
     for (int i = 0; i < 2; ++i) { mbar_init(&bfull[i], 1); mbar_init(&bempty[i], 1); mbar_init(&tfull[i], 1); }
     mbar_fence_init();
   }
@@ -320,7 +326,7 @@ __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaPar
     ep_wr[n] = __ldg(w.fc1_w + (int64_t)n * IN + 3 * D);
     ep_w2[n] = __ldg(w.fc2_w + n);
   }
-  if (warp == R_CWARPS) {  // the producer warp owns the tensor-memory allocation
+  if (warp == R_CWARPS + 1) {  // the MMA warp owns the tensor-memory allocation
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_base_p)), "n"(R_TMEM_COLS));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
@@ -328,10 +334,66 @@ __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaPar
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const uint32_t tmem = *tmem_base_p;
-  const int n_kc = (nq > 0) ? NKC : D / 64;    // without live query keys c = 0: its chunks are skipped
+
+  if (warp == R_CWARPS + 1) {
+    // ------------------------------------------------------------------ fc1 on tcgen05: chunk loader and MMA issuer.
+    // The kbar columns of A are written at kernel start, so their chunks are multiplied while the consumer warps are
+    // still in the Q projection and the cross attention; only the c chunks wait for them.
+    if (lane == 0) {
+      // instruction descriptor: D fp32, A and B bf16, both K-major, N = 128, M = 128
+      const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
+      const int n_k = 2 * KCK, n_chunks = n_k + (nq > 0 ? 4 : 0);
+      auto chunk_id = [&](int i, int& nh, int& kc) {  // kbar chunks of both halves first, then the c chunks
+        if (i < n_k) { nh = i / KCK; kc = i % KCK; } else { nh = (i - n_k) >> 1; kc = KCK + ((i - n_k) & 1); }
+      };
+      auto load_chunk = [&](int i) {
+        int nh, kc;
+        chunk_id(i, nh, kc);
+        const int b = i & 1;
+        mbar_arrive_expect_tx(&bfull[b], (uint32_t)W1C_CHUNK);
+        bulk_g2s(bbuf + b * W1C_CHUNK, p.w1_can + (size_t)(nh * NKC + kc) * W1C_CHUNK, (uint32_t)W1C_CHUNK, &bfull[b]);
+      };
+      load_chunk(0);
+      if (n_chunks > 1) load_chunk(1);
+      mbar_wait(&a_ready[0], 0u);
+      for (int i = 0; i < n_chunks; ++i) {
+        int nh, kc;
+        chunk_id(i, nh, kc);
+        const int b = i & 1;
+        if (i == n_k) mbar_wait(&a_ready[1], 0u);
+        mbar_wait(&bfull[b], (uint32_t)(i >> 1) & 1u);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const uint32_t bb = smem_u32(bbuf + b * W1C_CHUNK);
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks) {
+          const uint32_t a_off = (uint32_t)((kc * 8 + ks * 2) * 128);
+          const uint64_t dah = umma_desc(smem_u32(a_hi) + a_off, 128, A_SBO);
+          const uint64_t dal = umma_desc(smem_u32(a_lo) + a_off, 128, A_SBO);
+          const uint64_t dbh = umma_desc(bb + ks * 256, 128, 1024);
+          const uint64_t dbl = umma_desc(bb + W1C_PART + ks * 256, 128, 1024);
+          const uint32_t td = tmem + (uint32_t)(nh * 128);
+          umma_bf16(td, dah, dbh, idesc, (kc | ks) ? 1u : 0u);
+          umma_bf16(td, dal, dbh, idesc, 1u);
+          umma_bf16(td, dah, dbl, idesc, 1u);
+        }
+        umma_commit(&bempty[b]);
+        if (kc == (nq > 0 ? NKC : KCK) - 1) umma_commit(&tfull[nh]);
+        if (i + 2 < n_chunks) {
+          mbar_wait(&bempty[b], (uint32_t)(i >> 1) & 1u);  // the MMAs reading this buffer are done
+          load_chunk(i + 2);
+        }
+      }
+    }
+    __syncwarp();
+    __syncthreads();  // z halves written
+    __syncthreads();  // epilogue finished
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(R_TMEM_COLS));
+    return;
+  }
 
   if (warp == R_CWARPS) {
-    // ------------------------------------------------------------------ producer, then MMA issuer
+    // ------------------------------------------------------------------ ring producer (then joins the epilogue)
     if (lane == 0) {
       int s = 0;
       uint32_t ph = 0;
@@ -352,52 +414,9 @@ __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaPar
             push(p.vc_frag + ((int64_t)(hc * p.nks + (kc0 >> 4)) * 4) * 32, nv * 4 * 512, nullptr, 0);
           }
       }
-      // ---- fc1 on tcgen05: wait for the A rows (which also means the ring is dead), stream the chunks, issue
-      mbar_wait(a_ready, 0u);
-      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      const int n_chunks = 2 * n_kc;
-      auto chunk_src = [&](int i) { return p.w1_can + (size_t)((i / n_kc) * NKC + (i % n_kc)) * W1C_CHUNK; };
-      auto load_chunk = [&](int i) {
-        const int b = i & 1;
-        mbar_arrive_expect_tx(&bfull[b], (uint32_t)W1C_CHUNK);
-        bulk_g2s(ring + b * W1C_CHUNK, chunk_src(i), (uint32_t)W1C_CHUNK, &bfull[b]);
-      };
-      // instruction descriptor: D fp32, A and B bf16, both K-major, N = 128, M = 128
-      const uint32_t idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
-      load_chunk(0);
-      if (n_chunks > 1) load_chunk(1);
-      for (int i = 0; i < n_chunks; ++i) {
-        const int b = i & 1, nh = i / n_kc, kc = i % n_kc;
-        mbar_wait(&bfull[b], (uint32_t)(i >> 1) & 1u);
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint32_t bb = smem_u32(ring + b * W1C_CHUNK);
-#pragma unroll
-        for (int ks = 0; ks < 4; ++ks) {
-          const uint32_t a_off = (uint32_t)((kc * 8 + ks * 2) * 128);
-          const uint64_t dah = umma_desc(smem_u32(a_hi) + a_off, 128, A_SBO);
-          const uint64_t dal = umma_desc(smem_u32(a_lo) + a_off, 128, A_SBO);
-          const uint64_t dbh = umma_desc(bb + ks * 256, 128, 1024);
-          const uint64_t dbl = umma_desc(bb + W1C_PART + ks * 256, 128, 1024);
-          const uint32_t td = tmem + (uint32_t)(nh * 128);
-          umma_bf16(td, dah, dbh, idesc, (kc | ks) ? 1u : 0u);
-          umma_bf16(td, dal, dbh, idesc, 1u);
-          umma_bf16(td, dah, dbl, idesc, 1u);
-        }
-        umma_commit(&bempty[b]);
-        if (kc == n_kc - 1) umma_commit(&tfull[nh]);
-        if (i + 2 < n_chunks) {
-          mbar_wait(&bempty[b], (uint32_t)(i >> 1) & 1u);  // the MMAs reading this buffer are done
-          load_chunk(i + 2);
-        }
-      }
     }
     __syncwarp();
-    __syncthreads();  // epilogue finished (the consumer warps arrive below)
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(R_TMEM_COLS));
-    return;
-  }
-
+  } else {
   // -------------------------------------------------------------------- consumers
   const int t0 = (blockIdx.x * R_CWARPS + warp) * 16;
   const bool live = t0 < nc;  // warps past the end still walk the ring
@@ -438,6 +457,9 @@ __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaPar
     *reinterpret_cast<uint2*>(a_lo + a_row0 + ko) = make_uint2(akl[s][0], akl[s][2]);
     *reinterpret_cast<uint2*>(a_lo + a_row1 + ko) = make_uint2(akl[s][1], akl[s][3]);
   }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // publish the rows to the async proxy (tcgen05.mma)
+  __syncwarp();
+  if (lane == 0) mbar_arrive(&a_ready[0]);
 
   if (nq > 0) {
     // ---- Q = Wq' kbar + rule wq_r + bq'
@@ -551,43 +573,45 @@ __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaPar
     }
   }
 
-  // ---- fc1 on tcgen05 (issued by the producer warp): publish the A rows to the async proxy, then the epilogue
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the c columns of A
   __syncwarp();
-  if (lane == 0) mbar_arrive(a_ready);
-  if (warp < 4) {
-    // thread = token row m of the CTA tile = TMEM lane m: hid = acc + b1' + rule w_r -> erf-GELU -> fc2 dot
-    const int m = warp * 32 + lane;
+  if (lane == 0) mbar_arrive(&a_ready[1]);
+  (void)live; (void)rule0; (void)rule1;
+  }  // consumer warps
+
+  // ---- epilogue, warps 0..7: warp w reads TMEM lanes 32 (w % 4) .. + 31 (token rows) of accumulator half w / 4:
+  // hid = acc + b1' + rule w_r -> erf-GELU -> fc2 dot; the two halves of a row are added through shared memory
+  {
+    const int qd = warp & 3, nh = warp >> 2;
+    const int m = qd * 32 + lane;
     const int tok = blockIdx.x * R_CWARPS * 16 + m;
     const bool valid = (m < R_CWARPS * 16) && (tok < nc);
     const float rule = valid ? p.rule_c[tok] : 0.f;
     float z = 0.f;
+    mbar_wait(&tfull[nh], 0u);
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
-    for (int nh = 0; nh < 2; ++nh) {
-      mbar_wait(&tfull[nh], 0u);
-      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-#pragma unroll 1
-      for (int c0 = 0; c0 < 128; c0 += 16) {
-        uint32_t v[16];
-        const uint32_t taddr = tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(nh * 128 + c0);
-        asm volatile(
-            "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-            : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-              "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-            : "r"(taddr));
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    for (int c0 = 0; c0 < 128; c0 += 16) {
+      uint32_t v[16];
+      const uint32_t taddr = tmem + ((uint32_t)(qd * 32) << 16) + (uint32_t)(nh * 128 + c0);
+      asm volatile(
+          "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+          : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+            "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+          : "r"(taddr));
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const int n = nh * 128 + c0 + j;
-          z = fmaf(ep_w2[n], gelu_erf(__uint_as_float(v[j]) + fmaf(rule, ep_wr[n], ep_b1[n])), z);
-        }
+      for (int j = 0; j < 16; ++j) {
+        const int n = nh * 128 + c0 + j;
+        z = fmaf(ep_w2[n], gelu_erf(__uint_as_float(v[j]) + fmaf(rule, ep_wr[n], ep_b1[n])), z);
       }
     }
-    if (valid) p.scores[p.cand_pos[tok]] = rule + w.alpha * (z + w.fc2_b[0]);
+    ep_z[nh * 128 + m] = z;
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (nh == 0 && valid) p.scores[p.cand_pos[tok]] = rule + w.alpha * ((ep_z[m] + ep_z[128 + m]) + w.fc2_b[0]);
+    __syncthreads();  // the MMA warp frees the tensor memory after this
   }
-  (void)live; (void)rule0; (void)rule1;
-  __syncthreads();  // the producer warp frees the tensor memory after this
 }
 
 }  // namespace ikv
