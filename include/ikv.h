@@ -148,7 +148,9 @@ ikv_status ikv_select_evict(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req
  * Stream ordering (R27): the kernels of this call are launched with programmatic stream serialization and
  * read q, the slot maps and the K/V pools as soon as they start; they order only their WRITES after the preceding
  * kernel of the stream.  This is ordinary stream order as long as the producer of those inputs is a normally
- * completing kernel or copy (anything but this library's own decode kernels, which write none of them); a caller whose
+ * completing kernel or copy, or one of this library's kernels: the scoring kernels of ikv_score trigger their
+ * dependents early but wait on their own predecessor first and write none of these inputs, ikv_select_evict and the
+ * rescan, which write the survivor lists, never trigger early; a caller whose
  * own producer kernel triggers its dependents early (griddepcontrol.launch_dependents) must not do so before its
  * writes, or sets IKV_PDL=0 in the environment.  Up to 32 requests go into one launch; larger batches are chunked. */
 ikv_status ikv_decode_attn(ikv_ctx *ctx, int32_t layer, const ikv_request *reqs, int32_t n_req, const void *q,

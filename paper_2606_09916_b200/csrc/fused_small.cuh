@@ -14,6 +14,8 @@ template <int D, int G>
 __global__ __launch_bounds__(128) void k_mem_prep(const float* __restrict__ M, int L, int Hkv, float inv_sqrt_d,
                                                   uint4* __restrict__ frag, int n_frag_blocks, int LH,
                                                   float* __restrict__ mpart) {
+  pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
+  pdl_launch_dependents();
   const int bid = blockIdx.x;
   if (bid < n_frag_blocks) {
     memory_frags_item<D, G>(bid * 128 + threadIdx.x, M, L, Hkv, inv_sqrt_d, frag);
@@ -35,6 +37,8 @@ struct PostKeyParams {
 
 template <int D>
 __global__ __launch_bounds__(128) void k_post_key(const PostKeyParams p, const ResidW w) {
+  pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
+  pdl_launch_dependents();
   int bid = blockIdx.x;
   if (bid < p.n_lse) { score_lse_block(bid, p.partials, p.n_part, p.lse); return; }
   bid -= p.n_lse;
@@ -53,6 +57,8 @@ struct RuleParams {
 // kernel needs all three, and the small bodies hide under the rule blocks' stream of the logits.
 template <int D>
 __global__ __launch_bounds__(256) void k_rule_fused(const RuleParams r, const PostKeyParams p, const ResidW w) {
+  pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
+  pdl_launch_dependents();
   int bid = blockIdx.x;
   if (bid < r.n_rule) {
     score_rule4_block(bid, r.n_rule, r.logits, r.ldc, r.LH, r.lse, r.n_cand, r.cand_pos, r.rule_c, r.scores,

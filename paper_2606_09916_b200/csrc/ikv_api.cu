@@ -61,6 +61,7 @@ struct ikv_ctx {
   int max_smem = 48 * 1024;  // opt-in dynamic shared memory per CTA
   uint4* frag = nullptr;     // B fragments of M / sqrt(D) for the bf16 key pass
   bool use_pdl = true;       // programmatic dependent launch between decode kernels (IKV_PDL=0 disables)
+  bool pdl_prune = true;     // ... and along the kernels of the prune pass (IKV_PDL_PRUNE=0 disables)
   bool attr_done[2][2][9] = {};
 
   // scratch (per request, sized by ensure_scratch)
@@ -443,8 +444,8 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
                            cudaStream_t st) {
   const int L = c->cfg.n_layers, Hkv = c->cfg.n_kv_heads, Hq = c->cfg.n_q_heads;
   const int n_fb = mem_prep_frag_blocks<D, G>(L, Hkv);
-  k_mem_prep<D, G><<<n_fb + n_mpart, 128, 0, st>>>(M, L, Hkv, 1.0f / sqrtf((float)D), c->frag, n_fb, L * Hq, c->mpart);
-  LAUNCH_CHECK(c);
+  CU(c, launch_pdl(k_mem_prep<D, G>, dim3(n_fb + n_mpart), dim3(128), 0, st, c->pdl_prune, M, L, Hkv,
+                   1.0f / sqrtf((float)D), c->frag, n_fb, L * Hq, c->mpart));
   int ns = 0;
   const size_t smem = key_pass_smem(L, Hq, Hkv, D, kbar, c->max_smem, &ns);
   if (ns < 2) IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "key pass: L*Hq = %d and row of %d bytes do not fit shared memory", L * Hq,
@@ -460,11 +461,11 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
   if (kbar) {
     auto fn = k_key_pass<D, G, true>;
     CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    fn<<<grid, kp_threads(G, true), smem, st>>>(p);
+    CU(c, launch_pdl(fn, dim3(grid), dim3(kp_threads(G, true)), smem, st, c->pdl_prune, p));
   } else {
     auto fn = k_key_pass<D, G, false>;
     CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    fn<<<grid, kp_threads(G, false), smem, st>>>(p);
+    CU(c, launch_pdl(fn, dim3(grid), dim3(kp_threads(G, false)), smem, st, c->pdl_prune, p));
   }
   LAUNCH_CHECK(c);
   *n_part = grid;
@@ -513,15 +514,18 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
 #define IKV_PART_ARGS r.slot_map, N, c->cfg.dead_slot, r.prefix_len, r.q_start, r.q_end, scores, rule_out, \
                       c->cand_pos, c->cand_slot, c->d_ncand
 #define IKV_X_ARGS r.xattn_pos, n_x, c->xq_slot, c->d_nxq
-    if (N <= CL_CTAS * 1024 * 4) k_partition_cl<4><<<grid, 1024, 0, st>>>(IKV_PART_ARGS, IKV_X_ARGS);
-    else if (N <= CL_CTAS * 1024 * 8) k_partition_cl<8><<<grid, 1024, 0, st>>>(IKV_PART_ARGS, IKV_X_ARGS);
-    else if (N <= CL_MAX_N) k_partition_cl<16><<<grid, 1024, 0, st>>>(IKV_PART_ARGS, IKV_X_ARGS);
+#define IKV_PART_LAUNCH(MAXI) \
+  CU(c, launch_pdl(k_partition_cl<MAXI>, dim3(grid), dim3(1024), 0, st, c->pdl_prune, IKV_PART_ARGS, IKV_X_ARGS))
+    if (N <= CL_CTAS * 1024 * 4) IKV_PART_LAUNCH(4);
+    else if (N <= CL_CTAS * 1024 * 8) IKV_PART_LAUNCH(8);
+    else if (N <= CL_MAX_N) IKV_PART_LAUNCH(16);
     else {
       k_partition<<<1, 1024, 0, st>>>(IKV_PART_ARGS);
       if (n_x > 0)
         k_xattn_compact<<<1, 1024, 0, st>>>(r.slot_map, N, c->cfg.dead_slot, r.xattn_pos, n_x, r.q_start, c->xq_slot,
                                             c->d_nxq);
     }
+#undef IKV_PART_LAUNCH
 #undef IKV_PART_ARGS
 #undef IKV_X_ARGS
     LAUNCH_CHECK(c);
@@ -553,9 +557,8 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     pk.fold.bq_eff = c->bq_eff; pk.fold.b1_eff = c->b1_eff;
     pk.kq = c->kq; pk.n_xq = c->d_nxq; pk.nks = (int)(c->xq_cap / 16); pk.kc_frag = c->kc_frag; pk.vc_frag = c->vc_frag;
     pk.n_fold = 0; pk.n_kv = 0;
-    if (D == 128) k_post_key<128><<<pk.n_lse, 128, 0, st>>>(pk, c->rw);
-    else k_post_key<64><<<pk.n_lse, 128, 0, st>>>(pk, c->rw);
-    LAUNCH_CHECK(c);
+    CU(c, launch_pdl(D == 128 ? k_post_key<128> : k_post_key<64>, dim3(pk.n_lse), dim3(128), 0, st, c->pdl_prune, pk,
+                     c->rw));
     pk.n_fold = learn ? (D == 128 ? resid_fold_grid<128>() : resid_fold_grid<64>()) : 0;
     pk.n_kv = (learn && n_x > 0) ? 4 * ((n_x + 15) / 16) : 0;
     RuleParams rp;
@@ -563,9 +566,8 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     rp.cand_pos = c->cand_pos; rp.rule_c = c->rule_c; rp.scores = scores; rp.scatter_scores = learn ? 0 : 1;
     rp.rule_out = rule_out; rp.n_rule = (N + 63) / 64;
     const int grid = rp.n_rule + pk.n_fold + pk.n_kv;
-    if (D == 128) k_rule_fused<128><<<grid, 256, 0, st>>>(rp, pk, c->rw);
-    else k_rule_fused<64><<<grid, 256, 0, st>>>(rp, pk, c->rw);
-    LAUNCH_CHECK(c);
+    CU(c, launch_pdl(D == 128 ? k_rule_fused<128> : k_rule_fused<64>, dim3(grid), dim3(256), 0, st, c->pdl_prune, rp, pk,
+                     c->rw));
   }
   if (learn) {
     ResidMmaParams rp;
@@ -580,9 +582,8 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
       CU(c, cudaFuncSetAttribute(k_residual_mma<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, resid_smem<64>()));
       c->resid_attr_done = true;
     }
-    if (D == 128) k_residual_mma<128><<<nblk, R_THREADS, resid_smem<128>(), st>>>(rp, c->rw);
-    else k_residual_mma<64><<<nblk, R_THREADS, resid_smem<64>(), st>>>(rp, c->rw);
-    LAUNCH_CHECK(c);
+    CU(c, launch_pdl(D == 128 ? k_residual_mma<128> : k_residual_mma<64>, dim3(nblk), dim3(R_THREADS),
+                     D == 128 ? resid_smem<128>() : resid_smem<64>(), st, c->pdl_prune, rp, c->rw));
   }
   return IKV_OK;
 }
@@ -617,10 +618,9 @@ ikv_status select_prepare(ikv_ctx* c, const ikv_request& r, const float* scores,
 // One launch for up to SEL_MAX_REQ requests (one cluster each); longer maps take the single-CTA kernel one by one.
 ikv_status select_launch(ikv_ctx* c, const SelBatch& b, int n, int max_n, cudaStream_t st) {
   if (n == 0) return IKV_OK;
-  if (max_n <= CL_CTAS * 1024 * 4) k_select_evict_cl<4><<<n * CL_CTAS, 1024, 0, st>>>(b);
-  else if (max_n <= CL_CTAS * 1024 * 8) k_select_evict_cl<8><<<n * CL_CTAS, 1024, 0, st>>>(b);
-  else k_select_evict_cl<16><<<n * CL_CTAS, 1024, 0, st>>>(b);
-  LAUNCH_CHECK(c);
+  auto fn = max_n <= CL_CTAS * 1024 * 4 ? k_select_evict_cl<4>
+            : max_n <= CL_CTAS * 1024 * 8 ? k_select_evict_cl<8> : k_select_evict_cl<16>;
+  CU(c, launch_pdl(fn, dim3(n * CL_CTAS), dim3(1024), 0, st, c->pdl_prune, b));
   return IKV_OK;
 }
 
@@ -662,6 +662,8 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
   cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
   cudaDeviceGetAttribute(&c->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   if (const char* e = getenv("IKV_PDL")) c->use_pdl = atoi(e) != 0;
+  c->pdl_prune = c->use_pdl;
+  if (const char* e = getenv("IKV_PDL_PRUNE")) c->pdl_prune = atoi(e) != 0;
   const int row = cfg->n_kv_heads * cfg->head_dim;
   if (cfg->kv_dtype == IKV_BF16)
     k_init_dead<bf16><<<cfg->n_layers, 256>>>((bf16*)cfg->k_pool, (bf16*)cfg->v_pool, c->layer_stride, cfg->n_layers,

@@ -292,6 +292,8 @@ __global__ __launch_bounds__(R_THREADS, 1) void k_residual_mma(const ResidMmaPar
   constexpr int A_SBO = (KA / 8) * 128;        // byte distance between 8-row groups of A
   constexpr int KCK = D / 64;                  // 64-wide K chunks of the kbar columns
   constexpr int NKC = KCK + 2;                 // ... then the two c chunks
+  pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
+  pdl_launch_dependents();
   // A first: the MMA's unused rows 112..127 of a_lo then fall into the chunk buffers, inside the allocation
   extern __shared__ __align__(128) unsigned char a_hi[];
   unsigned char* a_lo = a_hi + A_PART;

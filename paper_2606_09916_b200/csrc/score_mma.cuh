@@ -102,6 +102,8 @@ struct KeyPassParams {
 // mean-key warp (kp_merged).
 template <int D, int G, bool KBAR>
 __global__ __launch_bounds__(kp_threads(G, KBAR), 1) void k_key_pass(const KeyPassParams p) {
+  pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
+  pdl_launch_dependents();
   constexpr int KS = D / 16, NI = D / 32, NT = (G <= 4) ? 1 : 2;
   constexpr bool MERGED = kp_merged(G, KBAR);
   constexpr int KP_THREADS = kp_threads(G, KBAR);

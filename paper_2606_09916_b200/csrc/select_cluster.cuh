@@ -7,6 +7,7 @@
 #pragma once
 #include <cooperative_groups.h>
 #include "common.cuh"
+#include "pipe.cuh"
 #include "select.cuh"
 
 namespace ikv {
@@ -43,6 +44,8 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_partit
     float* __restrict__ rule_out, int32_t* __restrict__ cand_pos, int32_t* __restrict__ cand_slot,
     int32_t* __restrict__ n_cand, const int32_t* __restrict__ xattn_pos, int n_x, int32_t* __restrict__ xq_slot,
     int32_t* __restrict__ n_xq) {
+  pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
+  pdl_launch_dependents();
   cg::cluster_group cl = cg::this_cluster();
   const int crank = (int)cl.block_rank();
   __shared__ int warp_tot[32];
@@ -118,6 +121,9 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_partit
 // ---------------------------------------------------------------------------------------------------------------
 template <int MAXI>
 __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select_evict_cl(const SelBatch batch) {
+  // waits on its predecessor; never triggers its dependents early: the decode kernel that may follow reads the
+  // survivor list written here before its own wait (R27)
+  pdl_wait();
   // one cluster per request of the batch.  Requests run concurrently on the shared kept-slot bitmap and
   // first-dropped-position table: they may share slots only below their radix_protected_len (forks, R19), where neither
   // structure is consulted, and every request clears exactly the bits it set.
