@@ -351,6 +351,58 @@ def test_decode_batched_and_empty(ikv, oracle):
     assert torch.count_nonzero(out[-1]) == 0
 
 
+def test_prune_decode_chain_without_host_sync(ikv, oracle):
+    """The kernels of the prune pass and of decode are all launched with programmatic stream serialization
+    (R27).  Six turns of score -> select/evict -> three decode layers are enqueued back to back on one
+    stream with no host synchronisation; the shared per-call scratch (candidate list, logits, fragment tables,
+    split-K partials) is reused by every turn, so a kernel that ran ahead of its predecessor would corrupt a
+    neighbouring turn.  Every turn is then checked against the oracle."""
+    shape = wl.ModelShape(3, 8, 2, 128, "bf16")
+    w = wl.small(seed=17, shape=shape, n_tokens=5000, budget=1200, kv_dtype="bf16")
+    ctx, s, M, kp, vp = run_memory(ikv, oracle, w)
+    g = gc.oracle_geom(oracle, w)
+    wts = wl.residual_weights(w.shape.D, 31)
+    ow = oracle.ResidualWeights(**wts)
+    ctx.residual_load(wts)
+    S0 = s.slot_map[:s.N].numpy().copy()
+    n_turn = 6
+    budgets = [1200, 900, 2000, 700, 1500, 1000]
+    modes = [ikv.MODE_LEARNABLE, ikv.MODE_MEMORY] * 3
+    S_dev = [torch.from_numpy(S0.copy()).cuda() for _ in range(n_turn)]
+    scores = [torch.empty(s.N, device="cuda") for _ in range(n_turn)]
+    freed = [torch.empty(s.N, dtype=torch.int32, device="cuda") for _ in range(n_turn)]
+    nf = torch.zeros(n_turn, dtype=torch.int32, device="cuda")
+    nk = torch.zeros(n_turn, dtype=torch.int32, device="cuda")
+    q = torch.randn((n_turn, 3, 1, 8, 128), generator=torch.Generator().manual_seed(3)).to(torch.bfloat16)
+    q_dev = q.cuda()
+    out = torch.zeros((n_turn, 3, 1, 8, 128), dtype=torch.bfloat16, device="cuda")
+    scale = 1 / math.sqrt(128)
+    reqs = [gc.request(ikv, s, S_dev[t], budget=budgets[t]) for t in range(n_turn)]
+    torch.cuda.synchronize()
+    for t in range(n_turn):
+        ctx.score([reqs[t]], modes[t], scores[t])
+        ctx.select_evict([reqs[t]], scores[t], freed[t], nf[t:t + 1], nk[t:t + 1])
+        for layer in range(3):
+            ctx.decode_attn(layer, [reqs[t]], q_dev[t, layer], out[t, layer], scale)
+    torch.cuda.synchronize()
+    for t in range(n_turn):
+        omode = oracle.MODE_LEARNABLE if modes[t] == ikv.MODE_LEARNABLE else oracle.MODE_MEMORY
+        want = oracle.score(g, kp, M, S0, s.pi, s.qs, s.qe, omode, 0, w=ow)
+        got = scores[t].cpu().numpy()
+        gc.assert_scores_close(got, want, f"turn {t}")
+        # select / rewrite are bit-exact on the scores the GPU produced
+        cls, _ = oracle.partition(S0, w.dead_slot, s.pi, s.qs, s.qe)
+        keep, n_kept = oracle.select(got, cls, budgets[t])
+        S2, _, freed_o = oracle.rewrite(S0, w.dead_slot, keep, s.pi, w.n_slots)
+        assert nk[t].item() == n_kept
+        assert np.array_equal(S_dev[t].cpu().numpy(), S2), f"turn {t}: slot map"
+        assert nf[t].item() == len(freed_o)
+        assert np.array_equal(freed[t].cpu().numpy()[:len(freed_o)], freed_o)
+        for layer in range(3):
+            o = oracle.decode(g, kp, vp, layer, S2, q[t, layer, 0].float().numpy(), scale)
+            gc.assert_decode_close(out[t, layer, 0].float().cpu().numpy(), o, True, f"turn {t} layer {layer}")
+
+
 def test_decode_back_to_back_calls(ikv, oracle):
     """Programmatic dependent launch (R27): 48 layer calls enqueued back to back without any host
     synchronisation share the split-K scratch; each must still see only its own partials."""
