@@ -56,7 +56,7 @@ struct RuleParams {
 // Kc / Vc fragments (latency-bound 128-thread bodies, warps 4-7 of their blocks exit) in one launch: the residual
 // kernel needs all three, and the small bodies hide under the rule blocks' stream of the logits.
 template <int D>
-__global__ __launch_bounds__(256) void k_rule_fused(const RuleParams r, const PostKeyParams p, const ResidW w) {
+__global__ __launch_bounds__(256, 4) void k_rule_fused(const RuleParams r, const PostKeyParams p, const ResidW w) {
   pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
   pdl_launch_dependents();
   int bid = blockIdx.x;
