@@ -1,8 +1,8 @@
 // fused_small.cuh -- the small per-call kernels around the key pass, fused into two launches (each launch costs
 // ~1.2 us of stream latency on B200, and several of these bodies are latency-bound on their own):
 //   k_mem_prep : B fragments of M / sqrt(D) for the key pass  |  partial sums of mbar (Eq. 5)
-//   k_post_key : lse[l,h] from the per-CTA partials (Eq. 3)   |  folded W_Q / fc1 operands  |  Kc / Vc fragments (Eq. 6)
-// Blocks of 128 threads; the block index selects the body.
+//   k_post_key : lse[l,h] from the per-CTA partials (Eq. 3), a warp per row
+//   k_rule_fused : rule_c (Eq. 3)  |  folded W_Q / fc1 operands  |  Kc / Vc fragments (Eq. 6); the block index selects the body.
 #pragma once
 #include "residual_mma.cuh"
 #include "score.cuh"
@@ -35,16 +35,26 @@ struct PostKeyParams {
   const float* kq; const int32_t* n_xq; int nks; uint4 *kc_frag, *vc_frag; int n_kv;  // Kc / Vc blocks
 };
 
+// lse[l,h] = log sum_c exp(x[l,h,c]) from the per-CTA (max, sum) partials of the key pass: one warp per (l,h) row, no
+// block barrier (the row has one partial per key-pass CTA, 148 of them).
 template <int D>
 __global__ __launch_bounds__(128) void k_post_key(const PostKeyParams p, const ResidW w) {
   pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
   pdl_launch_dependents();
-  int bid = blockIdx.x;
-  if (bid < p.n_lse) { score_lse_block(bid, p.partials, p.n_part, p.lse); return; }
-  bid -= p.n_lse;
-  if (bid < p.n_fold) { resid_fold_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.fold); return; }
-  bid -= p.n_fold;
-  resid_kv_frags_block(bid, p.kq, p.n_xq, D, w, p.nks, p.kc_frag, p.vc_frag);
+  (void)w;
+  const int row = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (row >= p.n_lse) return;
+  const float2* pp = p.partials + (int64_t)row * p.n_part;
+  float mx = -CUDART_INF_F;
+  for (int i = lane; i < p.n_part; i += 32) mx = fmaxf(mx, pp[i].x);
+  mx = warp_max(mx);
+  float s = 0.f;
+  for (int i = lane; i < p.n_part; i += 32) {
+    const float2 v = pp[i];
+    if (v.y > 0.f) s += v.y * expf(v.x - mx);
+  }
+  s = warp_sum(s);
+  if (lane == 0) p.lse[row] = mx + logf(s);
 }
 
 struct RuleParams {

@@ -557,7 +557,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     pk.fold.bq_eff = c->bq_eff; pk.fold.b1_eff = c->b1_eff;
     pk.kq = c->kq; pk.n_xq = c->d_nxq; pk.nks = (int)(c->xq_cap / 16); pk.kc_frag = c->kc_frag; pk.vc_frag = c->vc_frag;
     pk.n_fold = 0; pk.n_kv = 0;
-    CU(c, launch_pdl(D == 128 ? k_post_key<128> : k_post_key<64>, dim3(pk.n_lse), dim3(128), 0, st, c->pdl_prune, pk,
+    CU(c, launch_pdl(D == 128 ? k_post_key<128> : k_post_key<64>, dim3((pk.n_lse + 3) / 4), dim3(128), 0, st, c->pdl_prune, pk,
                      c->rw));
     pk.n_fold = learn ? (D == 128 ? resid_fold_grid<128>() : resid_fold_grid<64>()) : 0;
     pk.n_kv = (learn && n_x > 0) ? 4 * ((n_x + 15) / 16) : 0;

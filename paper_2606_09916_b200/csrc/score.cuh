@@ -172,29 +172,6 @@ __global__ __launch_bounds__(256) void k_score_logits(
   }
 }
 
-// lse[l,h] = log sum_c exp(x[l,h,c]) from the per-CTA partials.  One block of 128 threads per (l,h) row `row`.
-__device__ __forceinline__ void score_lse_block(int row, const float2* __restrict__ partials, int n_tiles,
-                                                float* __restrict__ lse) {
-  __shared__ float red[4];
-  const float2* p = partials + (int64_t)row * n_tiles;
-  float mx = -CUDART_INF_F;
-  for (int i = threadIdx.x; i < n_tiles; i += 128) mx = fmaxf(mx, p[i].x);
-  mx = warp_max(mx);
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
-  __syncthreads();
-  mx = fmaxf(fmaxf(red[0], red[1]), fmaxf(red[2], red[3]));
-  __syncthreads();
-  float s = 0.f;
-  for (int i = threadIdx.x; i < n_tiles; i += 128) {
-    const float2 v = p[i];
-    if (v.y > 0.f) s += v.y * expf(v.x - mx);
-  }
-  s = warp_sum(s);
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
-  __syncthreads();
-  if (threadIdx.x == 0) lse[row] = mx + logf(red[0] + red[1] + red[2] + red[3]);
-}
-
 // live cross-attention positions ("positions evicted in a prior round are excluded"):
 // compacts the slots of the live entries of xattn_pos (or of [qs,qe) when xattn_pos == NULL).  1 CTA of 1024.
 __global__ __launch_bounds__(1024) void k_xattn_compact(const int32_t* __restrict__ S, int N, int32_t dead,
