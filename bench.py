@@ -311,7 +311,8 @@ def run_ours(args):
     req_h = ikv.make_request(sid, None, T, sess.pi, sess.qs, sess.qe, C, sess.pi)
     e2e_t = []
     n_freed_h = 0
-    for i in range(args.warmup + args.steps):
+    n_e2e = max(args.steps, 20)     # a call takes well under a millisecond of wall clock: at least 20 of them, mean
+    for i in range(args.warmup + n_e2e):
         h_map.copy_(h_map0)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
@@ -319,7 +320,7 @@ def run_ours(args):
         dt = time.perf_counter() - t0
         if i >= args.warmup:
             e2e_t.append(dt)
-    e2e_total = sum(e2e_t)
+    e2e_total = sum(e2e_t) * args.steps / n_e2e     # scaled to the K steps of the device-timed region
     h2d = T * 4 + h_rows.numel() * h_rows.element_size()
     d2h = 16 + ((T + 1023) // 1024 * 1024) * 8 + T     # one copy: counts | slot map | freed list (capacity) | valid mask
 
@@ -374,7 +375,8 @@ def run_ours(args):
             "e2e": {"value": world * T * K / (e2e_ms_total * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": d2h,
                     "what": "ikv_prune_host: slot map + bf16 query rows H2D, memory update + score + select/evict, "
-                            "slot map + valid mask + freed list + counts D2H; the K/V pool is device-resident state"},
+                            "slot map + valid mask + freed list + counts D2H; the K/V pool is device-resident state; "
+                            "wall clock around each call, mean of max(steps, 20) calls"},
             "gpu_launches": K * (n_prune_launch + n_decode_launch),
             "roofline": {"kernel": "k_key_pass", "bound": "hbm", "achieved": ach, "peak": hbm_peak,
                          "unit": "GB/s", "frac": ach / hbm_peak, "frac_of_nominal_8TBs": ach / NOMINAL_HBM_GBS,
