@@ -210,6 +210,9 @@ def run_ours(args):
     sess = w.sessions[0]
     L, Hq, Hkv, D = shape.L, shape.Hq, shape.Hkv, shape.D
     ctx = ikv.Context(L, Hq, Hkv, D, w.k_pool, w.v_pool, dead_slot=w.dead_slot)
+    for kv in args.tune:                                  # experiment knobs (ikv_tune), e.g. --tune 2=0
+        k, v = kv.split("=")
+        ctx.tune(int(k), int(v))
     ctx.reserve(T + DEC, 1)
     ctx.residual_load(wl.residual_weights(D, w.seed + 5))
     sid = sess.spec.session_id
@@ -422,6 +425,7 @@ def main():
     ap.add_argument("--decode-steps", type=int, default=256)
     ap.add_argument("--ref-layers", type=int, default=12, help="layers in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--tune", action="append", default=[], help="ikv_tune knob=value (A/B experiments)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

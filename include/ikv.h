@@ -52,7 +52,14 @@ typedef int32_t ikv_status;
 #define IKV_FLAG_NO_RESIDUAL 0x200 /* "- residual": alpha = 0, recovers the rule scorer exactly      */
 
 /* request flags */
-#define IKV_REQ_RESCAN 1 /* ikv_decode_attn: ignore the cached live list, rescan the slot map       */
+#define IKV_REQ_RESCAN 1          /* ikv_decode_attn: ignore the cached live list, rescan the slot map            */
+#define IKV_REQ_INPUTS_COMPLETE 2 /* ikv_decode_attn: q, the slot-map tail and the K/V rows of this call were
+                                     complete before the PRECEDING kernel of the stream started (e.g. precomputed
+                                     queries): the kernel may read them before it orders itself after that kernel */
+
+/* ikv_config.flags */
+#define IKV_CFG_NO_PDL 1       /* never launch with programmatic stream serialization (plain stream order)          */
+#define IKV_CFG_NO_PDL_PRUNE 2 /* ... only the kernels of the pruning pass                                          */
 
 typedef struct {
   int32_t n_layers, n_q_heads, n_kv_heads, head_dim; /* L, H_q, H_kv, D; H_q % H_kv == 0; D in {64,128}   */
@@ -64,6 +71,7 @@ typedef struct {
                                                         layer                              */
   float lambda;                                      /* decay of Eq. 2; the paper uses 0.5 */
   int32_t max_sessions;                              /* LRU capacity; the paper uses 1024  */
+  int32_t flags;                                     /* IKV_CFG_*; 0 = defaults                           */
 } ikv_config;
 
 /* One request of a batch.  The array of requests lives on the HOST. */
@@ -80,6 +88,10 @@ typedef struct {
   const int32_t *xattn_pos;    /* DEVICE, positions forming K^q (Eq. 6); NULL => [q_s,q_e) (R7)           */
   int32_t n_xattn_pos;
   int32_t flags;               /* IKV_REQ_*                                                               */
+  uint32_t map_epoch;          /* version of the CONTENT behind slot_map: a caller that reuses a slot-map allocation
+                                  for different content (freed and reallocated at the same address, edited by hand)
+                                  bumps it; ikv_decode_attn rescans when it differs from the epoch seen by the last
+                                  ikv_select_evict / rescan of the session.  0 is an ordinary value.            */
 } ikv_request;
 
 /* Residual head parameters (R9), HOST fp32 arrays, row-major [out][in]:
@@ -95,6 +107,7 @@ typedef struct {
  * Synchronises.  *out receives the context. */
 ikv_status ikv_create(const ikv_config *cfg, ikv_ctx **out);
 ikv_status ikv_destroy(ikv_ctx *ctx);
+/* ctx == NULL: the reason of the last failed ikv_create on this thread. */
 const char *ikv_last_error(const ikv_ctx *ctx);
 
 /* Pre-sizes every scratch buffer so that later hot calls never allocate: `max_tokens` = largest sum of
@@ -166,13 +179,33 @@ ikv_status ikv_prune_host(ikv_ctx *ctx, const ikv_request *req, const void *q_ro
                           float *scores_host, int32_t *freed_host, int32_t *n_freed_host, int32_t *n_kept_host,
                           void *stream);
 
-/* Kernel-level timing for bench.py's roofline: while enabled, the library brackets its two dominant kernels
- * (the key pass k_key_pass / k_score_logits and the decode split kernel k_decode_mma / k_decode_split) with CUDA events on the caller's stream
- * (no host synchronisation; not allowed during stream capture).  ikv_profile_read synchronises, sums the
- * elapsed times recorded since the last read and clears them.
- * out_ms[0] = key-pass total ms, out_ms[1] = decode-split total ms; out_n[0], out_n[1] = launch counts. */
-ikv_status ikv_profile_enable(ikv_ctx *ctx, int32_t on);
+/* Kernel-level timing for bench.py's roofline and breakdown: while enabled, the library brackets kernels with CUDA
+ * events on the caller's stream (no host synchronisation; skipped during stream capture).  level 1: only the two dominant
+ * kernels (slots IKV_PROF_KEY_PASS, IKV_PROF_DECODE); level 2: every kernel of the path -- the events between the launches
+ * take away the overlap of programmatically launched kernels, so level 2 is a diagnostic, not a timing of the pass.
+ * ikv_profile_read synchronises, sums the elapsed times recorded per slot since the last read and clears them:
+ * out_ms[IKV_PROF_SLOTS] = total ms per slot, out_n[IKV_PROF_SLOTS] = launch counts. */
+#define IKV_PROF_KEY_PASS 0     /* k_key_pass / k_score_logits */
+#define IKV_PROF_DECODE 1       /* k_decode_mma / k_decode_split */
+#define IKV_PROF_MEM_UPDATE 2
+#define IKV_PROF_PARTITION 3
+#define IKV_PROF_MEM_PREP 4
+#define IKV_PROF_POST_KEY 5
+#define IKV_PROF_RULE 6
+#define IKV_PROF_RESIDUAL 7
+#define IKV_PROF_SELECT 8
+#define IKV_PROF_DECODE_MERGE 9
+#define IKV_PROF_SLOTS 12
+ikv_status ikv_profile_enable(ikv_ctx *ctx, int32_t level);
 ikv_status ikv_profile_read(ikv_ctx *ctx, float *out_ms, int32_t *out_n);
+
+/* Experiment knobs (A/B measurements; defaults are the tuned values).  Unknown knobs return
+ * IKV_ERR_INVALID_ARG.  Never needed for correctness. */
+#define IKV_TUNE_L2_HINTS 1 /* bit 0: key stream evict_first; bit 1: logits scratch evict_last; bit 2: rule reads
+                               evict_first (default 7)                                                         */
+#define IKV_TUNE_RESID_TC 2 /* 1 (default): residual head with folded cross attention on tcgen05 when the call has at
+                               most 64 cross-attention positions; 0: always the unfolded kernel                */
+ikv_status ikv_tune(ikv_ctx *ctx, int32_t knob, int32_t value);
 
 /* Library / build identification, e.g. "ikv 0.1 sm_100a". */
 const char *ikv_version(void);

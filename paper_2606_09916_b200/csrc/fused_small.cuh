@@ -5,6 +5,7 @@
 //   k_rule_fused : rule_c (Eq. 3)  |  folded W_Q / fc1 operands  |  Kc / Vc fragments (Eq. 6); the block index selects the body.
 #pragma once
 #include "residual_mma.cuh"
+#include "residual_tc.cuh"
 #include "score.cuh"
 #include "score_mma.cuh"
 
@@ -33,6 +34,7 @@ struct PostKeyParams {
   const float2* partials; int n_part; float* lse; int n_lse;          // lse rows
   const float* mpart; int n_mpart; int LH; FoldOut fold; int n_fold;  // fold blocks (0: not a learnable call)
   const float* kq; const int32_t* n_xq; int nks; uint4 *kc_frag, *vc_frag; int n_kv;  // Kc / Vc blocks
+  int tc; int nxp; RtFoldOut rt;  // tc != 0: operands of k_residual_tc instead (n_fold fc1 blocks, n_kv cross-attention blocks)
 };
 
 // lse[l,h] = log sum_c exp(x[l,h,c]) from the per-CTA (max, sum) partials of the key pass: one warp per (l,h) row, no
@@ -60,26 +62,35 @@ __global__ __launch_bounds__(128) void k_post_key(const PostKeyParams p, const R
 struct RuleParams {
   const float* logits; int64_t ldc; int LH; const float* lse; const int32_t* n_cand; const int32_t* cand_pos;
   float* rule_c; float* scores; int scatter_scores; float* rule_out; int n_rule;  // rule blocks (256 threads)
+  int l2_hints;
 };
 
 // rule_c of Eq. 3 (HBM-bound, 256-thread blocks) and, for a learnable call, the folded W_Q / fc1 operands and the
 // Kc / Vc fragments (latency-bound 128-thread bodies, warps 4-7 of their blocks exit) in one launch: the residual
 // kernel needs all three, and the small bodies hide under the rule blocks' stream of the logits.
-template <int D>
+template <int D, bool TC>
 __global__ __launch_bounds__(256, 4) void k_rule_fused(const RuleParams r, const PostKeyParams p, const ResidW w) {
   pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
   pdl_launch_dependents();
   int bid = blockIdx.x;
   if (bid < r.n_rule) {
     score_rule4_block(bid, r.n_rule, r.logits, r.ldc, r.LH, r.lse, r.n_cand, r.cand_pos, r.rule_c, r.scores,
-                      r.scatter_scores, r.rule_out);
+                      r.scatter_scores, r.rule_out, r.l2_hints);
     return;
   }
-  if (threadIdx.x >= 128) return;
   bid -= r.n_rule;
-  if (bid < p.n_fold) { resid_fold_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.fold); return; }
-  bid -= p.n_fold;
-  resid_kv_frags_block(bid, p.kq, p.n_xq, D, w, p.nks, p.kc_frag, p.vc_frag);
+  if constexpr (TC) {  // operands of k_residual_tc
+    if (bid < p.n_fold) {
+      if (threadIdx.x < 128) rt_fold_fc1_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.rt);
+      return;
+    }
+    rt_fold_xattn_block<D>(bid - p.n_fold, p.mpart, p.n_mpart, p.LH, p.kq, p.n_xq, p.nxp, w, p.rt);
+  } else {             // operands of k_residual_mma
+    if (threadIdx.x >= 128) return;
+    if (bid < p.n_fold) { resid_fold_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.fold); return; }
+    bid -= p.n_fold;
+    resid_kv_frags_block(bid, p.kq, p.n_xq, D, w, p.nks, p.kc_frag, p.vc_frag);
+  }
 }
 
 }  // namespace ikv

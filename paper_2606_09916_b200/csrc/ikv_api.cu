@@ -17,6 +17,7 @@
 #include "decode.cuh"
 #include "decode_mma.cuh"
 #include "residual_mma.cuh"
+#include "residual_tc.cuh"
 #include "score.cuh"
 #include "score_mma.cuh"
 #include "select.cuh"
@@ -40,6 +41,9 @@ struct Session {
   int covered = 0;            // positions [0, covered) are represented by the list
   int live_ub = 0;            // host upper bound of the list length
   const int32_t* map_ptr = nullptr;
+  uint32_t map_epoch = 0;     // ikv_request.map_epoch at the last select / rescan
+  bool list_fresh = false;    // live_slots was rewritten by the last library launch on this session: the next decode
+                              // launch is made WITHOUT programmatic serialization (full stream order), see R27
 };
 
 template <typename T>
@@ -63,6 +67,7 @@ struct ikv_ctx {
   bool use_pdl = true;       // programmatic dependent launch between decode kernels (IKV_PDL=0 disables)
   bool pdl_prune = true;     // ... and along the kernels of the prune pass (IKV_PDL_PRUNE=0 disables)
   bool attr_done[2][2][9] = {};
+  int dbg_l2 = 7;            // IKV_TUNE_L2_HINTS
 
   // scratch (per request, sized by ensure_scratch)
   int64_t cap_tokens = 0;
@@ -78,6 +83,8 @@ struct ikv_ctx {
   float *mpart = nullptr, *bq_eff = nullptr, *b1_eff = nullptr;
   uint4* wq_frag = nullptr;
   unsigned char* w1_can = nullptr;  // fc1' chunks for tcgen05 (residual_mma.cuh)
+  unsigned char* rt_wcan = nullptr; // operand chunks of k_residual_tc (residual_tc.cuh)
+  float* rt_svec = nullptr;         // s_r | s_b
   uint32_t* kept_bits = nullptr;
   int32_t* firstpos = nullptr;
   uint8_t* keepflag = nullptr;
@@ -94,12 +101,15 @@ struct ikv_ctx {
   unsigned char* st_host = nullptr;  // pinned host mirror of st_out
 
   // kernel-level profiling (ikv_profile_*)
-  bool prof_on = false;
-  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[2];
+  int prof_on = 0;           // 0 off, 1 the two dominant kernels, 2 every kernel of the path
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[IKV_PROF_SLOTS];
+  std::vector<cudaEvent_t> ev_pool;   // events are created once and reused (ikv_profile_read returns them here)
 
   // residual head (transposed on the device)
   bool has_resid = false;
   bool resid_attr_done = false;
+  bool resid_tc_attr_done = false;
+  int resid_tc = 1;          // IKV_TUNE_RESID_TC: 0 = always the unfolded kernel
   float* resid_blob = nullptr;
   ResidW rw{};
 };
@@ -135,13 +145,19 @@ namespace {
 struct ProfScope {  // brackets a launch with events when profiling is on and the stream is not capturing
   ikv_ctx* c; int which; cudaStream_t st; cudaEvent_t a = nullptr, b = nullptr;
   ProfScope(ikv_ctx* c_, int which_, cudaStream_t st_) : c(c_), which(which_), st(st_) {
-    if (!c->prof_on) return;
+    if (!c->prof_on || (c->prof_on < 2 && which > IKV_PROF_DECODE)) return;
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     cudaStreamIsCapturing(st, &cs);
     if (cs != cudaStreamCaptureStatusNone) return;
-    cudaEventCreate(&a);
-    cudaEventCreate(&b);
+    a = take();
+    b = take();
     cudaEventRecord(a, st);
+  }
+  cudaEvent_t take() {
+    if (!c->ev_pool.empty()) { cudaEvent_t e = c->ev_pool.back(); c->ev_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
   }
   ~ProfScope() {
     if (!a) return;
@@ -280,7 +296,10 @@ void session_free(Session& s) {
   cudaFree(s.d_n_live);
 }
 
-ikv_status session_create(ikv_ctx* c, uint64_t id, Session** out) {
+// M_0 = 0 (R3).  The zero fills are enqueued on `st`, the stream the session's first use is enqueued on; with
+// `sync` (ikv_session_open, which has no stream) the host waits for them, so that they are ordered before work on any
+// stream, including non-blocking ones.
+ikv_status session_create(ikv_ctx* c, uint64_t id, Session** out, cudaStream_t st, bool sync) {
   auto it = c->sessions.find(id);
   if (it == c->sessions.end()) {
     if ((int)c->sessions.size() >= c->cfg.max_sessions) {  // LRU eviction
@@ -300,10 +319,12 @@ ikv_status session_create(ikv_ctx* c, uint64_t id, Session** out) {
   }
   Session& s = it->second;
   const size_t n = (size_t)c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim;
-  CU(c, cudaMemset(s.d_mem, 0, n * sizeof(float)));  // M_0 = 0 (R3)
-  CU(c, cudaMemset(s.d_qenc, 0, n * sizeof(float)));
-  CU(c, cudaMemset(s.d_n_live, 0, sizeof(int32_t)));
+  CU(c, cudaMemsetAsync(s.d_mem, 0, n * sizeof(float), st));  // M_0 = 0 (R3)
+  CU(c, cudaMemsetAsync(s.d_qenc, 0, n * sizeof(float), st));
+  CU(c, cudaMemsetAsync(s.d_n_live, 0, sizeof(int32_t), st));
+  if (sync) CU(c, cudaStreamSynchronize(st));
   s.has_update = false;
+  s.list_fresh = false;
   s.covered = 0;
   s.map_ptr = nullptr;
   s.tick = ++c->tick;
@@ -376,7 +397,7 @@ ikv_status dispatch_logits(ikv_ctx* c, const Session& s, const float* M, int N, 
 
 template <typename T, int D, int G>
 ikv_status launch_decode(ikv_ctx* c, int layer, const DecBatch& batch, int n_req, int n_split, const void* q,
-                         void* out, float sm_scale, cudaStream_t st) {
+                         void* out, float sm_scale, cudaStream_t st, bool pdl_split) {
   const int Hkv = c->cfg.n_kv_heads, Hq = c->cfg.n_q_heads;
   const T* kl = (const T*)c->cfg.k_pool + (int64_t)layer * c->layer_stride;
   const T* vl = (const T*)c->cfg.v_pool + (int64_t)layer * c->layer_stride;
@@ -398,7 +419,7 @@ ikv_status launch_decode(ikv_ctx* c, int layer, const DecBatch& batch, int n_req
     }
     {
       ProfScope prof(c, 1, st);
-      CU(c, launch_pdl(fn, dim3(n_split, n_req, n_hg), dim3(DM_THREADS), smem, st, c->use_pdl, p, batch));
+      CU(c, launch_pdl(fn, dim3(n_split, n_req, n_hg), dim3(DM_THREADS), smem, st, pdl_split, p, batch));
     }
   } else {
     constexpr int VEC = Elem<T>::VEC;
@@ -411,6 +432,7 @@ ikv_status launch_decode(ikv_ctx* c, int layer, const DecBatch& batch, int n_req
                                                      c->part_o, c->part_ml, n_split);
     LAUNCH_CHECK(c);
   }
+  ProfScope prof(c, IKV_PROF_DECODE_MERGE, st);
   CU(c, launch_pdl(k_decode_merge4<T, D>, dim3(Hq, n_req), dim3(DMG_THREADS), 0, st, c->use_pdl, (const float*)c->part_o,
                    (const float2*)c->part_ml, n_split, batch, (T*)out));
   return IKV_OK;
@@ -418,24 +440,24 @@ ikv_status launch_decode(ikv_ctx* c, int layer, const DecBatch& batch, int n_req
 
 template <typename T, int D>
 ikv_status dispatch_decode_g(ikv_ctx* c, int layer, const DecBatch& b, int n_req, int n_split, const void* q,
-                             void* out, float sc, cudaStream_t st) {
+                             void* out, float sc, cudaStream_t st, bool pdl) {
   switch (c->G) {
-    case 1: return launch_decode<T, D, 1>(c, layer, b, n_req, n_split, q, out, sc, st);
-    case 2: return launch_decode<T, D, 2>(c, layer, b, n_req, n_split, q, out, sc, st);
-    case 4: return launch_decode<T, D, 4>(c, layer, b, n_req, n_split, q, out, sc, st);
-    case 5: return launch_decode<T, D, 5>(c, layer, b, n_req, n_split, q, out, sc, st);
-    case 8: return launch_decode<T, D, 8>(c, layer, b, n_req, n_split, q, out, sc, st);
+    case 1: return launch_decode<T, D, 1>(c, layer, b, n_req, n_split, q, out, sc, st, pdl);
+    case 2: return launch_decode<T, D, 2>(c, layer, b, n_req, n_split, q, out, sc, st, pdl);
+    case 4: return launch_decode<T, D, 4>(c, layer, b, n_req, n_split, q, out, sc, st, pdl);
+    case 5: return launch_decode<T, D, 5>(c, layer, b, n_req, n_split, q, out, sc, st, pdl);
+    case 8: return launch_decode<T, D, 8>(c, layer, b, n_req, n_split, q, out, sc, st, pdl);
   }
   IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "GQA group size %d not supported (1,2,4,5,8)", c->G);
 }
 
 ikv_status dispatch_decode(ikv_ctx* c, int layer, const DecBatch& b, int n_req, int n_split, const void* q,
-                           void* out, float sc, cudaStream_t st) {
+                           void* out, float sc, cudaStream_t st, bool pdl) {
   const bool bf = c->cfg.kv_dtype == IKV_BF16;
-  if (c->cfg.head_dim == 128) return bf ? dispatch_decode_g<bf16, 128>(c, layer, b, n_req, n_split, q, out, sc, st)
-                                        : dispatch_decode_g<float, 128>(c, layer, b, n_req, n_split, q, out, sc, st);
-  return bf ? dispatch_decode_g<bf16, 64>(c, layer, b, n_req, n_split, q, out, sc, st)
-            : dispatch_decode_g<float, 64>(c, layer, b, n_req, n_split, q, out, sc, st);
+  if (c->cfg.head_dim == 128) return bf ? dispatch_decode_g<bf16, 128>(c, layer, b, n_req, n_split, q, out, sc, st, pdl)
+                                        : dispatch_decode_g<float, 128>(c, layer, b, n_req, n_split, q, out, sc, st, pdl);
+  return bf ? dispatch_decode_g<bf16, 64>(c, layer, b, n_req, n_split, q, out, sc, st, pdl)
+            : dispatch_decode_g<float, 64>(c, layer, b, n_req, n_split, q, out, sc, st, pdl);
 }
 
 // bf16 key pass on the tensor pipe (score_mma.cuh).  Returns the number of partial (max, sum) columns.
@@ -444,8 +466,11 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
                            cudaStream_t st) {
   const int L = c->cfg.n_layers, Hkv = c->cfg.n_kv_heads, Hq = c->cfg.n_q_heads;
   const int n_fb = mem_prep_frag_blocks<D, G>(L, Hkv);
-  CU(c, launch_pdl(k_mem_prep<D, G>, dim3(n_fb + n_mpart), dim3(128), 0, st, c->pdl_prune, M, L, Hkv,
-                   1.0f / sqrtf((float)D), c->frag, n_fb, L * Hq, c->mpart));
+  {
+    ProfScope prof(c, IKV_PROF_MEM_PREP, st);
+    CU(c, launch_pdl(k_mem_prep<D, G>, dim3(n_fb + n_mpart), dim3(128), 0, st, c->pdl_prune, M, L, Hkv,
+                     1.0f / sqrtf((float)D), c->frag, n_fb, L * Hq, c->mpart));
+  }
   int ns = 0;
   const size_t smem = key_pass_smem(L, Hq, Hkv, D, kbar, c->max_smem, &ns);
   if (ns < 2) IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "key pass: L*Hq = %d and row of %d bytes do not fit shared memory", L * Hq,
@@ -456,6 +481,7 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
   p.xq_slot = with_xq ? c->xq_slot : nullptr; p.n_xq = with_xq ? c->d_nxq : nullptr;
   p.logits = c->logits; p.ldc = c->cap_tokens; p.partials = c->partials; p.kbar = c->kbar; p.kq = c->kq;
   p.n_stage = ns;
+  p.l2_hints = c->dbg_l2;
   const int grid = c->n_sm;
   ProfScope prof(c, 0, st);
   if (kbar) {
@@ -508,9 +534,13 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   const bool use_x = learn && !(mode & IKV_FLAG_NO_XATTN);
   const int n_x = use_x ? (r.xattn_pos ? r.n_xattn_pos : (r.q_end - r.q_start)) : 0;
   if (learn) TRY(ensure_xq(c, n_x > 0 ? n_x : 1));
+  // at most RT_NXMAX query positions: folded cross attention, the whole head on tcgen05 (residual_tc.cuh)
+  const bool tc = learn && c->resid_tc && n_x <= RT_NXMAX;
+  const int nxp = tc ? (n_x > 0 ? (n_x + 15) / 16 * 16 : 16) : 0;
   {
     // a1 (+ the compaction of the live cross-attention positions as a second cluster of the same launch)
     const int grid = CL_CTAS * (n_x > 0 ? 2 : 1);
+    ProfScope prof(c, IKV_PROF_PARTITION, st);
 #define IKV_PART_ARGS r.slot_map, N, c->cfg.dead_slot, r.prefix_len, r.q_start, r.q_end, scores, rule_out, \
                       c->cand_pos, c->cand_slot, c->d_ncand
 #define IKV_X_ARGS r.xattn_pos, n_x, c->xq_slot, c->d_nxq
@@ -556,20 +586,46 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     pk.fold.mbar = c->mbar; pk.fold.wq_frag = c->wq_frag; pk.fold.w1_can = c->w1_can;
     pk.fold.bq_eff = c->bq_eff; pk.fold.b1_eff = c->b1_eff;
     pk.kq = c->kq; pk.n_xq = c->d_nxq; pk.nks = (int)(c->xq_cap / 16); pk.kc_frag = c->kc_frag; pk.vc_frag = c->vc_frag;
-    pk.n_fold = 0; pk.n_kv = 0;
-    CU(c, launch_pdl(D == 128 ? k_post_key<128> : k_post_key<64>, dim3((pk.n_lse + 3) / 4), dim3(128), 0, st, c->pdl_prune, pk,
-                     c->rw));
-    pk.n_fold = learn ? (D == 128 ? resid_fold_grid<128>() : resid_fold_grid<64>()) : 0;
-    pk.n_kv = (learn && n_x > 0) ? 4 * ((n_x + 15) / 16) : 0;
+    pk.n_fold = 0; pk.n_kv = 0; pk.tc = 0; pk.nxp = 0; pk.rt = RtFoldOut{};
+    {
+      ProfScope prof(c, IKV_PROF_POST_KEY, st);
+      CU(c, launch_pdl(D == 128 ? k_post_key<128> : k_post_key<64>, dim3((pk.n_lse + 3) / 4), dim3(128), 0, st,
+                       c->pdl_prune, pk, c->rw));
+    }
+    pk.tc = tc ? 1 : 0; pk.nxp = nxp;
+    pk.rt.mbar = c->mbar; pk.rt.wcan = c->rt_wcan; pk.rt.svec = c->rt_svec; pk.rt.b1_eff = c->b1_eff;
+    if (tc) {
+      pk.n_fold = D == 128 ? rt_fold_fc1_grid<128>() : rt_fold_fc1_grid<64>();
+      pk.n_kv = n_x > 0 ? 4 * (nxp / 16) : 0;
+    } else {
+      pk.n_fold = learn ? (D == 128 ? resid_fold_grid<128>() : resid_fold_grid<64>()) : 0;
+      pk.n_kv = (learn && n_x > 0) ? 4 * ((n_x + 15) / 16) : 0;
+    }
     RuleParams rp;
     rp.logits = c->logits; rp.ldc = c->cap_tokens; rp.LH = LH; rp.lse = c->lse; rp.n_cand = c->d_ncand;
     rp.cand_pos = c->cand_pos; rp.rule_c = c->rule_c; rp.scores = scores; rp.scatter_scores = learn ? 0 : 1;
-    rp.rule_out = rule_out; rp.n_rule = (N + 63) / 64;
+    rp.rule_out = rule_out; rp.n_rule = (N + 63) / 64; rp.l2_hints = c->dbg_l2;
     const int grid = rp.n_rule + pk.n_fold + pk.n_kv;
-    CU(c, launch_pdl(D == 128 ? k_rule_fused<128> : k_rule_fused<64>, dim3(grid), dim3(256), 0, st, c->pdl_prune, rp, pk,
-                     c->rw));
+    auto rule_fn = tc ? (D == 128 ? k_rule_fused<128, true> : k_rule_fused<64, true>)
+                      : (D == 128 ? k_rule_fused<128, false> : k_rule_fused<64, false>);
+    ProfScope prof(c, IKV_PROF_RULE, st);
+    CU(c, launch_pdl(rule_fn, dim3(grid), dim3(256), 0, st, c->pdl_prune, rp, pk, c->rw));
   }
-  if (learn) {
+  if (learn && tc) {
+    ResidTcParams rp;
+    rp.rule_c = c->rule_c; rp.kbar = c->kbar; rp.n_cand = c->d_ncand; rp.cand_pos = c->cand_pos; rp.n_xq = c->d_nxq;
+    rp.wcan = c->rt_wcan; rp.svec = c->rt_svec; rp.b1_eff = c->b1_eff; rp.nxp = nxp;
+    rp.use_xattn = (use_x && n_x > 0) ? 1 : 0;
+    rp.scores = scores;
+    if (!c->resid_tc_attr_done) {
+      CU(c, cudaFuncSetAttribute(k_residual_tc<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt_smem<128>()));
+      CU(c, cudaFuncSetAttribute(k_residual_tc<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt_smem<64>()));
+      c->resid_tc_attr_done = true;
+    }
+    ProfScope prof(c, IKV_PROF_RESIDUAL, st);
+    CU(c, launch_pdl(D == 128 ? k_residual_tc<128> : k_residual_tc<64>, dim3((N + RT_M - 1) / RT_M), dim3(RT_THREADS),
+                     D == 128 ? rt_smem<128>() : rt_smem<64>(), st, c->pdl_prune, rp, c->rw));
+  } else if (learn) {
     ResidMmaParams rp;
     rp.rule_c = c->rule_c; rp.kbar = c->kbar; rp.n_cand = c->d_ncand; rp.cand_pos = c->cand_pos; rp.n_xq = c->d_nxq;
     rp.wq_frag = c->wq_frag; rp.w1_can = c->w1_can; rp.kc_frag = c->kc_frag; rp.vc_frag = c->vc_frag;
@@ -582,6 +638,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
       CU(c, cudaFuncSetAttribute(k_residual_mma<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, resid_smem<64>()));
       c->resid_attr_done = true;
     }
+    ProfScope prof(c, IKV_PROF_RESIDUAL, st);
     CU(c, launch_pdl(D == 128 ? k_residual_mma<128> : k_residual_mma<64>, dim3(nblk), dim3(R_THREADS),
                      D == 128 ? resid_smem<128>() : resid_smem<64>(), st, c->pdl_prune, rp, c->rw));
   }
@@ -606,6 +663,8 @@ ikv_status select_prepare(ikv_ctx* c, const ikv_request& r, const float* scores,
   *out = p;
   s->covered = N;
   s->map_ptr = r.slot_map;
+  s->map_epoch = r.map_epoch;
+  s->list_fresh = true;
   s->live_ub = N;
   if (N > r.budget) {
     const int forced_ub = r.prefix_len + (r.q_end - r.q_start);
@@ -620,6 +679,7 @@ ikv_status select_launch(ikv_ctx* c, const SelBatch& b, int n, int max_n, cudaSt
   if (n == 0) return IKV_OK;
   auto fn = max_n <= CL_CTAS * 1024 * 4 ? k_select_evict_cl<4>
             : max_n <= CL_CTAS * 1024 * 8 ? k_select_evict_cl<8> : k_select_evict_cl<16>;
+  ProfScope prof(c, IKV_PROF_SELECT, st);
   CU(c, launch_pdl(fn, dim3(n * CL_CTAS), dim3(1024), 0, st, c->pdl_prune, b));
   return IKV_OK;
 }
@@ -629,9 +689,18 @@ ikv_status select_launch(ikv_ctx* c, const SelBatch& b, int n, int max_n, cudaSt
 // ======================================================================================================
 extern "C" {
 
+#ifdef IKV_TRACE
+ikv_status ikv_debug_trace(long long* out) {
+  cudaDeviceSynchronize();
+  return cudaMemcpyFromSymbol(out, g_rt_trace, sizeof(long long) * 128) == cudaSuccess ? IKV_OK : IKV_ERR_CUDA;
+}
+#endif
+
 const char* ikv_version(void) { return "ikv 0.1 (sm_100a)"; }
 
-const char* ikv_last_error(const ikv_ctx* ctx) { return ctx ? ctx->err.c_str() : "null context"; }
+static thread_local std::string g_create_err;  // ikv_create has no context to hang its message on
+
+const char* ikv_last_error(const ikv_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 
 ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
   if (!cfg || !out) return IKV_ERR_INVALID_ARG;
@@ -639,7 +708,7 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
   ikv_ctx* c = new ikv_ctx();
   c->cfg = *cfg;
   auto fail = [&](ikv_status code, const char* msg) {
-    fprintf(stderr, "ikv_create: %s\n", msg);
+    g_create_err = std::string("ikv_create: ") + msg;
     delete c;
     return code;
   };
@@ -661,9 +730,8 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
   if (cudaGetDevice(&dev) != cudaSuccess) return fail(IKV_ERR_CUDA, "no CUDA device");
   cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, dev);
   cudaDeviceGetAttribute(&c->max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-  if (const char* e = getenv("IKV_PDL")) c->use_pdl = atoi(e) != 0;
-  c->pdl_prune = c->use_pdl;
-  if (const char* e = getenv("IKV_PDL_PRUNE")) c->pdl_prune = atoi(e) != 0;
+  c->use_pdl = !(cfg->flags & IKV_CFG_NO_PDL);
+  c->pdl_prune = c->use_pdl && !(cfg->flags & IKV_CFG_NO_PDL_PRUNE);
   const int row = cfg->n_kv_heads * cfg->head_dim;
   if (cfg->kv_dtype == IKV_BF16)
     k_init_dead<bf16><<<cfg->n_layers, 256>>>((bf16*)cfg->k_pool, (bf16*)cfg->v_pool, c->layer_stride, cfg->n_layers,
@@ -691,14 +759,16 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
     ok = ok && cudaMalloc((void**)&c->b1_eff, R_HID * 4) == cudaSuccess;
     ok = ok && cudaMalloc((void**)&c->wq_frag, (size_t)KS * 16 * 32 * sizeof(uint4)) == cudaSuccess;
     ok = ok && cudaMalloc((void**)&c->w1_can, (size_t)2 * (cfg->head_dim / 64 + 2) * W1C_CHUNK) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->rt_wcan, rt_wcan_bytes(cfg->head_dim)) == cudaSuccess;
+    ok = ok && cudaMalloc((void**)&c->rt_svec, 512 * 4) == cudaSuccess;
   }
   // B fragments: [L][Hkv][NT<=2][D/32][32 lanes] uint4
   ok = ok && cudaMalloc((void**)&c->frag, (size_t)cfg->n_layers * cfg->n_kv_heads * 2 * (cfg->head_dim / 32) * 32 *
                                               sizeof(uint4)) == cudaSuccess;
   ok = ok && cudaDeviceSynchronize() == cudaSuccess;
   if (!ok) {
+    g_create_err = std::string("ikv_create: CUDA initialisation failed: ") + cudaGetErrorString(cudaGetLastError());
     ikv_destroy(c);
-    fprintf(stderr, "ikv_create: CUDA initialisation failed: %s\n", cudaGetErrorString(cudaGetLastError()));
     return IKV_ERR_CUDA;
   }
   *out = c;
@@ -711,33 +781,45 @@ ikv_status ikv_destroy(ikv_ctx* c) {
   for (auto& kv : c->sessions) session_free(kv.second);
   void* bufs[] = {c->cand_pos, c->cand_slot, c->d_ncand, c->logits, c->partials, c->lse, c->rule_c, c->kbar, c->mbar,
                   c->xq_slot, c->d_nxq, c->kq, c->kc_frag, c->vc_frag, c->mpart, c->bq_eff, c->b1_eff, c->wq_frag,
-                  c->w1_can, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
+                  c->w1_can, c->rt_wcan, c->rt_svec, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
                   c->part_o, c->part_ml, c->st_out, c->st_scores,
                   c->st_qrows, c->resid_blob, c->frag};
   for (void* b : bufs) cudaFree(b);
   if (c->st_host) cudaFreeHost(c->st_host);
+  for (int w = 0; w < IKV_PROF_SLOTS; ++w)
+    for (auto& pr : c->prof_ev[w]) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+  for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
   const cudaError_t e = cudaGetLastError();
   delete c;
   return e == cudaSuccess ? IKV_OK : IKV_ERR_CUDA;
 }
 
+ikv_status ikv_tune(ikv_ctx* c, int32_t knob, int32_t value) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  switch (knob) {
+    case IKV_TUNE_L2_HINTS: c->dbg_l2 = value; return IKV_OK;
+    case IKV_TUNE_RESID_TC: c->resid_tc = value; return IKV_OK;
+  }
+  IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_tune: unknown knob %d", knob);
+}
+
 ikv_status ikv_profile_enable(ikv_ctx* c, int32_t on) {
   if (!c) return IKV_ERR_INVALID_ARG;
-  c->prof_on = on != 0;
+  c->prof_on = on < 0 ? 0 : (on > 2 ? 2 : on);
   return IKV_OK;
 }
 
 ikv_status ikv_profile_read(ikv_ctx* c, float* out_ms, int32_t* out_n) {
   if (!c || !out_ms || !out_n) return IKV_ERR_INVALID_ARG;
   CU(c, cudaDeviceSynchronize());
-  for (int w = 0; w < 2; ++w) {
+  for (int w = 0; w < IKV_PROF_SLOTS; ++w) {
     float tot = 0.f;
     for (auto& pr : c->prof_ev[w]) {
       float ms = 0.f;
       cudaEventElapsedTime(&ms, pr.first, pr.second);
       tot += ms;
-      cudaEventDestroy(pr.first);
-      cudaEventDestroy(pr.second);
+      c->ev_pool.push_back(pr.first);
+      c->ev_pool.push_back(pr.second);
     }
     out_ms[w] = tot;
     out_n[w] = (int32_t)c->prof_ev[w].size();
@@ -760,7 +842,7 @@ ikv_status ikv_reserve(ikv_ctx* c, int64_t max_tokens, int32_t max_requests) {
 ikv_status ikv_session_open(ikv_ctx* c, uint64_t id) {
   if (!c) return IKV_ERR_INVALID_ARG;
   Session* s;
-  return session_create(c, id, &s);
+  return session_create(c, id, &s, (cudaStream_t)0, true);
 }
 
 ikv_status ikv_session_fork(ikv_ctx* c, uint64_t parent, uint64_t child, void* stream) {
@@ -768,8 +850,14 @@ ikv_status ikv_session_fork(ikv_ctx* c, uint64_t parent, uint64_t child, void* s
   if (parent == child) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "fork onto itself");
   if (!session_find(c, parent)) IKV_FAIL(c, IKV_ERR_NO_SESSION, "parent session does not exist");
   Session* ch;
-  TRY(session_create(c, child, &ch));
+  TRY(session_create(c, child, &ch, (cudaStream_t)stream, false));
   Session* p = session_find(c, parent);  // re-find: the map may have rehashed
+  if (!p) {  // max_sessions == 1: creating the child evicted the parent
+    auto it = c->sessions.find(child);
+    if (it != c->sessions.end()) { session_free(it->second); c->sessions.erase(it); }
+    IKV_FAIL(c, IKV_ERR_CAPACITY, "ikv_session_fork: max_sessions = %d leaves no room for parent and child",
+             c->cfg.max_sessions);
+  }
   const size_t n = (size_t)c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim * sizeof(float);
   CU(c, cudaMemcpyAsync(ch->d_mem, p->d_mem, n, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
   CU(c, cudaMemcpyAsync(ch->d_qenc, p->d_qenc, n, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
@@ -804,6 +892,7 @@ ikv_status ikv_session_set_memory(ikv_ctx* c, uint64_t id, const float* host_in)
   const size_t n = (size_t)c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim * sizeof(float);
   CU(c, cudaDeviceSynchronize());
   CU(c, cudaMemcpy(s->d_mem, host_in, n, cudaMemcpyHostToDevice));
+  CU(c, cudaDeviceSynchronize());  // pageable copies may still be in flight when cudaMemcpy returns
   return IKV_OK;
 }
 
@@ -887,6 +976,7 @@ ikv_status ikv_residual_load(ikv_ctx* c, const ikv_residual_weights* w) {
   CU(c, cudaDeviceSynchronize());
   if (!c->resid_blob) CU(c, cudaMalloc((void**)&c->resid_blob, h.size() * 4));
   CU(c, cudaMemcpy(c->resid_blob, h.data(), h.size() * 4, cudaMemcpyHostToDevice));
+  CU(c, cudaDeviceSynchronize());  // pageable copies may still be in flight when cudaMemcpy returns
   float* b = c->resid_blob;
   c->rw.wq = b + off[0]; c->rw.bq = b + off[1]; c->rw.wk_t = b + off[2]; c->rw.bk = b + off[3];
   c->rw.wv_t = b + off[4]; c->rw.bv = b + off[5]; c->rw.fc1_w = b + off[6]; c->rw.fc1_b = b + off[7];
@@ -903,10 +993,11 @@ ikv_status ikv_memory_update(ikv_ctx* c, uint64_t id, const void* q_rows, int32_
   if (!q_rows || n <= 0) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_memory_update: need n > 0 query rows");
   if (q_dtype != IKV_F32 && q_dtype != IKV_BF16) IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "q_dtype must be IKV_F32 or IKV_BF16");
   Session* s = session_find(c, id);
-  if (!s) TRY(session_create(c, id, &s));
+  if (!s) TRY(session_create(c, id, &s, (cudaStream_t)stream, false));
   const int L = c->cfg.n_layers, Hq = c->cfg.n_q_heads, D = c->cfg.head_dim;
   const float decay = expf(-c->cfg.lambda);
   const int64_t rs = (int64_t)L * Hq * D;
+  ProfScope prof(c, IKV_PROF_MEM_UPDATE, (cudaStream_t)stream);
   if (q_dtype == IKV_F32)
     k_memory_update<float><<<L * Hq, D, 0, (cudaStream_t)stream>>>(s->d_mem, s->d_qenc, (const float*)q_rows, n, rs, D,
                                                                    decay);
@@ -940,6 +1031,9 @@ ikv_status ikv_select_evict(ikv_ctx* c, const ikv_request* reqs, int32_t n_req, 
   if (n_req < 0 || (n_req > 0 && (!reqs || !scores || !freed_slots || !n_freed || !n_kept)))
     IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_select_evict: NULL argument");
   for (int r = 0; r < n_req; ++r) TRY(check_request(c, reqs[r]));
+  for (int r = 0; r < n_req; ++r)  // validate the whole batch before any session bookkeeping changes
+    if (c->sessions.find(reqs[r].session_id) == c->sessions.end())
+      IKV_FAIL(c, IKV_ERR_NO_SESSION, "session %llu does not exist", (unsigned long long)reqs[r].session_id);
   int64_t off = 0;
   SelBatch batch;
   int nb = 0, max_n = 0;
@@ -978,12 +1072,14 @@ ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, i
     DecBatch batch;
     int max_items = 1;
     int items_of[DEC_MAX_REQ];
+    bool fresh = false;  // a survivor list of this batch was just rewritten: no programmatic launch (R27)
     for (int i = 0; i < nb; ++i) {
       const ikv_request& r = reqs[r0 + i];
       if (r.seq_len < 0 || (r.seq_len > 0 && !r.slot_map)) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "bad request %d", r0 + i);
       Session* s = session_find(c, r.session_id);
       if (!s) IKV_FAIL(c, IKV_ERR_NO_SESSION, "session %llu does not exist", (unsigned long long)r.session_id);
-      const bool stale = (r.flags & IKV_REQ_RESCAN) || s->map_ptr != r.slot_map || s->covered > r.seq_len ||
+      const bool stale = (r.flags & IKV_REQ_RESCAN) || s->map_ptr != r.slot_map || s->map_epoch != r.map_epoch ||
+                         s->covered > r.seq_len ||
                          (s->covered == 0 && r.seq_len > 0) || (r.seq_len - s->covered) > 4096;
       if (stale) {
         TRY(session_live_reserve(c, *s, r.seq_len > 0 ? r.seq_len : 1));
@@ -991,8 +1087,12 @@ ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, i
         LAUNCH_CHECK(c);
         s->covered = r.seq_len;
         s->map_ptr = r.slot_map;
+        s->map_epoch = r.map_epoch;
         s->live_ub = r.seq_len;
+        s->list_fresh = true;
       }
+      fresh = fresh || s->list_fresh;
+      s->list_fresh = false;
       batch.r[i].S = r.slot_map;
       batch.r[i].live_slots = s->live_slots;
       batch.r[i].n_live = s->d_n_live;
@@ -1036,7 +1136,7 @@ ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, i
     }
     TRY(ensure_parts(c, (int64_t)nb * Hq * n_split));
     TRY(dispatch_decode(c, layer, batch, nb, n_split, (const char*)q + (size_t)r0 * Hq * D * esz,
-                        (char*)out + (size_t)r0 * Hq * D * esz, sm_scale, st));
+                        (char*)out + (size_t)r0 * Hq * D * esz, sm_scale, st, c->use_pdl && !fresh));
   }
   return IKV_OK;
 }

@@ -95,6 +95,7 @@ struct KeyPassParams {
   float* kbar;             // [n_cand][D]   (KBAR)
   float* kq;               // [n_xq][D]     (KBAR)
   int n_stage;
+  int l2_hints;            // bit 0: keys evict_first, bit 1: logits evict_last
 };
 
 // Warp roles of k_key_pass: warps [0, KP_LWARPS) logit warps, [KP_LWARPS, KP_LWARPS + KP_KWARPS) mean-key warps
@@ -132,6 +133,8 @@ __global__ __launch_bounds__(kp_threads(G, KBAR), 1) void k_key_pass(const KeyPa
   }
   __syncthreads();
 
+  const uint64_t pol_keys = l2_policy_evict_first();  // keys are read exactly once per pass
+  const uint64_t pol_logits = l2_policy_evict_last();  // the rule kernel re-reads the logits scratch
   if (!MERGED && warp == KP_LWARPS + KP_KWARPS) {
     // ------------------------------------------------------------------ producer (a warp of its own)
     int s = 0;
@@ -149,9 +152,14 @@ __global__ __launch_bounds__(kp_threads(G, KBAR), 1) void k_key_pass(const KeyPa
           mbar_arrive_expect_tx(&full[s], (uint32_t)(nvalid * row_bytes));
         }
         __syncwarp();
-        if (lane < nvalid)
-          bulk_g2s(stage_base + (size_t)s * stage_bytes + lane * row_stride, src + (int64_t)l * p.layer_stride,
-                   (uint32_t)row_bytes, &full[s]);
+        if (lane < nvalid) {
+          if (p.l2_hints & 1)
+            bulk_g2s_hint(stage_base + (size_t)s * stage_bytes + lane * row_stride, src + (int64_t)l * p.layer_stride,
+                          (uint32_t)row_bytes, &full[s], pol_keys);
+          else
+            bulk_g2s(stage_base + (size_t)s * stage_bytes + lane * row_stride, src + (int64_t)l * p.layer_stride,
+                     (uint32_t)row_bytes, &full[s]);
+        }
         if (++s == NS) { s = 0; ph ^= 1u; }
       }
     }
@@ -254,7 +262,10 @@ __global__ __launch_bounds__(kp_threads(G, KBAR), 1) void k_key_pass(const KeyPa
               float mx = -CUDART_INF_F;
 #pragma unroll
               for (int e = 0; e < 4; ++e) {
-                if (gv && tv[e]) lrow[8 * e] = x[hh][e];
+                if (gv && tv[e]) {
+                  if (p.l2_hints & 2) st_f32_hint(lrow + 8 * e, x[hh][e], pol_logits);
+                  else lrow[8 * e] = x[hh][e];
+                }
                 mx = fmaxf(mx, tv[e] ? x[hh][e] : -CUDART_INF_F);
               }
               mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, 4));
@@ -322,9 +333,16 @@ __global__ __launch_bounds__(kp_threads(G, KBAR), 1) void k_key_pass(const KeyPa
       const int nv = min(KP_TOK, (tx ? nx : nc) - t0);
       if (lane == 0) mbar_arrive_expect_tx(&full[p_s], (uint32_t)(nv * row_bytes));
       __syncwarp();
-      if (lane < nv)
-        bulk_g2s(stage_base + (size_t)p_s * stage_bytes + lane * row_stride,
-                 p.k_pool + p_slot * (int64_t)(Hkv * D) + (int64_t)p_l * p.layer_stride, (uint32_t)row_bytes, &full[p_s]);
+      if (lane < nv) {
+        if (p.l2_hints & 1)
+          bulk_g2s_hint(stage_base + (size_t)p_s * stage_bytes + lane * row_stride,
+                        p.k_pool + p_slot * (int64_t)(Hkv * D) + (int64_t)p_l * p.layer_stride, (uint32_t)row_bytes,
+                        &full[p_s], pol_keys);
+        else
+          bulk_g2s(stage_base + (size_t)p_s * stage_bytes + lane * row_stride,
+                   p.k_pool + p_slot * (int64_t)(Hkv * D) + (int64_t)p_l * p.layer_stride, (uint32_t)row_bytes,
+                   &full[p_s]);
+      }
       if (++p_l == L) {
         p_l = 0;
         p_tile += gridDim.x;
@@ -408,8 +426,9 @@ __device__ __forceinline__ void score_rule4_block(int bid, int n_blocks, const f
                                                   const int32_t* __restrict__ n_cand_p,
                                                   const int32_t* __restrict__ cand_pos, float* __restrict__ rule_c,
                                                   float* __restrict__ scores, int scatter_scores,
-                                                  float* __restrict__ rule_out) {
+                                                  float* __restrict__ rule_out, int l2_hints) {
   __shared__ float4 part[16][16];
+  const uint64_t pol = l2_policy_evict_first();  // the logits are dead once read
   const int nc = *n_cand_p;
   // newest tiles first: the key pass wrote the logits in tile order, so the tail of the scratch is still in L2
   const int c0 = (n_blocks - 1 - bid) * 64;
@@ -420,7 +439,8 @@ __device__ __forceinline__ void score_rule4_block(int bid, int n_blocks, const f
   if (c < nc) {  // rows are padded to a multiple of 4 (ldc % 4 == 0); lanes past n_cand read scratch, never stored
 #pragma unroll 12
     for (int lh = lg; lh < LH; lh += 16) {
-      const float4 v = *reinterpret_cast<const float4*>(logits + (int64_t)lh * ldc + c);
+      const float* lp = logits + (int64_t)lh * ldc + c;
+      const float4 v = (l2_hints & 4) ? ld_f32x4_hint(lp, pol) : *reinterpret_cast<const float4*>(lp);
       const float e = __ldg(lse + lh);
       acc.x += __expf(v.x - e); acc.y += __expf(v.y - e); acc.z += __expf(v.z - e); acc.w += __expf(v.w - e);
     }

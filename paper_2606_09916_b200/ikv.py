@@ -23,25 +23,30 @@ ERR_INVALID_ARG, ERR_NO_SESSION, ERR_CAPACITY, ERR_OOM, ERR_CUDA, ERR_UNSUPPORTE
 F32, BF16 = 0, 1
 MODE_MEMORY, MODE_LEARNABLE, MODE_QUERY = 0, 1, 2
 FLAG_NO_XATTN, FLAG_NO_RESIDUAL = 0x100, 0x200
-REQ_RESCAN = 1
+REQ_RESCAN, REQ_INPUTS_COMPLETE = 1, 2
+CFG_NO_PDL, CFG_NO_PDL_PRUNE = 1, 2
+TUNE_L2_HINTS, TUNE_RESID_TC = 1, 2
+PROF_SLOTS = 12
+PROF_NAMES = ["key_pass", "decode_split", "memory_update", "partition", "mem_prep", "post_key", "rule_fold", "residual",
+              "select_evict", "decode_merge"]
 
 EXPORTS = ["ikv_create", "ikv_destroy", "ikv_last_error", "ikv_reserve", "ikv_session_open", "ikv_session_fork",
            "ikv_session_close", "ikv_session_get_memory", "ikv_session_set_memory", "ikv_residual_load",
-           "ikv_memory_update", "ikv_score", "ikv_select_evict", "ikv_decode_attn", "ikv_prune_host", "ikv_profile_enable", "ikv_profile_read", "ikv_version"]
+           "ikv_memory_update", "ikv_score", "ikv_select_evict", "ikv_decode_attn", "ikv_prune_host", "ikv_profile_enable", "ikv_profile_read", "ikv_tune", "ikv_version"]
 
 
 class Config(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("n_q_heads", C.c_int32), ("n_kv_heads", C.c_int32), ("head_dim", C.c_int32),
                 ("page_size", C.c_int32), ("kv_dtype", C.c_int32), ("n_slots", C.c_int64),
                 ("k_pool", C.c_void_p), ("v_pool", C.c_void_p), ("dead_slot", C.c_int32), ("lambda_", C.c_float),
-                ("max_sessions", C.c_int32)]
+                ("max_sessions", C.c_int32), ("flags", C.c_int32)]
 
 
 class Request(C.Structure):
     _fields_ = [("session_id", C.c_uint64), ("slot_map", C.c_void_p), ("valid_mask", C.c_void_p),
                 ("seq_len", C.c_int32), ("prefix_len", C.c_int32), ("q_start", C.c_int32), ("q_end", C.c_int32),
                 ("budget", C.c_int32), ("radix_protected_len", C.c_int32), ("xattn_pos", C.c_void_p),
-                ("n_xattn_pos", C.c_int32), ("flags", C.c_int32)]
+                ("n_xattn_pos", C.c_int32), ("flags", C.c_int32), ("map_epoch", C.c_uint32)]
 
 
 class ResidualWeights(C.Structure):
@@ -70,6 +75,7 @@ _lib.ikv_select_evict.argtypes = [C.c_void_p, C.POINTER(Request), C.c_int32, C.c
                                   C.c_void_p, C.c_void_p]
 _lib.ikv_decode_attn.argtypes = [C.c_void_p, C.c_int32, C.POINTER(Request), C.c_int32, C.c_void_p, C.c_void_p,
                                  C.c_float, C.c_void_p]
+_lib.ikv_tune.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
 _lib.ikv_profile_enable.argtypes = [C.c_void_p, C.c_int32]
 _lib.ikv_profile_read.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.ikv_prune_host.argtypes = [C.c_void_p, C.POINTER(Request), C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p,
@@ -97,7 +103,7 @@ def _stream(stream):
 
 
 def make_request(session_id, slot_map, seq_len, prefix_len, q_start, q_end, budget, radix_protected_len=0,
-                 valid_mask=None, xattn_pos=None, flags=0) -> Request:
+                 valid_mask=None, xattn_pos=None, flags=0, map_epoch=0) -> Request:
     r = Request()
     r.session_id = session_id
     r.slot_map = slot_map.data_ptr() if slot_map is not None else None
@@ -107,6 +113,7 @@ def make_request(session_id, slot_map, seq_len, prefix_len, q_start, q_end, budg
     r.xattn_pos = xattn_pos.data_ptr() if xattn_pos is not None else None
     r.n_xattn_pos = int(xattn_pos.numel()) if xattn_pos is not None else 0
     r.flags = flags
+    r.map_epoch = map_epoch
     return r
 
 
@@ -119,19 +126,19 @@ class Context:
     """Thin owner of an ikv_ctx*.  Methods have the names of the C entry points (without the prefix)."""
 
     def __init__(self, n_layers, n_q_heads, n_kv_heads, head_dim, k_pool, v_pool, dead_slot=0, page_size=16,
-                 lam=0.5, max_sessions=1024):
+                 lam=0.5, max_sessions=1024, flags=0):
         assert k_pool.is_cuda and v_pool.is_cuda and k_pool.is_contiguous() and v_pool.is_contiguous()
         assert k_pool.dtype == v_pool.dtype and k_pool.dtype in (torch.bfloat16, torch.float32)
         assert tuple(k_pool.shape) == (n_layers, k_pool.shape[1], n_kv_heads, head_dim) == tuple(v_pool.shape)
         self.k_pool, self.v_pool = k_pool, v_pool  # keep alive
         cfg = Config(n_layers, n_q_heads, n_kv_heads, head_dim, page_size,
                      BF16 if k_pool.dtype == torch.bfloat16 else F32, k_pool.shape[1], k_pool.data_ptr(),
-                     v_pool.data_ptr(), dead_slot, lam, max_sessions)
+                     v_pool.data_ptr(), dead_slot, lam, max_sessions, flags)
         self.cfg = cfg
         self._h = C.c_void_p()
         st = _lib.ikv_create(C.byref(cfg), C.byref(self._h))
         if st != OK:
-            raise IkvError(st, "ikv_create failed")
+            raise IkvError(st, _lib.ikv_last_error(None).decode() or "ikv_create failed")
 
     def _chk(self, st):
         if st != OK:
@@ -195,14 +202,20 @@ class Context:
         self._chk(_lib.ikv_decode_attn(self._h, layer, _req_array(reqs), len(reqs), _ptr(q), _ptr(out),
                                        C.c_float(sm_scale), _stream(stream)))
 
-    def profile_enable(self, on: bool):
-        self._chk(_lib.ikv_profile_enable(self._h, 1 if on else 0))
+    def tune(self, knob: int, value: int):
+        self._chk(_lib.ikv_tune(self._h, knob, value))
+
+    def profile_enable(self, level):
+        """0/False off, 1/True the two dominant kernels, 2 every kernel (diagnostic)."""
+        self._chk(_lib.ikv_profile_enable(self._h, int(level)))
 
     def profile_read(self) -> dict:
-        ms = (C.c_float * 2)()
-        n = (C.c_int32 * 2)()
+        ms = (C.c_float * PROF_SLOTS)()
+        n = (C.c_int32 * PROF_SLOTS)()
         self._chk(_lib.ikv_profile_read(self._h, ms, n))
-        return {"score_logits_ms": ms[0], "score_logits_n": n[0], "decode_split_ms": ms[1], "decode_split_n": n[1]}
+        out = {"score_logits_ms": ms[0], "score_logits_n": n[0], "decode_split_ms": ms[1], "decode_split_n": n[1]}
+        out["slots"] = {name: (ms[i], n[i]) for i, name in enumerate(PROF_NAMES) if n[i] > 0}
+        return out
 
     def prune_host(self, req, q_rows_host, mode, slot_map_host, valid_host, scores_host, freed_host, stream=None):
         """HOST-buffer variant. Tensors are CPU tensors (pinned or not). Returns (n_freed, n_kept)."""

@@ -39,7 +39,7 @@ def test_struct_layouts_match_header_sizes():
     """ctypes mirrors of ikv_config / ikv_request have the C sizes (LP64)."""
     from paper_2606_09916_b200 import ikv
     assert ctypes.sizeof(ikv.Config) == 64
-    assert ctypes.sizeof(ikv.Request) == 64
+    assert ctypes.sizeof(ikv.Request) == 72
     assert ctypes.sizeof(ikv.ResidualWeights) == 88
 
 
