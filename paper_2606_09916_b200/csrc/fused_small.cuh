@@ -38,25 +38,43 @@ struct PostKeyParams {
 };
 
 // lse[l,h] = log sum_c exp(x[l,h,c]) from the per-CTA (max, sum) partials of the key pass: one warp per (l,h) row, no
-// block barrier (the row has one partial per key-pass CTA, 148 of them).
-template <int D>
-__global__ __launch_bounds__(128) void k_post_key(const PostKeyParams p, const ResidW w) {
-  pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
-  pdl_launch_dependents();
-  (void)w;
-  const int row = blockIdx.x * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-  if (row >= p.n_lse) return;
-  const float2* pp = p.partials + (int64_t)row * p.n_part;
+// block barrier (the row has one partial per key-pass CTA, 148 of them).  TC: the launch also carries the fold bodies of
+// k_tail_tc (blocks of 256 threads; the lse and fc1 bodies use the first 128): n_fold fc1 blocks, then n_kv cross-attention
+// blocks, which need the mean keys of the query positions and hence the finished key pass.
+__device__ __forceinline__ void lse_rows_block(int bid, const float2* __restrict__ partials, int n_part,
+                                               float* __restrict__ lse, int n_lse) {
+  const int row = bid * 4 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (row >= n_lse) return;
+  const float2* pp = partials + (int64_t)row * n_part;
   float mx = -CUDART_INF_F;
-  for (int i = lane; i < p.n_part; i += 32) mx = fmaxf(mx, pp[i].x);
+  for (int i = lane; i < n_part; i += 32) mx = fmaxf(mx, pp[i].x);
   mx = warp_max(mx);
   float s = 0.f;
-  for (int i = lane; i < p.n_part; i += 32) {
+  for (int i = lane; i < n_part; i += 32) {
     const float2 v = pp[i];
     if (v.y > 0.f) s += v.y * expf(v.x - mx);
   }
   s = warp_sum(s);
-  if (lane == 0) p.lse[row] = mx + logf(s);
+  if (lane == 0) lse[row] = mx + logf(s);
+}
+template <int D, bool TC>
+__global__ __launch_bounds__(TC ? 256 : 128) void k_post_key(const PostKeyParams p, const ResidW w) {
+  pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
+  pdl_launch_dependents();
+  int bid = blockIdx.x;
+  const int n_lse_blocks = (p.n_lse + 3) / 4;
+  if (bid < n_lse_blocks) {
+    if (threadIdx.x < 128) lse_rows_block(bid, p.partials, p.n_part, p.lse, p.n_lse);
+    return;
+  }
+  if constexpr (TC) {
+    bid -= n_lse_blocks;
+    if (bid < p.n_fold) {
+      if (threadIdx.x < 128) rt_fold_fc1_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.rt);
+      return;
+    }
+    rt_fold_xattn_block<D>(bid - p.n_fold, p.mpart, p.n_mpart, p.LH, p.kq, p.n_xq, p.nxp, w, p.rt);
+  }
 }
 
 struct RuleParams {
@@ -68,7 +86,7 @@ struct RuleParams {
 // rule_c of Eq. 3 (HBM-bound, 256-thread blocks) and, for a learnable call, the folded W_Q / fc1 operands and the
 // Kc / Vc fragments (latency-bound 128-thread bodies, warps 4-7 of their blocks exit) in one launch: the residual
 // kernel needs all three, and the small bodies hide under the rule blocks' stream of the logits.
-template <int D, bool TC>
+template <int D>
 __global__ __launch_bounds__(256, 4) void k_rule_fused(const RuleParams r, const PostKeyParams p, const ResidW w) {
   pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
   pdl_launch_dependents();
@@ -79,18 +97,10 @@ __global__ __launch_bounds__(256, 4) void k_rule_fused(const RuleParams r, const
     return;
   }
   bid -= r.n_rule;
-  if constexpr (TC) {  // operands of k_residual_tc
-    if (bid < p.n_fold) {
-      if (threadIdx.x < 128) rt_fold_fc1_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.rt);
-      return;
-    }
-    rt_fold_xattn_block<D>(bid - p.n_fold, p.mpart, p.n_mpart, p.LH, p.kq, p.n_xq, p.nxp, w, p.rt);
-  } else {             // operands of k_residual_mma
-    if (threadIdx.x >= 128) return;
-    if (bid < p.n_fold) { resid_fold_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.fold); return; }
-    bid -= p.n_fold;
-    resid_kv_frags_block(bid, p.kq, p.n_xq, D, w, p.nks, p.kc_frag, p.vc_frag);
-  }
+  if (threadIdx.x >= 128) return;
+  if (bid < p.n_fold) { resid_fold_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.fold); return; }
+  bid -= p.n_fold;
+  resid_kv_frags_block(bid, p.kq, p.n_xq, D, w, p.nks, p.kc_frag, p.vc_frag);
 }
 
 }  // namespace ikv

@@ -108,7 +108,7 @@ struct ikv_ctx {
   // residual head (transposed on the device)
   bool has_resid = false;
   bool resid_attr_done = false;
-  bool resid_tc_attr_done = false;
+  int tail_smem_set = 0;     // dynamic shared memory k_tail_tc was last configured for
   int resid_tc = 1;          // IKV_TUNE_RESID_TC: 0 = always the unfolded kernel
   float* resid_blob = nullptr;
   ResidW rw{};
@@ -577,55 +577,71 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
       LAUNCH_CHECK(c);
     }
   }
-  {
-    // launch 1: lse rows.  launch 2: rule_c (Eq. 3) and, for a learnable call, the folded residual operands and the
-    // Kc / Vc fragments, whose latency-bound bodies hide under the rule blocks' stream of the logits.
-    PostKeyParams pk;
-    pk.partials = c->partials; pk.n_part = n_part; pk.lse = c->lse; pk.n_lse = LH;
-    pk.mpart = c->mpart; pk.n_mpart = n_mpart; pk.LH = LH;
-    pk.fold.mbar = c->mbar; pk.fold.wq_frag = c->wq_frag; pk.fold.w1_can = c->w1_can;
-    pk.fold.bq_eff = c->bq_eff; pk.fold.b1_eff = c->b1_eff;
-    pk.kq = c->kq; pk.n_xq = c->d_nxq; pk.nks = (int)(c->xq_cap / 16); pk.kc_frag = c->kc_frag; pk.vc_frag = c->vc_frag;
-    pk.n_fold = 0; pk.n_kv = 0; pk.tc = 0; pk.nxp = 0; pk.rt = RtFoldOut{};
+  PostKeyParams pk;
+  pk.partials = c->partials; pk.n_part = n_part; pk.lse = c->lse; pk.n_lse = LH;
+  pk.mpart = c->mpart; pk.n_mpart = n_mpart; pk.LH = LH;
+  pk.fold.mbar = c->mbar; pk.fold.wq_frag = c->wq_frag; pk.fold.w1_can = c->w1_can;
+  pk.fold.bq_eff = c->bq_eff; pk.fold.b1_eff = c->b1_eff;
+  pk.kq = c->kq; pk.n_xq = c->d_nxq; pk.nks = (int)(c->xq_cap / 16); pk.kc_frag = c->kc_frag; pk.vc_frag = c->vc_frag;
+  pk.n_fold = 0; pk.n_kv = 0; pk.tc = tc ? 1 : 0; pk.nxp = nxp;
+  pk.rt.mbar = c->mbar; pk.rt.wcan = c->rt_wcan; pk.rt.svec = c->rt_svec; pk.rt.b1_eff = c->b1_eff;
+  if (tc) {
+    // launch 1: lse rows and the folded operands of the residual head (they need the mean keys of the query positions,
+    // i.e. the finished key pass).  launch 2: rule_c (Eq. 3).  launch 3: k_tail_tc, the residual head (Eq. 4-6), one
+    // persistent CTA per SM.
+    pk.n_fold = D == 128 ? rt_fold_fc1_grid<128>() : rt_fold_fc1_grid<64>();
+    pk.n_kv = n_x > 0 ? rt_fold_xattn_grid(nxp) : 0;
     {
       ProfScope prof(c, IKV_PROF_POST_KEY, st);
-      CU(c, launch_pdl(D == 128 ? k_post_key<128> : k_post_key<64>, dim3((pk.n_lse + 3) / 4), dim3(128), 0, st,
+      CU(c, launch_pdl(D == 128 ? k_post_key<128, true> : k_post_key<64, true>, dim3((LH + 3) / 4 + pk.n_fold + pk.n_kv),
+                       dim3(256), 0, st, c->pdl_prune, pk, c->rw));
+    }
+    RuleParams rp;
+    rp.logits = c->logits; rp.ldc = c->cap_tokens; rp.LH = LH; rp.lse = c->lse; rp.n_cand = c->d_ncand;
+    rp.cand_pos = c->cand_pos; rp.rule_c = c->rule_c; rp.scores = scores; rp.scatter_scores = 0;
+    rp.rule_out = rule_out; rp.n_rule = (N + 63) / 64; rp.l2_hints = c->dbg_l2;
+    pk.n_fold = 0; pk.n_kv = 0;
+    {
+      ProfScope prof(c, IKV_PROF_RULE, st);
+      CU(c, launch_pdl(D == 128 ? k_rule_fused<128> : k_rule_fused<64>, dim3(rp.n_rule), dim3(256), 0, st, c->pdl_prune,
+                       rp, pk, c->rw));
+    }
+    TailParams tp;
+    tp.rule_c = c->rule_c; tp.kbar = c->kbar; tp.n_cand = c->d_ncand; tp.cand_pos = c->cand_pos; tp.n_xq = c->d_nxq;
+    tp.wcan = c->rt_wcan; tp.svec = c->rt_svec; tp.b1_eff = c->b1_eff; tp.nxp = nxp;
+    tp.use_xattn = (use_x && n_x > 0) ? 1 : 0; tp.scores = scores;
+    const int smem = D == 128 ? rt_tail_smem<128>() : rt_tail_smem<64>();
+    if (c->tail_smem_set != smem) {
+      CU(c, cudaFuncSetAttribute(k_tail_tc<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt_tail_smem<128>()));
+      CU(c, cudaFuncSetAttribute(k_tail_tc<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt_tail_smem<64>()));
+      c->tail_smem_set = smem;
+    }
+    const int n_tiles = (N + RT_M - 1) / RT_M;
+    ProfScope prof(c, IKV_PROF_RESIDUAL, st);
+    CU(c, launch_pdl(D == 128 ? k_tail_tc<128> : k_tail_tc<64>, dim3(n_tiles < c->n_sm ? n_tiles : c->n_sm),
+                     dim3(RT_TAIL_THREADS), smem, st, c->pdl_prune, tp, c->rw));
+    return IKV_OK;
+  }
+  {
+    // launch 1: lse rows.  launch 2: rule_c (Eq. 3) and, for a learnable call on the unfolded kernel, the folded residual
+    // operands and the Kc / Vc fragments, whose latency-bound bodies hide under the rule blocks' stream of the logits.
+    {
+      ProfScope prof(c, IKV_PROF_POST_KEY, st);
+      CU(c, launch_pdl(D == 128 ? k_post_key<128, false> : k_post_key<64, false>, dim3((LH + 3) / 4), dim3(128), 0, st,
                        c->pdl_prune, pk, c->rw));
     }
-    pk.tc = tc ? 1 : 0; pk.nxp = nxp;
-    pk.rt.mbar = c->mbar; pk.rt.wcan = c->rt_wcan; pk.rt.svec = c->rt_svec; pk.rt.b1_eff = c->b1_eff;
-    if (tc) {
-      pk.n_fold = D == 128 ? rt_fold_fc1_grid<128>() : rt_fold_fc1_grid<64>();
-      pk.n_kv = n_x > 0 ? 4 * (nxp / 16) : 0;
-    } else {
-      pk.n_fold = learn ? (D == 128 ? resid_fold_grid<128>() : resid_fold_grid<64>()) : 0;
-      pk.n_kv = (learn && n_x > 0) ? 4 * ((n_x + 15) / 16) : 0;
-    }
+    pk.n_fold = learn ? (D == 128 ? resid_fold_grid<128>() : resid_fold_grid<64>()) : 0;
+    pk.n_kv = (learn && n_x > 0) ? 4 * ((n_x + 15) / 16) : 0;
     RuleParams rp;
     rp.logits = c->logits; rp.ldc = c->cap_tokens; rp.LH = LH; rp.lse = c->lse; rp.n_cand = c->d_ncand;
     rp.cand_pos = c->cand_pos; rp.rule_c = c->rule_c; rp.scores = scores; rp.scatter_scores = learn ? 0 : 1;
     rp.rule_out = rule_out; rp.n_rule = (N + 63) / 64; rp.l2_hints = c->dbg_l2;
     const int grid = rp.n_rule + pk.n_fold + pk.n_kv;
-    auto rule_fn = tc ? (D == 128 ? k_rule_fused<128, true> : k_rule_fused<64, true>)
-                      : (D == 128 ? k_rule_fused<128, false> : k_rule_fused<64, false>);
     ProfScope prof(c, IKV_PROF_RULE, st);
-    CU(c, launch_pdl(rule_fn, dim3(grid), dim3(256), 0, st, c->pdl_prune, rp, pk, c->rw));
+    CU(c, launch_pdl(D == 128 ? k_rule_fused<128> : k_rule_fused<64>, dim3(grid), dim3(256), 0, st, c->pdl_prune, rp, pk,
+                     c->rw));
   }
-  if (learn && tc) {
-    ResidTcParams rp;
-    rp.rule_c = c->rule_c; rp.kbar = c->kbar; rp.n_cand = c->d_ncand; rp.cand_pos = c->cand_pos; rp.n_xq = c->d_nxq;
-    rp.wcan = c->rt_wcan; rp.svec = c->rt_svec; rp.b1_eff = c->b1_eff; rp.nxp = nxp;
-    rp.use_xattn = (use_x && n_x > 0) ? 1 : 0;
-    rp.scores = scores;
-    if (!c->resid_tc_attr_done) {
-      CU(c, cudaFuncSetAttribute(k_residual_tc<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt_smem<128>()));
-      CU(c, cudaFuncSetAttribute(k_residual_tc<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt_smem<64>()));
-      c->resid_tc_attr_done = true;
-    }
-    ProfScope prof(c, IKV_PROF_RESIDUAL, st);
-    CU(c, launch_pdl(D == 128 ? k_residual_tc<128> : k_residual_tc<64>, dim3((N + RT_M - 1) / RT_M), dim3(RT_THREADS),
-                     D == 128 ? rt_smem<128>() : rt_smem<64>(), st, c->pdl_prune, rp, c->rw));
-  } else if (learn) {
+  if (learn) {
     ResidMmaParams rp;
     rp.rule_c = c->rule_c; rp.kbar = c->kbar; rp.n_cand = c->d_ncand; rp.cand_pos = c->cand_pos; rp.n_xq = c->d_nxq;
     rp.wq_frag = c->wq_frag; rp.w1_can = c->w1_can; rp.kc_frag = c->kc_frag; rp.vc_frag = c->vc_frag;

@@ -96,9 +96,10 @@ __device__ __forceinline__ void rt_fold_fc1_block(int bid, const float* __restri
 template <int D>
 inline int rt_fold_fc1_grid() { return (R_HID * (D / 8) + R_HID * 32 + 127) / 128; }
 
-// Fold body, 256 threads: block (cross-attention head h, 16 query keys k0 .. k0+15) computes Kc_h, Vc_h of its keys
-// (Eq. 6) and from them its rows of W_S (S chunks), s_r, s_b and U (fc1 P chunks).  Keys >= n_xq are padding: zero rows,
-// s_b = RT_NEG.  nxp = number of key columns per head (multiple of 16).
+// Fold body, 256 threads: block (part, cross-attention head h, 16 query keys k0 .. k0+15).  part 0 computes Kc_h of its
+// keys (Eq. 6) and from it its rows of W_S (S chunks), s_r and s_b; part 1 computes Vc_h and its rows of U (fc1 P chunks).
+// Keys >= n_xq are padding: zero rows, s_b = RT_NEG.  nxp = key columns per head (multiple of 16).  The weight slices
+// are staged in shared memory with every load of a phase in flight at once: the body is a latency chain, not a stream.
 template <int D>
 __device__ __forceinline__ void rt_fold_xattn_block(int bid, const float* __restrict__ part, int n_part, int LH,
                                                     const float* __restrict__ kq, const int32_t* __restrict__ n_xq,
@@ -107,123 +108,140 @@ __device__ __forceinline__ void rt_fold_xattn_block(int bid, const float* __rest
   constexpr int KPT = 16 * D / 256;  // keys per thread in the W_S step
   __shared__ float mb[D];
   __shared__ float x[16][D];
-  __shared__ float kc[16][R_DH + 1], vc[16][R_DH + 1];
+  __shared__ float wbuf[8192];       // W_K_h / W_V_h as [D][32]; then W_Q rows of the head as [32][2D] or fc1's c columns [256][32]
+  __shared__ float kv[16][R_DH + 1]; // Kc (scaled) or Vc of the block's keys
   __shared__ float red[8][R_DH];
   __shared__ float bqh[R_DH];
-  __shared__ float wsT[16][D + 1];
   const int tid = threadIdx.x;
-  const int h = bid & 3, k0 = (bid >> 2) * 16;
+  const int pt = bid & 1, h = (bid >> 1) & 3, k0 = (bid >> 3) * 16;
   const int nq = *n_xq;
-  for (int d = tid; d < D; d += 256) {
-    float acc = 0.f;
-    for (int b = 0; b < n_part; ++b) acc += part[b * D + d];
-    mb[d] = acc / (float)LH;
-  }
-  for (int i = tid; i < 16 * D; i += 256) {
-    const int key = i / D, d = i % D;
-    x[key][d] = (k0 + key < nq) ? kq[(int64_t)(k0 + key) * D + d] : 0.f;
+  {  // stage W_K_h (part 0) or W_V_h (part 1): rows d of 32 consecutive floats
+    const float* src = (pt == 0 ? w.wk_t : w.wv_t) + h * R_DH;
+    float4 v[D / 32];
+#pragma unroll
+    for (int j = 0; j < D / 32; ++j) {
+      const int d = (tid >> 3) + 32 * j;
+      v[j] = __ldg(reinterpret_cast<const float4*>(src + d * R_DC) + (tid & 7));
+    }
+    for (int d = tid; d < D; d += 256) {
+      float acc = 0.f;
+      for (int b = 0; b < n_part; ++b) acc += part[b * D + d];
+      mb[d] = acc / (float)LH;
+    }
+    for (int i = tid; i < 16 * D; i += 256) {
+      const int key = i / D, d = i % D;
+      x[key][d] = (k0 + key < nq) ? kq[(int64_t)(k0 + key) * D + d] : 0.f;
+    }
+#pragma unroll
+    for (int j = 0; j < D / 32; ++j) *reinterpret_cast<float4*>(&wbuf[((tid >> 3) + 32 * j) * 32 + (tid & 7) * 4]) = v[j];
   }
   __syncthreads();
   const float sc = 1.4426950408889634f * 0.17677669529663689f;  // log2(e) / sqrt(32)  (R10)
-  {  // Kc, Vc of 2 keys per thread; partial sums of b_Q' over 16 columns of W_Qm per thread
+  float wreg[32];  // the next phase's weight slice, loaded while Kc / Vc are computed
+  if (pt == 0) {
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {  // W_Q rows h*32 + c: columns [0, D) and [2D, 3D), index e = tid + 256 j in [32][2D]
+      const int e = tid + 256 * j, c = e / (2 * D), dd = e % (2 * D);
+      wreg[j] = (e < 32 * 2 * D) ? __ldg(w.wq + (int64_t)(h * R_DH + c) * P + (dd < D ? dd : dd + D)) : 0.f;
+    }
+  } else {
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {  // fc1 columns P + h*32 + c of every hidden unit: [256][32]
+      const int n = (tid >> 5) + 8 * j, c = tid & 31;
+      wreg[j] = __ldg(w.fc1_w + (int64_t)n * IN + P + h * R_DH + c);
+    }
+  }
+  {  // Kc or Vc of 2 keys per thread
     const int c = tid & 31, ig = tid >> 5, oc = h * R_DH + c;
-    float ak0 = 0.f, ak1 = 0.f, av0 = 0.f, av1 = 0.f;
+    float a0 = 0.f, a1 = 0.f;
 #pragma unroll 8
     for (int d = 0; d < D; ++d) {
-      const float wk = __ldg(w.wk_t + d * R_DC + oc), wv = __ldg(w.wv_t + d * R_DC + oc);
-      const float x0 = x[2 * ig][d], x1 = x[2 * ig + 1][d];
-      ak0 = fmaf(wk, x0, ak0); ak1 = fmaf(wk, x1, ak1);
-      av0 = fmaf(wv, x0, av0); av1 = fmaf(wv, x1, av1);
+      const float wv = wbuf[d * 32 + c];
+      a0 = fmaf(wv, x[2 * ig][d], a0);
+      a1 = fmaf(wv, x[2 * ig + 1][d], a1);
     }
     const bool ok0 = k0 + 2 * ig < nq, ok1 = k0 + 2 * ig + 1 < nq;
-    kc[2 * ig][c] = ok0 ? (ak0 + w.bk[oc]) * sc : 0.f;
-    kc[2 * ig + 1][c] = ok1 ? (ak1 + w.bk[oc]) * sc : 0.f;
-    vc[2 * ig][c] = ok0 ? av0 + w.bv[oc] : 0.f;
-    vc[2 * ig + 1][c] = ok1 ? av1 + w.bv[oc] : 0.f;
-    const float* row = w.wq + (int64_t)oc * P + D;
-    float acc = 0.f;
-    for (int d = ig * (D / 8); d < (ig + 1) * (D / 8); ++d) acc = fmaf(row[d], mb[d], acc);
-    red[ig][c] = acc;
-  }
-  __syncthreads();
-  if (tid < R_DH) {
-    float acc = w.bq[h * R_DH + tid];
+    const float bias = pt == 0 ? w.bk[oc] : w.bv[oc], mul = pt == 0 ? sc : 1.f;
+    kv[2 * ig][c] = ok0 ? (a0 + bias) * mul : 0.f;
+    kv[2 * ig + 1][c] = ok1 ? (a1 + bias) * mul : 0.f;
+    if (pt == 0) {  // partial sums of b_Q' over D/8 columns of W_Qm per thread
+      const float* row = w.wq + (int64_t)oc * P + D;
+      float acc = 0.f;
 #pragma unroll
-    for (int g = 0; g < 8; ++g) acc += red[g][tid];
-    bqh[tid] = acc;
-  }
-  {  // W_S columns of this block: thread (d, group of KPT keys)
-    const int d = tid % D, kg = tid / D;
-    float acc[KPT];
-#pragma unroll
-    for (int j = 0; j < KPT; ++j) acc[j] = 0.f;
-#pragma unroll 4
-    for (int c = 0; c < R_DH; ++c) {
-      const float* row = w.wq + (int64_t)(h * R_DH + c) * P;
-      const float wqp = fmaf(__ldg(row + 2 * D + d), mb[d], __ldg(row + d));
-#pragma unroll
-      for (int j = 0; j < KPT; ++j) acc[j] = fmaf(wqp, kc[kg * KPT + j][c], acc[j]);
+      for (int d = ig * (D / 8); d < (ig + 1) * (D / 8); ++d) acc = fmaf(__ldg(row + d), mb[d], acc);
+      red[ig][c] = acc;
     }
-#pragma unroll
-    for (int j = 0; j < KPT; ++j) wsT[kg * KPT + j][d] = acc[j];
   }
-  __syncthreads();
-  if (tid < 32) {  // s_r (threads 0-15) and s_b (threads 16-31) of the block's keys
-    const int i = tid & 15;
-    float acc = 0.f;
-    if (tid < 16) {
-      for (int c = 0; c < R_DH; ++c) acc = fmaf(__ldg(w.wq + (int64_t)(h * R_DH + c) * P + 3 * D), kc[i][c], acc);
-    } else {
-      for (int c = 0; c < R_DH; ++c) acc = fmaf(bqh[c], kc[i][c], acc);
-      if (k0 + i >= nq) acc = RT_NEG;
+  __syncthreads();  // wbuf (W_K / W_V) is dead
+  if (pt == 0) {
+#pragma unroll
+    for (int j = 0; j < 32; ++j)
+      if (tid + 256 * j < 32 * 2 * D) wbuf[tid + 256 * j] = wreg[j];
+    if (tid < R_DH) {
+      float acc = w.bq[h * R_DH + tid];
+#pragma unroll
+      for (int g = 0; g < 8; ++g) acc += red[g][tid];
+      bqh[tid] = acc;
     }
-    o.svec[(tid < 16 ? 0 : 256) + h * nxp + k0 + i] = acc;
-  }
-  if (tid < 16 * (D / 8)) {  // W_S entries: row n = (h, key), 8 consecutive d
-    const int i = tid / (D / 8), k8 = tid % (D / 8), n = h * nxp + k0 + i;
-    float v[8];
+    __syncthreads();
+    {  // W_S columns of this block: thread (d, group of KPT keys); W_Q'[c][d] = W_Qk[c][d] + W_Qkm[c][d] mbar[d]
+      const int d = tid % D, kg = tid / D;
+      float acc[KPT];
 #pragma unroll
-    for (int e = 0; e < 8; ++e) v[e] = wsT[i][k8 * 8 + e];
-    rt_store8(o.wcan + (size_t)(k8 >> 1) * RT_CHUNK + rt_entry(n, k8), v);
-  }
-  {  // U rows (h, k0 .. k0+15) for hidden unit n = tid: B[n][k = (h, key)]
+      for (int j = 0; j < KPT; ++j) acc[j] = 0.f;
+      const float m = mb[d];
+#pragma unroll 8
+      for (int c = 0; c < R_DH; ++c) {
+        const float wqp = fmaf(wbuf[c * 2 * D + D + d], m, wbuf[c * 2 * D + d]);
+#pragma unroll
+        for (int j = 0; j < KPT; ++j) acc[j] = fmaf(wqp, kv[kg * KPT + j][c], acc[j]);
+      }
+      __syncthreads();  // every thread has read wbuf: reuse it as the transposed W_S tile [16][D + 1]
+#pragma unroll
+      for (int j = 0; j < KPT; ++j) wbuf[(kg * KPT + j) * (D + 1) + d] = acc[j];
+    }
+    if (tid >= 224) {  // s_r (lanes 0-15 of the last warp) and s_b (lanes 16-31) of the block's keys
+      const int t = tid - 224, i = t & 15;
+      float acc = 0.f;
+      if (t < 16) {
+        for (int c = 0; c < R_DH; ++c) acc = fmaf(__ldg(w.wq + (int64_t)(h * R_DH + c) * P + 3 * D), kv[i][c], acc);
+      } else {
+        for (int c = 0; c < R_DH; ++c) acc = fmaf(bqh[c], kv[i][c], acc);
+        if (k0 + i >= nq) acc = RT_NEG;
+      }
+      o.svec[(t < 16 ? 0 : 256) + h * nxp + k0 + i] = acc;
+    }
+    __syncthreads();
+    if (tid < 16 * (D / 8)) {  // W_S entries: row n = (h, key), 8 consecutive d
+      const int i = tid / (D / 8), k8 = tid % (D / 8), n = h * nxp + k0 + i;
+      float v[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) v[e] = wbuf[i * (D + 1) + k8 * 8 + e];
+      rt_store8(o.wcan + (size_t)(k8 >> 1) * RT_CHUNK + rt_entry(n, k8), v);
+    }
+  } else {
+    // U rows (h, k0 .. k0+15) for the hidden units n = warp + 8 j held in wreg: thread (c = lane) multiplies its column
+    // by Vc[:, c]; the sum over c is a warp reduction per (n, key) -- instead, transpose through shared memory:
+#pragma unroll
+    for (int j = 0; j < 32; ++j) wbuf[((tid >> 5) + 8 * j) * 32 + (tid & 31)] = wreg[j];
+    __syncthreads();
     const int n = tid;
-    const float* row = w.fc1_w + (int64_t)n * IN + P + h * R_DH;
     float a0[8], a1[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) { a0[i] = 0.f; a1[i] = 0.f; }
-#pragma unroll 4
+#pragma unroll 8
     for (int c = 0; c < R_DH; ++c) {
-      const float wv = __ldg(row + c);
+      const float wv = wbuf[n * 32 + ((c + n) & 31)];  // rotated column order: conflict-free rows of 32 floats
+      const int cc = (c + n) & 31;
 #pragma unroll
-      for (int i = 0; i < 8; ++i) { a0[i] = fmaf(wv, vc[i][c], a0[i]); a1[i] = fmaf(wv, vc[8 + i][c], a1[i]); }
+      for (int i = 0; i < 8; ++i) { a0[i] = fmaf(wv, kv[i][cc], a0[i]); a1[i] = fmaf(wv, kv[8 + i][cc], a1[i]); }
     }
     unsigned char* ch = o.wcan + (size_t)(2 * (D / 16) + (h * nxp + k0) / 16) * RT_CHUNK;
     rt_store8(ch + rt_entry(n, 0), a0);
     rt_store8(ch + rt_entry(n, 1), a1);
   }
 }
-
-#ifdef IKV_TRACE
-__device__ long long g_rt_trace[2][64];
-#define RT_T(w, i) do { if (blockIdx.x == 0) g_rt_trace[w][i] = clock64(); } while (0)
-#else
-#define RT_T(w, i) do { } while (0)
-#endif
-
-struct ResidTcParams {
-  const float* rule_c;       // [n_cand]
-  const float* kbar;         // [n_cand][D]
-  const int32_t* n_cand;
-  const int32_t* cand_pos;
-  const int32_t* n_xq;
-  const unsigned char* wcan;
-  const float* svec;
-  const float* b1_eff;
-  int nxp;                   // key columns per head (multiple of 16, <= RT_NXMAX)
-  int use_xattn;
-  float* scores;             // by position
-};
+inline int rt_fold_xattn_grid(int nxp) { return 8 * (nxp / 16); }
 
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float* v) {
   uint32_t r[16];
@@ -237,8 +255,46 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, float* v) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+#ifdef IKV_TRACE
+__device__ long long g_rt_trace[2][64];
+#define RT_T(w, i) do { if (blockIdx.x == 0) g_rt_trace[w][i] = clock64(); } while (0)
+#else
+#define RT_T(w, i) do { } while (0)
+#endif
+
+// ---------------------------------------------------------------------------------------------------------------
+// k_tail_tc: the residual head of Eq. 4-6 over 128-token tiles, one persistent CTA per SM.
+//   warps 0-7   tile loader (kbar rows -> A operand), per-head softmax, epilogue (GELU, fc2, s = rule + alpha z)
+//   warp  8     MMA issuer (one thread)            warp 9   bulk-copy chunk loader (one thread)
+// Per tile the compute warps run  fill(i) | epilogue(i-1) | softmax(i)  so that S(i) is multiplied under epilogue(i-1).
+// (Measured and rejected: four extra warps streaming the tile's logits for rule_c inside this kernel -- with 212 KB of
+// shared memory and 128 registers per thread a CTA keeps only 32 KB of loads in flight, 11 GB/s per SM, 110 k cycles per
+// tile; the rule kernel with 196 KB in flight per SM stays a launch of its own.)
+// ---------------------------------------------------------------------------------------------------------------
+constexpr int RT_CWARPS = 8;
+constexpr int RT_TAIL_THREADS = (RT_CWARPS + 2) * 32;
+
+struct TailParams {
+  const float* rule_c;       // [n_cand]  (Eq. 3)
+  const float* kbar;         // [n_cand][D]
+  const int32_t* n_cand;
+  const int32_t* cand_pos;
+  const int32_t* n_xq;
+  const unsigned char* wcan;
+  const float* svec;
+  const float* b1_eff;
+  int nxp;                   // key columns per head (multiple of 16, <= RT_NXMAX)
+  int use_xattn;
+  float* scores;             // by position
+};
+
 template <int D>
-__global__ __launch_bounds__(RT_THREADS, 1) void k_residual_tc(const ResidTcParams p, const ResidW w) {
+__host__ __device__ constexpr int rt_tail_smem() {
+  return rt_region0<D>() + RT_P01 + RT_STAGES * RT_CHUNK + (5 * 256 + 2 * 128) * 4 + 256;
+}
+
+template <int D>
+__global__ __launch_bounds__(RT_TAIL_THREADS, 1) void k_tail_tc(const TailParams p, const ResidW w) {
   constexpr int KS = D / 16;
   constexpr int A_PART = RT_M * D * 2;   // bytes of kbar hi (and of kbar lo)
   constexpr int A_SBO = (D / 8) * 128;   // byte distance between 8-row groups of the kbar rows
@@ -247,7 +303,7 @@ __global__ __launch_bounds__(RT_THREADS, 1) void k_residual_tc(const ResidTcPara
   pdl_launch_dependents();
   if (threadIdx.x == 0) RT_T(0, 1);
   extern __shared__ __align__(128) unsigned char rt_smem_raw[];
-  unsigned char* region0 = rt_smem_raw;                       // kbar hi | lo; later P of heads 2, 3
+  unsigned char* region0 = rt_smem_raw;                // kbar hi | lo; later P of heads 2, 3
   unsigned char* p01 = region0 + rt_region0<D>();      // P of heads 0, 1
   unsigned char* ring = p01 + RT_P01;                  // [RT_STAGES][RT_CHUNK]
   float* ep_b1 = reinterpret_cast<float*>(ring + RT_STAGES * RT_CHUNK);
@@ -255,20 +311,20 @@ __global__ __launch_bounds__(RT_THREADS, 1) void k_residual_tc(const ResidTcPara
   float* ep_w2 = ep_wr + 256;
   float* sv_r = ep_w2 + 256;
   float* sv_b = sv_r + 256;
-  float* ep_z = sv_b + 256;       // [2][128]
-  float* rule_s = ep_z + 256;     // [128]
-  uint64_t* bfull = reinterpret_cast<uint64_t*>(rule_s + 128);
+  float* ep_z = sv_b + 256;                  // [2][128]
+  uint64_t* bfull = reinterpret_cast<uint64_t*>(ep_z + 256);
   uint64_t* bempty = bfull + RT_STAGES;
   uint64_t* a_ready = bempty + RT_STAGES;   // kbar rows written (8 warps)
   uint64_t* s_full = a_ready + 1;           // S accumulator complete
   uint64_t* ak_free = s_full + 1;           // the MMAs reading the kbar rows have completed
   uint64_t* p_ready = ak_free + 1;          // [4] P of head h written (4 warps each)
-  uint64_t* fc1_full = p_ready + 4;
-  uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(fc1_full + 1);
+  uint64_t* fc1_full = p_ready + 4;         // fc1 accumulator complete (and every operand buffer of the tile is free)
+  uint64_t* tmem_free = fc1_full + 1;       // the epilogue has read the fc1 accumulator (8 warps)
+  uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(tmem_free + 1);
 
   const int nc = *p.n_cand;
-  const int t0 = blockIdx.x * RT_M;
-  if (t0 >= nc) return;
+  const int n_tiles = (nc + RT_M - 1) / RT_M;
+  if ((int)blockIdx.x >= n_tiles) return;
   const int nq = p.use_xattn ? *p.n_xq : 0;
   const bool xat = nq > 0;
   const int NXP = p.nxp;
@@ -276,21 +332,21 @@ __global__ __launch_bounds__(RT_THREADS, 1) void k_residual_tc(const ResidTcPara
   const int IN = 3 * D + 1 + R_DC;
   if (threadIdx.x == 0) {
     for (int s = 0; s < RT_STAGES; ++s) { mbar_init(&bfull[s], 1); mbar_init(&bempty[s], 1); }
-    mbar_init(a_ready, 8);
+    mbar_init(a_ready, RT_CWARPS);
     mbar_init(s_full, 1);
     mbar_init(ak_free, 1);
     for (int h = 0; h < 4; ++h) mbar_init(&p_ready[h], 4);
     mbar_init(fc1_full, 1);
+    mbar_init(tmem_free, RT_CWARPS);
     mbar_fence_init();
   }
-  for (int n = threadIdx.x; n < R_HID; n += RT_THREADS) {
+  for (int n = threadIdx.x; n < R_HID; n += RT_TAIL_THREADS) {
     ep_b1[n] = p.b1_eff[n];
     ep_wr[n] = __ldg(w.fc1_w + (int64_t)n * IN + 3 * D);
     ep_w2[n] = __ldg(w.fc2_w + n);
     sv_r[n] = xat ? p.svec[n] : 0.f;
     sv_b[n] = xat ? p.svec[256 + n] : 0.f;
   }
-  if (threadIdx.x < RT_M) rule_s[threadIdx.x] = (t0 + (int)threadIdx.x < nc) ? p.rule_c[t0 + threadIdx.x] : 0.f;
   if (warp == 8) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_base_p)), "n"(512));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
@@ -301,10 +357,10 @@ __global__ __launch_bounds__(RT_THREADS, 1) void k_residual_tc(const ResidTcPara
   const uint32_t tmem = *tmem_base_p;
   if (threadIdx.x == 0) RT_T(0, 2);
   const int HR = 512 * NXP;  // bytes of one head's P rows (hi | lo)
-
-  // chunk schedule (identical in the loader and the issuer): S chunks, fc1 kbar chunks, then the P chunks of heads 0, 2, 1, 3
-  // (warps 0-3 finish head 0 while warps 4-7 finish head 2).  Chunk index in wcan: S | fc1 kbar | fc1 P in head order.
+  // chunk schedule per tile (identical in the loader and the issuer): S chunks, fc1 kbar chunks, then the P chunks of
+  // heads 0, 2, 1, 3 (warps 0-3 finish head 0 while warps 4-7 finish head 2).  Order in wcan: S | fc1 kbar | fc1 P by head.
   const int n_s = xat ? KS : 0, spp = NXP / 16;
+
   if (warp == 9) {
     // ------------------------------------------------------------------ chunk loader (one thread)
     if (lane == 0) {
@@ -320,20 +376,18 @@ __global__ __launch_bounds__(RT_THREADS, 1) void k_residual_tc(const ResidTcPara
         bulk_g2s(ring + slot * RT_CHUNK + RT_PART, src + RT_PART, pb, &bfull[slot]);
         if (++slot == RT_STAGES) { slot = 0; ph ^= 1u; }
       };
-      for (int j = 0; j < n_s; ++j) push(src_s + (size_t)j * RT_CHUNK, (uint32_t)(128 * NXP));  // 4 NXP rows x 32 B
-      for (int j = 0; j < KS; ++j) push(src_k + (size_t)j * RT_CHUNK, (uint32_t)RT_PART);
-      if (xat) {
-        const int order[4] = {0, 2, 1, 3};
-        for (int o = 0; o < 4; ++o)
-          for (int st = 0; st < spp; ++st) push(src_p + (size_t)(order[o] * spp + st) * RT_CHUNK, (uint32_t)RT_PART);
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        for (int j = 0; j < n_s; ++j) push(src_s + (size_t)j * RT_CHUNK, (uint32_t)(128 * NXP));  // 4 NXP rows x 32 B
+        for (int j = 0; j < KS; ++j) push(src_k + (size_t)j * RT_CHUNK, (uint32_t)RT_PART);
+        if (xat) {
+          const int order[4] = {0, 2, 1, 3};
+          for (int o = 0; o < 4; ++o)
+            for (int st = 0; st < spp; ++st) push(src_p + (size_t)(order[o] * spp + st) * RT_CHUNK, (uint32_t)RT_PART);
+        }
       }
     }
     __syncwarp();
-    __syncthreads();  // z halves written
-    __syncthreads();  // epilogue finished
-    return;
-  }
-  if (warp == 8) {
+  } else if (warp == 8) {
     // ------------------------------------------------------------------ MMA issuer (one thread).  The descriptors are
     // kept as 64-bit values and advanced by additions: the issue loop is a serial instruction stream of one thread.
     if (lane == 0) {
@@ -357,140 +411,161 @@ __global__ __launch_bounds__(RT_THREADS, 1) void k_residual_tc(const ResidTcPara
         db += (RT_CHUNK >> 4);
         if (++slot == RT_STAGES) { slot = 0; ph ^= 1u; db = db0; }
       };
-      mbar_wait(a_ready, 0u);
-      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      for (int s = 0; s < n_s; ++s) chunk(da_k + (uint64_t)(s * 16), (uint32_t)A_PART, tmem, idesc_s, s ? 1u : 0u);
-      if (xat) umma_commit(s_full);
-      for (int s = 0; s < KS; ++s) chunk(da_k + (uint64_t)(s * 16), (uint32_t)A_PART, tmem + 256u, idesc_h, s ? 1u : 0u);
-      umma_commit(ak_free);
-      if (xat) {
-        const int order[4] = {0, 2, 1, 3};
-        for (int o = 0; o < 4; ++o) {
-          const int h = order[o];
-          mbar_wait(&p_ready[h], 0u);
+      uint32_t par = 0u;
+      for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, par ^= 1u) {
+        mbar_wait(a_ready, par);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        for (int s = 0; s < n_s; ++s) chunk(da_k + (uint64_t)(s * 16), (uint32_t)A_PART, tmem, idesc_s, s ? 1u : 0u);
+        if (xat) umma_commit(s_full);
+        if (tile != (int)blockIdx.x) {  // the previous tile's epilogue has read the fc1 accumulator
+          mbar_wait(tmem_free, par ^ 1u);
           asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-          const uint64_t da_p = umma_desc(h < 2 ? pp + (uint32_t)(h * HR) : r0 + (uint32_t)((h - 2) * HR), 128, (uint32_t)(16 * NXP));
-          for (int st = 0; st < spp; ++st) chunk(da_p + (uint64_t)(st * 16), (uint32_t)(HR / 2), tmem + 256u, idesc_h, 1u);
         }
-      }
-      umma_commit(fc1_full);
-    }
-    __syncwarp();
-    __syncthreads();  // z halves written
-    __syncthreads();  // epilogue finished
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
-    return;
-  }
-
-  // -------------------------------------------------------------------- warps 0-7
-  {  // kbar rows -> A operand (hi | lo).  A warp item = 8 rows x 4 groups of 8 columns: 128-byte global segments per
-     // row, 512 contiguous bytes of shared memory.  All loads of the warp's items are issued before the first use.
-    constexpr int KB = D / 32, NU = 16 * KB / 8;  // items per warp
-    float4 x0[NU], x1[NU];
-#pragma unroll
-    for (int u = 0; u < NU; ++u) {
-      const int unit = warp + 8 * u, rb = unit / KB, kb = unit % KB;
-      const int row = rb * 8 + (lane & 7), k8 = kb * 4 + (lane >> 3);
-      if (t0 + row < nc) {
-        const float4* src = reinterpret_cast<const float4*>(p.kbar + (int64_t)(t0 + row) * D + k8 * 8);
-        x0[u] = __ldg(src); x1[u] = __ldg(src + 1);
-      } else {
-        x0[u] = make_float4(0.f, 0.f, 0.f, 0.f); x1[u] = x0[u];
+        for (int s = 0; s < KS; ++s) chunk(da_k + (uint64_t)(s * 16), (uint32_t)A_PART, tmem + 256u, idesc_h, s ? 1u : 0u);
+        umma_commit(ak_free);
+        if (xat) {
+          const int order[4] = {0, 2, 1, 3};
+          for (int o = 0; o < 4; ++o) {
+            const int h = order[o];
+            mbar_wait(&p_ready[h], par);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint64_t da_p =
+                umma_desc(h < 2 ? pp + (uint32_t)(h * HR) : r0 + (uint32_t)((h - 2) * HR), 128, (uint32_t)(16 * NXP));
+            for (int st = 0; st < spp; ++st) chunk(da_p + (uint64_t)(st * 16), (uint32_t)(HR / 2), tmem + 256u, idesc_h, 1u);
+          }
+        }
+        umma_commit(fc1_full);
       }
     }
-#pragma unroll
-    for (int u = 0; u < NU; ++u) {
-      const int unit = warp + 8 * u, rb = unit / KB, kb = unit % KB;
-      const int k8 = kb * 4 + (lane >> 3);
-      uint32_t hi[4], lo[4];
-      split_bf16(x0[u].x, x0[u].y, hi[0], lo[0]); split_bf16(x0[u].z, x0[u].w, hi[1], lo[1]);
-      split_bf16(x1[u].x, x1[u].y, hi[2], lo[2]); split_bf16(x1[u].z, x1[u].w, hi[3], lo[3]);
-      unsigned char* dst = region0 + rb * A_SBO + k8 * 128 + (lane & 7) * 16;
-      *reinterpret_cast<uint4*>(dst) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-      *reinterpret_cast<uint4*>(dst + A_PART) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
-    }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // publish the rows to the async proxy (tcgen05.mma)
     __syncwarp();
-    if (lane == 0) mbar_arrive(a_ready);
-    if (threadIdx.x == 0) RT_T(0, 3);
-  }
-  const int qd = warp & 3, m = qd * 32 + lane;
-  const float rule = rule_s[m];
-  if (xat) {
-    // ---- per-head softmax of this thread's token row; warps 0-3 take heads 0, 1, warps 4-7 heads 2, 3
-    mbar_wait(s_full, 0u);
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    if (threadIdx.x == 0) RT_T(0, 4);
-    const int hp = warp >> 2;
+  } else {
+    // -------------------------------------------------------------------- warps 0-7
+    constexpr int KB = D / 32, NU = 16 * KB / 8;  // kbar items per warp: 8 rows x 4 groups of 8 columns each
+    const int qd = warp & 3, m = qd * 32 + lane, hp = warp >> 2, nh = warp >> 2;
+    // epilogue of one tile: warp w reads TMEM lanes 32 (w % 4) .. + 31 (token rows) of accumulator half w / 4:
+    // hid = acc + b1' + rule w_r -> erf-GELU -> fc2 dot; the two halves of a row are added through shared memory
+    auto epilogue = [&](int tile, float rule) {
+      const int tok = tile * RT_M + m;
+      float z = 0.f;
 #pragma unroll 1
-    for (int hh = 0; hh < 2; ++hh) {
-      const int h = hp * 2 + hh;
-      float x[RT_NXMAX];
+      for (int c0 = 0; c0 < 128; c0 += 16) {
+        float v[16];
+        tmem_ld16(tmem + ((uint32_t)(qd * 32) << 16) + (uint32_t)(256 + nh * 128 + c0), v);
+        tmem_ld_wait();
 #pragma unroll
-      for (int c0 = 0; c0 < RT_NXMAX; c0 += 16)
-        if (c0 < NXP) tmem_ld16(tmem + ((uint32_t)(qd * 32) << 16) + (uint32_t)(h * NXP + c0), &x[c0]);
-      tmem_ld_wait();
-      float mx = -CUDART_INF_F;
-#pragma unroll
-      for (int c = 0; c < RT_NXMAX; ++c)
-        if (c < NXP) {
-          x[c] = fmaf(rule, sv_r[h * NXP + c], x[c]) + sv_b[h * NXP + c];
-          mx = fmaxf(mx, x[c]);
+        for (int j = 0; j < 16; ++j) {
+          const int n = nh * 128 + c0 + j;
+          z = fmaf(ep_w2[n], gelu_erf(v[j] + fmaf(rule, ep_wr[n], ep_b1[n])), z);
         }
-      float l = 0.f;
-#pragma unroll
-      for (int c = 0; c < RT_NXMAX; ++c)
-        if (c < NXP) { x[c] = ex2f(x[c] - mx); l += x[c]; }
-      const float inv = 1.f / l;
-      if (hp == 1 && hh == 0) mbar_wait(ak_free, 0u);  // heads 2, 3 overwrite the kbar rows
-      unsigned char* base = (h < 2 ? p01 + h * HR : region0 + (h - 2) * HR) + (m >> 3) * (16 * NXP) + (m & 7) * 16;
-#pragma unroll
-      for (int g = 0; g < RT_NXMAX / 8; ++g)
-        if (g * 8 < NXP) {
-          uint32_t hi[4], lo[4];
-#pragma unroll
-          for (int e = 0; e < 4; ++e) split_bf16(x[g * 8 + 2 * e] * inv, x[g * 8 + 2 * e + 1] * inv, hi[e], lo[e]);
-          *reinterpret_cast<uint4*>(base + g * 128) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
-          *reinterpret_cast<uint4*>(base + g * 128 + HR / 2) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
-        }
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      }
+      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
       __syncwarp();
-      if (lane == 0) mbar_arrive(&p_ready[h]);
-      if (threadIdx.x == 0) RT_T(0, 5 + hh);
-      if (threadIdx.x == 128) RT_T(0, 7 + hh);
+      if (lane == 0) mbar_arrive(tmem_free);
+      ep_z[nh * 128 + m] = z;
+      bar_sync(1, RT_CWARPS * 32);
+      if (nh == 0 && tok < nc) p.scores[p.cand_pos[tok]] = rule + w.alpha * ((ep_z[m] + ep_z[128 + m]) + w.fc2_b[0]);
+      bar_sync(1, RT_CWARPS * 32);  // ep_z is free
+    };
+    int it = 0, prev_tile = -1;
+    float rule = 0.f, prev_rule = 0.f;
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+      const int t0 = tile * RT_M;
+      const uint32_t par = (uint32_t)it & 1u;
+      // kbar rows -> A operand (hi | lo): 128-byte global segments per row, 512 contiguous bytes of shared memory per warp
+      // item; all loads are issued before the wait on the previous tile's MMAs and before the first use
+      float4 x0[NU], x1[NU];
+#pragma unroll
+      for (int u = 0; u < NU; ++u) {
+        const int unit = warp + 8 * u, rb = unit / KB, kb = unit % KB;
+        const int row = rb * 8 + (lane & 7), k8 = kb * 4 + (lane >> 3);
+        if (t0 + row < nc) {
+          const float4* src = reinterpret_cast<const float4*>(p.kbar + (int64_t)(t0 + row) * D + k8 * 8);
+          x0[u] = __ldg(src); x1[u] = __ldg(src + 1);
+        } else {
+          x0[u] = make_float4(0.f, 0.f, 0.f, 0.f); x1[u] = x0[u];
+        }
+      }
+      if (it > 0) {  // the previous tile's MMAs are complete: its operand buffers are free, its accumulator is final
+        mbar_wait(fc1_full, par ^ 1u);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+      }
+#pragma unroll
+      for (int u = 0; u < NU; ++u) {
+        const int unit = warp + 8 * u, rb = unit / KB, kb = unit % KB;
+        const int k8 = kb * 4 + (lane >> 3);
+        uint32_t hi[4], lo[4];
+        split_bf16(x0[u].x, x0[u].y, hi[0], lo[0]); split_bf16(x0[u].z, x0[u].w, hi[1], lo[1]);
+        split_bf16(x1[u].x, x1[u].y, hi[2], lo[2]); split_bf16(x1[u].z, x1[u].w, hi[3], lo[3]);
+        unsigned char* dst = region0 + rb * A_SBO + k8 * 128 + (lane & 7) * 16;
+        *reinterpret_cast<uint4*>(dst) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+        *reinterpret_cast<uint4*>(dst + A_PART) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+      }
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // publish the rows to the async proxy (tcgen05.mma)
+      __syncwarp();
+      if (lane == 0) mbar_arrive(a_ready);
+      if (threadIdx.x == 0 && it == 0) RT_T(0, 3);
+      prev_rule = rule;
+      rule = (t0 + m < nc) ? p.rule_c[t0 + m] : 0.f;
+      if (it > 0) epilogue(prev_tile, prev_rule);   // S of this tile is multiplied meanwhile
+      if (threadIdx.x == 0 && it == 1) RT_T(0, 12);
+      if (xat) {
+        // ---- per-head softmax of this thread's token row; warps 0-3 take heads 0, 1, warps 4-7 heads 2, 3
+        mbar_wait(s_full, par);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        if (threadIdx.x == 0 && it == 0) RT_T(0, 4);
+#pragma unroll 1
+        for (int hh = 0; hh < 2; ++hh) {
+          const int h = hp * 2 + hh;
+          float x[RT_NXMAX];
+#pragma unroll
+          for (int c0 = 0; c0 < RT_NXMAX; c0 += 16)
+            if (c0 < NXP) tmem_ld16(tmem + ((uint32_t)(qd * 32) << 16) + (uint32_t)(h * NXP + c0), &x[c0]);
+          tmem_ld_wait();
+          float mx = -CUDART_INF_F;
+#pragma unroll
+          for (int c = 0; c < RT_NXMAX; ++c)
+            if (c < NXP) {
+              x[c] = fmaf(rule, sv_r[h * NXP + c], x[c]) + sv_b[h * NXP + c];
+              mx = fmaxf(mx, x[c]);
+            }
+          float l = 0.f;
+#pragma unroll
+          for (int c = 0; c < RT_NXMAX; ++c)
+            if (c < NXP) { x[c] = ex2f(x[c] - mx); l += x[c]; }
+          const float inv = 1.f / l;
+          if (hp == 1 && hh == 0) mbar_wait(ak_free, par);  // heads 2, 3 overwrite the kbar rows
+          unsigned char* base = (h < 2 ? p01 + h * HR : region0 + (h - 2) * HR) + (m >> 3) * (16 * NXP) + (m & 7) * 16;
+#pragma unroll
+          for (int g = 0; g < RT_NXMAX / 8; ++g)
+            if (g * 8 < NXP) {
+              uint32_t hi[4], lo[4];
+#pragma unroll
+              for (int e = 0; e < 4; ++e) split_bf16(x[g * 8 + 2 * e] * inv, x[g * 8 + 2 * e + 1] * inv, hi[e], lo[e]);
+              *reinterpret_cast<uint4*>(base + g * 128) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
+              *reinterpret_cast<uint4*>(base + g * 128 + HR / 2) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
+            }
+          asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&p_ready[h]);
+          if (threadIdx.x == 0 && it == 0) RT_T(0, 5 + hh);
+        }
+      }
+      prev_tile = tile;
     }
-  }
-
-  // ---- epilogue: warp w reads TMEM lanes 32 (w % 4) .. + 31 (token rows) of accumulator half w / 4:
-  // hid = acc + b1' + rule w_r -> erf-GELU -> fc2 dot; the two halves of a row are added through shared memory
-  {
-    const int nh = warp >> 2;
-    const int tok = t0 + m;
-    const bool valid = tok < nc;
-    float z = 0.f;
-    mbar_wait(fc1_full, 0u);
+    mbar_wait(fc1_full, (uint32_t)(it - 1) & 1u);
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     if (threadIdx.x == 0) RT_T(0, 9);
-#pragma unroll 1
-    for (int c0 = 0; c0 < 128; c0 += 16) {
-      float v[16];
-      tmem_ld16(tmem + ((uint32_t)(qd * 32) << 16) + (uint32_t)(256 + nh * 128 + c0), v);
-      tmem_ld_wait();
-#pragma unroll
-      for (int j = 0; j < 16; ++j) {
-        const int n = nh * 128 + c0 + j;
-        z = fmaf(ep_w2[n], gelu_erf(v[j] + fmaf(rule, ep_wr[n], ep_b1[n])), z);
-      }
-    }
-    ep_z[nh * 128 + m] = z;
+    epilogue(prev_tile, rule);
     if (threadIdx.x == 0) RT_T(0, 10);
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    if (nh == 0 && valid) p.scores[p.cand_pos[tok]] = rule + w.alpha * ((ep_z[m] + ep_z[128 + m]) + w.fc2_b[0]);
-    __syncthreads();  // the MMA warp frees the tensor memory after this
-    if (threadIdx.x == 0) RT_T(0, 11);
   }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (warp == 8) {
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+  }
+  if (threadIdx.x == 0) RT_T(0, 11);
 }
 
 }  // namespace ikv
