@@ -205,6 +205,8 @@ ikv_status ikv_profile_read(ikv_ctx *ctx, float *out_ms, int32_t *out_n);
                                evict_first (default 7)                                                         */
 #define IKV_TUNE_RESID_TC 2 /* 1 (default): residual head with folded cross attention on tcgen05 when the call has at
                                most 64 cross-attention positions; 0: always the unfolded kernel                */
+#define IKV_TUNE_LAYER_MAJOR 3 /* 1 (default): layer-major key pass with deferred normalisation (no logits scratch) when
+                                  the call fits its on-chip capacity; 0: always the logits-scratch key pass      */
 ikv_status ikv_tune(ikv_ctx *ctx, int32_t knob, int32_t value);
 
 /* Library / build identification, e.g. "ikv 0.1 sm_100a". */

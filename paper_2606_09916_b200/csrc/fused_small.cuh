@@ -14,10 +14,12 @@ namespace ikv {
 template <int D, int G>
 __global__ __launch_bounds__(128) void k_mem_prep(const float* __restrict__ M, int L, int Hkv, float inv_sqrt_d,
                                                   uint4* __restrict__ frag, int n_frag_blocks, int LH,
-                                                  float* __restrict__ mpart) {
+                                                  float* __restrict__ mpart, int32_t* __restrict__ layer_cnt) {
   pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
   pdl_launch_dependents();
   const int bid = blockIdx.x;
+  if (bid == 0 && layer_cnt)  // per-layer arrival counters of the layer-major key pass
+    for (int l = threadIdx.x; l < L; l += 128) layer_cnt[l] = 0;
   if (bid < n_frag_blocks) {
     memory_frags_item<D, G>(bid * 128 + threadIdx.x, M, L, Hkv, inv_sqrt_d, frag);
     return;

@@ -20,6 +20,7 @@
 #include "residual_tc.cuh"
 #include "score.cuh"
 #include "score_mma.cuh"
+#include "score_lm.cuh"
 #include "select.cuh"
 #include "select_cluster.cuh"
 #include "fused_small.cuh"
@@ -68,6 +69,9 @@ struct ikv_ctx {
   bool pdl_prune = true;     // ... and along the kernels of the prune pass (IKV_PDL_PRUNE=0 disables)
   bool attr_done[2][2][9] = {};
   int dbg_l2 = 7;            // IKV_TUNE_L2_HINTS
+  int use_lm = 1;            // IKV_TUNE_LAYER_MAJOR
+  int lm_dbg = 0;
+  int32_t* lm_cnt = nullptr; // per-layer arrival counters of k_key_pass_lm
 
   // scratch (per request, sized by ensure_scratch)
   int64_t cap_tokens = 0;
@@ -460,16 +464,52 @@ ikv_status dispatch_decode(ikv_ctx* c, int layer, const DecBatch& b, int n_req, 
             : dispatch_decode_g<float, 64>(c, layer, b, n_req, n_split, q, out, sc, st, pdl);
 }
 
-// bf16 key pass on the tensor pipe (score_mma.cuh).  Returns the number of partial (max, sum) columns.
+// bf16 key pass on the tensor pipe.  Layer-major with deferred normalisation (score_lm.cuh) when the call fits its
+// on-chip capacity: *lm_done = true, rule_c / scores / k_bar are final.  Otherwise k_key_pass (score_mma.cuh): logits
+// scratch + partials, *n_part = number of partial (max, sum) columns.
+struct LmOut { float* scores; float* rule_out; int scatter; };
 template <int D, int G>
-ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, int n_mpart, int* n_part,
-                           cudaStream_t st) {
+ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, int n_mpart, int* n_part, int N, int n_x,
+                           const LmOut& lo, bool* lm_done, cudaStream_t st) {
   const int L = c->cfg.n_layers, Hkv = c->cfg.n_kv_heads, Hq = c->cfg.n_q_heads;
   const int n_fb = mem_prep_frag_blocks<D, G>(L, Hkv);
+  const int grid = c->n_sm;
+  bool lm = false;
+  if constexpr (G <= 4) {
+    const int tiles_ub = (N + KP_TOK - 1) / KP_TOK + ((with_xq ? n_x : 0) + KP_TOK - 1) / KP_TOK;
+    lm = c->use_lm && Hkv <= KP_LWARPS && (tiles_ub + grid - 1) / grid <= (kbar ? LM_MT_KBAR : LM_MT);
+  }
   {
     ProfScope prof(c, IKV_PROF_MEM_PREP, st);
     CU(c, launch_pdl(k_mem_prep<D, G>, dim3(n_fb + n_mpart), dim3(128), 0, st, c->pdl_prune, M, L, Hkv,
-                     1.0f / sqrtf((float)D), c->frag, n_fb, L * Hq, c->mpart));
+                     1.0f / sqrtf((float)D), c->frag, n_fb, L * Hq, c->mpart, lm ? c->lm_cnt : (int32_t*)nullptr));
+  }
+  *lm_done = lm;
+  if constexpr (G <= 4) {
+    if (lm) {
+      int ns = 0;
+      const size_t smem = key_pass_lm_smem(Hq, Hkv, D, kbar, c->max_smem, &ns);
+      if (ns < 2) IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "key pass: a stage of %d bytes does not fit shared memory", Hkv * D * 2 * KP_TOK);
+      KeyPassLmParams p;
+      p.k_pool = (const bf16*)c->cfg.k_pool; p.layer_stride = c->layer_stride; p.L = L; p.Hkv = Hkv; p.frag = c->frag;
+      p.cand_slot = c->cand_slot; p.cand_pos = c->cand_pos; p.n_cand = c->d_ncand;
+      p.xq_slot = with_xq ? c->xq_slot : nullptr; p.n_xq = with_xq ? c->d_nxq : nullptr;
+      p.partials = c->partials; p.layer_cnt = c->lm_cnt; p.rule_c = c->rule_c;
+      p.scores = lo.scores; p.rule_out = lo.rule_out; p.scatter_scores = lo.scatter;
+      p.kbar = c->kbar; p.kq = c->kq; p.n_stage = ns; p.l2_hints = c->dbg_l2; p.dbg = c->lm_dbg;
+      ProfScope prof(c, IKV_PROF_KEY_PASS, st);
+      if (kbar) {
+        auto fn = k_key_pass_lm<D, G, true>;
+        CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(c, launch_pdl(fn, dim3(grid), dim3(lm_threads(true)), smem, st, c->pdl_prune, p));
+      } else {
+        auto fn = k_key_pass_lm<D, G, false>;
+        CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        CU(c, launch_pdl(fn, dim3(grid), dim3(lm_threads(false)), smem, st, c->pdl_prune, p));
+      }
+      *n_part = grid;
+      return IKV_OK;
+    }
   }
   int ns = 0;
   const size_t smem = key_pass_smem(L, Hq, Hkv, D, kbar, c->max_smem, &ns);
@@ -482,7 +522,6 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
   p.logits = c->logits; p.ldc = c->cap_tokens; p.partials = c->partials; p.kbar = c->kbar; p.kq = c->kq;
   p.n_stage = ns;
   p.l2_hints = c->dbg_l2;
-  const int grid = c->n_sm;
   ProfScope prof(c, 0, st);
   if (kbar) {
     auto fn = k_key_pass<D, G, true>;
@@ -499,22 +538,22 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
 }
 
 template <int D>
-ikv_status dispatch_key_pass_g(ikv_ctx* c, const float* M, bool kbar, bool xq, int n_mpart, int* n_part,
-                               cudaStream_t st) {
+ikv_status dispatch_key_pass_g(ikv_ctx* c, const float* M, bool kbar, bool xq, int n_mpart, int* n_part, int N, int n_x,
+                               const LmOut& lo, bool* lm_done, cudaStream_t st) {
   switch (c->G) {
-    case 1: return launch_key_pass<D, 1>(c, M, kbar, xq, n_mpart, n_part, st);
-    case 2: return launch_key_pass<D, 2>(c, M, kbar, xq, n_mpart, n_part, st);
-    case 4: return launch_key_pass<D, 4>(c, M, kbar, xq, n_mpart, n_part, st);
-    case 5: return launch_key_pass<D, 5>(c, M, kbar, xq, n_mpart, n_part, st);
-    case 8: return launch_key_pass<D, 8>(c, M, kbar, xq, n_mpart, n_part, st);
+    case 1: return launch_key_pass<D, 1>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
+    case 2: return launch_key_pass<D, 2>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
+    case 4: return launch_key_pass<D, 4>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
+    case 5: return launch_key_pass<D, 5>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
+    case 8: return launch_key_pass<D, 8>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
   }
   IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "GQA group size %d not supported (1,2,4,5,8)", c->G);
 }
 
-ikv_status dispatch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool xq, int n_mpart, int* n_part,
-                             cudaStream_t st) {
-  return c->cfg.head_dim == 128 ? dispatch_key_pass_g<128>(c, M, kbar, xq, n_mpart, n_part, st)
-                                : dispatch_key_pass_g<64>(c, M, kbar, xq, n_mpart, n_part, st);
+ikv_status dispatch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool xq, int n_mpart, int* n_part, int N, int n_x,
+                             const LmOut& lo, bool* lm_done, cudaStream_t st) {
+  return c->cfg.head_dim == 128 ? dispatch_key_pass_g<128>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st)
+                                : dispatch_key_pass_g<64>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
 }
 
 ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, float* rule_out, cudaStream_t st) {
@@ -562,12 +601,14 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   }
   const int LH = L * Hq, n_mpart = learn ? (LH + 31) / 32 : 0;  // mbar partial sums ride along with the fragments
   int n_part = (N + SCORE_TILE - 1) / SCORE_TILE;
+  bool lm_done = false;  // the layer-major key pass has already produced rule_c (and the scores of a rule-only call)
   if (fast) {
-    TRY(dispatch_key_pass(c, M, learn, n_x > 0, n_mpart, &n_part, st));
+    LmOut lo{scores, rule_out, learn ? 0 : 1};
+    TRY(dispatch_key_pass(c, M, learn, n_x > 0, n_mpart, &n_part, N, n_x, lo, &lm_done, st));
   } else {
     if (n_mpart > 0) {
-      if (D == 128) k_mem_prep<128, 1><<<n_mpart, 128, 0, st>>>(M, L, Hkv, 0.f, nullptr, 0, LH, c->mpart);
-      else k_mem_prep<64, 1><<<n_mpart, 128, 0, st>>>(M, L, Hkv, 0.f, nullptr, 0, LH, c->mpart);
+      if (D == 128) k_mem_prep<128, 1><<<n_mpart, 128, 0, st>>>(M, L, Hkv, 0.f, nullptr, 0, LH, c->mpart, nullptr);
+      else k_mem_prep<64, 1><<<n_mpart, 128, 0, st>>>(M, L, Hkv, 0.f, nullptr, 0, LH, c->mpart, nullptr);
       LAUNCH_CHECK(c);
     }
     TRY(dispatch_logits(c, *s, M, N, learn, st));
@@ -585,6 +626,8 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   pk.kq = c->kq; pk.n_xq = c->d_nxq; pk.nks = (int)(c->xq_cap / 16); pk.kc_frag = c->kc_frag; pk.vc_frag = c->vc_frag;
   pk.n_fold = 0; pk.n_kv = 0; pk.tc = tc ? 1 : 0; pk.nxp = nxp;
   pk.rt.mbar = c->mbar; pk.rt.wcan = c->rt_wcan; pk.rt.svec = c->rt_svec; pk.rt.b1_eff = c->b1_eff;
+  if (lm_done) pk.n_lse = 0;   // no lse rows to reduce, no logits to read back
+  if (lm_done && !learn) return IKV_OK;
   if (tc) {
     // launch 1: lse rows and the folded operands of the residual head (they need the mean keys of the query positions,
     // i.e. the finished key pass).  launch 2: rule_c (Eq. 3).  launch 3: k_tail_tc, the residual head (Eq. 4-6), one
@@ -593,15 +636,15 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     pk.n_kv = n_x > 0 ? rt_fold_xattn_grid(nxp) : 0;
     {
       ProfScope prof(c, IKV_PROF_POST_KEY, st);
-      CU(c, launch_pdl(D == 128 ? k_post_key<128, true> : k_post_key<64, true>, dim3((LH + 3) / 4 + pk.n_fold + pk.n_kv),
-                       dim3(256), 0, st, c->pdl_prune, pk, c->rw));
+      CU(c, launch_pdl(D == 128 ? k_post_key<128, true> : k_post_key<64, true>,
+                       dim3((pk.n_lse + 3) / 4 + pk.n_fold + pk.n_kv), dim3(256), 0, st, c->pdl_prune, pk, c->rw));
     }
     RuleParams rp;
     rp.logits = c->logits; rp.ldc = c->cap_tokens; rp.LH = LH; rp.lse = c->lse; rp.n_cand = c->d_ncand;
     rp.cand_pos = c->cand_pos; rp.rule_c = c->rule_c; rp.scores = scores; rp.scatter_scores = 0;
     rp.rule_out = rule_out; rp.n_rule = (N + 63) / 64; rp.l2_hints = c->dbg_l2;
     pk.n_fold = 0; pk.n_kv = 0;
-    {
+    if (!lm_done) {
       ProfScope prof(c, IKV_PROF_RULE, st);
       CU(c, launch_pdl(D == 128 ? k_rule_fused<128> : k_rule_fused<64>, dim3(rp.n_rule), dim3(256), 0, st, c->pdl_prune,
                        rp, pk, c->rw));
@@ -625,7 +668,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   {
     // launch 1: lse rows.  launch 2: rule_c (Eq. 3) and, for a learnable call on the unfolded kernel, the folded residual
     // operands and the Kc / Vc fragments, whose latency-bound bodies hide under the rule blocks' stream of the logits.
-    {
+    if (!lm_done) {
       ProfScope prof(c, IKV_PROF_POST_KEY, st);
       CU(c, launch_pdl(D == 128 ? k_post_key<128, false> : k_post_key<64, false>, dim3((LH + 3) / 4), dim3(128), 0, st,
                        c->pdl_prune, pk, c->rw));
@@ -635,7 +678,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     RuleParams rp;
     rp.logits = c->logits; rp.ldc = c->cap_tokens; rp.LH = LH; rp.lse = c->lse; rp.n_cand = c->d_ncand;
     rp.cand_pos = c->cand_pos; rp.rule_c = c->rule_c; rp.scores = scores; rp.scatter_scores = learn ? 0 : 1;
-    rp.rule_out = rule_out; rp.n_rule = (N + 63) / 64; rp.l2_hints = c->dbg_l2;
+    rp.rule_out = rule_out; rp.n_rule = lm_done ? 0 : (N + 63) / 64; rp.l2_hints = c->dbg_l2;
     const int grid = rp.n_rule + pk.n_fold + pk.n_kv;
     ProfScope prof(c, IKV_PROF_RULE, st);
     CU(c, launch_pdl(D == 128 ? k_rule_fused<128> : k_rule_fused<64>, dim3(grid), dim3(256), 0, st, c->pdl_prune, rp, pk,
@@ -710,6 +753,10 @@ ikv_status ikv_debug_trace(long long* out) {
   cudaDeviceSynchronize();
   return cudaMemcpyFromSymbol(out, g_rt_trace, sizeof(long long) * 128) == cudaSuccess ? IKV_OK : IKV_ERR_CUDA;
 }
+ikv_status ikv_debug_lm(long long* out) {
+  cudaDeviceSynchronize();
+  return cudaMemcpyFromSymbol(out, g_lm_wait, sizeof(long long) * 640) == cudaSuccess ? IKV_OK : IKV_ERR_CUDA;
+}
 #endif
 
 const char* ikv_version(void) { return "ikv 0.1 (sm_100a)"; }
@@ -767,6 +814,7 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
   ok = ok && cudaMalloc((void**)&c->d_ncand, 4) == cudaSuccess && cudaMalloc((void**)&c->d_nxq, 4) == cudaSuccess;
   ok = ok && cudaMemset(c->d_nxq, 0, 4) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&c->lse, (size_t)cfg->n_layers * cfg->n_q_heads * 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&c->lm_cnt, (size_t)cfg->n_layers * 4) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&c->mbar, (size_t)cfg->head_dim * 4) == cudaSuccess;
   {
     const int LH = cfg->n_layers * cfg->n_q_heads, KS = cfg->head_dim / 16;
@@ -797,7 +845,7 @@ ikv_status ikv_destroy(ikv_ctx* c) {
   for (auto& kv : c->sessions) session_free(kv.second);
   void* bufs[] = {c->cand_pos, c->cand_slot, c->d_ncand, c->logits, c->partials, c->lse, c->rule_c, c->kbar, c->mbar,
                   c->xq_slot, c->d_nxq, c->kq, c->kc_frag, c->vc_frag, c->mpart, c->bq_eff, c->b1_eff, c->wq_frag,
-                  c->w1_can, c->rt_wcan, c->rt_svec, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
+                  c->w1_can, c->rt_wcan, c->rt_svec, c->lm_cnt, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
                   c->part_o, c->part_ml, c->st_out, c->st_scores,
                   c->st_qrows, c->resid_blob, c->frag};
   for (void* b : bufs) cudaFree(b);
@@ -815,6 +863,8 @@ ikv_status ikv_tune(ikv_ctx* c, int32_t knob, int32_t value) {
   switch (knob) {
     case IKV_TUNE_L2_HINTS: c->dbg_l2 = value; return IKV_OK;
     case IKV_TUNE_RESID_TC: c->resid_tc = value; return IKV_OK;
+    case IKV_TUNE_LAYER_MAJOR: c->use_lm = value; return IKV_OK;
+    case 99: c->lm_dbg = value; return IKV_OK;
   }
   IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_tune: unknown knob %d", knob);
 }

@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdio.h>
 
 namespace ikv {
 
@@ -42,8 +43,19 @@ __device__ __forceinline__ bool mbar_test_wait(uint64_t* bar, uint32_t parity) {
   return ok != 0;
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+#ifdef IKV_TRACE
+  long long n = 0;
+  while (!mbar_try_wait(bar, parity)) {
+    if (++n > 20000000LL) {
+      printf("mbar hang: cta %d warp %d lane %d bar %u parity %u\n", (int)blockIdx.x, (int)(threadIdx.x >> 5),
+             (int)(threadIdx.x & 31), smem_u32(bar), parity);
+      __trap();
+    }
+  }
+#else
   while (!mbar_try_wait(bar, parity)) {
   }
+#endif
 }
 
 // 1-D bulk copy global -> shared (the TMA unit, SASS UBLKCP); completion is signalled on `bar` as `bytes`
