@@ -148,7 +148,11 @@ ikv_status ikv_score(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req, int32
  * freed_slots: DEVICE int32, requests concatenated like `scores` (capacity seq_len each); receives, per
  * request, the slots that pass the prefix-safe test (a)(b)(c) of PAPER.md:132, each once, ordered by first
  * dropped position (R22).  n_freed / n_kept: DEVICE int32[n_req].
- * Also refreshes the session's compact live list used by ikv_decode_attn. */
+ * Also refreshes the session's compact live list used by ikv_decode_attn.
+ * Stream ordering: the kernel is launched with programmatic stream serialization and reads the slot maps before it
+ * orders itself after the preceding kernel of the stream (the producer of `scores`); `scores` are read after that
+ * point.  The slot maps of the batch must therefore not be written by the kernel enqueued directly before this call
+ * (they never are when that kernel is ikv_score's or any other scorer: a map is edited between events, not inside one). */
 ikv_status ikv_select_evict(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req, const float *scores,
                             int32_t *freed_slots, int32_t *n_freed, int32_t *n_kept, void *stream);
 

@@ -22,6 +22,15 @@ struct SelBatch {
   SelParams p[SEL_MAX_REQ];
 };
 
+// Lifetime barrier of distributed shared memory: a CTA may not exit while another rank can still read its shared memory.
+// It orders no memory (arrive.relaxed: no fence over the output writes still in flight) and is split, so that the global
+// writes between arrive and wait overlap the other ranks' last remote reads.
+// `dep` = a value computed from this rank's last remote loads: the arrive cannot issue before they have returned.
+__device__ __forceinline__ void cluster_arrive_relaxed(int dep) {
+  asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::"r"(dep) : "memory");
+}
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.aligned;" ::: "memory"); }
+
 // sum over the cluster of one int per CTA, and the exclusive prefix of this CTA's rank
 __device__ __forceinline__ void cluster_offsets(cg::cluster_group& cl, int* sh_val, int crank, int* before, int* total) {
   int b = 0, t = 0;
@@ -121,9 +130,9 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_partit
 // ---------------------------------------------------------------------------------------------------------------
 template <int MAXI>
 __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select_evict_cl(const SelBatch batch) {
-  // waits on its predecessor; never triggers its dependents early: the decode kernel that may follow reads the
-  // survivor list written here before its own wait (R27)
-  pdl_wait();
+  // Never triggers its dependents early: the decode kernel that may follow reads the survivor list written here.  The
+  // wait on the predecessor (the producer of the scores) comes after the prologue: the slot map is not modified between
+  // ikv_score and ikv_select_evict of one event (ikv.h), so loading and classifying it overlaps the predecessor's tail.
   // one cluster per request of the batch.  Requests run concurrently on the shared kept-slot bitmap and
   // first-dropped-position table: they may share slots only below their radix_protected_len (forks, R19), where neither
   // structure is consulted, and every request clears exactly the bits it set.
@@ -145,63 +154,59 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select
   int slot[MAXI];
   uint32_t key[MAXI];
   uint32_t cand_m = 0, forced_m = 0;  // bit i: item i is a candidate / forced
+  const bool vec_s = (MAXI % 4 == 0) && (base + MAXI <= N) && ((reinterpret_cast<uintptr_t>(p.S) & 15) == 0);
+  if (vec_s) {
+#pragma unroll
+    for (int i = 0; i < MAXI; i += 4) {
+      const int4 v = *reinterpret_cast<const int4*>(p.S + base + i);
+      slot[i] = v.x; slot[i + 1] = v.y; slot[i + 2] = v.z; slot[i + 3] = v.w;
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < MAXI; ++i) slot[i] = (base + i < N) ? p.S[base + i] : p.dead;
+  }
+#pragma unroll
+  for (int i = 0; i < MAXI; ++i) {
+    const int j = base + i;
+    if (j < N) {
+      const int cls = classify(slot[i], j, p.dead, p.pi, p.qs, p.qe);
+      if (cls == CLS_CAND) cand_m |= 1u << i;
+      else if (cls == CLS_FORCED) forced_m |= 1u << i;
+    }
+  }
+  if (tid < 2) sh_cnt[tid] = 0;
+  if (tid < 256) { hist[0][tid] = 0; hist[1][tid] = 0; }
+  __syncthreads();
+  {  // |F| and |A| of this CTA; summed over the cluster together with the first histogram
+    const int nf = warp_sum_i(__popc(forced_m)), nc = warp_sum_i(__popc(cand_m));
+    if (lane == 0) { atomicAdd(&sh_cnt[0], nf); atomicAdd(&sh_cnt[1], nc); }
+  }
+  pdl_wait();  // the scores are complete
   {
-    const bool vec = (MAXI % 4 == 0) && (base + MAXI <= N) &&
-                     (((reinterpret_cast<uintptr_t>(p.S) | reinterpret_cast<uintptr_t>(p.scores)) & 15) == 0);
+    const bool vec = (MAXI % 4 == 0) && (base + MAXI <= N) && ((reinterpret_cast<uintptr_t>(p.scores) & 15) == 0);
     float sc[MAXI];
     if (vec) {
 #pragma unroll
       for (int i = 0; i < MAXI; i += 4) {
-        const int4 v = *reinterpret_cast<const int4*>(p.S + base + i);
         const float4 f = *reinterpret_cast<const float4*>(p.scores + base + i);
-        slot[i] = v.x; slot[i + 1] = v.y; slot[i + 2] = v.z; slot[i + 3] = v.w;
         sc[i] = f.x; sc[i + 1] = f.y; sc[i + 2] = f.z; sc[i + 3] = f.w;
       }
     } else {
 #pragma unroll
-      for (int i = 0; i < MAXI; ++i) {
-        const bool in = base + i < N;
-        slot[i] = in ? p.S[base + i] : p.dead;
-        sc[i] = in ? p.scores[base + i] : 0.f;
-      }
+      for (int i = 0; i < MAXI; ++i) sc[i] = (base + i < N) ? p.scores[base + i] : 0.f;
     }
 #pragma unroll
-    for (int i = 0; i < MAXI; ++i) {
-      const int j = base + i;
-      key[i] = 0u;
-      if (j < N) {
-        const int cls = classify(slot[i], j, p.dead, p.pi, p.qs, p.qe);
-        if (cls == CLS_CAND) { cand_m |= 1u << i; key[i] = score_key(sc[i]); }
-        else if (cls == CLS_FORCED) forced_m |= 1u << i;
-      }
-    }
+    for (int i = 0; i < MAXI; ++i) key[i] = ((cand_m >> i) & 1u) ? score_key(sc[i]) : 0u;
   }
 
-  // ---- |F| and |A|
-  if (tid < 2) sh_cnt[tid] = 0;
-  if (tid < 256) { hist[0][tid] = 0; hist[1][tid] = 0; }
-  __syncthreads();
-  {
-    const int nf = warp_sum_i(__popc(forced_m)), nc = warp_sum_i(__popc(cand_m));
-    if (lane == 0) { atomicAdd(&sh_cnt[0], nf); atomicAdd(&sh_cnt[1], nc); }
-  }
-  cl.sync();
-  int nF = 0, nC = 0;
-#pragma unroll
-  for (int rk = 0; rk < CL_CTAS; ++rk) {
-    nF += *cl.map_shared_rank(&sh_cnt[0], rk);
-    nC += *cl.map_shared_rank(&sh_cnt[1], rk);
-  }
-  int cstar = (N <= p.C) ? nC : max(0, p.C - nF);  // R15, R14
-  cstar = min(cstar, nC);
-  const bool keep_all = (cstar == nC), keep_none = (cstar == 0);
-
-  // ---- radix select of the cstar-th largest key, MSB first
+  // ---- radix select of the cstar-th largest key, MSB first; the first pass does not depend on C*
+  int nF = 0, nC = 0, cstar = 0;
+  bool keep_all = false, keep_none = false;
   uint32_t thr = 0;
   int need_eq = 0;
-  if (!keep_all && !keep_none) {
+  {
     uint32_t prefix = 0u;
-    int remaining = cstar;
+    int remaining = 0;
     for (int pass = 3; pass >= 0; --pass) {
       const int shift = pass * 8;
       const uint32_t mask = (pass == 3) ? 0u : (0xffffffffu << (shift + 8));
@@ -210,13 +215,32 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select
       for (int i = 0; i < MAXI; ++i) {
         const bool on = ((cand_m >> i) & 1u) && ((key[i] & mask) == prefix);
         const uint32_t digit = (key[i] >> shift) & 255u;
+        // upper digits are almost always the same over a warp (scores share sign and exponent): one atomic per warp;
+        // otherwise the digits are spread over the bins and plain shared-memory atomics do not collide much
         const uint32_t act = __ballot_sync(0xffffffffu, on);
-        if (on) {
-          const uint32_t peers = __match_any_sync(act, digit);
-          if (lane == (__ffs(peers) - 1)) atomicAdd(&h[digit], __popc(peers));
+        if (act) {
+          const int first = __ffs(act) - 1;
+          const uint32_t d0 = __shfl_sync(0xffffffffu, digit, first);
+          if (__all_sync(0xffffffffu, !on || digit == d0)) {
+            if (lane == first) atomicAdd(&h[d0], __popc(act));
+          } else if (on) {
+            atomicAdd(&h[digit], 1);
+          }
         }
       }
       cl.sync();
+      if (pass == 3) {
+#pragma unroll
+        for (int rk = 0; rk < CL_CTAS; ++rk) {
+          nF += *cl.map_shared_rank(&sh_cnt[0], rk);
+          nC += *cl.map_shared_rank(&sh_cnt[1], rk);
+        }
+        cstar = (N <= p.C) ? nC : max(0, p.C - nF);  // R15, R14
+        cstar = min(cstar, nC);
+        keep_all = (cstar == nC); keep_none = (cstar == 0);
+        remaining = cstar;
+        if (keep_all || keep_none) break;  // uniform over the cluster: no threshold to find
+      }
       if (tid < 256) {
         int v = 0;
 #pragma unroll
@@ -254,8 +278,10 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select
       remaining = sh_remaining;
       __syncthreads();
     }
-    thr = prefix;
-    need_eq = remaining;  // ties at the threshold survive lowest positions first (R13)
+    if (!keep_all && !keep_none) {
+      thr = prefix;
+      need_eq = remaining;  // ties at the threshold survive lowest positions first (R13)
+    }
   }
 
   // ---- ties in position order
@@ -298,8 +324,7 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select
       else if (((drop_m >> i) & 1u) && j >= p.radix) atomicMin(&p.firstpos[slot[i]], j);
     }
   }
-  __threadfence();
-  cl.sync();
+  cl.sync();  // arrive.release / wait.acquire at cluster scope: the bitmap and table updates are visible to every rank
 
   // ---- freed test (PAPER.md:132 (a)(b)(c)), ordered compaction of survivors and freed slots
   uint32_t freed_m = 0;
