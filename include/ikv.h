@@ -162,14 +162,14 @@ ikv_status ikv_select_evict(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req
  * q, out: DEVICE [n_req][H_q][D]; bf16 for a bf16 pool, fp32 for an fp32 pool.  Positions below the seq_len of
  * the last ikv_select_evict on the same (session, slot_map) come from the cached compact live list; positions
  * appended since are read from slot_map.  A caller that edited the slot map itself passes IKV_REQ_RESCAN.
- * Stream ordering (R27): the kernels of this call are launched with programmatic stream serialization and
- * read q, the slot maps and the K/V pools as soon as they start; they order only their WRITES after the preceding
- * kernel of the stream.  This is ordinary stream order as long as the producer of those inputs is a normally
- * completing kernel or copy, or one of this library's kernels: the scoring kernels of ikv_score trigger their
- * dependents early but wait on their own predecessor first and write none of these inputs, ikv_select_evict and the
- * rescan, which write the survivor lists, never trigger early; a caller whose
- * own producer kernel triggers its dependents early (griddepcontrol.launch_dependents) must not do so before its
- * writes, or sets IKV_PDL=0 in the environment.  Up to 32 requests go into one launch; larger batches are chunked. */
+ * Stream ordering (R27): the kernels of this call are launched with programmatic stream serialization.  Before
+ * they order themselves after the preceding kernel of the stream they read only the session's survivor list and the K/V
+ * rows of the positions it covers -- state that kernel cannot be producing (after ikv_select_evict or a rescan the library
+ * launches the first decode call without the programmatic attribute).  q, the slot-map tail and the K/V rows of positions
+ * appended since the last select are read after that point, so any producer kernel is safe, including one that triggers
+ * its dependents early.  IKV_REQ_INPUTS_COMPLETE lifts this for a request whose inputs were complete before the preceding
+ * kernel started (precomputed queries): the whole call then overlaps that kernel.  IKV_CFG_NO_PDL turns programmatic
+ * launches off.  Up to 32 requests go into one launch; larger batches are chunked. */
 ikv_status ikv_decode_attn(ikv_ctx *ctx, int32_t layer, const ikv_request *reqs, int32_t n_req, const void *q,
                            void *out, float sm_scale, void *stream);
 
@@ -212,6 +212,11 @@ ikv_status ikv_profile_read(ikv_ctx *ctx, float *out_ms, int32_t *out_n);
 #define IKV_TUNE_LAYER_MAJOR 3 /* 1 (default): layer-major key pass with deferred normalisation (no logits scratch) when
                                   the call fits its on-chip capacity; 0: always the logits-scratch key pass      */
 ikv_status ikv_tune(ikv_ctx *ctx, int32_t knob, int32_t value);
+
+/* Test support: enqueues a kernel that signals its dependents first (griddepcontrol.launch_dependents), idles for
+ * delay_us microseconds and only then copies `bytes` (a multiple of 16) from src to dst (both DEVICE).  Models a producer of
+ * q that triggers early; tests/test_gpu_parity.py uses it to check the stream ordering of ikv_decode_attn. */
+ikv_status ikv_test_late_writer(void *dst, const void *src, int64_t bytes, int32_t delay_us, void *stream);
 
 /* Library / build identification, e.g. "ikv 0.1 sm_100a". */
 const char *ikv_version(void);

@@ -14,6 +14,7 @@ struct DecReq {
   int seq_len, covered;
   int n_split;                // splits of this request (<= the launch's n_split, which is the scratch stride)
   int n_items;                // host-side upper bound of the list length; entries past *n_live hold the dead slot
+  int flags;                  // IKV_REQ_* of the request
 };
 struct DecBatch {
   DecReq r[DEC_MAX_REQ];

@@ -91,11 +91,12 @@ __global__ __launch_bounds__(DM_THREADS, 2) void k_decode_mma(const DecMmaParams
   __syncthreads();
   pdl_launch_dependents();
 
-  // Programmatic dependent launch: this grid may start while the previous decode call (its split and merge grids,
-  // the only kernels of the library that trigger their dependents early) is still running.  Everything READ here --
-  // slot lists, K/V pools, q -- was produced by kernels that never trigger early, so it is complete at this point;
-  // everything WRITTEN here (the partial buffers, which the previous merge may still be reading) is written only
-  // after pdl_wait(), which the consumers execute just before their stores (R27).
+  // Programmatic dependent launch: this grid may start while the preceding kernel of the stream is still running.
+  // What is read BEFORE griddepcontrol.wait is only what cannot be that kernel's output: the survivor list (rewritten
+  // only by ikv_select_evict / the rescan, after which the host launches this kernel without the programmatic attribute)
+  // and the K/V rows of positions that list covers.  The caller's inputs of THIS call -- q, the slot-map tail and the K/V
+  // rows of the appended positions -- are read after the wait, unless the request carries IKV_REQ_INPUTS_COMPLETE.
+  // Everything WRITTEN here (the partial buffers, which the previous merge may still be reading) is written after it.
   const DecReq rq = batch.r[req];
   const int n_cached = rq.n_items;
   const int total = n_cached + (rq.seq_len - rq.covered);
@@ -107,17 +108,20 @@ __global__ __launch_bounds__(DM_THREADS, 2) void k_decode_mma(const DecMmaParams
 
   if (warp == DM_CWARPS) {
     // ------------------------------------------------------------------ producer
-    auto slot_of = [&](int i) -> int {
+    bool waited = (rq.flags & 2) != 0;  // IKV_REQ_INPUTS_COMPLETE
+    auto slot_of = [&](int i0) -> int {  // slots i0 .. i0+31, one per lane (warp-uniform i0)
+      if (!waited && i0 + 32 > n_cached && i0 < end) { pdl_wait(); waited = true; }  // the slot-map tail is a caller input
+      const int i = i0 + lane;
       if (i >= end) return p.dead;
-      return (i < n_cached) ? __ldg(rq.live_slots + i) : __ldg(rq.S + rq.covered + (i - n_cached));
+      return (i < n_cached) ? rq.live_slots[i] : rq.S[rq.covered + (i - n_cached)];
     };
-    int cur = slot_of(begin + lane), nxt = slot_of(begin + 32 + lane);
+    int cur = slot_of(begin), nxt = slot_of(begin + 32);
     int s = 0;
     uint32_t ph = 0;
     for (int t = 0; t < n_tiles; ++t) {
       if (t > 0 && (t & 1) == 0) {
         cur = nxt;
-        nxt = slot_of(begin + (t + 2) * DM_TOK + lane);
+        nxt = slot_of(begin + (t + 2) * DM_TOK);
       }
       const int i = begin + t * DM_TOK + lane;
       const int slot = __shfl_sync(0xffffffffu, cur, (t & 1) * DM_TOK + (lane & (DM_TOK - 1)));
@@ -148,12 +152,13 @@ __global__ __launch_bounds__(DM_THREADS, 2) void k_decode_mma(const DecMmaParams
     uint32_t qb[KS][2];
 #pragma unroll
     for (int ks = 0; ks < KS; ++ks) { qb[ks][0] = 0u; qb[ks][1] = 0u; }
+    if (!(rq.flags & 2)) pdl_wait();  // q is a caller input of this call (IKV_REQ_INPUTS_COMPLETE: read it right away)
     if (active && r < G) {
       const uint32_t* qp = reinterpret_cast<const uint32_t*>(p.q + ((int64_t)req * Hq + kvh * G + r) * D);
 #pragma unroll
       for (int ks = 0; ks < KS; ++ks) {
-        qb[ks][0] = __ldg(qp + 8 * ks + q4);
-        qb[ks][1] = __ldg(qp + 8 * ks + 4 + q4);
+        qb[ks][0] = qp[8 * ks + q4];
+        qb[ks][1] = qp[8 * ks + 4 + q4];
       }
     }
     const float sc = p.sm_scale * 1.4426950408889634f;  // logits in log2 units

@@ -202,6 +202,16 @@ cudaError_t launch_pdl(void (*fn)(KArgs...), dim3 grid, dim3 block, size_t smem,
   return cudaLaunchKernelEx(&cfg, fn, KArgs(args)...);
 }
 
+// Test support (ikv_test_late_writer): a producer that triggers its dependents FIRST, idles, and only then writes.
+__global__ void k_late_writer(uint4* dst, const uint4* src, int64_t n16, int64_t delay_ns) {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  unsigned long long t0, t1;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+  do { asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1)); } while ((long long)(t1 - t0) < delay_ns);
+  for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n16; i += (int64_t)gridDim.x * blockDim.x)
+    dst[i] = src[i];
+}
+
 __global__ void k_fill_i32(int32_t* p, int64_t n, int32_t v) {
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
     p[i] = v;
@@ -759,6 +769,12 @@ ikv_status ikv_debug_lm(long long* out) {
 }
 #endif
 
+ikv_status ikv_test_late_writer(void* dst, const void* src, int64_t bytes, int32_t delay_us, void* stream) {
+  if (!dst || !src || bytes <= 0 || (bytes & 15)) return IKV_ERR_INVALID_ARG;
+  k_late_writer<<<1, 256, 0, (cudaStream_t)stream>>>((uint4*)dst, (const uint4*)src, bytes / 16, (int64_t)delay_us * 1000);
+  return cudaGetLastError() == cudaSuccess ? IKV_OK : IKV_ERR_CUDA;
+}
+
 const char* ikv_version(void) { return "ikv 0.1 (sm_100a)"; }
 
 static thread_local std::string g_create_err;  // ikv_create has no context to hang its message on
@@ -1165,6 +1181,7 @@ ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, i
       batch.r[i].seq_len = r.seq_len;
       batch.r[i].covered = s->covered;
       batch.r[i].n_items = s->live_ub;
+      batch.r[i].flags = r.flags;
       const int items = s->live_ub + (r.seq_len - s->covered);
       items_of[i] = items;
       if (items > max_items) max_items = items;

@@ -32,7 +32,7 @@ PROF_NAMES = ["key_pass", "decode_split", "memory_update", "partition", "mem_pre
 
 EXPORTS = ["ikv_create", "ikv_destroy", "ikv_last_error", "ikv_reserve", "ikv_session_open", "ikv_session_fork",
            "ikv_session_close", "ikv_session_get_memory", "ikv_session_set_memory", "ikv_residual_load",
-           "ikv_memory_update", "ikv_score", "ikv_select_evict", "ikv_decode_attn", "ikv_prune_host", "ikv_profile_enable", "ikv_profile_read", "ikv_tune", "ikv_version"]
+           "ikv_memory_update", "ikv_score", "ikv_select_evict", "ikv_decode_attn", "ikv_prune_host", "ikv_profile_enable", "ikv_profile_read", "ikv_tune", "ikv_test_late_writer", "ikv_version"]
 
 
 class Config(C.Structure):
@@ -76,6 +76,7 @@ _lib.ikv_select_evict.argtypes = [C.c_void_p, C.POINTER(Request), C.c_int32, C.c
 _lib.ikv_decode_attn.argtypes = [C.c_void_p, C.c_int32, C.POINTER(Request), C.c_int32, C.c_void_p, C.c_void_p,
                                  C.c_float, C.c_void_p]
 _lib.ikv_tune.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+_lib.ikv_test_late_writer.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p]
 _lib.ikv_profile_enable.argtypes = [C.c_void_p, C.c_int32]
 _lib.ikv_profile_read.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.ikv_prune_host.argtypes = [C.c_void_p, C.POINTER(Request), C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p,
@@ -201,6 +202,13 @@ class Context:
     def decode_attn(self, layer, reqs, q, out, sm_scale, stream=None):
         self._chk(_lib.ikv_decode_attn(self._h, layer, _req_array(reqs), len(reqs), _ptr(q), _ptr(out),
                                        C.c_float(sm_scale), _stream(stream)))
+
+    @staticmethod
+    def test_late_writer(dst, src, delay_us, stream=None):
+        """Test support: dst <- src by a kernel that triggers its dependents first and writes delay_us later."""
+        st = _lib.ikv_test_late_writer(_ptr(dst), _ptr(src), src.numel() * src.element_size(), delay_us, _stream(stream))
+        if st != OK:
+            raise IkvError(st, "ikv_test_late_writer failed")
 
     def tune(self, knob: int, value: int):
         self._chk(_lib.ikv_tune(self._h, knob, value))

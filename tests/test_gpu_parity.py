@@ -637,3 +637,83 @@ def test_errors_are_reported_not_thrown(ikv):
     # unsupported geometry is refused at create
     with pytest.raises(ikv.IkvError):
         ikv.Context(1, 3, 2, 64, w.k_pool[:1].contiguous(), w.v_pool[:1].contiguous())
+
+
+# ------------------------------------------------------------------------------------------- stream ordering
+def test_decode_after_a_producer_that_triggers_early(ikv, oracle):
+    """ikv_decode_attn is launched with programmatic stream serialization.  With default request flags it must read q
+    (and the slot-map tail) only after the preceding kernel of the stream has completed -- even when that kernel signals
+    its dependents BEFORE it writes q (R27; ikv.h).  The producer here triggers first, idles 200 us, then
+    writes the real q over a buffer of zeros."""
+    shape = wl.ModelShape(2, 8, 2, 128, "bf16")
+    w = wl.small(seed=41, shape=shape, n_tokens=3000, budget=700, kv_dtype="bf16")
+    ctx, s, M, kp, vp = run_memory(ikv, oracle, w)
+    g = gc.oracle_geom(oracle, w)
+    S_dev = s.slot_map.clone().cuda()
+    scores = torch.empty(s.N, device="cuda")
+    freed = torch.empty(s.N, dtype=torch.int32, device="cuda")
+    nf = torch.zeros(1, dtype=torch.int32, device="cuda")
+    nk = torch.zeros(1, dtype=torch.int32, device="cuda")
+    req = gc.request(ikv, s, S_dev)
+    ctx.score([req], ikv.MODE_MEMORY, scores)
+    ctx.select_evict([req], scores, freed, nf, nk)
+    scale = 1.0 / math.sqrt(shape.D)
+    q_true = torch.randn((shape.L, 1, shape.Hq, shape.D), generator=torch.Generator().manual_seed(9)).to(torch.bfloat16).cuda()
+    out = torch.zeros_like(q_true)
+    seq = s.N + 2                                           # two appended positions: the slot-map tail is read as well
+    r = gc.request(ikv, s, S_dev, seq_len=seq)
+    ctx.decode_attn(0, [r], q_true[0], out[0], scale)       # first call after the select (not programmatic)
+    torch.cuda.synchronize()
+    for rep in range(3):
+        q_buf = torch.zeros_like(q_true[1])
+        out[1].zero_()
+        torch.cuda.synchronize()
+        ikv.Context.test_late_writer(q_buf, q_true[1], 200)
+        ctx.decode_attn(1, [r], q_buf, out[1], scale)       # programmatic launch right behind the late writer
+        torch.cuda.synchronize()
+        want = oracle.decode(g, kp, vp, 1, S_dev.cpu().numpy()[:seq], q_true[1, 0].float().cpu().numpy(), scale)
+        err = gc.assert_decode_close(out[1, 0].float().cpu().numpy(), want, True, f"late writer rep {rep}")
+    print(f"decode behind an early-triggering producer: max abs err {err:.3e}")
+
+
+def test_sessions_on_a_non_blocking_stream(ikv, oracle):
+    """Session creation (auto-create in ikv_memory_update, ikv_session_fork) zero-fills the memory on the CALLER's stream:
+    on a non-blocking stream, with the legacy default stream busy, the fill must not land after the first update."""
+    shape = wl.ModelShape(2, 8, 2, 128, "bf16")
+    w = wl.small(seed=43, shape=shape, n_tokens=600, budget=200, kv_dtype="bf16")
+    gc.to_cuda(w)
+    ctx = gc.make_ctx(w)
+    s = w.sessions[0]
+    side = torch.cuda.Stream()                               # torch side streams are cudaStreamNonBlocking
+    busy = torch.empty(1 << 28, device="cuda")
+    rows = s.mem_rows[:4].cuda().contiguous()
+    torch.cuda.synchronize()
+    for sid in range(300, 306):
+        for _ in range(8):
+            busy.add_(1.0)                                   # keeps the default stream busy
+        with torch.cuda.stream(side):
+            ctx.memory_update(sid, rows, side)               # auto-create + first update, both on `side`
+            ctx.session_fork(sid, sid + 100, side)
+    torch.cuda.synchronize()
+    M = np.zeros((shape.L, shape.Hq, shape.D))
+    oracle.memory_update(M, s.mem_rows[:4].numpy(), 0.5)
+    for sid in range(300, 306):
+        assert np.abs(ctx.session_get_memory(sid).numpy() - M).max() < 2e-6
+        assert np.abs(ctx.session_get_memory(sid + 100).numpy() - M).max() < 2e-6
+
+
+def test_scores_are_bit_identical_from_run_to_run(ikv, oracle):
+    """Every sum of the scorer is taken in a fixed order (per-layer statistics in CTA order, deferred rule sums per
+    thread, KV heads in order): repeated calls give the same bits, in both scorer modes."""
+    w = wl.small(seed=47, shape=wl.ModelShape(4, 8, 2, 128, "bf16"), n_tokens=6000, budget=1500, kv_dtype="bf16")
+    ctx, s, M, kp, _ = run_memory(ikv, oracle, w)
+    ctx.residual_load(wl.residual_weights(w.shape.D, 31))
+    S_dev = s.slot_map[:s.N].cuda()
+    req = gc.request(ikv, s, S_dev)
+    for mode in (ikv.MODE_MEMORY, ikv.MODE_LEARNABLE):
+        ref = torch.empty(s.N, device="cuda")
+        ctx.score([req], mode, ref)
+        for _ in range(5):
+            again = torch.empty(s.N, device="cuda")
+            ctx.score([req], mode, again)
+            assert torch.equal(ref.view(torch.int32), again.view(torch.int32))
