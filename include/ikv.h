@@ -185,7 +185,8 @@ ikv_status ikv_prune_host(ikv_ctx *ctx, const ikv_request *req, const void *q_ro
 
 /* Kernel-level timing for bench.py's roofline and breakdown: while enabled, the library brackets kernels with CUDA
  * events on the caller's stream (no host synchronisation; skipped during stream capture).  level 1: only the two dominant
- * kernels (slots IKV_PROF_KEY_PASS, IKV_PROF_DECODE); level 2: every kernel of the path -- the events between the launches
+ * kernels (slots IKV_PROF_KEY_PASS, IKV_PROF_DECODE; the layer-major key pass stamps its own start and end with
+ * %globaltimer instead, so that no event sits between programmatically launched kernels); level 2: every kernel of the path -- the events between the launches
  * take away the overlap of programmatically launched kernels, so level 2 is a diagnostic, not a timing of the pass.
  * ikv_profile_read synchronises, sums the elapsed times recorded per slot since the last read and clears them:
  * out_ms[IKV_PROF_SLOTS] = total ms per slot, out_n[IKV_PROF_SLOTS] = launch counts. */
@@ -210,7 +211,8 @@ ikv_status ikv_profile_read(ikv_ctx *ctx, float *out_ms, int32_t *out_n);
 #define IKV_TUNE_RESID_TC 2 /* 1 (default): residual head with folded cross attention on tcgen05 when the call has at
                                most 64 cross-attention positions; 0: always the unfolded kernel                */
 #define IKV_TUNE_LAYER_MAJOR 3 /* 1 (default): layer-major key pass with deferred normalisation (no logits scratch) when
-                                  the call fits its on-chip capacity; 0: always the logits-scratch key pass      */
+                                  the call fits its on-chip capacity and has at least three 32-token tiles per SM;
+                                  2: whenever it fits; 0: always the logits-scratch key pass                      */
 ikv_status ikv_tune(ikv_ctx *ctx, int32_t knob, int32_t value);
 
 /* Test support: enqueues a kernel that signals its dependents first (griddepcontrol.launch_dependents), idles for

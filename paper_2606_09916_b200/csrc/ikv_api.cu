@@ -108,6 +108,11 @@ struct ikv_ctx {
   int prof_on = 0;           // 0 off, 1 the two dominant kernels, 2 every kernel of the path
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[IKV_PROF_SLOTS];
   std::vector<cudaEvent_t> ev_pool;   // events are created once and reused (ikv_profile_read returns them here)
+  // level 1 times the layer-major key pass by in-kernel %globaltimer stamps ({min start, max end} per launch): host
+  // events between programmatically launched kernels would take their overlap away and inflate the pass being timed
+  unsigned long long* ts_ring = nullptr;
+  int ts_used = 0;
+  static constexpr int TS_SLOTS = 4096;
 
   // residual head (transposed on the device)
   bool has_resid = false;
@@ -149,7 +154,7 @@ namespace {
 struct ProfScope {  // brackets a launch with events when profiling is on and the stream is not capturing
   ikv_ctx* c; int which; cudaStream_t st; cudaEvent_t a = nullptr, b = nullptr;
   ProfScope(ikv_ctx* c_, int which_, cudaStream_t st_) : c(c_), which(which_), st(st_) {
-    if (!c->prof_on || (c->prof_on < 2 && which > IKV_PROF_DECODE)) return;
+    if (!c->prof_on || which >= IKV_PROF_SLOTS || (c->prof_on < 2 && which > IKV_PROF_DECODE)) return;
     cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
     cudaStreamIsCapturing(st, &cs);
     if (cs != cudaStreamCaptureStatusNone) return;
@@ -487,7 +492,10 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
   bool lm = false;
   if constexpr (G <= 4) {
     const int tiles_ub = (N + KP_TOK - 1) / KP_TOK + ((with_xq ? n_x : 0) + KP_TOK - 1) / KP_TOK;
-    lm = c->use_lm && Hkv <= KP_LWARPS && (tiles_ub + grid - 1) / grid <= (kbar ? LM_MT_KBAR : LM_MT);
+    // every layer costs the grid one statistics round trip (~4 us): below three tiles per CTA the logits-scratch
+    // kernel is faster (IKV_TUNE_LAYER_MAJOR = 2 takes the layer-major kernel whenever the call fits its capacity)
+    lm = c->use_lm && Hkv <= KP_LWARPS && (tiles_ub + grid - 1) / grid <= (kbar ? LM_MT_KBAR : LM_MT) &&
+         (c->use_lm >= 2 || tiles_ub >= 3 * grid);
   }
   {
     ProfScope prof(c, IKV_PROF_MEM_PREP, st);
@@ -507,7 +515,9 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
       p.partials = c->partials; p.layer_cnt = c->lm_cnt; p.rule_c = c->rule_c;
       p.scores = lo.scores; p.rule_out = lo.rule_out; p.scatter_scores = lo.scatter;
       p.kbar = c->kbar; p.kq = c->kq; p.n_stage = ns; p.l2_hints = c->dbg_l2; p.dbg = c->lm_dbg;
-      ProfScope prof(c, IKV_PROF_KEY_PASS, st);
+      p.tstamp = nullptr;
+      if (c->prof_on == 1 && c->ts_ring && c->ts_used < ikv_ctx::TS_SLOTS) p.tstamp = c->ts_ring + 2 * (c->ts_used++);
+      ProfScope prof(c, c->prof_on == 1 ? IKV_PROF_SLOTS : IKV_PROF_KEY_PASS, st);  // level 1: stamps instead of events
       if (kbar) {
         auto fn = k_key_pass_lm<D, G, true>;
         CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -861,7 +871,7 @@ ikv_status ikv_destroy(ikv_ctx* c) {
   for (auto& kv : c->sessions) session_free(kv.second);
   void* bufs[] = {c->cand_pos, c->cand_slot, c->d_ncand, c->logits, c->partials, c->lse, c->rule_c, c->kbar, c->mbar,
                   c->xq_slot, c->d_nxq, c->kq, c->kc_frag, c->vc_frag, c->mpart, c->bq_eff, c->b1_eff, c->wq_frag,
-                  c->w1_can, c->rt_wcan, c->rt_svec, c->lm_cnt, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
+                  c->w1_can, c->rt_wcan, c->rt_svec, c->lm_cnt, c->ts_ring, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
                   c->part_o, c->part_ml, c->st_out, c->st_scores,
                   c->st_qrows, c->resid_blob, c->frag};
   for (void* b : bufs) cudaFree(b);
@@ -888,6 +898,16 @@ ikv_status ikv_tune(ikv_ctx* c, int32_t knob, int32_t value) {
 ikv_status ikv_profile_enable(ikv_ctx* c, int32_t on) {
   if (!c) return IKV_ERR_INVALID_ARG;
   c->prof_on = on < 0 ? 0 : (on > 2 ? 2 : on);
+  if (c->prof_on == 1) {
+    const size_t bytes = (size_t)ikv_ctx::TS_SLOTS * 16;
+    if (!c->ts_ring) CU(c, cudaMalloc((void**)&c->ts_ring, bytes));
+    std::vector<unsigned long long> init(2 * ikv_ctx::TS_SLOTS);
+    for (int i = 0; i < ikv_ctx::TS_SLOTS; ++i) { init[2 * i] = ~0ull; init[2 * i + 1] = 0ull; }
+    CU(c, cudaDeviceSynchronize());
+    CU(c, cudaMemcpy(c->ts_ring, init.data(), bytes, cudaMemcpyHostToDevice));
+    CU(c, cudaDeviceSynchronize());
+    c->ts_used = 0;
+  }
   return IKV_OK;
 }
 
@@ -906,6 +926,18 @@ ikv_status ikv_profile_read(ikv_ctx* c, float* out_ms, int32_t* out_n) {
     out_ms[w] = tot;
     out_n[w] = (int32_t)c->prof_ev[w].size();
     c->prof_ev[w].clear();
+  }
+  if (c->ts_ring && c->ts_used > 0) {  // stamps of the layer-major key pass (level 1)
+    std::vector<unsigned long long> h(2 * c->ts_used);
+    CU(c, cudaMemcpy(h.data(), c->ts_ring, h.size() * 8, cudaMemcpyDeviceToHost));
+    double tot = 0.0;
+    for (int i = 0; i < c->ts_used; ++i) tot += (double)(h[2 * i + 1] - h[2 * i]) * 1e-6;
+    out_ms[IKV_PROF_KEY_PASS] += (float)tot;
+    out_n[IKV_PROF_KEY_PASS] += c->ts_used;
+    for (int i = 0; i < c->ts_used; ++i) { h[2 * i] = ~0ull; h[2 * i + 1] = 0ull; }
+    CU(c, cudaMemcpy(c->ts_ring, h.data(), h.size() * 8, cudaMemcpyHostToDevice));
+    CU(c, cudaDeviceSynchronize());
+    c->ts_used = 0;
   }
   return IKV_OK;
 }

@@ -48,6 +48,7 @@ struct KeyPassLmParams {
   float* kq;               // [n_xq][D]     (KBAR)
   int n_stage;
   int l2_hints;
+  unsigned long long* tstamp;  // profiling: {min start, max end} of the launch in %globaltimer ns, or NULL
   int dbg;                 // experiment switches (bit 0: no TMEM traffic in the logit warps, bit 1: in the mean-key warps, bit 2: no stats/exp)
 };
 
@@ -123,6 +124,11 @@ __global__ __launch_bounds__(lm_threads(KBAR), 1) void k_key_pass_lm(const KeyPa
   static_assert(G <= 4, "layer-major key pass: G <= 4");
   pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
   pdl_launch_dependents();
+  if (p.tstamp && threadIdx.x == 0) {  // kernel time without host events between the launches (they cost the overlap)
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    atomicMin(p.tstamp, t);
+  }
   constexpr int KS = D / 16, NI = D / 32;
   constexpr int THREADS = lm_threads(KBAR);
   constexpr int MT = KBAR ? LM_MT_KBAR : LM_MT;
@@ -515,6 +521,11 @@ __global__ __launch_bounds__(lm_threads(KBAR), 1) void k_key_pass_lm(const KeyPa
   if (warp == W_STATS) {
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(512));
+  }
+  if (p.tstamp && threadIdx.x == 0) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    atomicMax(p.tstamp + 1, t);
   }
 }
 

@@ -121,7 +121,8 @@ def _fill_normal(shape: ModelShape, n_slots, seed, device, outlier_seed, chunk_l
     return pool
 
 
-def make_workload(shape: ModelShape, specs, seed: int, device="cpu", outliers=True, spare_pages=2) -> Workload:
+def make_workload(shape: ModelShape, specs, seed: int, device="cpu", outliers=True, spare_pages=2,
+                  with_values=True) -> Workload:
     """Build one shared paged pool holding every session in `specs`.
 
     Seeds: seed+1 keys, +2 values, +3 memory rows, +4 planted positions / noise,
@@ -132,7 +133,10 @@ def make_workload(shape: ModelShape, specs, seed: int, device="cpu", outliers=Tr
     pages_per = [(s.n_tokens + s.decode_tokens + PAGE - 1) // PAGE for s in specs]
     n_pages = 1 + sum(pages_per) + spare_pages
     n_slots = n_pages * PAGE
-    if outliers:
+    if not with_values:     # the pruning pass never reads V (the CPU baseline of bench.py uses the key pool only)
+        k_pool = _fill_normal(shape, n_slots, seed + 1, device, seed + 9)
+        v_pool = torch.empty((shape.L, 0, shape.Hkv, shape.D), dtype=shape.torch_dtype, device=device)
+    elif outliers:
         k_pool = _fill_normal(shape, n_slots, seed + 1, device, seed + 9)
         v_pool = _fill_normal(shape, n_slots, seed + 2, device, seed + 10)
     else:
@@ -187,12 +191,12 @@ def tiny(device="cpu", seed=0) -> Workload:
 
 
 def cfg1(device="cpu", seed=1000, n_tokens=32768, budget=8192, decode_tokens=256, shape=QWEN3_8B,
-         n_mem_rows=64) -> Workload:
+         n_mem_rows=64, with_values=True) -> Workload:
     """configs[1]: Qwen3-8B shape, 32,768 live tokens, M=64, 1% planted, C=8192, 256 decode steps."""
     n_cand = n_tokens - 256 - 64
     spec = SessionSpec(session_id=1, n_tokens=n_tokens, n_mem_rows=n_mem_rows, budget=budget,
                        n_planted=max(1, n_cand // 100), decode_tokens=decode_tokens)
-    return make_workload(shape, [spec], seed, device)
+    return make_workload(shape, [spec], seed, device, with_values=with_values)
 
 
 def cfg2(device="cpu", seed=2000, n_tokens=92160, budget=8192, decode_tokens=256) -> Workload:
@@ -211,7 +215,7 @@ def small(device="cpu", seed=77, shape=None, n_tokens=1500, budget=400, prefix_l
 
 
 def batched(device="cpu", seed=4000, shape=QWEN3_8B, n_sessions=64, median=16384, lo=4096, hi=65536,
-            sigma=0.5, budgets=(4096, 8192, 16384), decode_tokens=0) -> Workload:
+            sigma=0.5, budgets=(4096, 8192, 16384), decode_tokens=0, with_values=True) -> Workload:
     """configs[4]: concurrent sessions with lognormal live lengths in one shared pool."""
     g = _gen(seed + 8, "cpu")
     z = torch.randn(n_sessions, generator=g)
@@ -223,7 +227,7 @@ def batched(device="cpu", seed=4000, shape=QWEN3_8B, n_sessions=64, median=16384
         specs.append(SessionSpec(session_id=100 + i, n_tokens=int(n), n_mem_rows=int(m),
                                  budget=budgets[i % len(budgets)], n_planted=max(1, n_cand // 100),
                                  decode_tokens=decode_tokens))
-    return make_workload(shape, specs, seed, device)
+    return make_workload(shape, specs, seed, device, with_values=with_values)
 
 
 def residual_weights(D: int, seed: int, zero_init: bool = False) -> dict:

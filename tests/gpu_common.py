@@ -13,11 +13,16 @@ def oracle_geom(o, w):
                       o.BF16 if w.shape.kv_dtype == "bf16" else o.F32, w.dead_slot)
 
 
-def make_ctx(w, max_sessions=16):
+LAYER_MAJOR = 2   # ikv_tune(IKV_TUNE_LAYER_MAJOR): the small parity shapes take the layer-major key pass whenever it fits
+                  # (the library's default, 1, keeps it for calls with at least three tiles per SM)
+
+
+def make_ctx(w, max_sessions=16, layer_major=None):
     from paper_2606_09916_b200 import ikv
     assert w.k_pool.is_cuda
     ctx = ikv.Context(w.shape.L, w.shape.Hq, w.shape.Hkv, w.shape.D, w.k_pool, w.v_pool, dead_slot=w.dead_slot,
                       lam=0.5, max_sessions=max_sessions)
+    ctx.tune(ikv.TUNE_LAYER_MAJOR, LAYER_MAJOR if layer_major is None else layer_major)
     return ctx
 
 

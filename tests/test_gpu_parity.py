@@ -717,3 +717,29 @@ def test_scores_are_bit_identical_from_run_to_run(ikv, oracle):
             again = torch.empty(s.N, device="cuda")
             ctx.score([req], mode, again)
             assert torch.equal(ref.view(torch.int32), again.view(torch.int32))
+
+
+@pytest.mark.parametrize("lm", [0, 1], ids=["logits_scratch", "auto"])
+@pytest.mark.parametrize("name,shape", [SHAPES[1], SHAPES[2], SHAPES[5]], ids=["d128g4", "d64g2", "d128g8"])
+def test_key_pass_variants_match_oracle(ikv, oracle, name, shape, lm):
+    """The parity tests above run the layer-major key pass wherever it fits (gpu_common.LAYER_MAJOR = 2).  Here the same
+    scores come from the logits-scratch key pass (0) and from the library's default choice (1), in both scorer modes."""
+    w = build(name, shape)
+    kp, vp = gc.to_cuda(w)
+    ctx = gc.make_ctx(w, layer_major=lm)
+    s = w.sessions[0]
+    gc.fold_memory_gpu(ctx, s)
+    M = gc.fold_memory_oracle(oracle, s)
+    wts = wl.residual_weights(w.shape.D, 31)
+    ctx.residual_load(wts)
+    S = s.slot_map[:s.N].clone()
+    S[s.pi + 3: s.pi + 90: 4] = w.dead_slot
+    S_dev = S.cuda()
+    req = gc.request(ikv, s, S_dev)
+    g = gc.oracle_geom(oracle, w)
+    for mode, omode in ((ikv.MODE_MEMORY, oracle.MODE_MEMORY), (ikv.MODE_LEARNABLE, oracle.MODE_LEARNABLE)):
+        scores = torch.empty(s.N, device="cuda")
+        ctx.score([req], mode, scores)
+        want = oracle.score(g, kp, M, S.numpy(), s.pi, s.qs, s.qe, omode, 0, w=oracle.ResidualWeights(**wts))
+        mabs, mrel = gc.assert_scores_close(scores.cpu().numpy(), want, f"{name} lm={lm} mode={mode}")
+        print(f"[{name} lm={lm} mode={mode}] max abs err {mabs:.3e} rel {mrel:.3e}")
