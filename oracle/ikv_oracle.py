@@ -19,6 +19,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "ikv_oracle.c")
+_SRC_NEXT = os.path.join(_HERE, "ikv_oracle_next.c")      # SURVEY 8(f) follow-ups (N1-N3)
 _LIB = os.path.join(_HERE, "libikv_oracle.so")
 
 F32, BF16 = 0, 1
@@ -29,9 +30,10 @@ MODE_MEMORY, MODE_LEARNABLE = 0, 1
 
 def build(force: bool = False) -> str:
     """Compile the C oracle with gcc (plain C11 + OpenMP). Returns the .so path."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(_SRC),
+                                                                         os.path.getmtime(_SRC_NEXT)):
         cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra",
-               "-o", _LIB, _SRC, "-lm"]
+               "-o", _LIB, _SRC, _SRC_NEXT, "-lm"]
         subprocess.run(cmd, check=True, cwd=_HERE)
     return _LIB
 
@@ -243,3 +245,53 @@ def prune_event(g: Geometry, k_pool, M, S, pi, qs, qe, C_budget, radix_len, mode
     keep, n_kept = select(sc, cls, C_budget)
     S2, valid, freed = rewrite(S, g.dead_slot, keep, radix_len, g.n_slots)
     return dict(scores=sc, keep=keep, n_kept=n_kept, slot_map=S2, valid=valid, freed=freed)
+
+
+# ---------------------------------------------------------------------------------------------
+# SURVEY 8(f) follow-ups (ikv_oracle_next.c)
+# ---------------------------------------------------------------------------------------------
+def multirow_score(g: Geometry, k_pool, rows, weights, S, cls):
+    """N1: rows [R][L][Hq][D], weights [R] -> scores [N] (0 outside the candidates)."""
+    rows = _c(rows, np.float64)
+    w = _c(weights, np.float64)
+    S = _c(S, np.int32)
+    cls = _c(cls, np.uint8)
+    out = np.zeros(S.shape[0], np.float64)
+    lib().oracle_multirow_score(_p(_pool(g, k_pool)), g.kv_dtype, C.c_int64(g.n_slots), g.L, g.Hq, g.Hkv, g.D,
+                                _p(rows), rows.shape[0], _p(w), _p(S), _p(cls), S.shape[0], _p(out))
+    return out
+
+
+def maxpool_candidates(s, cls, kernel):
+    s = _c(s, np.float64)
+    cls = _c(cls, np.uint8)
+    out = np.zeros_like(s)
+    lib().oracle_maxpool_candidates(_p(s), _p(cls), s.shape[0], int(kernel), _p(out))
+    return out
+
+
+def streaming_scores(cls, n_sink):
+    cls = _c(cls, np.uint8)
+    out = np.zeros(cls.shape[0], np.float64)
+    lib().oracle_streaming_scores(_p(cls), cls.shape[0], int(n_sink), _p(out))
+    return out
+
+
+def h2o_scores(hh, cls, C_budget, ratio, floor_):
+    hh = _c(hh, np.float64)
+    cls = _c(cls, np.uint8)
+    out = np.zeros_like(hh)
+    lib().oracle_h2o_scores(_p(hh), _p(cls), hh.shape[0], int(C_budget), C.c_double(ratio), int(floor_), _p(out))
+    return out
+
+
+def prefill(g: Geometry, k_pool, v_pool, layer, S, q_pos0, q, sm_scale):
+    """N2: q [n_q][Hq][D] fp32 -> (out [n_q][Hq][D] float64, raw_reads, eff_reads)."""
+    q = _c(q, np.float32)
+    S = _c(S, np.int32)
+    out = np.zeros(q.shape, np.float64)
+    reads = np.zeros(2, np.int64)
+    lib().oracle_prefill(_p(_pool(g, k_pool)), _p(_pool(g, v_pool)), g.kv_dtype, C.c_int64(g.n_slots), g.Hq, g.Hkv,
+                         g.D, int(layer), _p(S), int(g.dead_slot), int(q_pos0), q.shape[0], _p(q),
+                         C.c_double(sm_scale), _p(out), _p(reads))
+    return out, int(reads[0]), int(reads[1])
