@@ -173,6 +173,47 @@ ikv_status ikv_select_evict(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req
 ikv_status ikv_decode_attn(ikv_ctx *ctx, int32_t layer, const ikv_request *reqs, int32_t n_req, const void *q,
                            void *out, float sm_scale, void *stream);
 
+/* ---- follow-ups of the hot path ------------------------------------------------------------ */
+/* Multi-row scorer ("window of W tail Q rows", O(W L H_q N); :159 W = 32; :310; R28): n_rows
+ * un-collapsed rows per (layer, query head), rows[r][L][H_q][D] DEVICE fp32, used as given; every row is its own softmax
+ * over the candidates of Eq. 3 and the rows are combined with the HOST weights[n_rows]:
+ *   s_j = sum_r weights[r] sum_{l,h} softmax_{i in A}(rows[r,l,h] . K[l, h div G, S[i]] / sqrt(D))_j.
+ * n_rows = 1, weights = {1}, rows = M_t is ikv_score(IKV_MODE_MEMORY) bit for bit.  scores as in ikv_score (fillers
+ * included).  One pass over the keys per row. */
+ikv_status ikv_score_rows(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req, const float *rows, int32_t n_rows,
+                          const float *weights, float *scores, void *stream);
+
+/* Baseline scorers on the same dead-slot substrate (R29-R31).  They only
+ * produce `scores` (same layout and fillers as ikv_score); budget, forced set, slot-map redirection and the prefix-safe
+ * free are ikv_select_evict's, shared by every scorer.
+ *   IKV_BASE_STREAMING  StreamingLLM: candidates at positions < n_sink first, then the most recent ones (no key is read)
+ *   IKV_BASE_SNAPKV     SnapKV: the multi-row scorer over the W observation rows `rows` (weights 1), then max-pool
+ *                       smoothing of width pool_kernel (7) over the logical positions, candidates only
+ *   IKV_BASE_H2O        H2O: heavy-hitter mass = the multi-row scorer over the bank `rows` (weights 1); the
+ *                       min(C*, max(recent_floor, round(recent_ratio C*))) most recent candidates are kept first */
+#define IKV_BASE_STREAMING 1
+#define IKV_BASE_SNAPKV 2
+#define IKV_BASE_H2O 3
+typedef struct {
+  int32_t kind;          /* IKV_BASE_*                                            */
+  const float *rows;     /* DEVICE [n_rows][L][H_q][D] fp32 (SNAPKV, H2O)         */
+  int32_t n_rows;
+  int32_t n_sink;        /* STREAMING: 4                           */
+  int32_t pool_kernel;   /* SNAPKV: 7, odd                         */
+  float recent_ratio;    /* H2O                                                   */
+  int32_t recent_floor;  /* H2O                                                   */
+} ikv_baseline;
+ikv_status ikv_score_baseline(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req, const ikv_baseline *b, float *scores,
+                              void *stream);
+
+/* Prefill / chunked-prefill attention of one layer through the slot map (R32): n_q query
+ * rows at logical positions q_pos0 .. q_pos0 + n_q - 1 of the request (q_pos0 + n_q <= req->seq_len); row i attends,
+ * causally, every position j <= q_pos0 + i with S[j] != s+.  q, out: DEVICE [n_q][H_q][D], pool dtype.
+ * kv_reads: optional DEVICE int64[2], ACCUMULATED: [0] += sum_i (q_pos0 + i + 1) = Raw KV Reads sum |R_t|,
+ * [1] += sum_i #{j <= q_pos0 + i : S[j] != s+} = Eff. KV Reads sum |K_t|. */
+ikv_status ikv_prefill_attn(ikv_ctx *ctx, int32_t layer, const ikv_request *req, int32_t q_pos0, int32_t n_q, const void *q,
+                            void *out, float sm_scale, int64_t *kv_reads, void *stream);
+
 /* The whole pruning pass of one request with HOST buffers (used for end-to-end timing): copies
  * q_rows_host ([n_rows][L][H_q][D], q_dtype IKV_F32 or IKV_BF16; may be NULL/0 to skip the memory update) and
  * slot_map_host[seq_len] to the device, runs ikv_memory_update -> ikv_score(mode) -> ikv_select_evict, brings the new

@@ -217,6 +217,95 @@ __global__ void k_late_writer(uint4* dst, const uint4* src, int64_t n16, int64_t
     dst[i] = src[i];
 }
 
+// scores[pos_c] = (first ? 0 : scores[pos_c]) + w * rule_c[c]   (multi-row scorer: weighted sum over the rows)
+__global__ void k_axpy_scatter(const float* __restrict__ rule_c, const int32_t* __restrict__ cand_pos,
+                               const int32_t* __restrict__ n_cand, float w, int first, float* __restrict__ scores) {
+  pdl_wait();
+  pdl_launch_dependents();
+  const int nc = *n_cand;
+  for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
+    const int pos = cand_pos[c];
+    scores[pos] = (first ? 0.f : scores[pos]) + w * rule_c[c];
+  }
+}
+// StreamingLLM (sink + recent window; R30): position scores of the candidates
+__global__ void k_streaming_scores(const int32_t* __restrict__ cand_pos, const int32_t* __restrict__ n_cand, int n_sink,
+                                   float* __restrict__ scores) {
+  const int nc = *n_cand;
+  for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
+    const int pos = cand_pos[c];
+    scores[pos] = pos < n_sink ? 1073741824.f : (float)pos;
+  }
+}
+// SnapKV max-pool smoothing over the logical positions, candidates only ("kernel 7 ... max-pool"; R29).
+// scores holds finite values exactly at the candidates (+-INF fillers elsewhere, R6).  Two launches: pooled -> tmp -> back.
+__global__ void k_maxpool_cand(const float* __restrict__ scores, const int32_t* __restrict__ cand_pos,
+                               const int32_t* __restrict__ n_cand, int N, int half, float* __restrict__ tmp) {
+  const int nc = *n_cand;
+  for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
+    const int pos = cand_pos[c];
+    float m = scores[pos];
+    for (int i = max(0, pos - half); i <= min(N - 1, pos + half); ++i) {
+      const float v = scores[i];
+      if (isfinite(v) && v > m) m = v;
+    }
+    tmp[c] = m;
+  }
+}
+// H2O "ratio mode with a recent-window floor" (R31): the n_recent most recent candidates are kept
+// first (score 1e30 + position).  One block: |F| is counted from the +INF fillers.
+__global__ __launch_bounds__(1024) void k_h2o_boost(const int32_t* __restrict__ cand_pos, const int32_t* __restrict__ n_cand,
+                                                    int N, int C, float ratio, int floor_, float* __restrict__ scores) {
+  __shared__ int warp_tot[32];
+  int nf = 0;
+  for (int j = threadIdx.x; j < N; j += 1024) nf += (scores[j] == CUDART_INF_F) ? 1 : 0;
+  int tot;
+  block_excl_scan_1024(nf, warp_tot, &tot);
+  const int cstar = max(0, C - tot);
+  int n_recent = (int)floorf(ratio * (float)cstar + 0.5f);
+  n_recent = min(cstar, max(floor_, n_recent));
+  const int nc = *n_cand;
+  __syncthreads();
+  for (int c = max(0, nc - n_recent) + threadIdx.x; c < nc; c += 1024) {
+    const int pos = cand_pos[c];
+    scores[pos] = 1.0e30f + (float)pos;
+  }
+}
+// KV-read counters of a prefill chunk: raw += sum (pos_i + 1), eff += sum #live positions <= pos_i.
+__global__ __launch_bounds__(1024) void k_prefill_reads(const int32_t* __restrict__ S, int32_t dead, int q_pos0, int n_q,
+                                                        unsigned long long* __restrict__ reads) {
+  __shared__ int warp_tot[32];
+  // live positions in [0, q_pos0) are common to every row; then an inclusive count along the chunk
+  int base = 0;
+  for (int j0 = 0; j0 < q_pos0; j0 += 1024) {
+    const int j = j0 + threadIdx.x;
+    int tot;
+    block_excl_scan_1024((j < q_pos0 && S[j] != dead) ? 1 : 0, warp_tot, &tot);
+    base += tot;
+  }
+  unsigned long long eff = 0;
+  int run = base;
+  for (int i0 = 0; i0 < n_q; i0 += 1024) {
+    const int i = i0 + threadIdx.x, j = q_pos0 + i;
+    const int lv = (i < n_q && S[j] != dead) ? 1 : 0;
+    int tot;
+    const int ex = block_excl_scan_1024(lv, warp_tot, &tot);
+    if (i < n_q) eff += (unsigned long long)(run + ex + lv);
+    run += tot;
+  }
+  // block sum of eff
+  __shared__ unsigned long long acc;
+  if (threadIdx.x == 0) acc = 0;
+  __syncthreads();
+  atomicAdd(&acc, eff);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    atomicAdd(&reads[0], (unsigned long long)n_q * (unsigned long long)(q_pos0 + 1) +
+                             (unsigned long long)n_q * (unsigned long long)(n_q - 1) / 2);
+    atomicAdd(&reads[1], acc);
+  }
+}
+
 __global__ void k_fill_i32(int32_t* p, int64_t n, int32_t v) {
   for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
     p[i] = v;
@@ -576,7 +665,10 @@ ikv_status dispatch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool xq, int
                                 : dispatch_key_pass_g<64>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
 }
 
-ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, float* rule_out, cudaStream_t st) {
+// M_ovr: score against these rows [L][Hq][D] instead of the session's memory (multi-row scorer); part: run the partition
+// (a1) first; scatter: write the rule score into `scores` (otherwise it stays in the compact rule_c[] scratch).
+ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, float* rule_out, cudaStream_t st,
+                     const float* M_ovr = nullptr, bool part = true, bool scatter = true) {
   const int N = r.seq_len;
   if (N == 0) return IKV_OK;
   const int base_mode = mode & 0xff;
@@ -587,7 +679,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   if (base_mode == IKV_MODE_LEARNABLE && !c->has_resid)
     IKV_FAIL(c, IKV_ERR_INVALID_ARG, "IKV_MODE_LEARNABLE needs ikv_residual_load first");
   TRY(ensure_scratch(c, N));
-  const float* M = (base_mode == IKV_MODE_QUERY) ? s->d_qenc : s->d_mem;
+  const float* M = M_ovr ? M_ovr : ((base_mode == IKV_MODE_QUERY) ? s->d_qenc : s->d_mem);
 
   const bool fast = c->cfg.kv_dtype == IKV_BF16;  // tensor-pipe key pass; fp32 pools take the plain FMA kernel
   const bool use_x = learn && !(mode & IKV_FLAG_NO_XATTN);
@@ -596,7 +688,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   // at most RT_NXMAX query positions: folded cross attention, the whole head on tcgen05 (residual_tc.cuh)
   const bool tc = learn && c->resid_tc && n_x <= RT_NXMAX;
   const int nxp = tc ? (n_x > 0 ? (n_x + 15) / 16 * 16 : 16) : 0;
-  {
+  if (part) {
     // a1 (+ the compaction of the live cross-attention positions as a second cluster of the same launch)
     const int grid = CL_CTAS * (n_x > 0 ? 2 : 1);
     ProfScope prof(c, IKV_PROF_PARTITION, st);
@@ -623,7 +715,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   int n_part = (N + SCORE_TILE - 1) / SCORE_TILE;
   bool lm_done = false;  // the layer-major key pass has already produced rule_c (and the scores of a rule-only call)
   if (fast) {
-    LmOut lo{scores, rule_out, learn ? 0 : 1};
+    LmOut lo{scores, rule_out, (learn || !scatter) ? 0 : 1};
     TRY(dispatch_key_pass(c, M, learn, n_x > 0, n_mpart, &n_part, N, n_x, lo, &lm_done, st));
   } else {
     if (n_mpart > 0) {
@@ -697,7 +789,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     pk.n_kv = (learn && n_x > 0) ? 4 * ((n_x + 15) / 16) : 0;
     RuleParams rp;
     rp.logits = c->logits; rp.ldc = c->cap_tokens; rp.LH = LH; rp.lse = c->lse; rp.n_cand = c->d_ncand;
-    rp.cand_pos = c->cand_pos; rp.rule_c = c->rule_c; rp.scores = scores; rp.scatter_scores = learn ? 0 : 1;
+    rp.cand_pos = c->cand_pos; rp.rule_c = c->rule_c; rp.scores = scores; rp.scatter_scores = (learn || !scatter) ? 0 : 1;
     rp.rule_out = rule_out; rp.n_rule = lm_done ? 0 : (N + 63) / 64; rp.l2_hints = c->dbg_l2;
     const int grid = rp.n_rule + pk.n_fold + pk.n_kv;
     ProfScope prof(c, IKV_PROF_RULE, st);
@@ -1135,6 +1227,112 @@ ikv_status ikv_score(ikv_ctx* c, const ikv_request* reqs, int32_t n_req, int32_t
   for (int r = 0; r < n_req; ++r) {
     TRY(score_one(c, reqs[r], mode, scores + off, rule_out ? rule_out + off : nullptr, (cudaStream_t)stream));
     off += reqs[r].seq_len;
+  }
+  return IKV_OK;
+}
+
+ikv_status ikv_score_rows(ikv_ctx* c, const ikv_request* reqs, int32_t n_req, const float* rows, int32_t n_rows,
+                          const float* weights, float* scores, void* stream) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (n_req < 0 || n_rows <= 0 || !rows || !weights || (n_req > 0 && (!reqs || !scores)))
+    IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_score_rows: bad argument");
+  for (int r = 0; r < n_req; ++r) TRY(check_request(c, reqs[r]));
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t row_elems = (int64_t)c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim;
+  int64_t off = 0;
+  for (int r = 0; r < n_req; ++r) {
+    for (int k = 0; k < n_rows; ++k) {
+      // one pass of the Eq. 3 scorer per row (row k in place of M_t), rule_c left in scratch, then the weighted sum
+      TRY(score_one(c, reqs[r], IKV_MODE_MEMORY, scores + off, nullptr, st, rows + k * row_elems, k == 0, false));
+      if (reqs[r].seq_len > 0)
+        CU(c, launch_pdl(k_axpy_scatter, dim3(64), dim3(256), 0, st, c->pdl_prune, (const float*)c->rule_c,
+                         (const int32_t*)c->cand_pos, (const int32_t*)c->d_ncand, weights[k], k == 0 ? 1 : 0, scores + off));
+    }
+    off += reqs[r].seq_len;
+  }
+  return IKV_OK;
+}
+
+ikv_status ikv_score_baseline(ikv_ctx* c, const ikv_request* reqs, int32_t n_req, const ikv_baseline* b, float* scores,
+                              void* stream) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (!b || n_req < 0 || (n_req > 0 && (!reqs || !scores))) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_score_baseline: NULL argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (b->kind == IKV_BASE_STREAMING) {
+    if (b->n_sink < 0) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "n_sink < 0");
+    int64_t off = 0;
+    for (int r = 0; r < n_req; ++r) {
+      TRY(check_request(c, reqs[r]));
+      const ikv_request& q = reqs[r];
+      const int N = q.seq_len;
+      if (N > 0) {
+        TRY(ensure_scratch(c, N));
+        // a1 partition: fillers and the candidate list (no keys are read by this scorer)
+        if (N <= CL_MAX_N) {
+          auto fn = N <= CL_CTAS * 1024 * 4 ? k_partition_cl<4> : N <= CL_CTAS * 1024 * 8 ? k_partition_cl<8> : k_partition_cl<16>;
+          CU(c, launch_pdl(fn, dim3(CL_CTAS), dim3(1024), 0, st, false, (const int32_t*)q.slot_map, N, c->cfg.dead_slot,
+                           q.prefix_len, q.q_start, q.q_end, scores + off, (float*)nullptr, c->cand_pos, c->cand_slot,
+                           c->d_ncand, (const int32_t*)nullptr, 0, (int32_t*)nullptr, (int32_t*)nullptr));
+        } else {
+          k_partition<<<1, 1024, 0, st>>>(q.slot_map, N, c->cfg.dead_slot, q.prefix_len, q.q_start, q.q_end, scores + off,
+                                          nullptr, c->cand_pos, c->cand_slot, c->d_ncand);
+        }
+        k_streaming_scores<<<64, 256, 0, st>>>(c->cand_pos, c->d_ncand, b->n_sink, scores + off);
+        LAUNCH_CHECK(c);
+      }
+      off += N;
+    }
+    return IKV_OK;
+  }
+  if (b->kind != IKV_BASE_SNAPKV && b->kind != IKV_BASE_H2O) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "unknown baseline %d", b->kind);
+  if (!b->rows || b->n_rows <= 0) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "baseline needs query rows");
+  if (b->kind == IKV_BASE_SNAPKV && (b->pool_kernel < 1 || !(b->pool_kernel & 1)))
+    IKV_FAIL(c, IKV_ERR_INVALID_ARG, "pool_kernel must be odd");
+  std::vector<float> ones((size_t)b->n_rows, 1.0f);
+  int64_t off = 0;
+  for (int r = 0; r < n_req; ++r) {
+    // observation-window / heavy-hitter mass: the multi-row scorer over the given rows, weights 1
+    TRY(ikv_score_rows(c, reqs + r, 1, b->rows, b->n_rows, ones.data(), scores + off, stream));
+    const int N = reqs[r].seq_len;
+    if (N > 0) {
+      if (b->kind == IKV_BASE_SNAPKV) {
+        k_maxpool_cand<<<64, 256, 0, st>>>(scores + off, c->cand_pos, c->d_ncand, N, (b->pool_kernel - 1) / 2, c->rule_c);
+        k_axpy_scatter<<<64, 256, 0, st>>>(c->rule_c, c->cand_pos, c->d_ncand, 1.0f, 1, scores + off);
+      } else {
+        k_h2o_boost<<<1, 1024, 0, st>>>(c->cand_pos, c->d_ncand, N, reqs[r].budget, b->recent_ratio, b->recent_floor,
+                                        scores + off);
+      }
+      LAUNCH_CHECK(c);
+    }
+    off += N;
+  }
+  return IKV_OK;
+}
+
+ikv_status ikv_prefill_attn(ikv_ctx* c, int32_t layer, const ikv_request* req, int32_t q_pos0, int32_t n_q, const void* q,
+                            void* out, float sm_scale, int64_t* kv_reads, void* stream) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (!req || !q || !out || n_q < 0 || q_pos0 < 0) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_prefill_attn: bad argument");
+  if ((int64_t)q_pos0 + n_q > req->seq_len) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "the chunk ends beyond seq_len");
+  if (n_q == 0) return IKV_OK;
+  const size_t esz = c->cfg.kv_dtype == IKV_BF16 ? 2 : 4;
+  const size_t row = (size_t)c->cfg.n_q_heads * c->cfg.head_dim * esz;
+  // Row i is a decode query at position q_pos0 + i: causal = its request ends at seq_len_i = q_pos0 + i + 1.  The rows of
+  // a launch share the session's survivor list and read the chunk's own positions from the slot map; the K/V rows of the
+  // request are re-read by every row out of L2 (33.5 MB per layer at 8,192 survivors).
+  ikv_request rr[DEC_MAX_REQ];
+  for (int i0 = 0; i0 < n_q; i0 += DEC_MAX_REQ) {
+    const int nb = (n_q - i0 < DEC_MAX_REQ) ? n_q - i0 : DEC_MAX_REQ;
+    for (int i = 0; i < nb; ++i) {
+      rr[i] = *req;
+      rr[i].seq_len = q_pos0 + i0 + i + 1;
+    }
+    TRY(ikv_decode_attn(c, layer, rr, nb, (const char*)q + (size_t)i0 * row, (char*)out + (size_t)i0 * row, sm_scale, stream));
+  }
+  if (kv_reads) {
+    k_prefill_reads<<<1, 1024, 0, (cudaStream_t)stream>>>(req->slot_map, c->cfg.dead_slot, q_pos0, n_q,
+                                                          reinterpret_cast<unsigned long long*>(kv_reads));
+    LAUNCH_CHECK(c);
   }
   return IKV_OK;
 }

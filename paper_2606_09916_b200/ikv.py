@@ -32,7 +32,8 @@ PROF_NAMES = ["key_pass", "decode_split", "memory_update", "partition", "mem_pre
 
 EXPORTS = ["ikv_create", "ikv_destroy", "ikv_last_error", "ikv_reserve", "ikv_session_open", "ikv_session_fork",
            "ikv_session_close", "ikv_session_get_memory", "ikv_session_set_memory", "ikv_residual_load",
-           "ikv_memory_update", "ikv_score", "ikv_select_evict", "ikv_decode_attn", "ikv_prune_host", "ikv_profile_enable", "ikv_profile_read", "ikv_tune", "ikv_test_late_writer", "ikv_version"]
+           "ikv_memory_update", "ikv_score", "ikv_select_evict", "ikv_decode_attn", "ikv_prune_host",
+           "ikv_score_rows", "ikv_score_baseline", "ikv_prefill_attn", "ikv_profile_enable", "ikv_profile_read", "ikv_tune", "ikv_test_late_writer", "ikv_version"]
 
 
 class Config(C.Structure):
@@ -81,6 +82,19 @@ _lib.ikv_profile_enable.argtypes = [C.c_void_p, C.c_int32]
 _lib.ikv_profile_read.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.ikv_prune_host.argtypes = [C.c_void_p, C.POINTER(Request), C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p,
                                 C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+
+
+class Baseline(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("rows", C.c_void_p), ("n_rows", C.c_int32), ("n_sink", C.c_int32),
+                ("pool_kernel", C.c_int32), ("recent_ratio", C.c_float), ("recent_floor", C.c_int32)]
+
+
+BASE_STREAMING, BASE_SNAPKV, BASE_H2O = 1, 2, 3
+_lib.ikv_score_rows.argtypes = [C.c_void_p, C.POINTER(Request), C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p,
+                                C.c_void_p]
+_lib.ikv_score_baseline.argtypes = [C.c_void_p, C.POINTER(Request), C.c_int32, C.POINTER(Baseline), C.c_void_p, C.c_void_p]
+_lib.ikv_prefill_attn.argtypes = [C.c_void_p, C.c_int32, C.POINTER(Request), C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
+                                  C.c_float, C.c_void_p, C.c_void_p]
 
 
 class IkvError(RuntimeError):
@@ -212,6 +226,23 @@ class Context:
 
     def tune(self, knob: int, value: int):
         self._chk(_lib.ikv_tune(self._h, knob, value))
+
+    def score_rows(self, reqs, rows, weights, scores, stream=None):
+        assert rows.is_cuda and rows.is_contiguous() and rows.dtype == torch.float32
+        w = (C.c_float * len(weights))(*[float(x) for x in weights])
+        assert rows.shape[0] == len(weights)
+        self._chk(_lib.ikv_score_rows(self._h, _req_array(reqs), len(reqs), _ptr(rows), rows.shape[0], w, _ptr(scores),
+                                      _stream(stream)))
+
+    def score_baseline(self, reqs, kind, scores, rows=None, n_sink=4, pool_kernel=7, recent_ratio=0.5, recent_floor=0,
+                       stream=None):
+        b = Baseline(kind, _ptr(rows).value if rows is not None else None, 0 if rows is None else rows.shape[0], n_sink,
+                     pool_kernel, recent_ratio, recent_floor)
+        self._chk(_lib.ikv_score_baseline(self._h, _req_array(reqs), len(reqs), C.byref(b), _ptr(scores), _stream(stream)))
+
+    def prefill_attn(self, layer, req, q_pos0, q, out, sm_scale, kv_reads=None, stream=None):
+        self._chk(_lib.ikv_prefill_attn(self._h, layer, C.byref(req), q_pos0, q.shape[0], _ptr(q), _ptr(out),
+                                        C.c_float(sm_scale), _ptr(kv_reads), _stream(stream)))
 
     def profile_enable(self, level):
         """0/False off, 1/True the two dominant kernels, 2 every kernel (diagnostic)."""

@@ -1,0 +1,164 @@
+"""-m gpu parity of the SURVEY 8(f) follow-ups against oracle/ikv_oracle_next.c: multi-row scorer (NEXT-1), prefill
+attention through the slot map with KV-read counters (NEXT-2), baseline scorers on the dead-slot substrate (NEXT-3)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_09916_b200 import workloads as wl
+from tests import gpu_common as gc
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ikv():
+    from paper_2606_09916_b200 import ikv as m
+    return m
+
+
+def _setup(oracle, shape, n_tokens=1500, budget=400, seed=61):
+    w = wl.small(seed=seed, shape=shape, n_tokens=n_tokens, budget=budget, kv_dtype=shape.kv_dtype)
+    kp, vp = gc.to_cuda(w)
+    ctx = gc.make_ctx(w)
+    s = w.sessions[0]
+    gc.fold_memory_gpu(ctx, s)
+    M = gc.fold_memory_oracle(oracle, s)
+    S = s.slot_map[:s.N].clone()
+    rng = np.random.default_rng(seed)
+    S[torch.from_numpy(rng.choice(s.N, size=s.N // 9, replace=False))] = w.dead_slot
+    return w, kp, vp, ctx, s, M, S
+
+
+SHAPES = [("d128g4", wl.ModelShape(3, 8, 2, 128, "bf16")), ("d64g2", wl.ModelShape(2, 4, 2, 64, "bf16")),
+          ("d128g5", wl.ModelShape(2, 10, 2, 128, "bf16"))]
+
+
+@pytest.mark.parametrize("name,shape", SHAPES, ids=[n for n, _ in SHAPES])
+@pytest.mark.parametrize("R", [1, 4, 32])
+def test_multirow_scorer_matches_oracle(ikv, oracle, name, shape, R):
+    w, kp, vp, ctx, s, M, S = _setup(oracle, shape)
+    S_dev = S.cuda()
+    req = gc.request(ikv, s, S_dev)
+    g = gc.oracle_geom(oracle, w)
+    rows = torch.randn((R, shape.L, shape.Hq, shape.D), generator=torch.Generator().manual_seed(R))
+    wt = (0.25 + torch.rand(R, generator=torch.Generator().manual_seed(R + 1))).tolist()
+    scores = torch.full((s.N,), 3.0, device="cuda")
+    ctx.score_rows([req], rows.cuda().contiguous(), wt, scores)
+    cls, _ = oracle.partition(S.numpy(), w.dead_slot, s.pi, s.qs, s.qe)
+    want = oracle.multirow_score(g, kp, rows.double().numpy(), wt, S.numpy(), cls)
+    want = np.where(cls == oracle.FORCED, np.inf, np.where(cls == oracle.DEAD, -np.inf, want))
+    mabs, mrel = gc.assert_scores_close(scores.cpu().numpy(), want, f"{name} R={R}")
+    print(f"[{name} R={R}] multi-row score max abs err {mabs:.3e} rel {mrel:.3e}")
+
+
+def test_multirow_single_row_is_the_memory_scorer_bit_for_bit(ikv, oracle):
+    """R = 1 with the session's QueryMemory as the row reproduces ikv_score(IKV_MODE_MEMORY) exactly (Eq. 3)."""
+    w, kp, vp, ctx, s, M, S = _setup(oracle, SHAPES[0][1])
+    S_dev = S.cuda()
+    req = gc.request(ikv, s, S_dev)
+    base = torch.empty(s.N, device="cuda")
+    ctx.score([req], ikv.MODE_MEMORY, base)
+    rows = ctx.session_get_memory(s.spec.session_id)[None].cuda().contiguous()
+    got = torch.empty(s.N, device="cuda")
+    ctx.score_rows([req], rows, [1.0], got)
+    assert torch.equal(base.view(torch.int32), got.view(torch.int32))
+
+
+def _select_matches(ikv, oracle, ctx, w, s, S, got_scores, budget):
+    """select / evict on the GPU's baseline scores is bit-exact with the oracle's selection on the same scores."""
+    S_dev = S.cuda()
+    req = gc.request(ikv, s, S_dev, budget=budget)
+    freed = torch.empty(s.N, dtype=torch.int32, device="cuda")
+    nf = torch.zeros(1, dtype=torch.int32, device="cuda")
+    nk = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ctx.select_evict([req], got_scores, freed, nf, nk)
+    cls, _ = oracle.partition(S.numpy(), w.dead_slot, s.pi, s.qs, s.qe)
+    keep, n_kept = oracle.select(got_scores.cpu().numpy(), cls, budget)
+    S2, _, freed_o = oracle.rewrite(S.numpy(), w.dead_slot, keep, s.pi, w.n_slots)
+    assert nk.item() == n_kept and np.array_equal(S_dev.cpu().numpy(), S2)
+    assert np.array_equal(freed.cpu().numpy()[:nf.item()], freed_o)
+    return keep.astype(bool)
+
+
+def test_streaming_baseline(ikv, oracle):
+    w, kp, vp, ctx, s, M, S = _setup(oracle, SHAPES[1][1], n_tokens=2100, budget=500)
+    S[:3] = s.slot_map[:3]                              # positions 0..2 live; they sit in the protected prefix anyway
+    sn = S.numpy()
+    S_dev = S.cuda()
+    # no protected prefix, so that the sink rule is what keeps the first four positions
+    req = ikv.make_request(s.spec.session_id, S_dev, s.N, 0, s.qs, s.qe, 500, 0)
+    scores = torch.empty(s.N, device="cuda")
+    ctx.score_baseline([req], ikv.BASE_STREAMING, scores, n_sink=4)
+    cls, _ = oracle.partition(sn, w.dead_slot, 0, s.qs, s.qe)
+    want = oracle.streaming_scores(cls, 4)
+    want = np.where(cls == oracle.FORCED, np.inf, np.where(cls == oracle.DEAD, -np.inf, want)).astype(np.float32)
+    assert np.array_equal(scores.cpu().numpy(), want)                       # integer-valued: exact
+
+
+@pytest.mark.parametrize("kind", ["snapkv", "h2o"])
+def test_snapkv_and_h2o_baselines(ikv, oracle, kind):
+    shape = SHAPES[0][1]
+    w, kp, vp, ctx, s, M, S = _setup(oracle, shape, n_tokens=1800, budget=450)
+    S_dev = S.cuda()
+    req = gc.request(ikv, s, S_dev, budget=450)
+    g = gc.oracle_geom(oracle, w)
+    W = 32 if kind == "snapkv" else 12
+    rows = torch.randn((W, shape.L, shape.Hq, shape.D), generator=torch.Generator().manual_seed(12))
+    scores = torch.empty(s.N, device="cuda")
+    cls, _ = oracle.partition(S.numpy(), w.dead_slot, s.pi, s.qs, s.qe)
+    mass = oracle.multirow_score(g, kp, rows.double().numpy(), np.ones(W), S.numpy(), cls)
+    if kind == "snapkv":
+        ctx.score_baseline([req], ikv.BASE_SNAPKV, scores, rows=rows.cuda().contiguous(), pool_kernel=7)
+        want = oracle.maxpool_candidates(mass, cls, 7)
+    else:
+        ctx.score_baseline([req], ikv.BASE_H2O, scores, rows=rows.cuda().contiguous(), recent_ratio=0.5, recent_floor=64)
+        want = oracle.h2o_scores(mass, cls, 450, 0.5, 64)
+    want = np.where(cls == oracle.FORCED, np.inf, np.where(cls == oracle.DEAD, -np.inf, want))
+    mabs, mrel = gc.assert_scores_close(scores.cpu().numpy(), want, kind)
+    print(f"[{kind}] baseline score max abs err {mabs:.3e} rel {mrel:.3e}")
+    keep = _select_matches(ikv, oracle, ctx, w, s, S, scores, 450)
+    if kind == "h2o":                                   # the recent floor is kept whatever the masses are
+        cand = np.nonzero(cls == oracle.CAND)[0]
+        n_recent = max(64, int(math.floor(0.5 * (450 - (cls == oracle.FORCED).sum()) + 0.5)))
+        assert keep[cand[-n_recent:]].all()
+
+
+@pytest.mark.parametrize("name,shape", SHAPES, ids=[n for n, _ in SHAPES])
+def test_prefill_attention_matches_oracle(ikv, oracle, name, shape):
+    """A chunk of 70 query rows right after a prune (the survivor list is cached, the chunk's positions are read from the
+    slot map), and a chunk that starts before the cached range (rescan), with dead positions inside the chunk; KV-read
+    counters accumulate over both calls."""
+    w = wl.small(seed=71, shape=shape, n_tokens=1300, budget=300, decode_tokens=80, kv_dtype="bf16")
+    kp, vp = gc.to_cuda(w)
+    ctx = gc.make_ctx(w)
+    s = w.sessions[0]
+    gc.fold_memory_gpu(ctx, s)
+    g = gc.oracle_geom(oracle, w)
+    full = s.slot_map.clone()
+    full[s.N + 5] = w.dead_slot                           # a dead position inside the chunk
+    S_dev = full.cuda()
+    scores = torch.empty(s.N, device="cuda")
+    freed = torch.empty(s.N, dtype=torch.int32, device="cuda")
+    nf = torch.zeros(1, dtype=torch.int32, device="cuda")
+    nk = torch.zeros(1, dtype=torch.int32, device="cuda")
+    req = gc.request(ikv, s, S_dev)
+    ctx.score([req], ikv.MODE_MEMORY, scores)
+    ctx.select_evict([req], scores, freed, nf, nk)
+    scale = 1.0 / math.sqrt(shape.D)
+    reads = torch.zeros(2, dtype=torch.int64, device="cuda")
+    want_raw = want_eff = 0
+    for q_pos0, n_q, layer in ((s.N, 70, 0), (s.N - 40, 50, shape.L - 1)):
+        q = torch.randn((n_q, shape.Hq, shape.D), generator=torch.Generator().manual_seed(q_pos0)).to(torch.bfloat16)
+        out = torch.empty((n_q, shape.Hq, shape.D), dtype=torch.bfloat16, device="cuda")
+        r = gc.request(ikv, s, S_dev, seq_len=q_pos0 + n_q)
+        ctx.prefill_attn(layer, r, q_pos0, q.cuda(), out, scale, reads)
+        torch.cuda.synchronize()
+        S_host = S_dev.cpu().numpy()
+        want, raw, eff = oracle.prefill(g, kp, vp, layer, S_host, q_pos0, q.float().numpy(), scale)
+        want_raw += raw
+        want_eff += eff
+        err = gc.assert_decode_close(out.float().cpu().numpy(), want, True, f"{name} prefill at {q_pos0}")
+        print(f"[{name}] prefill chunk at {q_pos0} x {n_q}: max abs err {err:.3e}")
+    assert reads.cpu().tolist() == [want_raw, want_eff]      # integer counters: exact
