@@ -76,13 +76,16 @@ def assert_scores_close(got, want, label=""):
 
 
 def assert_decode_close(got, want, is_bf16, label=""):
-    """north_star: "decode output within 2e-2 absolute in bf16".  The synthetic V has outlier channels (x8), so
-    |o| can exceed 5.12, where the final correctly-rounded bf16 store alone is already off by more than 2e-2
-    (half an ulp = 2^-9 |o|); the bound is therefore 2e-2 + 2^-8 |o| for bf16 (R25) and 1e-4 + 1e-5 |o|
-    for the fp32 (tiny) pool."""
+    """north_star: "decode output within 2e-2 absolute in bf16": asserted flat wherever |o| <= 2.56.  The synthetic V has
+    outlier channels (x8), so |o| can exceed 5.12, where the final correctly-rounded bf16 store alone is already off by
+    more than 2e-2 (half an ulp = 2^-9 |o|); beyond |o| = 2.56 the bound is 2e-2 + 2^-8 |o| (R25).  fp32 (tiny)
+    pool: 1e-4 + 1e-5 |o|.  Returns the observed max abs error."""
     got = np.asarray(got, np.float64)
     want = np.asarray(want, np.float64)
-    tol = (DECODE_ATOL + 2.0 ** -8 * np.abs(want)) if is_bf16 else (1e-4 + 1e-5 * np.abs(want))
+    if is_bf16:
+        tol = np.where(np.abs(want) <= 2.56, DECODE_ATOL, DECODE_ATOL + 2.0 ** -8 * np.abs(want))
+    else:
+        tol = 1e-4 + 1e-5 * np.abs(want)
     err = np.abs(got - want)
     worst = np.unravel_index(np.argmax(err - tol), err.shape)
     assert np.all(err <= tol), f"{label}: decode err {err[worst]:.3e} > tol {tol[worst]:.3e} at |o|={abs(want[worst]):.3f}"
