@@ -445,54 +445,72 @@ __global__ __launch_bounds__(lm_threads(KBAR), 1) void k_key_pass_lm(const KeyPa
     }
   } else if (KBAR && warp < KP_LWARPS + KP_KWARPS) {
     // ------------------------------------------------------------------ mean-key warps (Eq. 5): warp dq owns one quarter
-    // of D; the per-layer sum over the KV heads is added to the tile's accumulators in tensor memory
-    constexpr int CH = D / 32;                 // 16-byte chunks per token in a d-quarter
-    constexpr int TPL = 32 / CH;               // tokens per warp load
-    constexpr int NG = KP_TOK / TPL;           // token groups per warp
-    static_assert(NG * 8 <= 32, "mean-key accumulators: at most 32 columns per tile");
+    // of D.  The sum over the KV heads is a contraction with an identity matrix: the key tile is loaded as the A operand
+    // of mma.sync.m16n8k16 exactly like the logit warps load it (rows r, r+8; lane q takes the 16-byte chunk q of the
+    // quarter) and multiplied by B = [I8 | 0] and [0 | I8], accumulating over the heads in the fp32 accumulators --
+    // products with 1.0 are exact, and one HMMA replaces 16 unpack + 16 add instructions.  The tile's accumulators live
+    // in tensor memory between the layers.
+    // Thread (r, q) ends up with d = 8 q .. 8 q + 7 of the quarter for the tokens 16 mt + r and 16 mt + r + 8.
+    constexpr int CW = D / 32;                 // 16-byte chunks of a d-quarter (lanes q < CW hold data)
     const int dq = warp - KP_LWARPS;
-    const int tl = lane / CH, ch = lane % CH;
+    const int r = lane >> 2, q = lane & 3;
     const uint32_t stage_u32 = smem_u32(stage_base);
-    const uint32_t lane_off = (uint32_t)(tl * row_stride + dq * (D / 4) * 2 + ch * 16);
+    const uint32_t lane_off = (uint32_t)(r * row_stride + dq * (D / 4) * 2 + (q % CW) * 16);
     const uint32_t tcol = tmem + ((uint32_t)(dq * 32) << 16) + (uint32_t)KB_COL0;
     const float inv = 1.f / (float)(L * Hkv);
+    // identity fragments: n-tile t selects k = 8 t + n; b0 holds k = 2q, 2q+1 and b1 k = 2q+8, 2q+9 of column n = r
+    const uint32_t one_sel = (r == 2 * q) ? 0x00003f80u : ((r == 2 * q + 1) ? 0x3f800000u : 0u);
     int s = 0;
     uint32_t ph = 0;
     for (int l = 0; l < L; ++l) {
       for (int i = 0; i < my_tiles; ++i) {
-        float kb[32];  // NG * 8 of them are used
+        float c[2][2][2][4];  // [m-tile][k-step: xy | zw][n-tile][row r: cols 2q, 2q+1 | row r+8: cols 2q, 2q+1]
 #pragma unroll
-        for (int e = 0; e < 32; ++e) kb[e] = 0.f;
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+          for (int b = 0; b < 2; ++b)
+#pragma unroll
+            for (int t = 0; t < 2; ++t) c[a][b][t][0] = c[a][b][t][1] = c[a][b][t][2] = c[a][b][t][3] = 0.f;
         mbar_wait(&full[s], ph);
         const uint32_t sb = stage_u32 + (uint32_t)(s * stage_bytes) + lane_off;
-#pragma unroll 4
+#pragma unroll 2
         for (int kvh = 0; kvh < Hkv; ++kvh) {
 #pragma unroll
-          for (int gI = 0; gI < NG; ++gI) {
-            const uint4 u = lds128(sb + (uint32_t)(gI * TPL * row_stride + kvh * D * 2));
-            kb[gI * 8 + 0] += bf16lo(u.x); kb[gI * 8 + 1] += bf16hi(u.x);
-            kb[gI * 8 + 2] += bf16lo(u.y); kb[gI * 8 + 3] += bf16hi(u.y);
-            kb[gI * 8 + 4] += bf16lo(u.z); kb[gI * 8 + 5] += bf16hi(u.z);
-            kb[gI * 8 + 6] += bf16lo(u.w); kb[gI * 8 + 7] += bf16hi(u.w);
+          for (int mt = 0; mt < 2; ++mt) {
+            const uint4 ka = lds128(sb + (uint32_t)(mt * 16 * row_stride + kvh * D * 2));
+            const uint4 kc = lds128(sb + (uint32_t)((mt * 16 + 8) * row_stride + kvh * D * 2));
+            mma_bf16_16816(c[mt][0][0], ka.x, kc.x, ka.y, kc.y, one_sel, 0u);
+            mma_bf16_16816(c[mt][0][1], ka.x, kc.x, ka.y, kc.y, 0u, one_sel);
+            mma_bf16_16816(c[mt][1][0], ka.z, kc.z, ka.w, kc.w, one_sel, 0u);
+            mma_bf16_16816(c[mt][1][1], ka.z, kc.z, ka.w, kc.w, 0u, one_sel);
           }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[s]);
         if (++s == NS) { s = 0; ph ^= 1u; }
+        // kb[(mt * 2 + row) * 8 + e]: token 16 mt + r + 8 row, d = 8 q + e;  e = 4 ks + 2 t + {0, 1}
+        float kb[32];
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+          for (int ks = 0; ks < 2; ++ks)
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+              kb[(mt * 2 + 0) * 8 + 4 * ks + 2 * t + 0] = c[mt][ks][t][0];
+              kb[(mt * 2 + 0) * 8 + 4 * ks + 2 * t + 1] = c[mt][ks][t][1];
+              kb[(mt * 2 + 1) * 8 + 4 * ks + 2 * t + 0] = c[mt][ks][t][2];
+              kb[(mt * 2 + 1) * 8 + 4 * ks + 2 * t + 1] = c[mt][ks][t][3];
+            }
         const uint32_t ta = tcol + (uint32_t)(32 * i);
-        if (l >= 1 && !(p.dbg & 2)) {
+        if (l >= 1) {
           float acc[32];
           tmem_ld32(ta, acc);
           tmem_wait_ld();
 #pragma unroll
           for (int e = 0; e < 32; ++e) kb[e] += acc[e];
         }
-        if (!(p.dbg & 2)) {
-          tmem_st32(ta, kb);
-          tmem_wait_st();
-        } else if (kb[0] + kb[7] == 123.456f) {
-          p.kbar[0] = 1.f;
-        }
+        tmem_st32(ta, kb);
+        tmem_wait_st();
       }
     }
     bar_sync(1, (KP_LWARPS + KP_KWARPS) * 32);  // pairs with the logit warps' barrier before the ring is reused
@@ -505,13 +523,15 @@ __global__ __launch_bounds__(lm_threads(KBAR), 1) void k_key_pass_lm(const KeyPa
       tmem_ld32(tcol + (uint32_t)(32 * i), kb);
       tmem_wait_ld();
       float* outp = is_x ? p.kq : p.kbar;
+      if (q < CW) {
 #pragma unroll
-      for (int gI = 0; gI < NG; ++gI) {
-        const int tok = gI * TPL + tl;
-        if (tok < nvalid) {
-          float4* d4 = reinterpret_cast<float4*>(outp + (int64_t)(t0 + tok) * D + dq * (D / 4) + ch * 8);
-          d4[0] = make_float4(kb[gI * 8 + 0] * inv, kb[gI * 8 + 1] * inv, kb[gI * 8 + 2] * inv, kb[gI * 8 + 3] * inv);
-          d4[1] = make_float4(kb[gI * 8 + 4] * inv, kb[gI * 8 + 5] * inv, kb[gI * 8 + 6] * inv, kb[gI * 8 + 7] * inv);
+        for (int j = 0; j < 4; ++j) {
+          const int tok = (j >> 1) * 16 + r + 8 * (j & 1);
+          if (tok < nvalid) {
+            float4* d4 = reinterpret_cast<float4*>(outp + (int64_t)(t0 + tok) * D + dq * (D / 4) + q * 8);
+            d4[0] = make_float4(kb[j * 8 + 0] * inv, kb[j * 8 + 1] * inv, kb[j * 8 + 2] * inv, kb[j * 8 + 3] * inv);
+            d4[1] = make_float4(kb[j * 8 + 4] * inv, kb[j * 8 + 5] * inv, kb[j * 8 + 6] * inv, kb[j * 8 + 7] * inv);
+          }
         }
       }
     }
