@@ -765,6 +765,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     tp.rule_c = c->rule_c; tp.kbar = c->kbar; tp.n_cand = c->d_ncand; tp.cand_pos = c->cand_pos; tp.n_xq = c->d_nxq;
     tp.wcan = c->rt_wcan; tp.svec = c->rt_svec; tp.b1_eff = c->b1_eff; tp.nxp = nxp;
     tp.use_xattn = (use_x && n_x > 0) ? 1 : 0; tp.scores = scores;
+    tp.early = lm_done ? 1 : 0;  // rule_c and kbar then come from the key pass, complete before k_post_key started
     const int smem = D == 128 ? rt_tail_smem<128>() : rt_tail_smem<64>();
     if (c->tail_smem_set != smem) {
       CU(c, cudaFuncSetAttribute(k_tail_tc<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, rt_tail_smem<128>()));

@@ -285,6 +285,8 @@ struct TailParams {
   const float* b1_eff;
   int nxp;                   // key columns per head (multiple of 16, <= RT_NXMAX)
   int use_xattn;
+  int early;                 // rule_c and kbar are complete when this grid starts (they come from the layer-major key
+                             // pass, two kernels back): only the folded operands wait for the predecessor
   float* scores;             // by position
 };
 
@@ -299,7 +301,9 @@ __global__ __launch_bounds__(RT_TAIL_THREADS, 1) void k_tail_tc(const TailParams
   constexpr int A_PART = RT_M * D * 2;   // bytes of kbar hi (and of kbar lo)
   constexpr int A_SBO = (D / 8) * 128;   // byte distance between 8-row groups of the kbar rows
   if (threadIdx.x == 0) RT_T(0, 0);
-  pdl_wait();  // launched with programmatic stream serialization: nothing is read before the predecessor is complete
+  // Programmatic stream serialization.  p.early: the predecessor (k_post_key) only produces the folded operands, which
+  // warp 9 loads after its own griddepcontrol.wait; set-up and the first tile's fill run under the predecessor.
+  if (!p.early) pdl_wait();
   pdl_launch_dependents();
   if (threadIdx.x == 0) RT_T(0, 1);
   extern __shared__ __align__(128) unsigned char rt_smem_raw[];
@@ -320,7 +324,8 @@ __global__ __launch_bounds__(RT_TAIL_THREADS, 1) void k_tail_tc(const TailParams
   uint64_t* p_ready = ak_free + 1;          // [4] P of head h written (4 warps each)
   uint64_t* fc1_full = p_ready + 4;         // fc1 accumulator complete (and every operand buffer of the tile is free)
   uint64_t* tmem_free = fc1_full + 1;       // the epilogue has read the fc1 accumulator (8 warps)
-  uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(tmem_free + 1);
+  uint64_t* vec_ready = tmem_free + 1;      // b1', s_r, s_b (outputs of the fold) are in shared memory (warp 9)
+  uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(vec_ready + 1);
 
   const int nc = *p.n_cand;
   const int n_tiles = (nc + RT_M - 1) / RT_M;
@@ -338,14 +343,12 @@ __global__ __launch_bounds__(RT_TAIL_THREADS, 1) void k_tail_tc(const TailParams
     for (int h = 0; h < 4; ++h) mbar_init(&p_ready[h], 4);
     mbar_init(fc1_full, 1);
     mbar_init(tmem_free, RT_CWARPS);
+    mbar_init(vec_ready, 1);
     mbar_fence_init();
   }
-  for (int n = threadIdx.x; n < R_HID; n += RT_TAIL_THREADS) {
-    ep_b1[n] = p.b1_eff[n];
+  for (int n = threadIdx.x; n < R_HID; n += RT_TAIL_THREADS) {  // static weights: no dependency on the predecessor
     ep_wr[n] = __ldg(w.fc1_w + (int64_t)n * IN + 3 * D);
     ep_w2[n] = __ldg(w.fc2_w + n);
-    sv_r[n] = xat ? p.svec[n] : 0.f;
-    sv_b[n] = xat ? p.svec[256 + n] : 0.f;
   }
   if (warp == 8) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_base_p)), "n"(512));
@@ -362,7 +365,16 @@ __global__ __launch_bounds__(RT_TAIL_THREADS, 1) void k_tail_tc(const TailParams
   const int n_s = xat ? KS : 0, spp = NXP / 16;
 
   if (warp == 9) {
-    // ------------------------------------------------------------------ chunk loader (one thread)
+    // ------------------------------------------------------------------ chunk loader (one thread); first the folded
+    // vectors, which like the chunks are outputs of the predecessor
+    pdl_wait();
+    for (int n = lane; n < R_HID; n += 32) {
+      ep_b1[n] = p.b1_eff[n];
+      sv_r[n] = xat ? p.svec[n] : 0.f;
+      sv_b[n] = xat ? p.svec[256 + n] : 0.f;
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(vec_ready);
     if (lane == 0) {
       const unsigned char* src_s = p.wcan;
       const unsigned char* src_k = p.wcan + (size_t)KS * RT_CHUNK;
@@ -506,6 +518,7 @@ __global__ __launch_bounds__(RT_TAIL_THREADS, 1) void k_tail_tc(const TailParams
       if (threadIdx.x == 0 && it == 0) RT_T(0, 3);
       prev_rule = rule;
       rule = (t0 + m < nc) ? p.rule_c[t0 + m] : 0.f;
+      if (it == 0) mbar_wait(vec_ready, 0u);  // b1', s_r, s_b
       if (it > 0) epilogue(prev_tile, prev_rule);   // S of this tile is multiplied meanwhile
       if (threadIdx.x == 0 && it == 1) RT_T(0, 12);
       if (xat) {
