@@ -55,26 +55,13 @@ struct DevBuf {
 
 }  // namespace
 
-struct ikv_ctx {
-  ikv_config cfg;
-  int G = 1;
-  int64_t layer_stride = 0;  // elements
-  std::unordered_map<uint64_t, Session> sessions;
-  uint64_t tick = 0;
-  std::string err;
-  int n_sm = 148;
-  int max_smem = 48 * 1024;  // opt-in dynamic shared memory per CTA
+// Scratch of one score pass (a1-a5 of one request).  The context derives from it: its own copy is the set in use; a
+// batched ikv_score gives every lane a set of its own and swaps it in around that lane's launches (the kernels take
+// the pointers by value).
+struct Scratch {
   uint4* frag = nullptr;     // B fragments of M / sqrt(D) for the bf16 key pass
-  bool use_pdl = true;       // programmatic dependent launch between decode kernels (IKV_PDL=0 disables)
-  bool pdl_prune = true;     // ... and along the kernels of the prune pass (IKV_PDL_PRUNE=0 disables)
-  bool attr_done[2][2][9] = {};
-  int dbg_l2 = 7;            // IKV_TUNE_L2_HINTS
-  int use_lm = 1;            // IKV_TUNE_LAYER_MAJOR
-  int lm_dbg = 0;
   int32_t* lm_cnt = nullptr; // per-layer arrival counters of k_key_pass_lm
-
-  // scratch (per request, sized by ensure_scratch)
-  int64_t cap_tokens = 0;
+  int64_t cap_tokens = 0;    // token-sized buffers (ensure_scratch)
   int32_t *cand_pos = nullptr, *cand_slot = nullptr, *d_ncand = nullptr;
   float* logits = nullptr;
   float2* partials = nullptr;
@@ -89,10 +76,37 @@ struct ikv_ctx {
   unsigned char* w1_can = nullptr;  // fc1' chunks for tcgen05 (residual_mma.cuh)
   unsigned char* rt_wcan = nullptr; // operand chunks of k_residual_tc (residual_tc.cuh)
   float* rt_svec = nullptr;         // s_r | s_b
+  uint8_t* keepflag = nullptr;      // select fallback (maps > CL_MAX_N)
+  int32_t* tmp_slot = nullptr;
+};
+constexpr int IKV_MAX_LANES = 8;
+
+struct ikv_ctx : Scratch {
+  ikv_config cfg;
+  int G = 1;
+  int64_t layer_stride = 0;  // elements
+  std::unordered_map<uint64_t, Session> sessions;
+  uint64_t tick = 0;
+  std::string err;
+  int n_sm = 148;
+  int max_smem = 48 * 1024;  // opt-in dynamic shared memory per CTA
+  bool use_pdl = true;       // programmatic dependent launch between decode kernels (IKV_CFG_NO_PDL disables)
+  bool pdl_prune = true;     // ... and along the kernels of the prune pass (IKV_CFG_NO_PDL_PRUNE disables)
+  bool attr_done[2][2][9] = {};
+  int dbg_l2 = 7;            // IKV_TUNE_L2_HINTS
+  int use_lm = 1;            // IKV_TUNE_LAYER_MAJOR
+
+  // lanes of a batched ikv_score: the small kernels of request r run on stream r % n_lanes with that lane's scratch,
+  // the key passes in request order on the caller's stream (lane 0 uses the context's own set)
+  int n_lanes = 4;           // IKV_TUNE_BATCH_LANES
+  int lanes_ready = 0;
+  Scratch lane_set[IKV_MAX_LANES];
+  cudaStream_t lane_stream[IKV_MAX_LANES] = {};
+  cudaEvent_t lane_ev[IKV_MAX_LANES][3] = {};  // small -> key, key -> small, join
+  cudaEvent_t fork_ev = nullptr;
+
   uint32_t* kept_bits = nullptr;
   int32_t* firstpos = nullptr;
-  uint8_t* keepflag = nullptr;
-  int32_t* tmp_slot = nullptr;
   float* part_o = nullptr;
   float2* part_ml = nullptr;
   int64_t part_cap = 0;  // in (req*Hq*split) units
@@ -321,6 +335,35 @@ __global__ void k_init_dead(T* k_pool, T* v_pool, int64_t layer_stride, int L, i
 }
 
 int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
+
+// The buffers of a scratch set whose size depends on the model shape only.
+bool scratch_alloc_fixed(Scratch& s, const ikv_config& cfg) {
+  const int LH = cfg.n_layers * cfg.n_q_heads, KS = cfg.head_dim / 16;
+  bool ok = cudaMalloc((void**)&s.d_ncand, 4) == cudaSuccess && cudaMalloc((void**)&s.d_nxq, 4) == cudaSuccess;
+  ok = ok && cudaMemset(s.d_nxq, 0, 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&s.lse, (size_t)LH * 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&s.lm_cnt, (size_t)cfg.n_layers * 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&s.mbar, (size_t)cfg.head_dim * 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&s.mpart, (size_t)((LH + 31) / 32) * cfg.head_dim * 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&s.bq_eff, R_DC * 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&s.b1_eff, R_HID * 4) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&s.wq_frag, (size_t)KS * 16 * 32 * sizeof(uint4)) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&s.w1_can, (size_t)2 * (cfg.head_dim / 64 + 2) * W1C_CHUNK) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&s.rt_wcan, rt_wcan_bytes(cfg.head_dim)) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&s.rt_svec, 512 * 4) == cudaSuccess;
+  // B fragments: [L][Hkv][NT<=2][D/32][32 lanes] uint4
+  ok = ok && cudaMalloc((void**)&s.frag, (size_t)cfg.n_layers * cfg.n_kv_heads * 2 * (cfg.head_dim / 32) * 32 *
+                                             sizeof(uint4)) == cudaSuccess;
+  return ok;
+}
+
+void scratch_free(Scratch& s) {
+  void* bufs[] = {s.frag, s.lm_cnt, s.cand_pos, s.cand_slot, s.d_ncand, s.logits, s.partials, s.lse, s.rule_c, s.kbar,
+                  s.mbar, s.xq_slot, s.d_nxq, s.kq, s.kc_frag, s.vc_frag, s.mpart, s.bq_eff, s.b1_eff, s.wq_frag,
+                  s.w1_can, s.rt_wcan, s.rt_svec, s.keepflag, s.tmp_slot};
+  for (void* b : bufs) cudaFree(b);
+  s = Scratch{};
+}
 
 ikv_status ensure_scratch(ikv_ctx* c, int64_t tokens) {
   if (tokens <= c->cap_tokens) return IKV_OK;
@@ -572,9 +615,13 @@ ikv_status dispatch_decode(ikv_ctx* c, int layer, const DecBatch& b, int n_req, 
 // on-chip capacity: *lm_done = true, rule_c / scores / k_bar are final.  Otherwise k_key_pass (score_mma.cuh): logits
 // scratch + partials, *n_part = number of partial (max, sum) columns.
 struct LmOut { float* scores; float* rule_out; int scatter; };
+// lane != nullptr (batched ikv_score): the key pass goes on lane->kst, after the work enqueued on st so far, and st
+// continues after it.
+struct KeyLane { cudaStream_t kst; cudaEvent_t to_key, from_key; };
+
 template <int D, int G>
 ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, int n_mpart, int* n_part, int N, int n_x,
-                           const LmOut& lo, bool* lm_done, cudaStream_t st) {
+                           const LmOut& lo, bool* lm_done, cudaStream_t st, const KeyLane* lane) {
   const int L = c->cfg.n_layers, Hkv = c->cfg.n_kv_heads, Hq = c->cfg.n_q_heads;
   const int n_fb = mem_prep_frag_blocks<D, G>(L, Hkv);
   const int grid = c->n_sm;
@@ -592,6 +639,19 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
                      1.0f / sqrtf((float)D), c->frag, n_fb, L * Hq, c->mpart, lm ? c->lm_cnt : (int32_t*)nullptr));
   }
   *lm_done = lm;
+  cudaStream_t ks = st;
+  if (lane) {
+    ks = lane->kst;
+    CU(c, cudaEventRecord(lane->to_key, st));
+    CU(c, cudaStreamWaitEvent(ks, lane->to_key, 0));
+  }
+  auto rejoin = [&]() -> ikv_status {
+    if (lane) {
+      CU(c, cudaEventRecord(lane->from_key, ks));
+      CU(c, cudaStreamWaitEvent(st, lane->from_key, 0));
+    }
+    return IKV_OK;
+  };
   if constexpr (G <= 4) {
     if (lm) {
       int ns = 0;
@@ -603,21 +663,21 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
       p.xq_slot = with_xq ? c->xq_slot : nullptr; p.n_xq = with_xq ? c->d_nxq : nullptr;
       p.partials = c->partials; p.layer_cnt = c->lm_cnt; p.rule_c = c->rule_c;
       p.scores = lo.scores; p.rule_out = lo.rule_out; p.scatter_scores = lo.scatter;
-      p.kbar = c->kbar; p.kq = c->kq; p.n_stage = ns; p.l2_hints = c->dbg_l2; p.dbg = c->lm_dbg;
+      p.kbar = c->kbar; p.kq = c->kq; p.n_stage = ns; p.l2_hints = c->dbg_l2;
       p.tstamp = nullptr;
       if (c->prof_on == 1 && c->ts_ring && c->ts_used < ikv_ctx::TS_SLOTS) p.tstamp = c->ts_ring + 2 * (c->ts_used++);
-      ProfScope prof(c, c->prof_on == 1 ? IKV_PROF_SLOTS : IKV_PROF_KEY_PASS, st);  // level 1: stamps instead of events
+      ProfScope prof(c, c->prof_on == 1 ? IKV_PROF_SLOTS : IKV_PROF_KEY_PASS, ks);  // level 1: stamps instead of events
       if (kbar) {
         auto fn = k_key_pass_lm<D, G, true>;
         CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(c, launch_pdl(fn, dim3(grid), dim3(lm_threads(true)), smem, st, c->pdl_prune, p));
+        CU(c, launch_pdl(fn, dim3(grid), dim3(lm_threads(true)), smem, ks, c->pdl_prune, p));
       } else {
         auto fn = k_key_pass_lm<D, G, false>;
         CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        CU(c, launch_pdl(fn, dim3(grid), dim3(lm_threads(false)), smem, st, c->pdl_prune, p));
+        CU(c, launch_pdl(fn, dim3(grid), dim3(lm_threads(false)), smem, ks, c->pdl_prune, p));
       }
       *n_part = grid;
-      return IKV_OK;
+      return rejoin();
     }
   }
   int ns = 0;
@@ -631,44 +691,71 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
   p.logits = c->logits; p.ldc = c->cap_tokens; p.partials = c->partials; p.kbar = c->kbar; p.kq = c->kq;
   p.n_stage = ns;
   p.l2_hints = c->dbg_l2;
-  ProfScope prof(c, 0, st);
-  if (kbar) {
-    auto fn = k_key_pass<D, G, true>;
-    CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    CU(c, launch_pdl(fn, dim3(grid), dim3(kp_threads(G, true)), smem, st, c->pdl_prune, p));
-  } else {
-    auto fn = k_key_pass<D, G, false>;
-    CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    CU(c, launch_pdl(fn, dim3(grid), dim3(kp_threads(G, false)), smem, st, c->pdl_prune, p));
+  {
+    ProfScope prof(c, 0, ks);
+    if (kbar) {
+      auto fn = k_key_pass<D, G, true>;
+      CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      CU(c, launch_pdl(fn, dim3(grid), dim3(kp_threads(G, true)), smem, ks, c->pdl_prune, p));
+    } else {
+      auto fn = k_key_pass<D, G, false>;
+      CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      CU(c, launch_pdl(fn, dim3(grid), dim3(kp_threads(G, false)), smem, ks, c->pdl_prune, p));
+    }
+    LAUNCH_CHECK(c);
   }
-  LAUNCH_CHECK(c);
   *n_part = grid;
-  return IKV_OK;
+  return rejoin();
 }
 
 template <int D>
 ikv_status dispatch_key_pass_g(ikv_ctx* c, const float* M, bool kbar, bool xq, int n_mpart, int* n_part, int N, int n_x,
-                               const LmOut& lo, bool* lm_done, cudaStream_t st) {
+                               const LmOut& lo, bool* lm_done, cudaStream_t st, const KeyLane* lane) {
   switch (c->G) {
-    case 1: return launch_key_pass<D, 1>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
-    case 2: return launch_key_pass<D, 2>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
-    case 4: return launch_key_pass<D, 4>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
-    case 5: return launch_key_pass<D, 5>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
-    case 8: return launch_key_pass<D, 8>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
+    case 1: return launch_key_pass<D, 1>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st, lane);
+    case 2: return launch_key_pass<D, 2>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st, lane);
+    case 4: return launch_key_pass<D, 4>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st, lane);
+    case 5: return launch_key_pass<D, 5>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st, lane);
+    case 8: return launch_key_pass<D, 8>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st, lane);
   }
   IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "GQA group size %d not supported (1,2,4,5,8)", c->G);
 }
 
 ikv_status dispatch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool xq, int n_mpart, int* n_part, int N, int n_x,
-                             const LmOut& lo, bool* lm_done, cudaStream_t st) {
-  return c->cfg.head_dim == 128 ? dispatch_key_pass_g<128>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st)
-                                : dispatch_key_pass_g<64>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st);
+                             const LmOut& lo, bool* lm_done, cudaStream_t st, const KeyLane* lane) {
+  return c->cfg.head_dim == 128 ? dispatch_key_pass_g<128>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st, lane)
+                                : dispatch_key_pass_g<64>(c, M, kbar, xq, n_mpart, n_part, N, n_x, lo, lm_done, st, lane);
+}
+
+// Swaps lane k's scratch set with the context's own for the lifetime of the object (lane 0 is the context's own).
+struct LaneSwap {
+  ikv_ctx* c; int k;
+  LaneSwap(ikv_ctx* c_, int k_) : c(c_), k(k_) { if (k > 0) std::swap(static_cast<Scratch&>(*c), c->lane_set[k]); }
+  ~LaneSwap() { if (k > 0) std::swap(static_cast<Scratch&>(*c), c->lane_set[k]); }
+};
+
+ikv_status lanes_prepare(ikv_ctx* c, int K) {
+  if (!c->fork_ev) CU(c, cudaEventCreateWithFlags(&c->fork_ev, cudaEventDisableTiming));
+  for (int k = c->lanes_ready; k < K; ++k) {
+    if (!c->lane_stream[k]) CU(c, cudaStreamCreateWithFlags(&c->lane_stream[k], cudaStreamNonBlocking));
+    for (cudaEvent_t& e : c->lane_ev[k])
+      if (!e) CU(c, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    if (k > 0 && !c->lane_set[k].frag) {
+      if (!scratch_alloc_fixed(c->lane_set[k], c->cfg)) {
+        scratch_free(c->lane_set[k]);
+        IKV_FAIL(c, IKV_ERR_OOM, "ikv_score: scratch of lane %d: %s", k, cudaGetErrorString(cudaGetLastError()));
+      }
+      CU(c, cudaDeviceSynchronize());  // the memset of d_nxq is on the legacy stream
+    }
+    c->lanes_ready = k + 1;
+  }
+  return IKV_OK;
 }
 
 // M_ovr: score against these rows [L][Hq][D] instead of the session's memory (multi-row scorer); part: run the partition
 // (a1) first; scatter: write the rule score into `scores` (otherwise it stays in the compact rule_c[] scratch).
 ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, float* rule_out, cudaStream_t st,
-                     const float* M_ovr = nullptr, bool part = true, bool scatter = true) {
+                     const float* M_ovr = nullptr, bool part = true, bool scatter = true, const KeyLane* lane = nullptr) {
   const int N = r.seq_len;
   if (N == 0) return IKV_OK;
   const int base_mode = mode & 0xff;
@@ -716,7 +803,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   bool lm_done = false;  // the layer-major key pass has already produced rule_c (and the scores of a rule-only call)
   if (fast) {
     LmOut lo{scores, rule_out, (learn || !scatter) ? 0 : 1};
-    TRY(dispatch_key_pass(c, M, learn, n_x > 0, n_mpart, &n_part, N, n_x, lo, &lm_done, st));
+    TRY(dispatch_key_pass(c, M, learn, n_x > 0, n_mpart, &n_part, N, n_x, lo, &lm_done, st, lane));
   } else {
     if (n_mpart > 0) {
       if (D == 128) k_mem_prep<128, 1><<<n_mpart, 128, 0, st>>>(M, L, Hkv, 0.f, nullptr, 0, LH, c->mpart, nullptr);
@@ -930,24 +1017,7 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
     k_fill_i32<<<256, 256>>>(c->firstpos, cfg->n_slots, INT_MAX);
     ok = cudaGetLastError() == cudaSuccess;
   }
-  ok = ok && cudaMalloc((void**)&c->d_ncand, 4) == cudaSuccess && cudaMalloc((void**)&c->d_nxq, 4) == cudaSuccess;
-  ok = ok && cudaMemset(c->d_nxq, 0, 4) == cudaSuccess;
-  ok = ok && cudaMalloc((void**)&c->lse, (size_t)cfg->n_layers * cfg->n_q_heads * 4) == cudaSuccess;
-  ok = ok && cudaMalloc((void**)&c->lm_cnt, (size_t)cfg->n_layers * 4) == cudaSuccess;
-  ok = ok && cudaMalloc((void**)&c->mbar, (size_t)cfg->head_dim * 4) == cudaSuccess;
-  {
-    const int LH = cfg->n_layers * cfg->n_q_heads, KS = cfg->head_dim / 16;
-    ok = ok && cudaMalloc((void**)&c->mpart, (size_t)((LH + 31) / 32) * cfg->head_dim * 4) == cudaSuccess;
-    ok = ok && cudaMalloc((void**)&c->bq_eff, R_DC * 4) == cudaSuccess;
-    ok = ok && cudaMalloc((void**)&c->b1_eff, R_HID * 4) == cudaSuccess;
-    ok = ok && cudaMalloc((void**)&c->wq_frag, (size_t)KS * 16 * 32 * sizeof(uint4)) == cudaSuccess;
-    ok = ok && cudaMalloc((void**)&c->w1_can, (size_t)2 * (cfg->head_dim / 64 + 2) * W1C_CHUNK) == cudaSuccess;
-    ok = ok && cudaMalloc((void**)&c->rt_wcan, rt_wcan_bytes(cfg->head_dim)) == cudaSuccess;
-    ok = ok && cudaMalloc((void**)&c->rt_svec, 512 * 4) == cudaSuccess;
-  }
-  // B fragments: [L][Hkv][NT<=2][D/32][32 lanes] uint4
-  ok = ok && cudaMalloc((void**)&c->frag, (size_t)cfg->n_layers * cfg->n_kv_heads * 2 * (cfg->head_dim / 32) * 32 *
-                                              sizeof(uint4)) == cudaSuccess;
+  ok = ok && scratch_alloc_fixed(*c, *cfg);
   ok = ok && cudaDeviceSynchronize() == cudaSuccess;
   if (!ok) {
     g_create_err = std::string("ikv_create: CUDA initialisation failed: ") + cudaGetErrorString(cudaGetLastError());
@@ -962,11 +1032,15 @@ ikv_status ikv_destroy(ikv_ctx* c) {
   if (!c) return IKV_ERR_INVALID_ARG;
   cudaDeviceSynchronize();
   for (auto& kv : c->sessions) session_free(kv.second);
-  void* bufs[] = {c->cand_pos, c->cand_slot, c->d_ncand, c->logits, c->partials, c->lse, c->rule_c, c->kbar, c->mbar,
-                  c->xq_slot, c->d_nxq, c->kq, c->kc_frag, c->vc_frag, c->mpart, c->bq_eff, c->b1_eff, c->wq_frag,
-                  c->w1_can, c->rt_wcan, c->rt_svec, c->lm_cnt, c->ts_ring, c->kept_bits, c->firstpos, c->keepflag, c->tmp_slot,
-                  c->part_o, c->part_ml, c->st_out, c->st_scores,
-                  c->st_qrows, c->resid_blob, c->frag};
+  scratch_free(*c);
+  for (int k = 1; k < IKV_MAX_LANES; ++k) scratch_free(c->lane_set[k]);
+  for (int k = 0; k < IKV_MAX_LANES; ++k) {
+    if (c->lane_stream[k]) cudaStreamDestroy(c->lane_stream[k]);
+    for (cudaEvent_t e : c->lane_ev[k]) if (e) cudaEventDestroy(e);
+  }
+  if (c->fork_ev) cudaEventDestroy(c->fork_ev);
+  void* bufs[] = {c->ts_ring, c->kept_bits, c->firstpos, c->part_o, c->part_ml, c->st_out, c->st_scores,
+                  c->st_qrows, c->resid_blob};
   for (void* b : bufs) cudaFree(b);
   if (c->st_host) cudaFreeHost(c->st_host);
   for (int w = 0; w < IKV_PROF_SLOTS; ++w)
@@ -983,7 +1057,9 @@ ikv_status ikv_tune(ikv_ctx* c, int32_t knob, int32_t value) {
     case IKV_TUNE_L2_HINTS: c->dbg_l2 = value; return IKV_OK;
     case IKV_TUNE_RESID_TC: c->resid_tc = value; return IKV_OK;
     case IKV_TUNE_LAYER_MAJOR: c->use_lm = value; return IKV_OK;
-    case 99: c->lm_dbg = value; return IKV_OK;
+    case IKV_TUNE_BATCH_LANES:
+      c->n_lanes = value < 1 ? 1 : (value > IKV_MAX_LANES ? IKV_MAX_LANES : value);
+      return IKV_OK;
   }
   IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_tune: unknown knob %d", knob);
 }
@@ -1224,12 +1300,61 @@ ikv_status ikv_score(ikv_ctx* c, const ikv_request* reqs, int32_t n_req, int32_t
   if (bm != IKV_MODE_MEMORY && bm != IKV_MODE_LEARNABLE && bm != IKV_MODE_QUERY)
     IKV_FAIL(c, IKV_ERR_INVALID_ARG, "unknown scorer mode %d", bm);
   for (int r = 0; r < n_req; ++r) TRY(check_request(c, reqs[r]));
+  cudaStream_t st = (cudaStream_t)stream;
+  int n_busy = 0;
+  for (int r = 0; r < n_req; ++r) n_busy += reqs[r].seq_len > 0;
+  const int K = n_busy < c->n_lanes ? n_busy : c->n_lanes;
+  if (K < 2 || c->cfg.kv_dtype != IKV_BF16) {
+    int64_t off = 0;
+    for (int r = 0; r < n_req; ++r) {
+      TRY(score_one(c, reqs[r], mode, scores + off, rule_out ? rule_out + off : nullptr, st));
+      off += reqs[r].seq_len;
+    }
+    return IKV_OK;
+  }
+  // Batch: the latency chain of one request (partition, fragments, fold, residual head: ~60 us of small kernels) runs
+  // beside the key passes of the others.  Lane k = stream + scratch set; request r takes lane r % K; the key passes
+  // stay on the caller's stream in request order (two layer-major passes must never be resident together: each
+  // waits for all of its own CTAs).
+  TRY(lanes_prepare(c, K));
+  const bool learn = (mode & 0xff) == IKV_MODE_LEARNABLE && !(mode & IKV_FLAG_NO_RESIDUAL);
+  {  // every allocation before the first launch: cudaMalloc would serialise the lanes
+    int64_t need[IKV_MAX_LANES] = {}, need_x[IKV_MAX_LANES] = {};
+    int k = 0;
+    for (int r = 0; r < n_req; ++r) {
+      if (reqs[r].seq_len == 0) continue;
+      need[k] = std::max<int64_t>(need[k], reqs[r].seq_len);
+      const int n_x = reqs[r].xattn_pos ? reqs[r].n_xattn_pos : (reqs[r].q_end - reqs[r].q_start);
+      need_x[k] = std::max<int64_t>(need_x[k], n_x > 0 ? n_x : 1);
+      k = (k + 1) % K;
+    }
+    for (k = 0; k < K; ++k) {
+      LaneSwap sw(c, k);
+      TRY(ensure_scratch(c, need[k]));
+      if (learn) TRY(ensure_xq(c, need_x[k]));
+    }
+  }
+  CU(c, cudaEventRecord(c->fork_ev, st));
+  for (int k = 0; k < K; ++k) CU(c, cudaStreamWaitEvent(c->lane_stream[k], c->fork_ev, 0));
+  ikv_status rc = IKV_OK;
   int64_t off = 0;
-  for (int r = 0; r < n_req; ++r) {
-    TRY(score_one(c, reqs[r], mode, scores + off, rule_out ? rule_out + off : nullptr, (cudaStream_t)stream));
+  for (int r = 0, k = 0; r < n_req && rc == IKV_OK; ++r) {
+    if (reqs[r].seq_len > 0) {
+      LaneSwap sw(c, k);
+      const KeyLane lane{st, c->lane_ev[k][0], c->lane_ev[k][1]};
+      rc = score_one(c, reqs[r], mode, scores + off, rule_out ? rule_out + off : nullptr, c->lane_stream[k], nullptr,
+                     true, true, &lane);
+      k = (k + 1) % K;
+    }
     off += reqs[r].seq_len;
   }
-  return IKV_OK;
+  for (int k = 0; k < K; ++k) {  // join, also after a failure: the caller's stream must not run ahead of the lanes
+    if (cudaEventRecord(c->lane_ev[k][2], c->lane_stream[k]) != cudaSuccess ||
+        cudaStreamWaitEvent(st, c->lane_ev[k][2], 0) != cudaSuccess) {
+      if (rc == IKV_OK) { c->err = "ikv_score: joining the lanes failed"; rc = IKV_ERR_CUDA; }
+    }
+  }
+  return rc;
 }
 
 ikv_status ikv_score_rows(ikv_ctx* c, const ikv_request* reqs, int32_t n_req, const float* rows, int32_t n_rows,

@@ -49,7 +49,6 @@ struct KeyPassLmParams {
   int n_stage;
   int l2_hints;
   unsigned long long* tstamp;  // profiling: {min start, max end} of the launch in %globaltimer ns, or NULL
-  int dbg;                 // experiment switches (bit 0: no TMEM traffic in the logit warps, bit 1: in the mean-key warps, bit 2: no stats/exp)
 };
 
 __device__ __forceinline__ void tmem_ld4(uint32_t taddr, float (&v)[4]) {
@@ -352,7 +351,7 @@ __global__ __launch_bounds__(lm_threads(KBAR), 1) void k_key_pass_lm(const KeyPa
             // tensor-memory scratch of the tile: [rule_acc | x of layer l-1 | x of layer l-2], 4 tokens each
             const uint32_t ta = tcol + (uint32_t)(12 * i);
             float racc[4] = {0.f, 0.f, 0.f, 0.f}, xa[4] = {0.f, 0.f, 0.f, 0.f}, xb[4] = {0.f, 0.f, 0.f, 0.f};
-            if (l >= 1 && !(p.dbg & 1)) {
+            if (l >= 1) {
               tmem_ld4(ta, racc);
               tmem_ld4(ta + 4, xa);
               tmem_ld4(ta + 8, xb);
@@ -362,14 +361,10 @@ __global__ __launch_bounds__(lm_threads(KBAR), 1) void k_key_pass_lm(const KeyPa
 #pragma unroll
               for (int e = 0; e < 4; ++e) racc[e] += __expf(xb[e] - lse2);
             }
-            if (!(p.dbg & 1)) {
-              tmem_st4(ta, racc);
-              tmem_st4(ta + 4, x);
-              tmem_st4(ta + 8, xa);
-              tmem_wait_st();
-            } else if (racc[0] + xa[1] + x[2] == 123.456f) {
-              p.rule_c[0] = 1.f;
-            }
+            tmem_st4(ta, racc);
+            tmem_st4(ta + 4, x);
+            tmem_st4(ta + 8, xa);
+            tmem_wait_st();
           }
           __syncwarp();
           if (lane == 0) mbar_arrive(&empty[s]);

@@ -532,6 +532,56 @@ def test_batched_score_select(ikv, oracle):
         off += s.N
 
 
+@pytest.mark.parametrize("mode_name", ["memory", "learnable"])
+def test_batched_score_lanes(ikv, oracle, mode_name):
+    """A batch on 1, 3 and 8 lanes (IKV_TUNE_BATCH_LANES: small kernels of different requests on internal streams, each
+    lane with its own scratch) gives bit-identical scores, on a non-blocking stream with the default stream busy, and
+    agrees with the oracle; an empty request sits in the middle of the batch."""
+    shape = wl.ModelShape(2, 8, 2, 128, "bf16")
+    lens = [(700, 200), (4500, 256), (130, 64), (2300, 512), (1, 1), (5200, 300), (3100, 128)]
+    specs = [wl.SessionSpec(60 + i, n, 8, c, prefix_len=min(16, n // 4), span_len=min(16, n // 4), n_planted=min(5, n // 8))
+             for i, (n, c) in enumerate(lens)]
+    w = wl.make_workload(shape, specs, 23)
+    kp, vp = gc.to_cuda(w)
+    ctx = gc.make_ctx(w, max_sessions=16)
+    rw = wl.residual_weights(shape.D, 77)
+    ctx.residual_load(rw)
+    g = gc.oracle_geom(oracle, w)
+    maps = [s.slot_map[:s.N].clone().cuda() for s in w.sessions]
+    reqs = []
+    for s, m in zip(w.sessions, maps):
+        gc.fold_memory_gpu(ctx, s)
+        reqs.append(gc.request(ikv, s, m))
+    ctx.session_open(999)
+    empty = ikv.make_request(999, maps[0], 0, 0, 0, 0, 1, 0)
+    reqs.insert(3, empty)
+    tot = sum(s.N for s in w.sessions)
+    mode = ikv.MODE_MEMORY if mode_name == "memory" else ikv.MODE_LEARNABLE
+    stream = torch.cuda.Stream()
+    busy = torch.empty(64 << 20, device="cuda")
+    outs = []
+    for lanes in (1, 3, 8):
+        ctx.tune(ikv.TUNE_BATCH_LANES, lanes)
+        sc = torch.full((tot,), float("nan"), device="cuda")
+        torch.cuda.synchronize()
+        for _ in range(4):
+            busy.add_(1.0)
+        ctx.score(reqs, mode, sc, None, stream)
+        stream.synchronize()
+        outs.append(sc.cpu().numpy())
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+    off = 0
+    for i, s in enumerate(w.sessions):
+        M = gc.fold_memory_oracle(oracle, s)
+        S = s.slot_map[:s.N].numpy()
+        if mode_name == "memory":
+            want = oracle.score(g, kp, M, S, s.pi, s.qs, s.qe)
+        else:
+            want = oracle.score(g, kp, M, S, s.pi, s.qs, s.qe, oracle.MODE_LEARNABLE, 0, w=oracle.ResidualWeights(**rw))
+        gc.assert_scores_close(outs[0][off:off + s.N], want, f"lanes request {i}")
+        off += s.N
+
+
 def test_batched_select_many_requests(ikv, oracle):
     """20 requests in one ikv_select_evict call (two launches of one cluster per request) on pages interleaved in one
     pool: mixed lengths (one beyond 32,768 positions), heavy ties, dead positions; every request bit-exact."""
