@@ -440,11 +440,11 @@ __global__ __launch_bounds__(lm_threads(KBAR), 1) void k_key_pass_lm(const KeyPa
     }
   } else if (KBAR && warp < KP_LWARPS + KP_KWARPS) {
     // ------------------------------------------------------------------ mean-key warps (Eq. 5): warp dq owns one quarter
-    // of D.  The sum over the KV heads is a contraction with an identity matrix: the key tile is loaded as the A operand
-    // of mma.sync.m16n8k16 exactly like the logit warps load it (rows r, r+8; lane q takes the 16-byte chunk q of the
-    // quarter) and multiplied by B = [I8 | 0] and [0 | I8], accumulating over the heads in the fp32 accumulators --
-    // products with 1.0 are exact, and one HMMA replaces 16 unpack + 16 add instructions.  The tile's accumulators live
-    // in tensor memory between the layers.
+    // of D.  The sum over the KV heads is a contraction with a stacked identity matrix: for every pair of KV heads the
+    // 4-byte piece j of the lane's 16-byte chunk (rows r, r+8) of head kvh is the k < 8 half of an mma.sync.m16n8k16
+    // A tile and the same piece of head kvh + 1 the k >= 8 half; B = [I8; I8] adds the two heads into the fp32
+    // accumulators -- products with 1.0 are exact, and one HMMA replaces 32 unpack + 32 add instructions.  The tile's
+    // accumulators live in tensor memory between the layers.
     // Thread (r, q) ends up with d = 8 q .. 8 q + 7 of the quarter for the tokens 16 mt + r and 16 mt + r + 8.
     constexpr int CW = D / 32;                 // 16-byte chunks of a d-quarter (lanes q < CW hold data)
     const int dq = warp - KP_LWARPS;
@@ -453,13 +453,13 @@ __global__ __launch_bounds__(lm_threads(KBAR), 1) void k_key_pass_lm(const KeyPa
     const uint32_t lane_off = (uint32_t)(r * row_stride + dq * (D / 4) * 2 + (q % CW) * 16);
     const uint32_t tcol = tmem + ((uint32_t)(dq * 32) << 16) + (uint32_t)KB_COL0;
     const float inv = 1.f / (float)(L * Hkv);
-    // identity fragments: n-tile t selects k = 8 t + n; b0 holds k = 2q, 2q+1 and b1 k = 2q+8, 2q+9 of column n = r
+    // B = [I8; I8]: b0 holds rows k = 2q, 2q+1 and b1 rows k = 2q+8, 2q+9 of column n = r -- the same pattern
     const uint32_t one_sel = (r == 2 * q) ? 0x00003f80u : ((r == 2 * q + 1) ? 0x3f800000u : 0u);
     int s = 0;
     uint32_t ph = 0;
     for (int l = 0; l < L; ++l) {
       for (int i = 0; i < my_tiles; ++i) {
-        float c[2][2][2][4];  // [m-tile][k-step: xy | zw][n-tile][row r: cols 2q, 2q+1 | row r+8: cols 2q, 2q+1]
+        float c[2][2][2][4];  // [m-tile][piece j = 2 ks + t of the chunk][row r: d 2j, 2j+1 | row r+8: d 2j, 2j+1]
 #pragma unroll
         for (int a = 0; a < 2; ++a)
 #pragma unroll
@@ -468,16 +468,31 @@ __global__ __launch_bounds__(lm_threads(KBAR), 1) void k_key_pass_lm(const KeyPa
             for (int t = 0; t < 2; ++t) c[a][b][t][0] = c[a][b][t][1] = c[a][b][t][2] = c[a][b][t][3] = 0.f;
         mbar_wait(&full[s], ph);
         const uint32_t sb = stage_u32 + (uint32_t)(s * stage_bytes) + lane_off;
+        // two KV heads per HMMA: k = 0..7 of the A tile come from head kvh, k = 8..15 from head kvh + 1, B = [I8; I8]
 #pragma unroll 2
-        for (int kvh = 0; kvh < Hkv; ++kvh) {
+        for (int kvh = 0; kvh + 1 < Hkv; kvh += 2) {
 #pragma unroll
           for (int mt = 0; mt < 2; ++mt) {
             const uint4 ka = lds128(sb + (uint32_t)(mt * 16 * row_stride + kvh * D * 2));
             const uint4 kc = lds128(sb + (uint32_t)((mt * 16 + 8) * row_stride + kvh * D * 2));
-            mma_bf16_16816(c[mt][0][0], ka.x, kc.x, ka.y, kc.y, one_sel, 0u);
-            mma_bf16_16816(c[mt][0][1], ka.x, kc.x, ka.y, kc.y, 0u, one_sel);
-            mma_bf16_16816(c[mt][1][0], ka.z, kc.z, ka.w, kc.w, one_sel, 0u);
-            mma_bf16_16816(c[mt][1][1], ka.z, kc.z, ka.w, kc.w, 0u, one_sel);
+            const uint4 kd = lds128(sb + (uint32_t)(mt * 16 * row_stride + (kvh + 1) * D * 2));
+            const uint4 ke = lds128(sb + (uint32_t)((mt * 16 + 8) * row_stride + (kvh + 1) * D * 2));
+            mma_bf16_16816(c[mt][0][0], ka.x, kc.x, kd.x, ke.x, one_sel, one_sel);
+            mma_bf16_16816(c[mt][0][1], ka.y, kc.y, kd.y, ke.y, one_sel, one_sel);
+            mma_bf16_16816(c[mt][1][0], ka.z, kc.z, kd.z, ke.z, one_sel, one_sel);
+            mma_bf16_16816(c[mt][1][1], ka.w, kc.w, kd.w, ke.w, one_sel, one_sel);
+          }
+        }
+        if (Hkv & 1) {
+          const int kvh = Hkv - 1;
+#pragma unroll
+          for (int mt = 0; mt < 2; ++mt) {
+            const uint4 ka = lds128(sb + (uint32_t)(mt * 16 * row_stride + kvh * D * 2));
+            const uint4 kc = lds128(sb + (uint32_t)((mt * 16 + 8) * row_stride + kvh * D * 2));
+            mma_bf16_16816(c[mt][0][0], ka.x, kc.x, 0u, 0u, one_sel, 0u);
+            mma_bf16_16816(c[mt][0][1], ka.y, kc.y, 0u, 0u, one_sel, 0u);
+            mma_bf16_16816(c[mt][1][0], ka.z, kc.z, 0u, 0u, one_sel, 0u);
+            mma_bf16_16816(c[mt][1][1], ka.w, kc.w, 0u, 0u, one_sel, 0u);
           }
         }
         __syncwarp();
