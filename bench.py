@@ -6,7 +6,7 @@ configs[1]): ikv_memory_update (4 rows) -> ikv_score (LEARNABLE: rule + residual
 (C = 8192) -> 256 decode steps x 36 layers of ikv_decode_attn through the pruned slot map (CUDA graph).
 `value` = live history tokens / time of the pruning pass (memory update + score + select/evict), the metric
 BASELINE.json names; the decode stage is reported beside it (`decode`, `roofline_decode`), and configs[2] / configs[4]
-as sub-objects `cfg2` / `cfg4` of the same line.
+as sub-objects `cfg2` / `cfg4` of the same line; `next` holds the widened rows (multi-row scorer, baselines, prefill).
 
   python bench.py [--gpus N] [--steps K] [--warmup W]            # our arm (N>1: under torchrun, replicas)
   python bench.py --impl reference ...                           # the CPU oracle timed on the host cores
@@ -275,6 +275,80 @@ def prune_breakdown(rig, reps=10):
     pr = rig.ctx.profile_read()
     rig.ctx.profile_enable(0)
     return {k: round(1e3 * ms / n, 2) for k, (ms, n) in pr["slots"].items()}
+
+
+def run_next(rig, hbm_peak):
+    """The widened rows of SURVEY section 8(f), measured on the headline workload (configs[1]) through the C-ABI: NEXT-1
+    multi-row scorer (R = 4, 32), NEXT-3 baseline scorers, NEXT-2 one chunk of prefill attention through the pruned slot
+    map with its KV-read counters.  Each entry carries its own roofline: the time the algorithmic bytes (or flops) would
+    take at the measured peaks."""
+    torch, ikv = rig.torch, rig.ikv
+    ctx, st, dev, shape, T = rig.ctx, rig.stream, rig.dev, rig.shape, rig.T
+    L, Hq, Hkv, D = shape.L, shape.Hq, shape.Hkv, shape.D
+    key_bytes = L * Hkv * T * D * shape.elem_bytes
+    hbm_ms = key_bytes / (hbm_peak * 1e9) * 1e3
+    tensor_peak = 1679.3e12
+    mp = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(mp):
+        tensor_peak = float(json.load(open(mp)).get("bf16_tflops", 1679.3)) * 1e12
+
+    def timed(fn, n=3):
+        ts = []
+        for i in range(n + 1):
+            with torch.cuda.stream(st):
+                a, b = rig.ev(), rig.ev()
+                a.record(st); fn(); b.record(st)
+            st.synchronize()
+            ts.append(a.elapsed_time(b))
+        return statistics.median(ts[1:])
+
+    with torch.cuda.stream(st):
+        rig.S_dev.copy_(rig.pristine)
+    st.synchronize()
+    res = {"workload": "configs[1], un-pruned 32k-token map for the scorers; pruned map (C = 8k) for the prefill chunk"}
+    gen = torch.Generator(device="cpu").manual_seed(4242)
+    for R in (4, 32):
+        rows = torch.randn((R, L, Hq, D), generator=gen).to(dev).contiguous()
+        wts = [1.0 / R] * R
+        ms = timed(lambda: ctx.score_rows([rig.req], rows, wts, rig.scores, st))
+        # the bank is a bf16 hi + lo pair: two tensor passes per product; the keys are read twice (statistics, sums)
+        flop_ms = 2 * 2 * 2.0 * R * L * Hq * T * D / tensor_peak * 1e3
+        tc = R >= 6
+        roof = max(hbm_ms, flop_ms)
+        res[f"multirow_R{R}"] = {"ms": ms, "roofline_ms": roof, "frac_of_roofline": roof / ms,
+                                 "bound": "hbm" if hbm_ms >= flop_ms else "tensor",
+                                 "passes_over_the_keys": 2 if tc else R,
+                                 "what": ("ikv_score_rows on tcgen05: one bank of 128 bank rows, two sweeps over the keys"
+                                          if tc else "ikv_score_rows: R passes of the single-row key pass (below 6 rows)")}
+    rows32 = torch.randn((32, L, Hq, D), generator=gen).to(dev).contiguous()
+    res["baseline_streaming"] = {"ms": timed(lambda: ctx.score_baseline([rig.req], ikv.BASE_STREAMING, rig.scores, n_sink=4,
+                                                                        stream=st)),
+                                 "what": "sink 4 + recency scores: no keys are read"}
+    for name, kind, kw in (("baseline_snapkv", ikv.BASE_SNAPKV, {"pool_kernel": 7}),
+                           ("baseline_h2o", ikv.BASE_H2O, {"recent_ratio": 0.5, "recent_floor": 64})):
+        ms = timed(lambda: ctx.score_baseline([rig.req], kind, rig.scores, rows=rows32, stream=st, **kw), n=2)
+        res[name] = {"ms": ms, "roofline_ms": hbm_ms, "frac_of_roofline": hbm_ms / ms,
+                     "what": "window of 32 query rows through the tcgen05 multi-row scorer + pooling / recency rule"}
+    # NEXT-2: prune, then one chunk of 64 prefill rows at layer 0 through the pruned map
+    with torch.cuda.stream(st):
+        rig.prune()
+    st.synchronize()
+    n_kept = int(rig.nk.item())
+    n_q = 64
+    q = torch.randn((n_q, Hq, D), generator=gen).to(torch.bfloat16).to(dev)
+    out = torch.empty_like(q)
+    reads = torch.zeros(2, dtype=torch.int64, device=dev)
+    r = ikv.make_request(rig.sid, rig.S_dev, T + n_q, rig.sess.pi, rig.sess.qs, rig.sess.qe, rig.C, rig.sess.pi)
+    n_rep = 4
+    ms = timed(lambda: ctx.prefill_attn(0, r, T, q, out, rig.scale, reads, st), n=n_rep - 1)
+    raw, eff = [int(x) // n_rep for x in reads.cpu().tolist()]
+    kv_bytes = (n_kept + n_q) * Hkv * D * 2 * shape.elem_bytes          # the survivors' K and V rows, read once per chunk
+    roof = kv_bytes / (hbm_peak * 1e9) * 1e3
+    res["prefill_chunk"] = {"n_q": n_q, "layer_calls": 1, "live_tokens": n_kept, "ms": ms, "roofline_ms": roof,
+                            "frac_of_roofline": roof / ms, "raw_kv_reads": raw, "effective_kv_reads": eff,
+                            "what": "ikv_prefill_attn: the decode kernels row by row (32 rows per launch), K/V re-read "
+                                    "from L2 for every row; counters per PAPER.md:163-175"}
+    return res
 
 
 def run_cfg2(args, dev, hbm_peak):
@@ -583,6 +657,11 @@ def run_ours(args):
                                 "ms": dec_kernel_ms},
             "clocks": clocks, "wall_s_timed_region": t_wall,
         }
+        if not args.no_extra and world == 1:
+            try:
+                line["next"] = run_next(rig, hbm_peak)
+            except Exception as e:  # a sub-object must not take the headline down
+                line["next"] = {"error": repr(e)}
         del rig, graph, chain, w
         torch.cuda.empty_cache()
         if not args.no_extra and world == 1:

@@ -21,6 +21,7 @@
 #include "score.cuh"
 #include "score_mma.cuh"
 #include "score_lm.cuh"
+#include "score_rows_tc.cuh"
 #include "select.cuh"
 #include "select_cluster.cuh"
 #include "fused_small.cuh"
@@ -104,6 +105,13 @@ struct ikv_ctx : Scratch {
   cudaStream_t lane_stream[IKV_MAX_LANES] = {};
   cudaEvent_t lane_ev[IKV_MAX_LANES][3] = {};  // small -> key, key -> small, join
   cudaEvent_t fork_ev = nullptr;
+
+  // multi-row scorer on tcgen05 (score_rows_tc.cuh)
+  int rows_tc = 1;           // IKV_TUNE_ROWS_TC
+  unsigned char* rows_bank = nullptr;
+  float2* rows_partials = nullptr;
+  size_t rows_partials_cap = 0;
+  bool rows_attr_done = false;
 
   uint32_t* kept_bits = nullptr;
   int32_t* firstpos = nullptr;
@@ -752,6 +760,33 @@ ikv_status lanes_prepare(ikv_ctx* c, int K) {
   return IKV_OK;
 }
 
+// a1: fillers, candidate list and (n_x > 0) the compaction of the live cross-attention positions as a second cluster of
+// the same launch.
+ikv_status launch_partition(ikv_ctx* c, const ikv_request& r, int n_x, float* scores, float* rule_out, cudaStream_t st) {
+  const int N = r.seq_len;
+  const int grid = CL_CTAS * (n_x > 0 ? 2 : 1);
+  ProfScope prof(c, IKV_PROF_PARTITION, st);
+#define IKV_PART_ARGS r.slot_map, N, c->cfg.dead_slot, r.prefix_len, r.q_start, r.q_end, scores, rule_out, \
+                      c->cand_pos, c->cand_slot, c->d_ncand
+#define IKV_X_ARGS r.xattn_pos, n_x, c->xq_slot, c->d_nxq
+#define IKV_PART_LAUNCH(MAXI) \
+  CU(c, launch_pdl(k_partition_cl<MAXI>, dim3(grid), dim3(1024), 0, st, c->pdl_prune, IKV_PART_ARGS, IKV_X_ARGS))
+  if (N <= CL_CTAS * 1024 * 4) IKV_PART_LAUNCH(4);
+  else if (N <= CL_CTAS * 1024 * 8) IKV_PART_LAUNCH(8);
+  else if (N <= CL_MAX_N) IKV_PART_LAUNCH(16);
+  else {
+    k_partition<<<1, 1024, 0, st>>>(IKV_PART_ARGS);
+    if (n_x > 0)
+      k_xattn_compact<<<1, 1024, 0, st>>>(r.slot_map, N, c->cfg.dead_slot, r.xattn_pos, n_x, r.q_start, c->xq_slot,
+                                          c->d_nxq);
+  }
+#undef IKV_PART_LAUNCH
+#undef IKV_PART_ARGS
+#undef IKV_X_ARGS
+  LAUNCH_CHECK(c);
+  return IKV_OK;
+}
+
 // M_ovr: score against these rows [L][Hq][D] instead of the session's memory (multi-row scorer); part: run the partition
 // (a1) first; scatter: write the rule score into `scores` (otherwise it stays in the compact rule_c[] scratch).
 ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, float* rule_out, cudaStream_t st,
@@ -775,29 +810,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   // at most RT_NXMAX query positions: folded cross attention, the whole head on tcgen05 (residual_tc.cuh)
   const bool tc = learn && c->resid_tc && n_x <= RT_NXMAX;
   const int nxp = tc ? (n_x > 0 ? (n_x + 15) / 16 * 16 : 16) : 0;
-  if (part) {
-    // a1 (+ the compaction of the live cross-attention positions as a second cluster of the same launch)
-    const int grid = CL_CTAS * (n_x > 0 ? 2 : 1);
-    ProfScope prof(c, IKV_PROF_PARTITION, st);
-#define IKV_PART_ARGS r.slot_map, N, c->cfg.dead_slot, r.prefix_len, r.q_start, r.q_end, scores, rule_out, \
-                      c->cand_pos, c->cand_slot, c->d_ncand
-#define IKV_X_ARGS r.xattn_pos, n_x, c->xq_slot, c->d_nxq
-#define IKV_PART_LAUNCH(MAXI) \
-  CU(c, launch_pdl(k_partition_cl<MAXI>, dim3(grid), dim3(1024), 0, st, c->pdl_prune, IKV_PART_ARGS, IKV_X_ARGS))
-    if (N <= CL_CTAS * 1024 * 4) IKV_PART_LAUNCH(4);
-    else if (N <= CL_CTAS * 1024 * 8) IKV_PART_LAUNCH(8);
-    else if (N <= CL_MAX_N) IKV_PART_LAUNCH(16);
-    else {
-      k_partition<<<1, 1024, 0, st>>>(IKV_PART_ARGS);
-      if (n_x > 0)
-        k_xattn_compact<<<1, 1024, 0, st>>>(r.slot_map, N, c->cfg.dead_slot, r.xattn_pos, n_x, r.q_start, c->xq_slot,
-                                            c->d_nxq);
-    }
-#undef IKV_PART_LAUNCH
-#undef IKV_PART_ARGS
-#undef IKV_X_ARGS
-    LAUNCH_CHECK(c);
-  }
+  if (part) TRY(launch_partition(c, r, n_x, scores, rule_out, st));
   const int LH = L * Hq, n_mpart = learn ? (LH + 31) / 32 : 0;  // mbar partial sums ride along with the fragments
   int n_part = (N + SCORE_TILE - 1) / SCORE_TILE;
   bool lm_done = false;  // the layer-major key pass has already produced rule_c (and the scores of a rule-only call)
@@ -901,6 +914,57 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
     CU(c, launch_pdl(D == 128 ? k_residual_mma<128> : k_residual_mma<64>, dim3(nblk), dim3(R_THREADS),
                      D == 128 ? resid_smem<128>() : resid_smem<64>(), st, c->pdl_prune, rp, c->rw));
   }
+  return IKV_OK;
+}
+
+// NEXT-1 on tcgen05 (score_rows_tc.cuh): banks of 128 / G rows, two sweeps over the keys per bank.
+template <int D>
+ikv_status score_rows_tc(ikv_ctx* c, const ikv_request& r, const float* rows, int n_rows, const float* weights,
+                         float* scores, cudaStream_t st) {
+  const int N = r.seq_len, L = c->cfg.n_layers, Hkv = c->cfg.n_kv_heads, G = c->G;
+  if (!session_find(c, r.session_id))
+    IKV_FAIL(c, IKV_ERR_NO_SESSION, "session %llu does not exist", (unsigned long long)r.session_id);
+  TRY(ensure_scratch(c, N));
+  const int n_items = L * Hkv;
+  if (!c->rows_bank) CU(c, cudaMalloc((void**)&c->rows_bank, (size_t)n_items * rb_item(D)));
+  const int tiles = (N + RB_TOK - 1) / RB_TOK;
+  const int grid = std::max(1, std::min(c->n_sm, (tiles + 1) / 2));
+  const int n_pairs = (tiles + 2 * grid - 1) / (2 * grid);
+  const int n_slots = n_pairs * grid * 4;   // (pair, CTA, tile of the pair, column half)
+  const size_t need = (size_t)n_items * n_slots * RB_ROWS;
+  if (need > c->rows_partials_cap) {
+    c->rows_partials_cap = 0;
+    TRY(grow(c, &c->rows_partials, need));
+    c->rows_partials_cap = need;
+  }
+  if (!c->rows_attr_done) {
+    CU(c, cudaFuncSetAttribute(k_rows_pass<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(128)));
+    CU(c, cudaFuncSetAttribute(k_rows_pass<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(128)));
+    CU(c, cudaFuncSetAttribute(k_rows_pass<64, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(64)));
+    CU(c, cudaFuncSetAttribute(k_rows_pass<64, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(64)));
+    c->rows_attr_done = true;
+  }
+  TRY(launch_partition(c, r, 0, scores, nullptr, st));
+  const int64_t row_elems = (int64_t)L * c->cfg.n_q_heads * D;
+  const int rpb = RB_ROWS / G;  // rows per bank
+  RowsPassParams p;
+  p.k_pool = (const bf16*)c->cfg.k_pool; p.layer_stride = c->layer_stride; p.L = L; p.Hkv = Hkv;
+  p.bank = c->rows_bank; p.cand_slot = c->cand_slot; p.n_cand = c->d_ncand; p.partials = c->rows_partials;
+  p.n_slots = n_slots; p.n_pairs = n_pairs; p.rule_c = c->rule_c;
+  for (int r0 = 0; r0 < n_rows; r0 += rpb) {
+    const int nr = std::min(rpb, n_rows - r0);
+    RowsWeights wts;
+    for (int cc = 0; cc < RB_ROWS; ++cc) wts.w[cc] = cc < nr * G ? weights[r0 + cc / G] : 0.f;
+    p.n_cols = nr * G;
+    p.accumulate = r0 > 0 ? 1 : 0;
+    k_rows_prep<D><<<n_items, 256, 0, st>>>(rows + r0 * row_elems, nr, L, Hkv, G, wts, c->rows_bank);
+    k_rows_pass<D, 1><<<grid, RB_THREADS, rb_smem(D), st>>>(p);
+    k_rows_lse<D><<<n_items, RB_ROWS, 0, st>>>(c->rows_partials, n_slots, c->rows_bank);
+    k_rows_pass<D, 2><<<grid, RB_THREADS, rb_smem(D), st>>>(p);
+    LAUNCH_CHECK(c);
+  }
+  k_axpy_scatter<<<64, 256, 0, st>>>(c->rule_c, c->cand_pos, c->d_ncand, 1.0f, 1, scores);
+  LAUNCH_CHECK(c);
   return IKV_OK;
 }
 
@@ -1039,7 +1103,7 @@ ikv_status ikv_destroy(ikv_ctx* c) {
     for (cudaEvent_t e : c->lane_ev[k]) if (e) cudaEventDestroy(e);
   }
   if (c->fork_ev) cudaEventDestroy(c->fork_ev);
-  void* bufs[] = {c->ts_ring, c->kept_bits, c->firstpos, c->part_o, c->part_ml, c->st_out, c->st_scores,
+  void* bufs[] = {c->rows_bank, c->rows_partials, c->ts_ring, c->kept_bits, c->firstpos, c->part_o, c->part_ml, c->st_out, c->st_scores,
                   c->st_qrows, c->resid_blob};
   for (void* b : bufs) cudaFree(b);
   if (c->st_host) cudaFreeHost(c->st_host);
@@ -1057,6 +1121,7 @@ ikv_status ikv_tune(ikv_ctx* c, int32_t knob, int32_t value) {
     case IKV_TUNE_L2_HINTS: c->dbg_l2 = value; return IKV_OK;
     case IKV_TUNE_RESID_TC: c->resid_tc = value; return IKV_OK;
     case IKV_TUNE_LAYER_MAJOR: c->use_lm = value; return IKV_OK;
+    case IKV_TUNE_ROWS_TC: c->rows_tc = value; return IKV_OK;
     case IKV_TUNE_BATCH_LANES:
       c->n_lanes = value < 1 ? 1 : (value > IKV_MAX_LANES ? IKV_MAX_LANES : value);
       return IKV_OK;
@@ -1365,6 +1430,17 @@ ikv_status ikv_score_rows(ikv_ctx* c, const ikv_request* reqs, int32_t n_req, co
   for (int r = 0; r < n_req; ++r) TRY(check_request(c, reqs[r]));
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t row_elems = (int64_t)c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim;
+  // six rows and up: banks on tcgen05 (two sweeps over the keys cost about six single-row passes); rows_tc = 2 forces it
+  if (c->rows_tc && c->cfg.kv_dtype == IKV_BF16 && (n_rows >= 6 || (c->rows_tc >= 2 && n_rows >= 2))) {
+    int64_t off = 0;
+    for (int r = 0; r < n_req; ++r) {
+      if (reqs[r].seq_len > 0)
+        TRY(c->cfg.head_dim == 128 ? score_rows_tc<128>(c, reqs[r], rows, n_rows, weights, scores + off, st)
+                                   : score_rows_tc<64>(c, reqs[r], rows, n_rows, weights, scores + off, st));
+      off += reqs[r].seq_len;
+    }
+    return IKV_OK;
+  }
   int64_t off = 0;
   for (int r = 0; r < n_req; ++r) {
     for (int k = 0; k < n_rows; ++k) {

@@ -36,9 +36,13 @@ SHAPES = [("d128g4", wl.ModelShape(3, 8, 2, 128, "bf16")), ("d64g2", wl.ModelSha
 
 
 @pytest.mark.parametrize("name,shape", SHAPES, ids=[n for n, _ in SHAPES])
-@pytest.mark.parametrize("R", [1, 4, 32])
+@pytest.mark.parametrize("R", [1, 4, 7, 32])
 def test_multirow_scorer_matches_oracle(ikv, oracle, name, shape, R):
+    """R = 1: one single-row pass; R = 7, 32: banks of 128 / G rows on tcgen05 (R = 32 at G = 5 needs two banks); R = 4
+    is forced through the tcgen05 path (IKV_TUNE_ROWS_TC = 2)."""
     w, kp, vp, ctx, s, M, S = _setup(oracle, shape)
+    if R == 4:
+        ctx.tune(ikv.TUNE_ROWS_TC, 2)
     S_dev = S.cuda()
     req = gc.request(ikv, s, S_dev)
     g = gc.oracle_geom(oracle, w)
@@ -51,6 +55,34 @@ def test_multirow_scorer_matches_oracle(ikv, oracle, name, shape, R):
     want = np.where(cls == oracle.FORCED, np.inf, np.where(cls == oracle.DEAD, -np.inf, want))
     mabs, mrel = gc.assert_scores_close(scores.cpu().numpy(), want, f"{name} R={R}")
     print(f"[{name} R={R}] multi-row score max abs err {mabs:.3e} rel {mrel:.3e}")
+
+
+def test_multirow_tc_several_tile_pairs(ikv, oracle):
+    """40,000 tokens: more than 2 x 148 tiles of 128, so the CTAs of the tcgen05 scorer walk two pairs of tiles (the
+    gather runs ahead into the next pair); ragged last tile, dead positions, 5 rows at G = 2 (10 of 128 bank rows).
+    Checked against the oracle and against the row-by-row path."""
+    shape = wl.ModelShape(1, 2, 1, 64, "bf16")
+    w, kp, vp, ctx, s, M, S = _setup(oracle, shape, n_tokens=40000, budget=1000)
+    S_dev = S.cuda()
+    req = gc.request(ikv, s, S_dev)
+    g = gc.oracle_geom(oracle, w)
+    R = 5
+    rows = torch.randn((R, shape.L, shape.Hq, shape.D), generator=torch.Generator().manual_seed(3))
+    wt = [0.5, 1.0, 0.0, 2.0, 0.25]
+    ctx.tune(ikv.TUNE_ROWS_TC, 2)
+    scores = torch.full((s.N,), 3.0, device="cuda")
+    ctx.score_rows([req], rows.cuda().contiguous(), wt, scores)
+    cls, _ = oracle.partition(S.numpy(), w.dead_slot, s.pi, s.qs, s.qe)
+    want = oracle.multirow_score(g, kp, rows.double().numpy(), wt, S.numpy(), cls)
+    want = np.where(cls == oracle.FORCED, np.inf, np.where(cls == oracle.DEAD, -np.inf, want))
+    mabs, mrel = gc.assert_scores_close(scores.cpu().numpy(), want, "several pairs")
+    print(f"[several pairs] multi-row score max abs err {mabs:.3e} rel {mrel:.3e}")
+    ctx.tune(ikv.TUNE_ROWS_TC, 0)
+    ref = torch.empty_like(scores)
+    ctx.score_rows([req], rows.cuda().contiguous(), wt, ref)
+    fin = torch.isfinite(ref)
+    assert torch.equal(torch.isfinite(scores), fin)
+    assert torch.allclose(scores[fin], ref[fin], rtol=1e-4, atol=1e-6)
 
 
 def test_multirow_single_row_is_the_memory_scorer_bit_for_bit(ikv, oracle):
