@@ -173,6 +173,23 @@ ikv_status ikv_select_evict(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req
 ikv_status ikv_decode_attn(ikv_ctx *ctx, int32_t layer, const ikv_request *reqs, int32_t n_req, const void *q,
                            void *out, float sm_scale, void *stream);
 
+/* a8 without any allocation, for callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses
+ * that forbid it).  One request, no session: every position [0, seq_len) is read through req->slot_map, entries equal to
+ * the dead slot are skipped (session_id, budget and the span fields of the request are ignored); q and out as in
+ * ikv_decode_attn with n_req = 1.  The split partials -- the only scratch of the decode kernels -- live in a file-scope
+ * device array of IKV_STATIC_SCRATCH_BYTES that every GPU holds from the moment it loads the library until exit; its
+ * address is resolved once, in ikv_create (cudaGetSymbolAddress on the context's device).  The call performs no
+ * cudaMalloc / cudaFree and calls no allocating routine.
+ * Limit: 256 + n_q_heads * n_split * (head_dim + 2) * 4 bytes must fit the array, n_split being the split count the
+ * library picks for seq_len (at most one per SM; 32 or 40 query heads at head_dim 128 always fit, 64 heads up to 92
+ * splits = sequences up to 1,472 positions); beyond it the call returns IKV_ERR_CAPACITY and enqueues nothing.
+ * Every call on a device shares the array, which keeps the previous call's contents (the call clears the one word that
+ * must start at zero): calls that can overlap on the GPU (different streams, or a captured graph replayed concurrently)
+ * race on it -- keep them on one stream.  Errors: IKV_ERR_INVALID_ARG, IKV_ERR_CAPACITY, IKV_ERR_CUDA. */
+#define IKV_STATIC_SCRATCH_BYTES (3 * 1024 * 1024)
+ikv_status ikv_decode_attn_static(ikv_ctx *ctx, int32_t layer, const ikv_request *req, const void *q, void *out,
+                                  float sm_scale, void *stream);
+
 /* ---- follow-ups of the hot path ------------------------------------------------------------ */
 /* Multi-row scorer ("window of W tail Q rows", O(W L H_q N); :159 W = 32; :310; R28): n_rows
  * un-collapsed rows per (layer, query head), rows[r][L][H_q][D] DEVICE fp32, used as given; every row is its own softmax

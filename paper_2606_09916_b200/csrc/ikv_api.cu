@@ -56,6 +56,10 @@ struct DevBuf {
 
 }  // namespace
 
+// Scratch of ikv_decode_attn_static: [0, 256) a zero word (the empty survivor list's length) | split partials.  In host
+// code this name is a host-side stand-in, never a device address: ikv_create resolves it with cudaGetSymbolAddress.
+static __device__ __align__(256) unsigned char g_static_scratch[IKV_STATIC_SCRATCH_BYTES];
+
 // Scratch of one score pass (a1-a5 of one request).  The context derives from it: its own copy is the set in use; a
 // batched ikv_score gives every lane a set of its own and swaps it in around that lane's launches (the kernels take
 // the pointers by value).
@@ -105,6 +109,9 @@ struct ikv_ctx : Scratch {
   cudaStream_t lane_stream[IKV_MAX_LANES] = {};
   cudaEvent_t lane_ev[IKV_MAX_LANES][3] = {};  // small -> key, key -> small, join
   cudaEvent_t fork_ev = nullptr;
+
+  unsigned char* static_scratch = nullptr;  // device address of g_static_scratch on this context's device
+  std::string static_scratch_err;           // why it could not be resolved
 
   // multi-row scorer on tcgen05 (score_rows_tc.cuh)
   int rows_tc = 1;           // IKV_TUNE_ROWS_TC
@@ -1088,6 +1095,13 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
     ikv_destroy(c);
     return IKV_ERR_CUDA;
   }
+  {  // ikv_decode_attn_static: the static array's device address, once per context, with its device current
+    void* sp = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&sp, g_static_scratch);
+    if (e == cudaSuccess) c->static_scratch = (unsigned char*)sp;
+    else c->static_scratch_err = cudaGetErrorString(e);
+    cudaGetLastError();
+  }
   *out = c;
   return IKV_OK;
 }
@@ -1654,6 +1668,63 @@ ikv_status ikv_decode_attn(ikv_ctx* c, int32_t layer, const ikv_request* reqs, i
                         (char*)out + (size_t)r0 * Hq * D * esz, sm_scale, st, c->use_pdl && !fresh));
   }
   return IKV_OK;
+}
+
+ikv_status ikv_decode_attn_static(ikv_ctx* c, int32_t layer, const ikv_request* req, const void* q, void* out,
+                                  float sm_scale, void* stream) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (!req || !q || !out) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_decode_attn_static: NULL argument");
+  if (layer < 0 || layer >= c->cfg.n_layers) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "layer %d out of range", layer);
+  if (req->seq_len < 0 || (req->seq_len > 0 && !req->slot_map)) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "bad request");
+  if (!c->static_scratch)
+    IKV_FAIL(c, IKV_ERR_CUDA, "ikv_decode_attn_static: cudaGetSymbolAddress failed in ikv_create: %s",
+             c->static_scratch_err.c_str());
+  cudaStream_t st = (cudaStream_t)stream;
+  const int Hq = c->cfg.n_q_heads, Hkv = c->cfg.n_kv_heads, D = c->cfg.head_dim;
+  const int items = req->seq_len;
+  // split plan of ikv_decode_attn for one request
+  int n_split;
+  if (c->cfg.kv_dtype == IKV_BF16) {
+    const int n_hg = (Hkv + DM_CWARPS - 1) / DM_CWARPS;
+    int reserve = (Hq + 1) / 2;
+    if (reserve > c->n_sm / 4) reserve = c->n_sm / 4;
+    n_split = (c->n_sm - reserve) / n_hg;
+    const int by_len = (items + 15) / 16;
+    if (n_split > by_len) n_split = by_len;
+  } else {
+    n_split = (4 * c->n_sm + Hkv - 1) / Hkv;
+    const int by_len = (items + 63) / 64;
+    if (n_split > by_len) n_split = by_len;
+  }
+  if (n_split < 1) n_split = 1;
+  if (n_split > DMG_MAX_SPLIT) n_split = DMG_MAX_SPLIT;
+  const size_t o_bytes = (size_t)Hq * n_split * D * sizeof(float), ml_bytes = (size_t)Hq * n_split * sizeof(float2);
+  const size_t need = 256 + o_bytes + ml_bytes;
+  if (need > (size_t)IKV_STATIC_SCRATCH_BYTES)
+    IKV_FAIL(c, IKV_ERR_CAPACITY,
+             "ikv_decode_attn_static: %d query heads x %d splits x head_dim %d need %zu bytes of partials, the static "
+             "scratch holds %d (use ikv_decode_attn)", Hq, n_split, D, need, (int)IKV_STATIC_SCRATCH_BYTES);
+  // the array keeps the previous call's contents: the list length must read zero; the partials are overwritten
+  CU(c, cudaMemsetAsync(c->static_scratch, 0, 256, st));
+  DecBatch batch;
+  memset(&batch, 0, sizeof batch);
+  batch.r[0].S = req->slot_map;
+  batch.r[0].live_slots = reinterpret_cast<const int32_t*>(c->static_scratch);  // empty list: never indexed
+  batch.r[0].n_live = reinterpret_cast<const int32_t*>(c->static_scratch);
+  batch.r[0].seq_len = req->seq_len;
+  batch.r[0].covered = 0;       // every position comes from the slot map
+  batch.r[0].n_items = 0;
+  batch.r[0].flags = req->flags & IKV_REQ_INPUTS_COMPLETE;
+  batch.r[0].n_split = n_split;
+  // the kernels take their scratch from the context: lend them the static array for this launch
+  float* po = c->part_o;
+  float2* pm = c->part_ml;
+  c->part_o = reinterpret_cast<float*>(c->static_scratch + 256);
+  c->part_ml = reinterpret_cast<float2*>(c->static_scratch + 256 + o_bytes);
+  const ikv_status rc = dispatch_decode(c, layer, batch, 1, n_split, q, out, sm_scale, st, false);
+  c->part_o = po;
+  c->part_ml = pm;
+  return rc;
 }
 
 ikv_status ikv_prune_host(ikv_ctx* c, const ikv_request* req, const void* q_rows_host, int32_t n_rows, int32_t q_dtype,

@@ -33,7 +33,7 @@ PROF_NAMES = ["key_pass", "decode_split", "memory_update", "partition", "mem_pre
 EXPORTS = ["ikv_create", "ikv_destroy", "ikv_last_error", "ikv_reserve", "ikv_session_open", "ikv_session_fork",
            "ikv_session_close", "ikv_session_get_memory", "ikv_session_set_memory", "ikv_residual_load",
            "ikv_memory_update", "ikv_score", "ikv_select_evict", "ikv_decode_attn", "ikv_prune_host",
-           "ikv_score_rows", "ikv_score_baseline", "ikv_prefill_attn", "ikv_profile_enable", "ikv_profile_read", "ikv_tune", "ikv_test_late_writer", "ikv_version"]
+           "ikv_score_rows", "ikv_score_baseline", "ikv_prefill_attn", "ikv_decode_attn_static", "ikv_profile_enable", "ikv_profile_read", "ikv_tune", "ikv_test_late_writer", "ikv_version"]
 
 
 class Config(C.Structure):
@@ -76,6 +76,8 @@ _lib.ikv_select_evict.argtypes = [C.c_void_p, C.POINTER(Request), C.c_int32, C.c
                                   C.c_void_p, C.c_void_p]
 _lib.ikv_decode_attn.argtypes = [C.c_void_p, C.c_int32, C.POINTER(Request), C.c_int32, C.c_void_p, C.c_void_p,
                                  C.c_float, C.c_void_p]
+_lib.ikv_decode_attn_static.argtypes = [C.c_void_p, C.c_int32, C.POINTER(Request), C.c_void_p, C.c_void_p, C.c_float,
+                                        C.c_void_p]
 _lib.ikv_tune.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
 _lib.ikv_test_late_writer.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p]
 _lib.ikv_profile_enable.argtypes = [C.c_void_p, C.c_int32]
@@ -90,6 +92,7 @@ class Baseline(C.Structure):
 
 
 BASE_STREAMING, BASE_SNAPKV, BASE_H2O = 1, 2, 3
+STATIC_SCRATCH_BYTES = 3 * 1024 * 1024
 _lib.ikv_score_rows.argtypes = [C.c_void_p, C.POINTER(Request), C.c_int32, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p,
                                 C.c_void_p]
 _lib.ikv_score_baseline.argtypes = [C.c_void_p, C.POINTER(Request), C.c_int32, C.POINTER(Baseline), C.c_void_p, C.c_void_p]
@@ -216,6 +219,11 @@ class Context:
     def decode_attn(self, layer, reqs, q, out, sm_scale, stream=None):
         self._chk(_lib.ikv_decode_attn(self._h, layer, _req_array(reqs), len(reqs), _ptr(q), _ptr(out),
                                        C.c_float(sm_scale), _stream(stream)))
+
+    def decode_attn_static(self, layer, req, q, out, sm_scale, stream=None):
+        """One request, no session, no allocation: split partials in the library's static device array."""
+        self._chk(_lib.ikv_decode_attn_static(self._h, layer, C.byref(req), _ptr(q), _ptr(out), C.c_float(sm_scale),
+                                              _stream(stream)))
 
     @staticmethod
     def test_late_writer(dst, src, delay_us, stream=None):
