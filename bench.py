@@ -384,6 +384,8 @@ def run_cfg2(args, dev, hbm_peak):
                        "92,160 live tokens, M=256, C=8192", "mode": "learnable", "prune_ms": prune_ms,
            "tokens_per_s": T / (prune_ms * 1e-3), "key_pass_ms": key_ms, "key_pass_gbs": key_bytes / (key_ms * 1e-3) / 1e9,
            "key_pass_frac_of_measured_peak": key_bytes / (key_ms * 1e-3) / 1e9 / hbm_peak,
+           # 92k tokens exceed the on-chip capacity of the layer-major kernel: k_key_pass also writes L*Hq*T fp32 logits
+           "key_pass_traffic_frac_of_measured_peak": (key_bytes + shape.L * shape.Hq * T * 4) / (key_ms * 1e-3) / 1e9 / hbm_peak,
            "prune_frac_of_measured_peak": key_bytes / (prune_ms * 1e-3) / 1e9 / hbm_peak, "n_kept": n_kept,
            "decode_ms_per_step": dec_ms, "decode_kv_gbs": dec_bytes / (dec_ms * 1e-3) / 1e9,
            "decode_frac_of_measured_peak": dec_bytes / (dec_ms * 1e-3) / 1e9 / hbm_peak,

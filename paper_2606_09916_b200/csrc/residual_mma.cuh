@@ -103,6 +103,21 @@ struct FoldOut {
 
 // Folds mbar into W_Q and fc1 (see the header of this file).  Blocks of 128 threads; resid_fold_grid() blocks cover
 // D/16*16*32 W_Q fragment items, 256*D/8 canonical fc1 rows and 384 bias warps.
+// sum over the partial rows part[b][d], b ascending (the order is part of the result); eight loads in flight
+__device__ __forceinline__ float sum_parts(const float* __restrict__ part, int n_part, int D, int d) {
+  float acc = 0.f;
+  int b = 0;
+  for (; b + 8 <= n_part; b += 8) {
+    float v[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) v[j] = part[(b + j) * D + d];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc += v[j];
+  }
+  for (; b < n_part; ++b) acc += part[b * D + d];
+  return acc;
+}
+
 template <int D>
 __device__ __forceinline__ void resid_fold_block(int bid, const float* __restrict__ part, int n_part, int LH,
                                                  const ResidW& w, const FoldOut& o) {
@@ -110,8 +125,7 @@ __device__ __forceinline__ void resid_fold_block(int bid, const float* __restric
   constexpr int N_WQ = KS * 16 * 32, N_W1 = R_HID * (D / 8), N_B = R_DC + R_HID;
   __shared__ float mb[D];
   for (int d = threadIdx.x; d < D; d += 128) {
-    float acc = 0.f;
-    for (int b = 0; b < n_part; ++b) acc += part[b * D + d];
+    const float acc = sum_parts(part, n_part, D, d);
     mb[d] = acc / (float)LH;
   }
   __syncthreads();

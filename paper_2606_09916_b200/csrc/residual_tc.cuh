@@ -65,8 +65,7 @@ __device__ __forceinline__ void rt_fold_fc1_block(int bid, const float* __restri
   constexpr int N_W1 = R_HID * (D / 8);
   __shared__ float mb[D];
   for (int d = threadIdx.x; d < D; d += 128) {
-    float acc = 0.f;
-    for (int b = 0; b < n_part; ++b) acc += part[b * D + d];
+    const float acc = sum_parts(part, n_part, D, d);
     mb[d] = acc / (float)LH;
   }
   __syncthreads();
@@ -124,8 +123,7 @@ __device__ __forceinline__ void rt_fold_xattn_block(int bid, const float* __rest
       v[j] = __ldg(reinterpret_cast<const float4*>(src + d * R_DC) + (tid & 7));
     }
     for (int d = tid; d < D; d += 256) {
-      float acc = 0.f;
-      for (int b = 0; b < n_part; ++b) acc += part[b * D + d];
+      const float acc = sum_parts(part, n_part, D, d);
       mb[d] = acc / (float)LH;
     }
     for (int i = tid; i < 16 * D; i += 256) {

@@ -25,11 +25,20 @@ constexpr int KP_TOK = 32;       // tokens per stage = two m16 tiles of the mma
 constexpr int KP_LWARPS = 8;     // logit warps
 constexpr int KP_KWARPS = 4;     // mean-key warps
 // G <= 4: a producer warp of its own (13 warps, 128 registers per thread).  G > 4 with mean keys: the two-tile B
-// fragments need more registers than a 13-warp CTA leaves, so the first mean-key warp also produces (12 warps, 170
-// registers); measured at configs[2]: 2.38 -> 1.98 ms.  (At G = 4 the shared producer costs 20 %: it refills a slot only
-// between its own stages.)
-__host__ __device__ constexpr bool kp_merged(int G, bool kbar) { return kbar && G > 4; }
-__host__ __device__ constexpr int kp_threads(int G, bool kbar) { return (KP_LWARPS + KP_KWARPS + (kp_merged(G, kbar) ? 0 : 1)) * 32; }
+// fragments need ~170 registers in the logit warps, more than a 13-warp CTA leaves.  Round 1 let the first mean-key
+// warp also produce (12 warps; -DIKV_KP_MERGED=1 still builds it); now the CTA has four whole warpgroups and the logit
+// warps take registers from the others with setmaxnreg (configs[2]: 2.00 -> 1.96 ms).
+#ifndef IKV_KP_MERGED
+#define IKV_KP_MERGED 0
+#endif
+__host__ __device__ constexpr bool kp_merged(int G, bool kbar) { return IKV_KP_MERGED && kbar && G > 4; }
+// G > 4 with mean keys, not merged: four whole warpgroups (logit | logit | mean-key | producer + three idle warps), so
+// that setmaxnreg can move registers from the last two to the logit warps (KP_REG_*)
+__host__ __device__ constexpr bool kp_regsplit(int G, bool kbar) { return !IKV_KP_MERGED && kbar && G > 4; }
+__host__ __device__ constexpr int kp_threads(int G, bool kbar) {
+  return kp_regsplit(G, kbar) ? 512 : (KP_LWARPS + KP_KWARPS + (kp_merged(G, kbar) ? 0 : 1)) * 32;
+}
+constexpr int KP_REG_LOGIT = 184, KP_REG_OTHER = 72;   // 256 x 184 + 256 x 72 = 65,536 registers
 constexpr int KP_ROWPAD = 64;    // bytes added to each staged token row (bank spread for the 16-byte reads)
 
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
@@ -135,6 +144,10 @@ __global__ __launch_bounds__(kp_threads(G, KBAR), 1) void k_key_pass(const KeyPa
 
   const uint64_t pol_keys = l2_policy_evict_first();  // keys are read exactly once per pass
   const uint64_t pol_logits = l2_policy_evict_last();  // the rule kernel re-reads the logits scratch
+  if constexpr (kp_regsplit(G, KBAR)) {
+    if (warp < KP_LWARPS) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(KP_REG_LOGIT));
+    else asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(KP_REG_OTHER));
+  }
   if (!MERGED && warp == KP_LWARPS + KP_KWARPS) {
     // ------------------------------------------------------------------ producer (a warp of its own)
     int s = 0;
