@@ -334,20 +334,27 @@ def run_next(rig, hbm_peak):
         rig.prune()
     st.synchronize()
     n_kept = int(rig.nk.item())
-    n_q = 64
-    q = torch.randn((n_q, Hq, D), generator=gen).to(torch.bfloat16).to(dev)
-    out = torch.empty_like(q)
-    reads = torch.zeros(2, dtype=torch.int64, device=dev)
-    r = ikv.make_request(rig.sid, rig.S_dev, T + n_q, rig.sess.pi, rig.sess.qs, rig.sess.qe, rig.C, rig.sess.pi)
-    n_rep = 4
-    ms = timed(lambda: ctx.prefill_attn(0, r, T, q, out, rig.scale, reads, st), n=n_rep - 1)
-    raw, eff = [int(x) // n_rep for x in reads.cpu().tolist()]
-    kv_bytes = (n_kept + n_q) * Hkv * D * 2 * shape.elem_bytes          # the survivors' K and V rows, read once per chunk
-    roof = kv_bytes / (hbm_peak * 1e9) * 1e3
-    res["prefill_chunk"] = {"n_q": n_q, "layer_calls": 1, "live_tokens": n_kept, "ms": ms, "roofline_ms": roof,
-                            "frac_of_roofline": roof / ms, "raw_kv_reads": raw, "effective_kv_reads": eff,
-                            "what": "ikv_prefill_attn: the decode kernels row by row (32 rows per launch), K/V re-read "
-                                    "from L2 for every row; counters per PAPER.md:163-175"}
+    for n_q in (64, 2048):
+        q = torch.randn((n_q, Hq, D), generator=gen).to(torch.bfloat16).to(dev)
+        out = torch.empty_like(q)
+        reads = torch.zeros(2, dtype=torch.int64, device=dev)
+        S_map = rig.S_dev
+        if T + n_q > S_map.numel():   # the workload's map ends 256 positions after T: the new positions reuse live slots
+            head_map = rig.S_dev[:T]
+            S_map = torch.cat([head_map, head_map[head_map != rig.w.dead_slot][:n_q]]).contiguous()
+        r = ikv.make_request(rig.sid, S_map, T + n_q, rig.sess.pi, rig.sess.qs, rig.sess.qe, rig.C, rig.sess.pi)
+        n_rep = 4
+        ms = timed(lambda: ctx.prefill_attn(0, r, T, q, out, rig.scale, reads, st), n=n_rep - 1)
+        raw, eff = [int(x) // n_rep for x in reads.cpu().tolist()]
+        kv_bytes = (n_kept + n_q) * Hkv * D * 2 * shape.elem_bytes      # the survivors' K and V rows, read once per chunk
+        flops = 2 * 2.0 * Hq * D * eff                                  # QK^T and PV over the (row, visible item) pairs
+        hbm_t, mma_t = kv_bytes / (hbm_peak * 1e9) * 1e3, flops / tensor_peak * 1e3
+        roof = max(hbm_t, mma_t)
+        res[f"prefill_chunk_{n_q}"] = {"n_q": n_q, "layer_calls": 1, "live_tokens": n_kept, "ms": ms, "roofline_ms": roof,
+                                       "bound": "hbm" if hbm_t >= mma_t else "tensor (bf16 peak; the kernel is mma.sync)",
+                                       "frac_of_roofline": roof / ms, "raw_kv_reads": raw, "effective_kv_reads": eff,
+                                       "what": "ikv_prefill_attn, tiled kernel: 32 query rows per CTA share each K/V tile; "
+                                               "counters per PAPER.md:163-175"}
     return res
 
 

@@ -22,6 +22,7 @@
 #include "score_mma.cuh"
 #include "score_lm.cuh"
 #include "score_rows_tc.cuh"
+#include "prefill_mma.cuh"
 #include "select.cuh"
 #include "select_cluster.cuh"
 #include "fused_small.cuh"
@@ -113,6 +114,8 @@ struct ikv_ctx : Scratch {
   unsigned char* static_scratch = nullptr;  // device address of g_static_scratch on this context's device
   std::string static_scratch_err;           // why it could not be resolved
 
+  bool pf_attr_done[2][9] = {};
+  int prefill_tiled = 1;     // IKV_TUNE_PREFILL_TILED: 0 = ikv_prefill_attn row by row through the decode kernels
   // multi-row scorer on tcgen05 (score_rows_tc.cuh)
   int rows_tc = 1;           // IKV_TUNE_ROWS_TC
   unsigned char* rows_bank = nullptr;
@@ -301,12 +304,14 @@ __global__ __launch_bounds__(1024) void k_h2o_boost(const int32_t* __restrict__ 
   }
 }
 // KV-read counters of a prefill chunk: raw += sum (pos_i + 1), eff += sum #live positions <= pos_i.
+// n_live (may be NULL) = number of live positions in [0, covered), covered <= q_pos0: only the gap is scanned.
 __global__ __launch_bounds__(1024) void k_prefill_reads(const int32_t* __restrict__ S, int32_t dead, int q_pos0, int n_q,
-                                                        unsigned long long* __restrict__ reads) {
+                                                        unsigned long long* __restrict__ reads,
+                                                        const int32_t* __restrict__ n_live, int covered) {
   __shared__ int warp_tot[32];
   // live positions in [0, q_pos0) are common to every row; then an inclusive count along the chunk
-  int base = 0;
-  for (int j0 = 0; j0 < q_pos0; j0 += 1024) {
+  int base = n_live ? *n_live : 0;
+  for (int j0 = n_live ? covered : 0; j0 < q_pos0; j0 += 1024) {
     const int j = j0 + threadIdx.x;
     int tot;
     block_excl_scan_1024((j < q_pos0 && S[j] != dead) ? 1 : 0, warp_tot, &tot);
@@ -924,6 +929,75 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   return IKV_OK;
 }
 
+template <int D, int G>
+ikv_status launch_prefill(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaStream_t st) {
+  auto fn = k_prefill_mma<D, G>;
+  if (!c->pf_attr_done[D == 128][G]) {
+    CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pf_smem<D>()));
+    c->pf_attr_done[D == 128][G] = true;
+  }
+  fn<<<dim3(p.n_split, p.Hkv, (p.n_q + PF_BR - 1) / PF_BR), 64 * G, pf_smem<D>(), st>>>(p);
+  LAUNCH_CHECK(c);
+  k_prefill_merge<D><<<dim3(p.Hkv * G, p.n_q), D, 0, st>>>(p.part_o, p.part_ml, p.n_split, out);
+  LAUNCH_CHECK(c);
+  return IKV_OK;
+}
+template <int D>
+ikv_status dispatch_prefill(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaStream_t st) {
+  switch (c->G) {
+    case 1: return launch_prefill<D, 1>(c, p, out, st);
+    case 2: return launch_prefill<D, 2>(c, p, out, st);
+    case 4: return launch_prefill<D, 4>(c, p, out, st);
+    case 5: return launch_prefill<D, 5>(c, p, out, st);
+    case 8: return launch_prefill<D, 8>(c, p, out, st);
+  }
+  IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "GQA group size %d not supported (1,2,4,5,8)", c->G);
+}
+
+// The tiled kernel (prefill_mma.cuh).  The session's survivor list is made to cover a prefix [0, covered) with
+// covered <= q_pos0 (rebuilt for [0, q_pos0) when it is stale, reaches into the chunk, or lags it by more than 4,096
+// positions); the rest of the positions come from the slot map.  Chunks of more than 1,024 rows go in groups of 1,024
+// (bounds the partials).
+ikv_status prefill_tiled(ikv_ctx* c, int layer, const ikv_request& r, int q_pos0, int n_q, const bf16* q, bf16* out,
+                         float sm_scale, cudaStream_t st) {
+  Session* s = session_find(c, r.session_id);
+  if (!s) IKV_FAIL(c, IKV_ERR_NO_SESSION, "session %llu does not exist", (unsigned long long)r.session_id);
+  const int Hq = c->cfg.n_q_heads, Hkv = c->cfg.n_kv_heads, D = c->cfg.head_dim;
+  const bool stale = (r.flags & IKV_REQ_RESCAN) || s->map_ptr != r.slot_map || s->map_epoch != r.map_epoch ||
+                     s->covered > q_pos0 || (q_pos0 - s->covered) > 4096;
+  if (stale) {
+    TRY(session_live_reserve(c, *s, q_pos0 > 0 ? q_pos0 : 1));
+    k_build_live<<<1, 1024, 0, st>>>(r.slot_map, q_pos0, c->cfg.dead_slot, s->live_slots, s->d_n_live);
+    LAUNCH_CHECK(c);
+    s->covered = q_pos0;
+    s->map_ptr = r.slot_map;
+    s->map_epoch = r.map_epoch;
+    s->live_ub = q_pos0;
+    s->list_fresh = true;
+  }
+  PrefillParams p;
+  p.k_layer = (const bf16*)c->cfg.k_pool + (int64_t)layer * c->layer_stride;
+  p.v_layer = (const bf16*)c->cfg.v_pool + (int64_t)layer * c->layer_stride;
+  p.Hkv = Hkv; p.dead = c->cfg.dead_slot; p.S = r.slot_map; p.live_slots = s->live_slots;
+  p.n_live = s->d_n_live; p.n_cached = s->live_ub; p.covered = s->covered;
+  p.scale_log2 = sm_scale * 1.4426950408889634f;
+  for (int g0 = 0; g0 < n_q; g0 += 1024) {
+    const int ng = std::min(1024, n_q - g0);
+    p.q_pos0 = q_pos0 + g0; p.n_q = ng;
+    p.q = q + (size_t)g0 * Hq * D;
+    const int rbs = (ng + PF_BR - 1) / PF_BR;
+    const int tiles = (p.n_cached + (p.q_pos0 + ng - p.covered) + PF_TOK - 1) / PF_TOK;   // upper bound
+    int ns = c->n_sm / (Hkv * rbs);   // one wave: the kernel's registers leave room for one CTA per SM
+    ns = std::max(1, std::min(std::min(ns, tiles), 32));
+    p.n_split = ns;
+    TRY(ensure_parts(c, (int64_t)ng * Hq * ns));
+    p.part_o = c->part_o; p.part_ml = c->part_ml;
+    TRY(D == 128 ? dispatch_prefill<128>(c, p, out + (size_t)g0 * Hq * D, st)
+                 : dispatch_prefill<64>(c, p, out + (size_t)g0 * Hq * D, st));
+  }
+  return IKV_OK;
+}
+
 // NEXT-1 on tcgen05 (score_rows_tc.cuh): banks of 128 / G rows, two sweeps over the keys per bank.
 template <int D>
 ikv_status score_rows_tc(ikv_ctx* c, const ikv_request& r, const float* rows, int n_rows, const float* weights,
@@ -1136,6 +1210,7 @@ ikv_status ikv_tune(ikv_ctx* c, int32_t knob, int32_t value) {
     case IKV_TUNE_RESID_TC: c->resid_tc = value; return IKV_OK;
     case IKV_TUNE_LAYER_MAJOR: c->use_lm = value; return IKV_OK;
     case IKV_TUNE_ROWS_TC: c->rows_tc = value; return IKV_OK;
+    case IKV_TUNE_PREFILL_TILED: c->prefill_tiled = value; return IKV_OK;
     case IKV_TUNE_BATCH_LANES:
       c->n_lanes = value < 1 ? 1 : (value > IKV_MAX_LANES ? IKV_MAX_LANES : value);
       return IKV_OK;
@@ -1536,6 +1611,19 @@ ikv_status ikv_prefill_attn(ikv_ctx* c, int32_t layer, const ikv_request* req, i
   // Row i is a decode query at position q_pos0 + i: causal = its request ends at seq_len_i = q_pos0 + i + 1.  The rows of
   // a launch share the session's survivor list and read the chunk's own positions from the slot map; the K/V rows of the
   // request are re-read by every row out of L2 (33.5 MB per layer at 8,192 survivors).
+  if (c->prefill_tiled && c->cfg.kv_dtype == IKV_BF16) {
+    if (req->seq_len < 0 || !req->slot_map) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "bad request");
+    if (layer < 0 || layer >= c->cfg.n_layers) IKV_FAIL(c, IKV_ERR_INVALID_ARG, "layer %d out of range", layer);
+    TRY(prefill_tiled(c, layer, *req, q_pos0, n_q, (const bf16*)q, (bf16*)out, sm_scale, (cudaStream_t)stream));
+    if (kv_reads) {  // the session's list now covers [0, covered), covered <= q_pos0: its length is the count up to there
+      const Session* s = session_find(c, req->session_id);
+      k_prefill_reads<<<1, 1024, 0, (cudaStream_t)stream>>>(req->slot_map, c->cfg.dead_slot, q_pos0, n_q,
+                                                            reinterpret_cast<unsigned long long*>(kv_reads),
+                                                            s->d_n_live, s->covered);
+      LAUNCH_CHECK(c);
+    }
+    return IKV_OK;
+  }
   ikv_request rr[DEC_MAX_REQ];
   for (int i0 = 0; i0 < n_q; i0 += DEC_MAX_REQ) {
     const int nb = (n_q - i0 < DEC_MAX_REQ) ? n_q - i0 : DEC_MAX_REQ;
@@ -1547,7 +1635,7 @@ ikv_status ikv_prefill_attn(ikv_ctx* c, int32_t layer, const ikv_request* req, i
   }
   if (kv_reads) {
     k_prefill_reads<<<1, 1024, 0, (cudaStream_t)stream>>>(req->slot_map, c->cfg.dead_slot, q_pos0, n_q,
-                                                          reinterpret_cast<unsigned long long*>(kv_reads));
+                                                          reinterpret_cast<unsigned long long*>(kv_reads), nullptr, 0);
     LAUNCH_CHECK(c);
   }
   return IKV_OK;

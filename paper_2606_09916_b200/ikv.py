@@ -25,7 +25,7 @@ MODE_MEMORY, MODE_LEARNABLE, MODE_QUERY = 0, 1, 2
 FLAG_NO_XATTN, FLAG_NO_RESIDUAL = 0x100, 0x200
 REQ_RESCAN, REQ_INPUTS_COMPLETE = 1, 2
 CFG_NO_PDL, CFG_NO_PDL_PRUNE = 1, 2
-TUNE_L2_HINTS, TUNE_RESID_TC, TUNE_LAYER_MAJOR, TUNE_BATCH_LANES, TUNE_ROWS_TC = 1, 2, 3, 4, 5
+TUNE_L2_HINTS, TUNE_RESID_TC, TUNE_LAYER_MAJOR, TUNE_BATCH_LANES, TUNE_ROWS_TC, TUNE_PREFILL_TILED = 1, 2, 3, 4, 5, 6
 PROF_SLOTS = 12
 PROF_NAMES = ["key_pass", "decode_split", "memory_update", "partition", "mem_prep", "post_key", "rule_fold", "residual",
               "select_evict", "decode_merge"]
