@@ -403,12 +403,12 @@ def run_cfg2(args, dev, hbm_peak):
 
 
 def run_cfg4(args, dev, hbm_peak):
-    """configs[4] (64 concurrent sessions, lognormal lengths, budgets {4096, 8192, 16384}) as a sub-object, on L_res = 8
-    resident layers (all 36 layers of K+V of 1.2 M tokens are ~180 GB: they do not fit beside anything else).  Batched
+    """configs[4] (64 concurrent sessions, lognormal lengths, budgets {4096, 8192, 16384}) as a sub-object, on L_res = 24
+    resident layers (all 36 layers of K+V of 1.12 M tokens are 165 GB: they do not fit beside anything else).  Batched
     score / select / evict, then batched decode, all through the C-ABI with n_req = 64."""
     import torch
     from paper_2606_09916_b200 import ikv, workloads as wl
-    L_RES = 8
+    L_RES = 24      # K+V of 1.12 M tokens: 4.6 GB per layer; 24 layers = 110 GB of the 180 GB
     shape = wl.ModelShape(L_RES, 32, 8, 128)
     w = wl.batched(device="cuda", shape=shape, decode_tokens=1)
     ctx = ikv.Context(shape.L, shape.Hq, shape.Hkv, shape.D, w.k_pool, w.v_pool, dead_slot=w.dead_slot)
