@@ -1043,7 +1043,7 @@ ikv_status score_rows_tc(ikv_ctx* c, const ikv_request& r, const float* rows, in
     p.accumulate = r0 > 0 ? 1 : 0;
     k_rows_prep<D><<<n_items, 256, 0, st>>>(rows + r0 * row_elems, nr, L, Hkv, G, wts, c->rows_bank);
     k_rows_pass<D, 1><<<grid, RB_THREADS, rb_smem(D), st>>>(p);
-    k_rows_lse<D><<<n_items, RB_ROWS, 0, st>>>(c->rows_partials, n_slots, c->rows_bank);
+    k_rows_lse<D><<<n_items, 1024, 0, st>>>(c->rows_partials, n_slots, c->rows_bank);
     k_rows_pass<D, 2><<<grid, RB_THREADS, rb_smem(D), st>>>(p);
     LAUNCH_CHECK(c);
   }

@@ -59,21 +59,29 @@ __global__ void k_rows_prep(const float* __restrict__ rows, int n_rows, int L, i
   for (int c = threadIdx.x; c < RB_ROWS; c += blockDim.x) { tail[c] = 0.f; tail[RB_ROWS + c] = wts.w[c]; }
 }
 
-// lse[item, c] = log2 sum 2^x over all candidates, from the partials of sweep 1 (slots in fixed order: deterministic)
+// lse[item, c] = log2 sum 2^x over all candidates, from the partials of sweep 1.  Block = item, 1,024 threads: thread
+// (c, sg) folds the slots sg, sg + 8, ... in ascending order, the eight folds are combined in sg order (deterministic).
 template <int D>
-__global__ void k_rows_lse(const float2* __restrict__ partials, int n_slots, unsigned char* __restrict__ bank) {
-  const int item = blockIdx.x, c = threadIdx.x;
+__global__ __launch_bounds__(1024) void k_rows_lse(const float2* __restrict__ partials, int n_slots,
+                                                   unsigned char* __restrict__ bank) {
+  __shared__ float2 part_s[8][RB_ROWS];
+  const int item = blockIdx.x, c = threadIdx.x & (RB_ROWS - 1), sg = threadIdx.x >> 7;
   const float2* p = partials + (size_t)item * n_slots * RB_ROWS + c;
   float m = -CUDART_INF_F, s = 0.f;
-  for (int j = 0; j < n_slots; ++j) {
-    const float2 v = p[(size_t)j * RB_ROWS];
+  auto fold = [&](float2 v) {
     if (v.y > 0.f) {
       const float mn = fmaxf(m, v.x);
       s = s * exp2f(m - mn) + v.y * exp2f(v.x - mn);
       m = mn;
     }
+  };
+  for (int j = sg; j < n_slots; j += 8) fold(p[(size_t)j * RB_ROWS]);
+  part_s[sg][c] = make_float2(m, s);
+  __syncthreads();
+  if (sg == 0) {
+    for (int k = 1; k < 8; ++k) fold(part_s[k][c]);
+    reinterpret_cast<float*>(bank + (size_t)item * rb_item(D) + 2 * rb_part(D))[c] = m + log2f(s);  // no candidates: unused
   }
-  reinterpret_cast<float*>(bank + (size_t)item * rb_item(D) + 2 * rb_part(D))[c] = m + log2f(s);  // no candidates: unused
 }
 
 struct RowsPassParams {
