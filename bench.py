@@ -351,10 +351,10 @@ def run_next(rig, hbm_peak):
         hbm_t, mma_t = kv_bytes / (hbm_peak * 1e9) * 1e3, flops / tensor_peak * 1e3
         roof = max(hbm_t, mma_t)
         res[f"prefill_chunk_{n_q}"] = {"n_q": n_q, "layer_calls": 1, "live_tokens": n_kept, "ms": ms, "roofline_ms": roof,
-                                       "bound": "hbm" if hbm_t >= mma_t else "tensor (bf16 peak; the kernel is mma.sync)",
+                                       "bound": "hbm" if hbm_t >= mma_t else "tensor",
                                        "frac_of_roofline": roof / ms, "raw_kv_reads": raw, "effective_kv_reads": eff,
-                                       "what": "ikv_prefill_attn, tiled kernel: 32 query rows per CTA share each K/V tile; "
-                                               "counters per PAPER.md:163-175"}
+                                       "what": "ikv_prefill_attn on tcgen05 (k_prefill_tc): 128 / G query rows x G heads per CTA "
+                                               "share each gathered K/V tile; counters per PAPER.md:163-175"}
     return res
 
 

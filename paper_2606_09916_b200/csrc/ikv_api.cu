@@ -23,6 +23,7 @@
 #include "score_lm.cuh"
 #include "score_rows_tc.cuh"
 #include "prefill_mma.cuh"
+#include "prefill_tc.cuh"
 #include "select.cuh"
 #include "select_cluster.cuh"
 #include "fused_small.cuh"
@@ -115,6 +116,7 @@ struct ikv_ctx : Scratch {
   std::string static_scratch_err;           // why it could not be resolved
 
   bool pf_attr_done[2][9] = {};
+  bool pt_attr_done[2][9] = {};
   int prefill_tiled = 1;     // IKV_TUNE_PREFILL_TILED: 0 = ikv_prefill_attn row by row through the decode kernels
   // multi-row scorer on tcgen05 (score_rows_tc.cuh)
   int rows_tc = 1;           // IKV_TUNE_ROWS_TC
@@ -945,8 +947,30 @@ ikv_status launch_prefill(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaStr
   LAUNCH_CHECK(c);
   return IKV_OK;
 }
+template <int D, int G>
+ikv_status launch_prefill_tc(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaStream_t st) {
+  auto fn = k_prefill_tc<D, G>;
+  if (!c->pt_attr_done[D == 128][G]) {
+    CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pt_smem<D>()));
+    c->pt_attr_done[D == 128][G] = true;
+  }
+  constexpr int BR = 128 / G;
+  fn<<<dim3(p.n_split, p.Hkv, (p.n_q + BR - 1) / BR), PT_THREADS, pt_smem<D>(), st>>>(p);
+  LAUNCH_CHECK(c);
+  k_prefill_merge<D><<<dim3(p.Hkv * G, p.n_q), D, 0, st>>>(p.part_o, p.part_ml, p.n_split, out);
+  LAUNCH_CHECK(c);
+  return IKV_OK;
+}
 template <int D>
 ikv_status dispatch_prefill(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaStream_t st) {
+  if (c->prefill_tiled == 1) {   // tcgen05 where 128 / G rows x G heads make a 128-row tile
+    switch (c->G) {
+      case 1: return launch_prefill_tc<D, 1>(c, p, out, st);
+      case 2: return launch_prefill_tc<D, 2>(c, p, out, st);
+      case 4: return launch_prefill_tc<D, 4>(c, p, out, st);
+      case 8: return launch_prefill_tc<D, 8>(c, p, out, st);
+    }
+  }
   switch (c->G) {
     case 1: return launch_prefill<D, 1>(c, p, out, st);
     case 2: return launch_prefill<D, 2>(c, p, out, st);
@@ -988,7 +1012,9 @@ ikv_status prefill_tiled(ikv_ctx* c, int layer, const ikv_request& r, int q_pos0
     const int ng = std::min(1024, n_q - g0);
     p.q_pos0 = q_pos0 + g0; p.n_q = ng;
     p.q = q + (size_t)g0 * Hq * D;
-    const int rbs = (ng + PF_BR - 1) / PF_BR;
+    const bool tc = c->prefill_tiled == 1 && c->G != 5;
+    const int br = tc ? 128 / c->G : PF_BR;
+    const int rbs = (ng + br - 1) / br;
     const int tiles = (p.n_cached + (p.q_pos0 + ng - p.covered) + PF_TOK - 1) / PF_TOK;   // upper bound
     int ns = c->n_sm / (Hkv * rbs);   // one wave: the kernel's registers leave room for one CTA per SM
     ns = std::max(1, std::min(std::min(ns, tiles), 32));

@@ -198,8 +198,8 @@ def test_prefill_attention_matches_oracle(ikv, oracle, name, shape):
 
 def test_prefill_tiled_long_chunk_and_row_by_row_agree(ikv, oracle):
     """A 300-row chunk (ten 32-row blocks, the last one ragged) far behind a stale survivor list, dead positions inside
-    the chunk and before it: the tiled kernel agrees with the oracle and with the row-by-row path
-    (IKV_TUNE_PREFILL_TILED = 0); a first chunk at position 0 (empty survivor list) works too."""
+    the chunk and before it: the tcgen05 kernel, the mma.sync tiled kernel (IKV_TUNE_PREFILL_TILED = 2) and the
+    row-by-row path (= 0) all agree with the oracle; a first chunk at position 0 (empty survivor list) works too."""
     shape = wl.ModelShape(2, 8, 2, 128, "bf16")
     w = wl.small(seed=73, shape=shape, n_tokens=2600, budget=700, decode_tokens=320, kv_dtype="bf16")
     kp, vp = gc.to_cuda(w)
@@ -216,7 +216,7 @@ def test_prefill_tiled_long_chunk_and_row_by_row_agree(ikv, oracle):
         q = torch.randn((n_q, shape.Hq, shape.D), generator=torch.Generator().manual_seed(q_pos0 + 1)).to(torch.bfloat16)
         r = gc.request(ikv, s, S_dev, seq_len=q_pos0 + n_q)
         outs = []
-        for tiled in (1, 0):
+        for tiled in (1, 2, 0):      # tcgen05 kernel, mma.sync tiled kernel, row by row
             ctx.tune(ikv.TUNE_PREFILL_TILED, tiled)
             out = torch.full((n_q, shape.Hq, shape.D), float("nan"), dtype=torch.bfloat16, device="cuda")
             reads = torch.zeros(2, dtype=torch.int64, device="cuda")
@@ -224,8 +224,8 @@ def test_prefill_tiled_long_chunk_and_row_by_row_agree(ikv, oracle):
             torch.cuda.synchronize()
             outs.append((out.float().cpu().numpy(), reads.cpu().tolist()))
         want, raw, eff = oracle.prefill(g, kp, vp, layer, S_dev.cpu().numpy(), q_pos0, q.float().numpy(), scale)
-        e1 = gc.assert_decode_close(outs[0][0], want, True, f"tiled prefill at {q_pos0}")
-        e0 = gc.assert_decode_close(outs[1][0], want, True, f"row-by-row prefill at {q_pos0}")
-        assert outs[0][1] == [raw, eff] and outs[1][1] == [raw, eff]
-        print(f"prefill at {q_pos0} x {n_q}: max abs err tiled {e1:.3e}, row by row {e0:.3e}, "
-              f"between them {np.abs(outs[0][0] - outs[1][0]).max():.3e}")
+        e1 = gc.assert_decode_close(outs[0][0], want, True, f"tcgen05 prefill at {q_pos0}")
+        e2 = gc.assert_decode_close(outs[1][0], want, True, f"mma.sync prefill at {q_pos0}")
+        e0 = gc.assert_decode_close(outs[2][0], want, True, f"row-by-row prefill at {q_pos0}")
+        assert outs[0][1] == [raw, eff] and outs[1][1] == [raw, eff] and outs[2][1] == [raw, eff]
+        print(f"prefill at {q_pos0} x {n_q}: max abs err tcgen05 {e1:.3e}, mma.sync {e2:.3e}, row by row {e0:.3e}")
