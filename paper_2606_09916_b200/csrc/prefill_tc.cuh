@@ -19,7 +19,8 @@ namespace ikv {
 
 constexpr int PT_TOK = 64;            // items per tile
 constexpr int PT_THREADS = 9 * 32;    // 4 softmax warps, 4 producer warps, MMA warp
-constexpr int PT_NB = 3;               // K / V^T / staging buffers: the gathers run two tiles ahead of the MMAs
+constexpr int PT_NB = 4;               // K / V^T buffers: the gathers run three tiles ahead of the MMAs
+constexpr int PT_PB = 1;               // P buffers (shared memory: 4 K / V^T buffers leave room for one)
 constexpr float PT_GROW = 8.f;        // log2 units a tile's maximum may exceed the reference before it moves
 
 template <int D>
@@ -27,7 +28,7 @@ __host__ __device__ constexpr int pt_vst() { return D * 2 + 16; }   // staged V 
 template <int D>
 __host__ __device__ constexpr int pt_smem() {
   // Q | K[3] | V^T[3] | V staging[2] | P[2] | minrow[3][64] | barriers
-  return 128 * D * 2 + PT_NB * (PT_TOK * D * 2 + D * PT_TOK * 2) + 2 * PT_TOK * pt_vst<D>() + 2 * 128 * PT_TOK * 2 +
+  return 128 * D * 2 + PT_NB * (PT_TOK * D * 2 + D * PT_TOK * 2) + 2 * PT_TOK * pt_vst<D>() + PT_PB * 128 * PT_TOK * 2 +
          PT_NB * PT_TOK * 4 + 256;
 }
 // canonical K-major (no swizzle) offset of the 16-byte entry (row n, k-group k8) of an operand with kdim elements of K
@@ -57,26 +58,24 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
   unsigned char* vt_s = k_s + PT_NB * KB;        // [3][VTB]
   unsigned char* vst_s = vt_s + PT_NB * VTB;     // [2][VSB]: one per producer group
   unsigned char* p_s = vst_s + 2 * VSB;          // [2][PB]
-  int* minrow_s = reinterpret_cast<int*>(p_s + 2 * PB);   // [3][PT_TOK]
+  int* minrow_s = reinterpret_cast<int*>(p_s + PT_PB * PB);   // [3][PT_TOK]
   uint64_t* bars = reinterpret_cast<uint64_t*>(minrow_s + PT_NB * PT_TOK);
-  uint64_t* kv_full = bars;        // [3] operands K, V^T and minrow of a tile are in shared memory (64 producer threads)
-  uint64_t* kv_free = bars + 3;    // [3] the MMAs that read them have completed
-  uint64_t* s_full = bars + 6;     // [2] S accumulator complete
-  uint64_t* s_free = bars + 8;     // [2] every softmax thread has read it
-  uint64_t* p_full = bars + 10;    // [2] P written (and O rescaled) by every softmax thread
-  uint64_t* p_free = bars + 12;    // [2] P V of the buffer's tile complete
-  uint64_t* q_ready = bars + 14;
-  uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(bars + 15);
+  uint64_t* kv_full = bars;                 // [PT_NB] operands K, V^T and minrow of a tile are in shared memory (64 threads)
+  uint64_t* kv_free = kv_full + PT_NB;      // [PT_NB] the MMAs that read them have completed
+  uint64_t* s_full = kv_free + PT_NB;       // [2] S accumulator complete
+  uint64_t* s_free = s_full + 2;            // [2] every softmax thread has read it
+  uint64_t* p_full = s_free + 2;            // [PT_PB] P written (and O rescaled) by every softmax thread
+  uint64_t* p_free = p_full + PT_PB;        // [PT_PB] P V of the buffer's tile complete
+  uint64_t* q_ready = p_free + PT_PB;
+  uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(q_ready + 1);
 
   const int split = blockIdx.x, kvh = blockIdx.y, rb = blockIdx.z;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int Hq = p.Hkv * G;
   if (threadIdx.x == 0) {
     for (int b = 0; b < PT_NB; ++b) { mbar_init(&kv_full[b], 64); mbar_init(&kv_free[b], 1); }
-    for (int b = 0; b < 2; ++b) {
-      mbar_init(&s_full[b], 1);    mbar_init(&s_free[b], 128);
-      mbar_init(&p_full[b], 128);  mbar_init(&p_free[b], 1);
-    }
+    for (int b = 0; b < 2; ++b) { mbar_init(&s_full[b], 1); mbar_init(&s_free[b], 128); }
+    for (int b = 0; b < PT_PB; ++b) { mbar_init(&p_full[b], 128); mbar_init(&p_free[b], 1); }
     mbar_init(q_ready, 128);
     mbar_fence_init();
   }
@@ -171,16 +170,16 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
       mbar_wait(q_ready, 0u);
       issue_s(0);
       for (int it = 0; it < n_t; ++it) {
-        const int b = it & 1;
         if (it + 1 < n_t) issue_s(it + 1);      // S of the next tile runs under this tile's softmax
-        mbar_wait(&p_full[b], (uint32_t)(it >> 1) & 1u);
+        const int pb = it % PT_PB;
+        mbar_wait(&p_full[pb], (uint32_t)(it / PT_PB) & 1u);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint64_t dp = umma_desc(smem_u32(p_s) + (uint32_t)(b * PB), 128, SBO_T);
+        const uint64_t dp = umma_desc(smem_u32(p_s) + (uint32_t)(pb * PB), 128, SBO_T);
         const uint64_t dv = umma_desc(smem_u32(vt_s) + (uint32_t)((it % PT_NB) * VTB), 128, SBO_T);
 #pragma unroll
         for (int ks = 0; ks < PT_TOK / 16; ++ks)
           umma_bf16(tmem + O_COL, dp + (uint64_t)(ks * 16), dv + (uint64_t)(ks * 16), idesc_o, (it | ks) ? 1u : 0u);
-        umma_commit(&p_free[b]);
+        umma_commit(&p_free[pb]);
         umma_commit(&kv_free[it % PT_NB]);
       }
     }
@@ -230,7 +229,7 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
         const float m_new = grow ? tmax : m_ref;
         const float corr = (m_new == -CUDART_INF_F) ? 1.f : fast_exp2(m_ref - m_new);   // m_ref = -inf: 0
         if (it > 0) {   // O exists from the first P V on; wait for the previous tile's
-          mbar_wait(&p_free[b ^ 1], (uint32_t)((it - 1) >> 1) & 1u);
+          mbar_wait(&p_free[(it - 1) % PT_PB], (uint32_t)((it - 1) / PT_PB) & 1u);
           asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
           for (int c0 = 0; c0 < D; c0 += 32) {
@@ -257,8 +256,9 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
         s0 += x[c]; s1 += x[c + 1];
       }
       l += s0 + s1;
-      mbar_wait(&p_free[b], par ^ 1u);   // P V of tile it - 2 has read this buffer
-      unsigned char* pd = p_s + (size_t)b * PB;
+      const int pb = it % PT_PB;
+      mbar_wait(&p_free[pb], ((uint32_t)(it / PT_PB) & 1u) ^ 1u);   // the P V that read this buffer has completed
+      unsigned char* pd = p_s + (size_t)pb * PB;
 #pragma unroll
       for (int k8 = 0; k8 < PT_TOK / 8; ++k8) {
         const uint4 v = make_uint4(pack2_bf16(x[8 * k8], x[8 * k8 + 1]), pack2_bf16(x[8 * k8 + 2], x[8 * k8 + 3]),
@@ -267,11 +267,11 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-      mbar_arrive(&p_full[b]);
+      mbar_arrive(&p_full[pb]);
     }
     // ---- partials of the split (an empty split writes m = -inf, l = 0: the scratch is not cleared)
     if (n_t > 0) {
-      mbar_wait(&p_free[(n_t - 1) & 1], (uint32_t)((n_t - 1) >> 1) & 1u);
+      mbar_wait(&p_free[(n_t - 1) % PT_PB], (uint32_t)((n_t - 1) / PT_PB) & 1u);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     }
     const int64_t ph = ((int64_t)row * Hq + head) * p.n_split + split;
