@@ -143,7 +143,6 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select
   __shared__ int comb[256];
   __shared__ int warp_tot[32];
   __shared__ int sh_cnt[2];   // |F|, |A| of this CTA
-  __shared__ int sh_eq;       // threshold ties of this CTA
   __shared__ int sh_kf[2];    // kept, freed of this CTA
   __shared__ uint32_t sh_prefix;
   __shared__ int sh_remaining;
@@ -293,12 +292,13 @@ __global__ __cluster_dims__(CL_CTAS, 1, 1) __launch_bounds__(1024) void k_select
   }
   int eq_before = 0;
   {
+    // ties of the lower ranks: their last-pass histograms (pass 0 counted, in bin thr & 255, exactly the keys equal to
+    // the threshold) are complete since that pass' cluster barrier and are not written again -- no barrier of its own
     int tot;
     const int ex = block_excl_scan_1024(__popc(eq_m), warp_tot, &tot);
-    if (tid == 0) sh_eq = tot;
-    cl.sync();
-    int before, total;
-    cluster_offsets(cl, &sh_eq, crank, &before, &total);
+    int before = 0;
+    if (!keep_all && !keep_none)
+      for (int rk = 0; rk < crank; ++rk) before += *cl.map_shared_rank(&hist[0][thr & 255u], rk);
     eq_before = before + ex;
   }
 
