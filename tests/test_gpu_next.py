@@ -229,3 +229,37 @@ def test_prefill_tiled_long_chunk_and_row_by_row_agree(ikv, oracle):
         e0 = gc.assert_decode_close(outs[2][0], want, True, f"row-by-row prefill at {q_pos0}")
         assert outs[0][1] == [raw, eff] and outs[1][1] == [raw, eff] and outs[2][1] == [raw, eff]
         print(f"prefill at {q_pos0} x {n_q}: max abs err tcgen05 {e1:.3e}, mma.sync {e2:.3e}, row by row {e0:.3e}")
+
+
+@pytest.mark.parametrize("name,shape", [("d128g1", wl.ModelShape(2, 2, 2, 128, "bf16")), ("d64g8", wl.ModelShape(2, 16, 2, 64, "bf16")),
+                                        ("d128g8", wl.ModelShape(1, 8, 1, 128, "bf16")), ("d64g4", wl.ModelShape(2, 8, 2, 64, "bf16"))],
+                         ids=["d128g1", "d64g8", "d128g8", "d64g4"])
+def test_prefill_tcgen05_head_layouts(ikv, oracle, name, shape):
+    """k_prefill_tc on the remaining tile shapes (128 rows x 1 head, 16 rows x 8 heads, D = 64): chunks of 1, 33 and 150
+    rows over several splits and tiles (the 150-row chunk lags the survivor list and crosses row blocks), against the
+    oracle and against the mma.sync kernel."""
+    w = wl.small(seed=81, shape=shape, n_tokens=2100, budget=500, decode_tokens=200, kv_dtype="bf16")
+    kp, vp = gc.to_cuda(w)
+    ctx = gc.make_ctx(w)
+    s = w.sessions[0]
+    gc.fold_memory_gpu(ctx, s)
+    g = gc.oracle_geom(oracle, w)
+    full = s.slot_map.clone()
+    rng = np.random.default_rng(9)
+    full[torch.from_numpy(rng.choice(s.N + 200, size=400, replace=False))] = w.dead_slot
+    S_dev = full.cuda()
+    scale = 1.0 / math.sqrt(shape.D)
+    for q_pos0, n_q in ((s.N, 1), (s.N + 1, 33), (s.N + 40, 150)):
+        q = torch.randn((n_q, shape.Hq, shape.D), generator=torch.Generator().manual_seed(q_pos0)).to(torch.bfloat16)
+        r = gc.request(ikv, s, S_dev, seq_len=q_pos0 + n_q)
+        outs = []
+        for tiled in (1, 2):
+            ctx.tune(ikv.TUNE_PREFILL_TILED, tiled)
+            out = torch.full((n_q, shape.Hq, shape.D), float("nan"), dtype=torch.bfloat16, device="cuda")
+            ctx.prefill_attn(shape.L - 1, r, q_pos0, q.cuda(), out, scale)
+            torch.cuda.synchronize()
+            outs.append(out.float().cpu().numpy())
+        want, _, _ = oracle.prefill(g, kp, vp, shape.L - 1, S_dev.cpu().numpy(), q_pos0, q.float().numpy(), scale)
+        e1 = gc.assert_decode_close(outs[0], want, True, f"{name} tcgen05 prefill at {q_pos0} x {n_q}")
+        e2 = gc.assert_decode_close(outs[1], want, True, f"{name} mma.sync prefill at {q_pos0} x {n_q}")
+        print(f"[{name}] prefill at {q_pos0} x {n_q}: max abs err tcgen05 {e1:.3e}, mma.sync {e2:.3e}")
