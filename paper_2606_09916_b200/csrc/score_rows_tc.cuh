@@ -6,17 +6,20 @@
 // Up to 128 / G rows form a BANK: per (layer l, KV head) a 128 x D operand whose row c = r*G + g is row r's query head
 // kvh*G + g (scaled by log2(e)/sqrt(D), split into bf16 hi + lo; rows beyond R*G are zero).  A CTA owns fixed
 // 128-token tiles (two at a time) and walks (layer, KV head) items with the bank of the item resident in shared memory
-// (double-buffered bulk copies); per (item, tile) = sub-item its compute warps gather the tile's keys of that head
+// (double-buffered bulk copies); per (item, tile) = sub-item the gather warps copy the tile's keys of that head
 // through the slot map straight into the canonical K-major operand layout (8-token x 16-byte core matrices, cp.async),
-// and one thread issues 2 * D/16 tcgen05.mma (hi, lo) into a 128-column TMEM accumulator.  Three key buffers and two
-// accumulators: the MMAs of one sub-item run under the statistics of the previous one and the gathers of the next two.
+// and one thread issues 2 * D/16 tcgen05.mma (hi, lo) into a 128-column TMEM accumulator.  Three key buffers and
+// three accumulators: the MMAs of one sub-item run under the statistics of the previous ones and the gathers of the
+// next two.  The gather is the limit: 256-byte pieces of random rows arrive at ~15 bytes per cycle per SM whatever the
+// copy instruction (measured: cp.async 16 B, bulk copies of 256 B), a third of what 2 KB rows reach in the key pass.
 //   sweep 1 (statistics):  D[bank row, token] = bank . keys^T   -- thread = bank row: (max, sum 2^x) over the tile's
 //                          tokens is thread-local; partials per (item, slot) -> k_rows_lse -> lse[item, c].
 //   sweep 2 (sums):        D[token, bank row] = keys . bank^T   -- thread = token: sum_c w_c 2^(x - lse_c) is
 //                          thread-local and accumulates in a register over all items; written to rule_c per tile pair.
 // The same two shared-memory operands serve both sweeps with the A / B roles exchanged (both are K-major, no swizzle).
-// Eight compute warps: warps w and w + 4 own the same 32 TMEM lanes and take half of the accumulator's columns each
-// (the statistics are MUFU-bound: 8 cycles per ex2 warp instruction per SM sub-partition, measured).
+// Sixteen compute warps: warps w, w + 4, w + 8, w + 12 own the same 32 TMEM lanes and take a quarter of the
+// accumulator's columns each (the statistics are MUFU-bound: 8 cycles per ex2 warp instruction per SM sub-partition,
+// measured); eight more warps gather the keys.
 #pragma once
 #include "residual_tc.cuh"
 #include "score_lm.cuh"
@@ -26,9 +29,13 @@ namespace ikv {
 constexpr int RB_ROWS = 128;                 // bank rows = MMA M (sweep 1) / N (sweep 2)
 constexpr int RB_TOK = 128;                  // tokens per tile
 constexpr int RB_TAIL = 1024;                // bytes after the operands: lse[128] | w[128]
-constexpr int RB_CWARPS = 8;                 // compute warps
-constexpr int RB_THREADS = (RB_CWARPS + 2) * 32;  // + the bank loader warp + the MMA issuer warp
+constexpr int RB_CWARPS = 16;                // compute warps
+constexpr int RB_CQ = RB_CWARPS / 4;         // column groups of the accumulator (one warp per lane quarter each)
+constexpr int RB_CG = 128 / RB_CQ;           // columns per group
+constexpr int RB_PWARPS = 8;                 // key gather warps: warp (token quarter, half of the row's chunks)
+constexpr int RB_THREADS = (RB_CWARPS + 2 + RB_PWARPS) * 32;  // + the bank loader warp + the MMA issuer warp
 constexpr int RB_KBUF = 3;                   // key operand buffers
+constexpr int RB_TB = 3;                     // TMEM accumulators (128 columns each; exchange columns behind them)
 __host__ __device__ constexpr int rb_part(int D) { return RB_ROWS * D * 2; }          // bytes of hi (or lo)
 __host__ __device__ constexpr int rb_item(int D) { return 2 * rb_part(D) + RB_TAIL; }  // bank bytes per (l, kvh)
 // canonical K-major offset of the 16-byte entry (row n, 8 consecutive k starting at 8 * k8) of an [rows x D] operand
@@ -91,7 +98,7 @@ struct RowsPassParams {
   const unsigned char* bank;
   const int32_t* cand_slot;
   const int32_t* n_cand;
-  float2* partials;      // sweep 1: [item][slot][128], slot = (pair, cta, tile of the pair, column half)
+  float2* partials;      // sweep 1: [item][slot][128], slot = (pair, cta, tile of the pair, column group)
   int n_slots, n_pairs;
   float* rule_c;         // sweep 2
   int accumulate;        // sweep 2: add to rule_c (second and later banks)
@@ -113,7 +120,8 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// Roles: warps 0-7 gather the keys and take the statistics from TMEM; warp 8 streams the banks; warp 9 issues the MMAs.
+// Roles: warps [0, RB_CWARPS) take the statistics from TMEM; then one warp streams the banks, one issues the MMAs and
+// RB_PWARPS warps gather the keys.
 // Sub-item K = (pair of tiles, item, tile t): key buffer K % 3, TMEM buffer K & 1, bank buffer (item count) & 1.
 template <int D, int SWEEP>
 __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParams p) {
@@ -129,24 +137,23 @@ __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParam
   uint64_t* bars = reinterpret_cast<uint64_t*>(keys_s + RB_KBUF * KB);
   uint64_t* bank_full = bars;             // [2]  bulk copy landed
   uint64_t* bank_empty = bars + 2;        // [2]  sweep 1: the item's MMAs completed; sweep 2: every thread read lse / w
-  uint64_t* mma_done = bars + 4;          // [2]  accumulator of the TMEM buffer complete
-  uint64_t* tmem_free = bars + 6;         // [2]  every compute thread has read the accumulator
-  uint64_t* keys_ready = bars + 8;        // [RB_KBUF] every compute thread's part of the operand is in shared memory
-  uint64_t* keys_free = bars + 8 + RB_KBUF;  // [RB_KBUF] the MMAs that read the operand completed
-  uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(bars + 8 + 2 * RB_KBUF);
+  uint64_t* mma_done = bars + 4;          // [RB_TB]  accumulator of the TMEM buffer complete
+  uint64_t* tmem_free = mma_done + RB_TB; // [RB_TB]  every compute thread has read the accumulator
+  uint64_t* keys_ready = tmem_free + RB_TB;   // [RB_KBUF] every gather thread's part of the operand is in shared memory
+  uint64_t* keys_free = keys_ready + RB_KBUF; // [RB_KBUF] the MMAs that read the operand completed
+  uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(keys_free + RB_KBUF);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   if (threadIdx.x == 0) {
     for (int b = 0; b < 2; ++b) {
       mbar_init(&bank_full[b], 1);
       mbar_init(&bank_empty[b], SWEEP == 1 ? 1 : CT);
-      mbar_init(&mma_done[b], 1);
-      mbar_init(&tmem_free[b], CT);
     }
-    for (int b = 0; b < RB_KBUF; ++b) { mbar_init(&keys_ready[b], CT); mbar_init(&keys_free[b], 1); }
+    for (int b = 0; b < RB_TB; ++b) { mbar_init(&mma_done[b], 1); mbar_init(&tmem_free[b], CT); }
+    for (int b = 0; b < RB_KBUF; ++b) { mbar_init(&keys_ready[b], RB_PWARPS * 32); mbar_init(&keys_free[b], 1); }
     mbar_fence_init();
   }
-  if (warp == 0) {  // columns [0, 256): two accumulators; [256, 260): exchange between the column halves (sweep 2)
+  if (warp == 0) {  // columns [0, 384): three accumulators; [384, 400): exchange between the column groups (sweep 2)
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_base_p)), "n"(512));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
@@ -180,10 +187,10 @@ __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParam
       uint32_t kph = 0u;
       for (int K = 0; K < total; ++K) {
         const int j = K >> 1, t = K & 1, b = j & 1;      // j = item count over the pairs
-        const uint32_t buf = (uint32_t)K & 1u;
+        const uint32_t buf = (uint32_t)(K % RB_TB);
         mbar_wait(&keys_ready[kb], kph);
         if (t == 0) mbar_wait(&bank_full[b], (uint32_t)(j >> 1) & 1u);
-        mbar_wait(&tmem_free[buf], ((uint32_t)(K >> 1) & 1u) ^ 1u);
+        mbar_wait(&tmem_free[buf], ((uint32_t)(K / RB_TB) & 1u) ^ 1u);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint64_t d_keys = umma_desc(keys_u32 + (uint32_t)(kb * KB), 128, SBO);
         const uint64_t d_hi = umma_desc(bank_u32 + (uint32_t)(b * ITEM), 128, SBO);
@@ -206,26 +213,65 @@ __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParam
         if (++kb == RB_KBUF) { kb = 0; kph ^= 1u; }
       }
     }
-  } else {
-    // ------------------------------------------------------------------ compute warps
-    const int wq = warp & 3, half = warp >> 2, tid = wq * 32 + lane;   // tid = TMEM lane (bank row / token)
-    const int tok8 = lane & 7, c4 = lane >> 3;
+  } else if (warp >= RB_CWARPS + 2) {
+    // ------------------------------------------------------------------ key gather warps: sub-item K into buffer K % 3
+    // as soon as the MMAs of K - 3 have completed; published one iteration later, so that two gathers are in flight and
+    // the wait never depends on a sub-item these warps have not published yet
+    const int pw = (warp - (RB_CWARPS + 2)) & 3, ph2 = (warp - (RB_CWARPS + 2)) >> 2, tok8 = lane & 7, c4 = lane >> 3;
     const uint32_t keys_u32 = smem_u32(keys_s);
-    const uint32_t tlane = tmem + ((uint32_t)(wq * 32) << 16);          // this warp's 32 TMEM lanes
-    // The gather runs two sub-items ahead of the statistics and may already belong to the next pair of tiles: the
-    // slot registers describe the GATHER's pair, c_t0 / c_nv the pair the statistics are on.
-    int64_t slot[2][4];   // lane = (token % 8, chunk % 4) of the gather: tokens wq*32 + i*8 + tok8 of tile 0 / 1
+    int64_t slot[2][4];   // lane = (token % 8, chunk % 4): tokens pw*32 + i*8 + tok8 of tile 0 / 1 of the pair
     auto load_slots = [&](int pr) {
 #pragma unroll
       for (int t = 0; t < 2; ++t) {
         const int t0 = ((2 * pr + t) * (int)gridDim.x + (int)blockIdx.x) * RB_TOK;
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-          const int tok = t0 + wq * 32 + i * 8 + tok8;
+          const int tok = t0 + pw * 32 + i * 8 + tok8;
           slot[t][i] = tok < nc ? (int64_t)p.cand_slot[tok] : -1;
         }
       }
     };
+    int g_l = 0, g_kvh = 0, g_sub = 0, g_pr = 0, kb = 0;
+    uint32_t kph = 0u;
+    if (total > 0) load_slots(0);
+    for (int K = 0; K < total; ++K) {
+      const int t = K & 1;
+      mbar_wait(&keys_free[kb], kph ^ 1u);
+      const bf16* base = p.k_pool + (int64_t)g_l * p.layer_stride + (int64_t)g_kvh * D;
+      const uint32_t dst0 = keys_u32 + (uint32_t)(kb * KB);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const int64_t sl = t ? slot[1][i] : slot[0][i];
+        const bf16* src = base + (sl >= 0 ? sl : 0) * (int64_t)(p.Hkv * D);
+#pragma unroll
+        for (int jj = 0; jj < CH / 8; ++jj) {
+          const int jc = ph2 * (CH / 8) + jj;
+          cp_async16_zfill(dst0 + (uint32_t)rb_entry(pw * 32 + i * 8 + tok8, jc * 4 + c4, D), src + (jc * 4 + c4) * 8,
+                           sl >= 0 ? 16u : 0u);  // tokens beyond the candidates: zero rows
+        }
+      }
+      cp_async_commit();
+      if (K > 0) {
+        cp_async_wait<1>();
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_arrive(&keys_ready[kb == 0 ? RB_KBUF - 1 : kb - 1]);
+      }
+      if (++kb == RB_KBUF) { kb = 0; kph ^= 1u; }
+      if (t == 1) {   // next (layer, head); after the last one the next pair of tiles
+        if (++g_kvh == p.Hkv) { g_kvh = 0; if (++g_l == p.L) g_l = 0; }
+      }
+      if (++g_sub == n_sub) { g_sub = 0; if (++g_pr < p.n_pairs) load_slots(g_pr); }
+    }
+    if (total > 0) {
+      cp_async_wait<0>();
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_arrive(&keys_ready[kb == 0 ? RB_KBUF - 1 : kb - 1]);
+    }
+  } else {
+    // ------------------------------------------------------------------ compute warps: statistics only.  Warp w owns
+    // the TMEM lane quarter w % 4 and the column group cq = w / 4 (RB_CG columns of the 128)
+    const int wq = warp & 3, cq = warp >> 2, tid = wq * 32 + lane;   // tid = TMEM lane (bank row / token)
+    const uint32_t tlane = tmem + ((uint32_t)(wq * 32) << 16);        // this warp's 32 TMEM lanes
     int c_t0[2], c_nv[2];
     auto set_pair = [&](int pr) {
 #pragma unroll
@@ -234,81 +280,57 @@ __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParam
         c_nv[t] = max(0, min(RB_TOK, nc - c_t0[t]));
       }
     };
-    int g_kb = 0, g_l = 0, g_kvh = 0;   // key buffer and (layer, KV head) of the next gather
-    uint32_t g_ph = 0u;
-    auto gather = [&](int Kg) {
-      const int t = Kg & 1;
-      mbar_wait(&keys_free[g_kb], g_ph ^ 1u);
-      const bf16* base = p.k_pool + (int64_t)g_l * p.layer_stride + (int64_t)g_kvh * D;
-      const uint32_t dst0 = keys_u32 + (uint32_t)(g_kb * KB);
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const int64_t sl = t ? slot[1][i] : slot[0][i];
-        const bf16* src = base + (sl >= 0 ? sl : 0) * (int64_t)(p.Hkv * D);
-#pragma unroll
-        for (int jj = 0; jj < CH / 8; ++jj) {   // the two warps of a lane quarter take half of the row's chunks each
-          const int jc = half * (CH / 8) + jj;
-          cp_async16_zfill(dst0 + (uint32_t)rb_entry(wq * 32 + i * 8 + tok8, jc * 4 + c4, D), src + (jc * 4 + c4) * 8,
-                           sl >= 0 ? 16u : 0u);  // tokens beyond the candidates: zero rows
-        }
-      }
-      cp_async_commit();
-      if (++g_kb == RB_KBUF) { g_kb = 0; g_ph ^= 1u; }
-      if (t == 1) {   // both tiles of the item are under way: next (layer, head); the next pair starts over
-        if (++g_kvh == p.Hkv) { g_kvh = 0; if (++g_l == p.L) g_l = 0; }
-      }
-    };
     float acc[2] = {0.f, 0.f};   // sweep 2: this thread's token of tile 0 / tile 1 of the statistics' pair
     // statistics of sub-item Ks: item `it` of pair `prs`, tile t
     auto stats = [&](int Ks, int it, int prs) {
       const int t = Ks & 1, j = Ks >> 1, b = j & 1;
       const int snv = t ? c_nv[1] : c_nv[0];
-      const uint32_t buf = (uint32_t)Ks & 1u;
-      mbar_wait(&mma_done[buf], (uint32_t)(Ks >> 1) & 1u);
+      const uint32_t buf = (uint32_t)(Ks % RB_TB);
+      mbar_wait(&mma_done[buf], (uint32_t)(Ks / RB_TB) & 1u);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      const uint32_t tl = tlane + buf * 128u;
+      const uint32_t tl = tlane + buf * 128u + (uint32_t)(cq * RB_CG);
+      float x[RB_CG];
       if (SWEEP == 1) {
         float m = -CUDART_INF_F, s = 0.f;
-        const int q0 = half * 64, nq = min(64, snv - q0);   // this warp's half of the token columns
+        const int nq = min(RB_CG, snv - cq * RB_CG);   // this warp's share of the token columns
         if (nq > 0) {
-          float x[64];
-          tmem_ld32f(tl + (uint32_t)q0, x);
-          tmem_ld32f(tl + (uint32_t)q0 + 32, x + 32);   // columns beyond the tile's tokens: read, not used
+#pragma unroll
+          for (int c0 = 0; c0 < RB_CG; c0 += 16) tmem_ld16(tl + (uint32_t)c0, x + c0);   // beyond the tile: read, not used
           tmem_ld_wait();
-          if (nq == 64) {
+          if (nq == RB_CG) {
             float c0 = x[0], c1 = x[1];
 #pragma unroll
-            for (int e = 2; e < 64; e += 2) { c0 = fmaxf(c0, x[e]); c1 = fmaxf(c1, x[e + 1]); }
+            for (int e = 2; e < RB_CG; e += 2) { c0 = fmaxf(c0, x[e]); c1 = fmaxf(c1, x[e + 1]); }
             m = fmaxf(c0, c1);
             float s0 = 0.f, s1 = 0.f;
 #pragma unroll
-            for (int e = 0; e < 64; e += 2) { s0 += ex2_approx(x[e] - m); s1 += ex2_approx(x[e + 1] - m); }
+            for (int e = 0; e < RB_CG; e += 2) { s0 += ex2_approx(x[e] - m); s1 += ex2_approx(x[e + 1] - m); }
             s = s0 + s1;
           } else {
 #pragma unroll
-            for (int e = 0; e < 64; ++e)
+            for (int e = 0; e < RB_CG; ++e)
               if (e < nq) m = fmaxf(m, x[e]);
 #pragma unroll
-            for (int e = 0; e < 64; ++e)
+            for (int e = 0; e < RB_CG; ++e)
               if (e < nq) s += ex2_approx(x[e] - m);
           }
         }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         mbar_arrive(&tmem_free[buf]);
-        const int slot_id = ((prs * (int)gridDim.x + (int)blockIdx.x) * 2 + t) * 2 + half;
+        const int slot_id = ((prs * (int)gridDim.x + (int)blockIdx.x) * 2 + t) * RB_CQ + cq;
         p.partials[((size_t)it * p.n_slots + slot_id) * RB_ROWS + tid] = make_float2(m, s);
       } else {
-        const int q0 = half * 64, nq = min(64, p.n_cols - q0);   // this warp's half of the bank rows
+        const int q0 = cq * RB_CG, nq = min(RB_CG, p.n_cols - q0);   // this warp's share of the bank rows
         if (snv > 0 && nq > 0) {
           mbar_wait(&bank_full[b], (uint32_t)(j >> 1) & 1u);   // the bulk copy's bytes (lse, w) are visible to this thread
           const float* tail = reinterpret_cast<const float*>(bank_s + (size_t)b * ITEM + 2 * PART);
           float a0 = 0.f, a1 = 0.f;
-          float x[64];
-          tmem_ld32f(tl + (uint32_t)q0, x);
-          if (nq > 32) tmem_ld32f(tl + (uint32_t)q0 + 32, x + 32);
+#pragma unroll
+          for (int c0 = 0; c0 < RB_CG; c0 += 16)
+            if (c0 < nq) tmem_ld16(tl + (uint32_t)c0, x + c0);
           tmem_ld_wait();
 #pragma unroll
-          for (int e = 0; e < 64; e += 4) {
+          for (int e = 0; e < RB_CG; e += 4) {
             if (e < nq) {   // groups of four columns: the bank's padding rows have w = 0 and a finite lse
               const float4 ls = *reinterpret_cast<const float4*>(tail + q0 + e);
               const float4 ws = *reinterpret_cast<const float4*>(tail + RB_ROWS + q0 + e);
@@ -325,36 +347,35 @@ __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParam
         if (t == 1) mbar_arrive(&bank_empty[b]);   // this thread is done with the item's lse / w
       }
     };
-    // end of a pair (sweep 2): the two column halves of a token meet through four spare TMEM columns (warps w and
-    // w + 4 own the same lanes); the lower half writes the sums
+    // end of a pair (sweep 2): the column groups of a token meet through spare TMEM columns (four per group; the warps
+    // w, w + 4, ... own the same lanes); group 0 adds them in group order and writes the sums
     auto flush = [&]() {
-      const uint32_t tx = tlane + 256u;
-      if (half == 1) {
+      const uint32_t tx = tlane + (uint32_t)(RB_TB * 128);
+      if (cq > 0) {
         const float v4[4] = {acc[0], acc[1], 0.f, 0.f};
-        tmem_st4(tx, v4);
+        tmem_st4(tx + (uint32_t)(4 * cq), v4);
         tmem_wait_st();
       }
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
       bar_sync(1, CT);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      if (half == 0) {
-        float o[4];
-        tmem_ld4(tx, o);
-        tmem_wait_ld();
+      if (cq == 0) {
+        float s0 = acc[0], s1 = acc[1];
 #pragma unroll
-        for (int t = 0; t < 2; ++t) {
-          const int tok = c_t0[t] + tid;
-          if (tid < c_nv[t]) p.rule_c[tok] = (p.accumulate ? p.rule_c[tok] : 0.f) + acc[t] + o[t];
+        for (int k = 1; k < RB_CQ; ++k) {
+          float o[4];
+          tmem_ld4(tx + (uint32_t)(4 * k), o);
+          tmem_wait_ld();
+          s0 += o[0]; s1 += o[1];
         }
+        if (tid < c_nv[0]) { const int tok = c_t0[0] + tid; p.rule_c[tok] = (p.accumulate ? p.rule_c[tok] : 0.f) + s0; }
+        if (tid < c_nv[1]) { const int tok = c_t0[1] + tid; p.rule_c[tok] = (p.accumulate ? p.rule_c[tok] : 0.f) + s1; }
       }
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
       bar_sync(1, CT);
       acc[0] = acc[1] = 0.f;
     };
-    load_slots(0);
     set_pair(0);
-    int g_pair = 0;
-    for (int Kg = 0; Kg < 2 && Kg < total; ++Kg) gather(Kg);
     int s_sub = 0, s_pr = 0;   // statistics: sub-item inside its pair, pair
     auto stats_next = [&](int Ks) {
       stats(Ks, s_sub >> 1, s_pr);
@@ -364,22 +385,7 @@ __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParam
         if (++s_pr < p.n_pairs) set_pair(s_pr);
       }
     };
-    for (int K = 0; K < total; ++K) {
-      // sub-item K's operand first (its gather was issued two iterations ago): the issuer can then start its MMAs the
-      // moment those of K - 1 complete.  Then the statistics of K - 1, and only then the gather of K + 2: its buffer is
-      // the one of K - 1, whose MMAs the statistics have just waited for (gather first: 1.4 k idle cycles per sub-item)
-      if (K + 1 < total) cp_async_wait<1>(); else cp_async_wait<0>();
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_arrive(&keys_ready[K % RB_KBUF]);
-      if (K > 0) stats_next(K - 1);
-      const int Kg = K + 2;
-      if (Kg < total) {
-        const int prg = Kg / n_sub;
-        if (prg != g_pair) { load_slots(prg); g_pair = prg; }
-        gather(Kg);
-      }
-    }
-    stats_next(total - 1);
+    for (int K = 0; K < total; ++K) stats_next(K);
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
