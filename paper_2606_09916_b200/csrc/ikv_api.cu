@@ -1040,7 +1040,7 @@ ikv_status score_rows_tc(ikv_ctx* c, const ikv_request& r, const float* rows, in
   const int tiles = (N + RB_TOK - 1) / RB_TOK;
   const int grid = std::max(1, std::min(c->n_sm, (tiles + 1) / 2));
   const int n_pairs = (tiles + 2 * grid - 1) / (2 * grid);
-  const int n_slots = n_pairs * grid * 2 * RB_CQ;   // (pair, CTA, tile of the pair, column group)
+  const int n_slots = n_pairs * grid * RB_CQ;   // (pair, CTA, column group)
   const size_t need = (size_t)n_items * n_slots * RB_ROWS;
   if (need > c->rows_partials_cap) {
     c->rows_partials_cap = 0;

@@ -98,7 +98,7 @@ struct RowsPassParams {
   const unsigned char* bank;
   const int32_t* cand_slot;
   const int32_t* n_cand;
-  float2* partials;      // sweep 1: [item][slot][128], slot = (pair, cta, tile of the pair, column group)
+  float2* partials;      // sweep 1: [item][slot][128], slot = (pair, cta, column group)
   int n_slots, n_pairs;
   float* rule_c;         // sweep 2
   int accumulate;        // sweep 2: add to rule_c (second and later banks)
@@ -281,6 +281,7 @@ __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParam
       }
     };
     float acc[2] = {0.f, 0.f};   // sweep 2: this thread's token of tile 0 / tile 1 of the statistics' pair
+    float pm = -CUDART_INF_F, ps = 0.f;   // sweep 1: (max, sum) of tile 0 until tile 1 of the same item is done
     // statistics of sub-item Ks: item `it` of pair `prs`, tile t
     auto stats = [&](int Ks, int it, int prs) {
       const int t = Ks & 1, j = Ks >> 1, b = j & 1;
@@ -317,8 +318,14 @@ __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParam
         }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         mbar_arrive(&tmem_free[buf]);
-        const int slot_id = ((prs * (int)gridDim.x + (int)blockIdx.x) * 2 + t) * RB_CQ + cq;
-        p.partials[((size_t)it * p.n_slots + slot_id) * RB_ROWS + tid] = make_float2(m, s);
+        if (t == 0) {   // the two tiles of the pair are the same bank row of the same item: one partial for both
+          pm = m; ps = s;
+        } else {
+          const float mn = fmaxf(pm, m);
+          if (mn > -CUDART_INF_F) { s = ps * ex2_approx(pm - mn) + s * ex2_approx(m - mn); m = mn; }
+          const int slot_id = (prs * (int)gridDim.x + (int)blockIdx.x) * RB_CQ + cq;
+          p.partials[((size_t)it * p.n_slots + slot_id) * RB_ROWS + tid] = make_float2(m, s);
+        }
       } else {
         const int q0 = cq * RB_CG, nq = min(RB_CG, p.n_cols - q0);   // this warp's share of the bank rows
         if (snv > 0 && nq > 0) {
