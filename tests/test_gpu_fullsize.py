@@ -233,3 +233,50 @@ def test_cfg4_sixty_four_sessions(ikv, oracle):
         want_o = oracle.decode(_layer_geom(oracle, w), k1, v1, 0, finals[i], q[i].float().numpy(), 1 / math.sqrt(shape.D))
         gc.assert_decode_close(out[i].float().cpu().numpy(), want_o, True, f"cfg4 decode session {i}")
     print(f"cfg4 full: 64 sessions, {tot} tokens, worst score abs err {worst:.3e}")
+
+
+def test_next_rows_and_prefill_at_full_width(ikv, oracle):
+    """The widened rows at the width and length of configs[1] (32 Q / 8 KV heads, D 128, 32,768 live tokens), on 4
+    layers so that the oracle finishes in seconds: the 32-row window scorer on tcgen05 (one bank of 128 rows, every CTA
+    on its full pair of tiles) against the oracle, then prune to C = 8,192 and a 256-row prefill chunk through the pruned
+    map (tcgen05 kernel, 8 row blocks x 8 KV heads x 2 splits) against the oracle, counters exact."""
+    shape = wl.ModelShape(4, 32, 8, 128, "bf16")
+    w = wl.cfg1(device="cuda", shape=shape, n_tokens=32768, decode_tokens=256)
+    s = w.sessions[0]
+    ctx = ikv.Context(shape.L, shape.Hq, shape.Hkv, shape.D, w.k_pool, w.v_pool, dead_slot=w.dead_slot)
+    kp = _host_bits(w.k_pool)
+    ctx.reserve(s.N + 256, 1)
+    gc.fold_memory_gpu(ctx, s)
+    g = gc.oracle_geom(oracle, w)
+    S = s.slot_map[:s.N].numpy().copy()
+    S_dev = s.slot_map.clone().cuda()
+    req = ikv.make_request(s.spec.session_id, S_dev, s.N, s.pi, s.qs, s.qe, 8192, s.pi)
+    R = 32
+    rows = torch.randn((R, shape.L, shape.Hq, shape.D), generator=torch.Generator().manual_seed(77))
+    wt = [1.0 / R] * R
+    scores = torch.empty(s.N, device="cuda")
+    ctx.score_rows([req], rows.cuda().contiguous(), wt, scores)
+    cls, _ = oracle.partition(S, w.dead_slot, s.pi, s.qs, s.qe)
+    want = oracle.multirow_score(g, kp, rows.double().numpy(), wt, S, cls)
+    want = np.where(cls == oracle.FORCED, np.inf, np.where(cls == oracle.DEAD, -np.inf, want))
+    mabs, mrel = gc.assert_scores_close(scores.cpu().numpy(), want, "32-row scorer at full width")
+    print(f"full width: 32-row scorer max abs err {mabs:.3e} rel {mrel:.3e}")
+    # prune on these scores, then a prefill chunk through the pruned map
+    freed = torch.empty(s.N, dtype=torch.int32, device="cuda")
+    nf = torch.zeros(1, dtype=torch.int32, device="cuda")
+    nk = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ctx.select_evict([req], scores, freed, nf, nk)
+    torch.cuda.synchronize()
+    assert nk.item() == 8192
+    n_q, layer = 256, 2
+    q = torch.randn((n_q, shape.Hq, shape.D), generator=torch.Generator().manual_seed(78)).to(torch.bfloat16)
+    out = torch.empty((n_q, shape.Hq, shape.D), dtype=torch.bfloat16, device="cuda")
+    reads = torch.zeros(2, dtype=torch.int64, device="cuda")
+    r = ikv.make_request(s.spec.session_id, S_dev, s.N + n_q, s.pi, s.qs, s.qe, 8192, s.pi)
+    ctx.prefill_attn(layer, r, s.N, q.cuda(), out, 1.0 / math.sqrt(shape.D), reads)
+    torch.cuda.synchronize()
+    vp = _host_bits(w.v_pool)
+    want_o, raw, eff = oracle.prefill(g, kp, vp, layer, S_dev.cpu().numpy(), s.N, q.float().numpy(), 1.0 / math.sqrt(shape.D))
+    err = gc.assert_decode_close(out.float().cpu().numpy(), want_o, True, "prefill chunk at full width")
+    assert reads.cpu().tolist() == [raw, eff]
+    print(f"full width: 256-row prefill chunk over {nk.item()} survivors max abs err {err:.3e}, reads {raw} / {eff}")
