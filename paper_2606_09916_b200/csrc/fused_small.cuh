@@ -35,6 +35,7 @@ inline int mem_prep_frag_blocks(int L, int Hkv) {
 struct PostKeyParams {
   const float2* partials; int n_part; float* lse; int n_lse;          // lse rows
   const float* mpart; int n_mpart; int LH; FoldOut fold; int n_fold;  // fold blocks (0: not a learnable call)
+  int mbar_ready;  // rt.mbar was reduced by the layer-major key pass
   const float* kq; const int32_t* n_xq; int nks; uint4 *kc_frag, *vc_frag; int n_kv;  // Kc / Vc blocks
   int tc; int nxp; RtFoldOut rt;  // tc != 0: operands of k_residual_tc instead (n_fold fc1 blocks, n_kv cross-attention blocks)
 };
@@ -72,10 +73,10 @@ __global__ __launch_bounds__(TC ? 256 : 128) void k_post_key(const PostKeyParams
   if constexpr (TC) {
     bid -= n_lse_blocks;
     if (bid < p.n_fold) {
-      if (threadIdx.x < 128) rt_fold_fc1_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.rt);
+      if (threadIdx.x < 128) rt_fold_fc1_block<D>(bid, p.mpart, p.n_mpart, p.LH, w, p.rt, p.mbar_ready != 0);
       return;
     }
-    rt_fold_xattn_block<D>(bid - p.n_fold, p.mpart, p.n_mpart, p.LH, p.kq, p.n_xq, p.nxp, w, p.rt);
+    rt_fold_xattn_block<D>(bid - p.n_fold, p.mpart, p.n_mpart, p.LH, p.kq, p.n_xq, p.nxp, w, p.rt, p.mbar_ready != 0);
   }
 }
 

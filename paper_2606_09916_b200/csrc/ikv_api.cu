@@ -690,6 +690,7 @@ ikv_status launch_key_pass(ikv_ctx* c, const float* M, bool kbar, bool with_xq, 
       p.scores = lo.scores; p.rule_out = lo.rule_out; p.scatter_scores = lo.scatter;
       p.kbar = c->kbar; p.kq = c->kq; p.n_stage = ns; p.l2_hints = c->dbg_l2;
       p.tstamp = nullptr;
+      p.mpart = c->mpart; p.n_mpart = n_mpart; p.LH = L * Hq; p.mbar_out = (kbar && n_mpart > 0) ? c->mbar : nullptr;
       if (c->prof_on == 1 && c->ts_ring && c->ts_used < ikv_ctx::TS_SLOTS) p.tstamp = c->ts_ring + 2 * (c->ts_used++);
       ProfScope prof(c, c->prof_on == 1 ? IKV_PROF_SLOTS : IKV_PROF_KEY_PASS, ks);  // level 1: stamps instead of events
       if (kbar) {
@@ -856,6 +857,7 @@ ikv_status score_one(ikv_ctx* c, const ikv_request& r, int mode, float* scores, 
   pk.n_fold = 0; pk.n_kv = 0; pk.tc = tc ? 1 : 0; pk.nxp = nxp;
   pk.rt.mbar = c->mbar; pk.rt.wcan = c->rt_wcan; pk.rt.svec = c->rt_svec; pk.rt.b1_eff = c->b1_eff;
   if (lm_done) pk.n_lse = 0;   // no lse rows to reduce, no logits to read back
+  pk.mbar_ready = (lm_done && learn) ? 1 : 0;
   if (lm_done && !learn) return IKV_OK;
   if (tc) {
     // launch 1: lse rows and the folded operands of the residual head (they need the mean keys of the query positions,

@@ -60,17 +60,21 @@ __device__ __forceinline__ void rt_store8(unsigned char* dst, const float (&v)[8
 // Fold bodies, 128 threads: fc1's kbar columns (W_1k') as chunks D/16 .. 2D/16-1, b_1', mbar.
 template <int D>
 __device__ __forceinline__ void rt_fold_fc1_block(int bid, const float* __restrict__ part, int n_part, int LH,
-                                                  const ResidW& w, const RtFoldOut& o) {
+                                                  const ResidW& w, const RtFoldOut& o, bool mbar_ready) {
   constexpr int P = 3 * D + 1, IN = P + R_DC;
   constexpr int N_W1 = R_HID * (D / 8);
   __shared__ float mb[D];
   for (int d = threadIdx.x; d < D; d += 128) {
-    const float acc = sum_parts(part, n_part, D, d);
-    mb[d] = acc / (float)LH;
+    if (mbar_ready) {   // reduced by the layer-major key pass (same order of additions)
+      mb[d] = o.mbar[d];
+    } else {
+      const float acc = sum_parts(part, n_part, D, d);
+      mb[d] = acc / (float)LH;
+    }
   }
   __syncthreads();
   int idx = bid * 128 + threadIdx.x;
-  if (bid == 0)
+  if (bid == 0 && !mbar_ready)
     for (int d = threadIdx.x; d < D; d += 128) o.mbar[d] = mb[d];
   if (idx < N_W1) {
     const int n = idx / (D / 8), k8 = idx % (D / 8), k0 = k8 * 8;
@@ -102,7 +106,7 @@ inline int rt_fold_fc1_grid() { return (R_HID * (D / 8) + R_HID * 32 + 127) / 12
 template <int D>
 __device__ __forceinline__ void rt_fold_xattn_block(int bid, const float* __restrict__ part, int n_part, int LH,
                                                     const float* __restrict__ kq, const int32_t* __restrict__ n_xq,
-                                                    int nxp, const ResidW& w, const RtFoldOut& o) {
+                                                    int nxp, const ResidW& w, const RtFoldOut& o, bool mbar_ready) {
   constexpr int P = 3 * D + 1, IN = P + R_DC;
   constexpr int KPT = 16 * D / 256;  // keys per thread in the W_S step
   __shared__ float mb[D];
@@ -123,8 +127,12 @@ __device__ __forceinline__ void rt_fold_xattn_block(int bid, const float* __rest
       v[j] = __ldg(reinterpret_cast<const float4*>(src + d * R_DC) + (tid & 7));
     }
     for (int d = tid; d < D; d += 256) {
-      const float acc = sum_parts(part, n_part, D, d);
-      mb[d] = acc / (float)LH;
+      if (mbar_ready) {
+        mb[d] = o.mbar[d];
+      } else {
+        const float acc = sum_parts(part, n_part, D, d);
+        mb[d] = acc / (float)LH;
+      }
     }
     for (int i = tid; i < 16 * D; i += 256) {
       const int key = i / D, d = i % D;

@@ -49,6 +49,9 @@ struct KeyPassLmParams {
   int n_stage;
   int l2_hints;
   unsigned long long* tstamp;  // profiling: {min start, max end} of the launch in %globaltimer ns, or NULL
+  const float* mpart;      // partial sums of the memory rows (k_mem_prep), [n_mpart][D]; with mbar_out != NULL one
+  int n_mpart, LH;         // statistics warp of CTA 0 reduces them to mbar (Eq. 5) while the keys stream, in the order
+  float* mbar_out;         // the fold blocks would use (b ascending): they then start with one load instead of a chain
 };
 
 __device__ __forceinline__ void tmem_ld4(uint32_t taddr, float (&v)[4]) {
@@ -215,6 +218,21 @@ __global__ __launch_bounds__(lm_threads(KBAR), 1) void k_key_pass_lm(const KeyPa
     const int hq2 = (Hq + 1) & ~1;
     const int sw = warp - W_STATS;
     const int per = (n_cta + LM_SWARPS - 1) / LM_SWARPS, j_lo = sw * per, j_hi = min(n_cta, j_lo + per);
+    if (KBAR && blockIdx.x == 0 && sw == LM_SWARPS - 1 && p.mbar_out) {
+      for (int d = lane; d < D; d += 32) {
+        float acc = 0.f;
+        int b = 0;
+        for (; b + 8 <= p.n_mpart; b += 8) {
+          float v[8];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) v[j] = p.mpart[(b + j) * D + d];
+#pragma unroll
+          for (int j = 0; j < 8; ++j) acc += v[j];
+        }
+        for (; b < p.n_mpart; ++b) acc += p.mpart[b * D + d];
+        p.mbar_out[d] = acc / (float)p.LH;
+      }
+    }
     for (int l = 0; l < L; ++l) {
       if (sw == 0) {
         // publish this CTA's partials of layer l (the logit warps only write shared memory: the fence and the atomic
