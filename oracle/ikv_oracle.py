@@ -295,3 +295,18 @@ def prefill(g: Geometry, k_pool, v_pool, layer, S, q_pos0, q, sm_scale):
                          g.D, int(layer), _p(S), int(g.dead_slot), int(q_pos0), q.shape[0], _p(q),
                          C.c_double(sm_scale), _p(out), _p(reads))
     return out, int(reads[0]), int(reads[1])
+
+
+def train_loss(s, y, mem_rows=None, rho=0.05, gamma=0.01, eta=0.001):
+    """N4: Eq. 8 and dL/ds.  s [n] float64, y [n] int32 (1 / 0 / -100), mem_rows [R][D] or None.
+    Returns (terms[5] = L, L_BCE, L_rank, keep, norm; grad [n])."""
+    s = _c(s, np.float64)
+    y = _c(y, np.int32)
+    if mem_rows is None:
+        mem_rows = np.zeros((0, 1), np.float64)
+    mem_rows = _c(mem_rows, np.float64)
+    terms = np.zeros(5, np.float64)
+    grad = np.zeros(s.shape[0], np.float64)
+    lib().oracle_train_loss(_p(s), _p(y), s.shape[0], _p(mem_rows), mem_rows.shape[0], mem_rows.shape[1],
+                            C.c_double(rho), C.c_double(gamma), C.c_double(eta), _p(terms), _p(grad))
+    return terms, grad

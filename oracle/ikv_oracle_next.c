@@ -197,3 +197,87 @@ void oracle_prefill(const void *k_pool, const void *v_pool, int kv_dtype, int64_
       free(x);
     }
 }
+
+/* ------------------------------------------------------------------------
+ * N4  training objective of the residual head, Eq. 8, and its gradient
+ * with respect to the scores (readings R34-R37):
+ *   L = L_BCE(s, y) + rho L_rank + gamma mean sigma(s) + eta (||M_t||_2 - 1)^2
+ * s[n]: scores (logits) of the candidate tokens of one (session, turn) row; y[n]: 1 = positive
+ * ("matches a literal substring of a future tool argument"), 0 = negative, anything else
+ * (-100) = excluded from the loss.  V = valid entries, n_v = |V|, P = positives.
+ *   p = |P| / n_v,  p~ = clip(p, 0.02, 0.5),  w+ = (1 - p~) / p~                        (:147)
+ *   L_BCE  = (1/n_v) sum_V [ w+ y softplus(-s) + (1 - y) softplus(s) ]
+ *   L_rank = (1 / (|P| |H|)) sum_{i in P} sum_{j in H} softplus(s_j - s_i),
+ *            H = the 64 highest-scored negatives (ties: lower position first); 0 if P or H is empty
+ *   keep   = (1/n_v) sum_V sigma(s)
+ *   norm   = mean over the rows r of mem_rows[R][D] of (||row_r||_2 - 1)^2   (0 if R = 0)
+ * terms[5] = {L, L_BCE, L_rank, keep, norm} (L_rank, keep, norm unweighted); grad[n] = dL/ds
+ * (0 at excluded entries).  n_v = 0: everything 0 except the norm term.
+ * ---------------------------------------------------------------------- */
+static double softplus_d(double x) { return x > 0 ? x + log1p(exp(-x)) : log1p(exp(x)); }
+static double sigmoid_d(double x) { return x >= 0 ? 1.0 / (1.0 + exp(-x)) : exp(x) / (1.0 + exp(x)); }
+
+void oracle_train_loss(const double *s, const int32_t *y, int n, const double *mem_rows, int R, int D,
+                       double rho, double gamma, double eta, double *terms, double *grad) {
+  int n_v = 0, n_p = 0;
+  for (int i = 0; i < n; ++i) {
+    grad[i] = 0.0;
+    if (y[i] == 0 || y[i] == 1) { ++n_v; n_p += y[i]; }
+  }
+  double bce = 0.0, rank = 0.0, keep = 0.0, norm = 0.0;
+  if (n_v > 0) {
+    double p = (double)n_p / (double)n_v;
+    double pt = p < 0.02 ? 0.02 : (p > 0.5 ? 0.5 : p);
+    const double wp = (1.0 - pt) / pt;
+    for (int i = 0; i < n; ++i) {
+      if (y[i] != 0 && y[i] != 1) continue;
+      if (y[i] == 1) {
+        bce += wp * softplus_d(-s[i]);
+        grad[i] += -wp * sigmoid_d(-s[i]) / n_v;
+      } else {
+        bce += softplus_d(s[i]);
+        grad[i] += sigmoid_d(s[i]) / n_v;
+      }
+      const double sg = sigmoid_d(s[i]);
+      keep += sg;
+      grad[i] += gamma * sg * (1.0 - sg) / n_v;
+    }
+    bce /= n_v;
+    keep /= n_v;
+    /* hard negatives: repeatedly take the best remaining negative */
+    int hn[64], n_h = 0;
+    char *taken = (char *)calloc((size_t)n, 1);
+    for (int k = 0; k < 64; ++k) {
+      int best = -1;
+      for (int i = 0; i < n; ++i)
+        if (y[i] == 0 && !taken[i] && (best < 0 || s[i] > s[best])) best = i;  /* lower position wins ties */
+      if (best < 0) break;
+      taken[best] = 1;
+      hn[n_h++] = best;
+    }
+    free(taken);
+    if (n_p > 0 && n_h > 0) {
+      const double c = 1.0 / ((double)n_p * (double)n_h);
+      for (int i = 0; i < n; ++i) {
+        if (y[i] != 1) continue;
+        for (int k = 0; k < n_h; ++k) {
+          const double z = s[hn[k]] - s[i];
+          rank += softplus_d(z);
+          const double gz = sigmoid_d(z) * c * rho;
+          grad[hn[k]] += gz;
+          grad[i] -= gz;
+        }
+      }
+      rank *= c;
+    }
+  }
+  for (int r = 0; r < R; ++r) {
+    double q = 0.0;
+    for (int d = 0; d < D; ++d) q += mem_rows[(int64_t)r * D + d] * mem_rows[(int64_t)r * D + d];
+    const double e = sqrt(q) - 1.0;
+    norm += e * e;
+  }
+  if (R > 0) norm /= R;
+  terms[1] = bce; terms[2] = rank; terms[3] = keep; terms[4] = norm;
+  terms[0] = bce + rho * rank + gamma * keep + eta * norm;
+}

@@ -162,3 +162,72 @@ def test_prefill_single_row_is_decode(oracle):
     out, raw, eff = oracle.prefill(g, kp, vp, 0, S, 149, q.numpy(), 0.125)
     want = oracle.decode(g, kp, vp, 0, S[:150], q[0].numpy(), 0.125)
     assert np.array_equal(out[0], want) and raw == 150 and eff == int((S[:150] != w.dead_slot).sum())
+
+
+# ------------------------------------------------------------------------------------------- N4: Eq. 8 and dL/ds
+def _loss_case(seed, n=400, pos_rate=0.03, excl=0.1):
+    rng = np.random.default_rng(seed)
+    s = rng.standard_normal(n) * 2.0
+    y = (rng.random(n) < pos_rate).astype(np.int32)
+    y[rng.random(n) < excl] = -100
+    return s, y
+
+
+def test_train_loss_bce_term_is_torch_bce_with_logits(oracle):
+    """L_BCE against the library routine (pos_weight = (1 - p~) / p~, mean over the valid entries), for a
+    positive rate below, inside and above the clip [0.02, 0.5]."""
+    import torch.nn.functional as F
+    for seed, rate in ((1, 0.005), (2, 0.1), (3, 0.8)):
+        s, y = _loss_case(seed, pos_rate=rate)
+        terms, _ = oracle.train_loss(s, y)
+        v = y >= 0
+        p = y[v].mean()
+        pt = min(max(p, 0.02), 0.5)
+        want = F.binary_cross_entropy_with_logits(torch.from_numpy(s[v]), torch.from_numpy(y[v].astype(np.float64)),
+                                                  pos_weight=torch.tensor((1 - pt) / pt, dtype=torch.float64))
+        assert abs(terms[1] - want.item()) < 1e-12 * max(1.0, abs(want.item()))
+        assert abs(terms[3] - torch.sigmoid(torch.from_numpy(s[v])).mean().item()) < 1e-14
+
+
+def test_train_loss_rank_term_brute_force(oracle):
+    """L_rank by brute force in Python: every positive against the 64 highest negatives (ties: lower position first),
+    pairwise softplus, mean over the pairs; fewer than 64 negatives and heavy ties included."""
+    import math
+    for seed, n, q in ((4, 300, None), (5, 50, None), (6, 500, 0.5)):
+        s, y = _loss_case(seed, n=n, pos_rate=0.1)
+        if q:
+            s = np.round(s / q) * q
+        terms, _ = oracle.train_loss(s, y)
+        neg = sorted([i for i in range(n) if y[i] == 0], key=lambda i: (-s[i], i))[:64]
+        pos = [i for i in range(n) if y[i] == 1]
+        tot = sum(math.log1p(math.exp(s[j] - s[i])) for i in pos for j in neg)
+        want = tot / (len(pos) * len(neg)) if pos and neg else 0.0
+        assert abs(terms[2] - want) < 1e-12 * max(1.0, want)
+
+
+def test_train_loss_total_gradient_and_special_cases(oracle):
+    """L = L_BCE + rho L_rank + gamma keep + eta norm; dL/ds against central differences of L itself (away from ties the
+    hard-negative set is locally constant); excluded entries get no gradient; no positives: rank term 0 and p~ = 0.02;
+    nothing valid: only the norm term; rows of norm 2 give norm term 1."""
+    s, y = _loss_case(7, n=200, pos_rate=0.08)
+    rows = np.random.default_rng(8).standard_normal((6, 16))
+    rho, gamma, eta = 0.05, 0.01, 0.001
+    terms, grad = oracle.train_loss(s, y, rows, rho, gamma, eta)
+    assert abs(terms[0] - (terms[1] + rho * terms[2] + gamma * terms[3] + eta * terms[4])) < 1e-15
+    want_norm = np.mean((np.linalg.norm(rows, axis=1) - 1.0) ** 2)
+    assert abs(terms[4] - want_norm) < 1e-14
+    eps = 1e-6
+    for i in range(0, 200, 7):
+        sp, sm = s.copy(), s.copy()
+        sp[i] += eps
+        sm[i] -= eps
+        fd = (oracle.train_loss(sp, y, rows, rho, gamma, eta)[0][0] - oracle.train_loss(sm, y, rows, rho, gamma, eta)[0][0]) / (2 * eps)
+        assert abs(grad[i] - fd) < 1e-8, (i, grad[i], fd)
+    assert np.all(grad[y < 0] == 0.0)
+    y0 = np.where(y == 1, 0, y)
+    t0, _ = oracle.train_loss(s, y0)
+    v = y0 >= 0
+    assert t0[2] == 0.0
+    assert abs(t0[1] - np.mean(np.logaddexp(0.0, s[v]))) < 1e-13          # only negatives: plain softplus, w+ unused
+    tn, gn = oracle.train_loss(s, np.full_like(y, -100), 2.0 * np.eye(4), rho, gamma, eta)
+    assert tn[1] == tn[2] == tn[3] == 0.0 and abs(tn[4] - 1.0) < 1e-15 and abs(tn[0] - eta) < 1e-18 and not gn.any()
