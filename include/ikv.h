@@ -282,6 +282,20 @@ ikv_status ikv_profile_read(ikv_ctx *ctx, float *out_ms, int32_t *out_n);
                                  passes in request order on the caller's stream; 1 = one request after another      */
 ikv_status ikv_tune(ikv_ctx *ctx, int32_t knob, int32_t value);
 
+/* NEXT-4: the training objective of the residual head, Eq. 8, and its gradient with respect to the
+ * scores, for one (session, turn) row:  L = L_BCE + rho L_rank + gamma mean sigma(s) + eta mean_r (||row_r||_2 - 1)^2
+ * (readings R34-R37 in DESIGN.md).  scores [n] DEVICE fp32 logits; labels [n] DEVICE int32: 1 positive, 0 negative, any
+ * other value (-100) excluded; mem_rows [n_rows][row_dim] DEVICE fp32, the un-normalised memory rows of the norm term
+ * (NULL / 0: term 0); terms [5] DEVICE = {L, L_BCE, L_rank, keep, norm}, the last three unweighted; grad [n] DEVICE =
+ * dL/dscores (0 at excluded entries).  The backward pass through the residual head and the optimiser are not part of
+ * the library.  n <= 131,072 (one CTA), else IKV_ERR_UNSUPPORTED.  Enqueues on `stream`; no host synchronisation. */
+typedef struct {
+  float rho, gamma, eta; /* the paper's defaults: 0.05, 0.01, 0.001 */
+} ikv_loss_cfg;
+ikv_status ikv_train_loss(ikv_ctx *ctx, const float *scores, const int32_t *labels, int32_t n, const float *mem_rows,
+                          int32_t n_rows, int32_t row_dim, const ikv_loss_cfg *cfg, float *terms, float *grad,
+                          void *stream);
+
 /* Test support: enqueues a kernel that signals its dependents first (griddepcontrol.launch_dependents), idles for
  * delay_us microseconds and only then copies `bytes` (a multiple of 16) from src to dst (both DEVICE).  Models a producer of
  * q that triggers early; tests/test_gpu_parity.py uses it to check the stream ordering of ikv_decode_attn. */

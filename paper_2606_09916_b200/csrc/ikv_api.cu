@@ -24,6 +24,7 @@
 #include "score_rows_tc.cuh"
 #include "prefill_mma.cuh"
 #include "prefill_tc.cuh"
+#include "loss.cuh"
 #include "select.cuh"
 #include "select_cluster.cuh"
 #include "fused_small.cuh"
@@ -1844,6 +1845,21 @@ ikv_status ikv_decode_attn_static(ikv_ctx* c, int32_t layer, const ikv_request* 
   c->part_o = po;
   c->part_ml = pm;
   return rc;
+}
+
+ikv_status ikv_train_loss(ikv_ctx* c, const float* scores, const int32_t* labels, int32_t n, const float* mem_rows,
+                          int32_t n_rows, int32_t row_dim, const ikv_loss_cfg* cfg, float* terms, float* grad,
+                          void* stream) {
+  if (!c) return IKV_ERR_INVALID_ARG;
+  if (n < 0 || !cfg || !terms || (n > 0 && (!scores || !labels || !grad)) || n_rows < 0 || (n_rows > 0 && (!mem_rows || row_dim <= 0)))
+    IKV_FAIL(c, IKV_ERR_INVALID_ARG, "ikv_train_loss: bad argument");
+  if (n > LOSS_MAX_N) IKV_FAIL(c, IKV_ERR_UNSUPPORTED, "ikv_train_loss: n = %d exceeds %d", n, LOSS_MAX_N);
+  LossParams p;
+  p.s = scores; p.y = labels; p.n = n; p.mem_rows = mem_rows; p.n_rows = n_rows; p.row_dim = row_dim;
+  p.rho = cfg->rho; p.gamma = cfg->gamma; p.eta = cfg->eta; p.terms = terms; p.grad = grad;
+  k_train_loss<<<1, 1024, 0, (cudaStream_t)stream>>>(p);
+  LAUNCH_CHECK(c);
+  return IKV_OK;
 }
 
 ikv_status ikv_prune_host(ikv_ctx* c, const ikv_request* req, const void* q_rows_host, int32_t n_rows, int32_t q_dtype,

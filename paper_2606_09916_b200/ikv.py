@@ -33,7 +33,7 @@ PROF_NAMES = ["key_pass", "decode_split", "memory_update", "partition", "mem_pre
 EXPORTS = ["ikv_create", "ikv_destroy", "ikv_last_error", "ikv_reserve", "ikv_session_open", "ikv_session_fork",
            "ikv_session_close", "ikv_session_get_memory", "ikv_session_set_memory", "ikv_residual_load",
            "ikv_memory_update", "ikv_score", "ikv_select_evict", "ikv_decode_attn", "ikv_prune_host",
-           "ikv_score_rows", "ikv_score_baseline", "ikv_prefill_attn", "ikv_decode_attn_static", "ikv_profile_enable", "ikv_profile_read", "ikv_tune", "ikv_test_late_writer", "ikv_version"]
+           "ikv_score_rows", "ikv_score_baseline", "ikv_prefill_attn", "ikv_decode_attn_static", "ikv_train_loss", "ikv_profile_enable", "ikv_profile_read", "ikv_tune", "ikv_test_late_writer", "ikv_version"]
 
 
 class Config(C.Structure):
@@ -78,6 +78,12 @@ _lib.ikv_decode_attn.argtypes = [C.c_void_p, C.c_int32, C.POINTER(Request), C.c_
                                  C.c_float, C.c_void_p]
 _lib.ikv_decode_attn_static.argtypes = [C.c_void_p, C.c_int32, C.POINTER(Request), C.c_void_p, C.c_void_p, C.c_float,
                                         C.c_void_p]
+class LossCfg(C.Structure):
+    _fields_ = [("rho", C.c_float), ("gamma", C.c_float), ("eta", C.c_float)]
+
+
+_lib.ikv_train_loss.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int32, C.c_int32,
+                                C.POINTER(LossCfg), C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.ikv_tune.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
 _lib.ikv_test_late_writer.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p]
 _lib.ikv_profile_enable.argtypes = [C.c_void_p, C.c_int32]
@@ -219,6 +225,13 @@ class Context:
     def decode_attn(self, layer, reqs, q, out, sm_scale, stream=None):
         self._chk(_lib.ikv_decode_attn(self._h, layer, _req_array(reqs), len(reqs), _ptr(q), _ptr(out),
                                        C.c_float(sm_scale), _stream(stream)))
+
+    def train_loss(self, scores, labels, terms, grad, mem_rows=None, rho=0.05, gamma=0.01, eta=0.001, stream=None):
+        """Eq. 8 and dL/dscores for one row of scores (device tensors; terms [5], grad [n] are written)."""
+        cfg = LossCfg(rho, gamma, eta)
+        nr, rd = (0, 0) if mem_rows is None else (mem_rows.shape[0], mem_rows.shape[1])
+        self._chk(_lib.ikv_train_loss(self._h, _ptr(scores), _ptr(labels), scores.numel(), _ptr(mem_rows), nr, rd,
+                                      C.byref(cfg), _ptr(terms), _ptr(grad), _stream(stream)))
 
     def decode_attn_static(self, layer, req, q, out, sm_scale, stream=None):
         """One request, no session, no allocation: split partials in the library's static device array."""

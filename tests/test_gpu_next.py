@@ -263,3 +263,32 @@ def test_prefill_tcgen05_head_layouts(ikv, oracle, name, shape):
         e1 = gc.assert_decode_close(outs[0], want, True, f"{name} tcgen05 prefill at {q_pos0} x {n_q}")
         e2 = gc.assert_decode_close(outs[1], want, True, f"{name} mma.sync prefill at {q_pos0} x {n_q}")
         print(f"[{name}] prefill at {q_pos0} x {n_q}: max abs err tcgen05 {e1:.3e}, mma.sync {e2:.3e}")
+
+
+@pytest.mark.parametrize("n,pos_rate", [(1, 1.0), (700, 0.05), (33000, 0.004), (5000, 0.0), (40, 0.5)])
+def test_train_loss_matches_oracle(ikv, oracle, n, pos_rate):
+    """Eq. 8 and dL/ds (ikv_train_loss) against the fp64 oracle: terms within 1e-5 relative, gradient within
+    1e-7 + 1e-4 |g|; quantised scores (ties among the hard negatives), excluded labels, fewer than 64 negatives, no
+    positives; run twice: bit-identical."""
+    rng = np.random.default_rng(n)
+    s = (np.round(rng.standard_normal(n) * 8) / 4).astype(np.float32)
+    y = (rng.random(n) < pos_rate).astype(np.int32)
+    y[rng.random(n) < 0.1] = -100
+    rows = rng.standard_normal((12, 64)).astype(np.float32) * 0.2
+    want_t, want_g = oracle.train_loss(s.astype(np.float64), y, rows.astype(np.float64))
+    w = wl.small(seed=3, shape=wl.ModelShape(1, 2, 1, 64, "bf16"), n_tokens=64, budget=16, kv_dtype="bf16")
+    gc.to_cuda(w)
+    ctx = gc.make_ctx(w)
+    outs = []
+    for _ in range(2):
+        terms = torch.full((5,), float("nan"), device="cuda")
+        grad = torch.full((n,), float("nan"), device="cuda")
+        ctx.train_loss(torch.from_numpy(s).cuda(), torch.from_numpy(y).cuda(), terms, grad, torch.from_numpy(rows).cuda())
+        torch.cuda.synchronize()
+        outs.append((terms.cpu().numpy().astype(np.float64), grad.cpu().numpy().astype(np.float64)))
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    got_t, got_g = outs[0]
+    assert np.all(np.abs(got_t - want_t) <= 1e-5 * np.maximum(1e-3, np.abs(want_t))), (got_t, want_t)
+    assert np.all(np.abs(got_g - want_g) <= 1e-7 + 1e-4 * np.abs(want_g)), np.abs(got_g - want_g).max()
+    assert np.all(got_g[(y != 0) & (y != 1)] == 0.0)
+    print(f"[n={n}] Eq. 8 terms {got_t}, max |dL/ds err| {np.abs(got_g - want_g).max():.2e}")
