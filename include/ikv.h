@@ -196,7 +196,9 @@ ikv_status ikv_decode_attn_static(ikv_ctx *ctx, int32_t layer, const ikv_request
  * over the candidates of Eq. 3 and the rows are combined with the HOST weights[n_rows]:
  *   s_j = sum_r weights[r] sum_{l,h} softmax_{i in A}(rows[r,l,h] . K[l, h div G, S[i]] / sqrt(D))_j.
  * n_rows = 1, weights = {1}, rows = M_t is ikv_score(IKV_MODE_MEMORY) bit for bit.  scores as in ikv_score (fillers
- * included).  One pass over the keys per row. */
+ * included).  Below six rows: one pass over the keys per row.  From six rows on (bf16 pools): banks of 128 / G rows as a
+ * dense tile on tcgen05, two sweeps over the keys per bank (IKV_TUNE_ROWS_TC).  The first call allocates the bank and
+ * its partials (cudaMalloc). */
 ikv_status ikv_score_rows(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req, const float *rows, int32_t n_rows,
                           const float *weights, float *scores, void *stream);
 
@@ -227,7 +229,10 @@ ikv_status ikv_score_baseline(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_r
  * rows at logical positions q_pos0 .. q_pos0 + n_q - 1 of the request (q_pos0 + n_q <= req->seq_len); row i attends,
  * causally, every position j <= q_pos0 + i with S[j] != s+.  q, out: DEVICE [n_q][H_q][D], pool dtype.
  * kv_reads: optional DEVICE int64[2], ACCUMULATED: [0] += sum_i (q_pos0 + i + 1) = Raw KV Reads sum |R_t|,
- * [1] += sum_i #{j <= q_pos0 + i : S[j] != s+} = Eff. KV Reads sum |K_t|. */
+ * [1] += sum_i #{j <= q_pos0 + i : S[j] != s+} = Eff. KV Reads sum |K_t|.
+ * bf16 pools: one tiled launch per 1,024 rows (IKV_TUNE_PREFILL_TILED); the session's cached survivor list is brought to
+ * cover a prefix [0, covered), covered <= q_pos0 (rebuilt from the slot map when it is stale or reaches into the chunk),
+ * exactly as ikv_decode_attn maintains it; the scratch for the split partials grows on demand (cudaMalloc). */
 ikv_status ikv_prefill_attn(ikv_ctx *ctx, int32_t layer, const ikv_request *req, int32_t q_pos0, int32_t n_q, const void *q,
                             void *out, float sm_scale, int64_t *kv_reads, void *stream);
 
