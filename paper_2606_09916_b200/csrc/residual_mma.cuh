@@ -251,24 +251,72 @@ struct ResidMmaParams {
   float* scores;             // by position
 };
 
-__device__ __forceinline__ float ex2f(float x);
-// erf-GELU (exact GELU, not the tanh form) with erf from Abramowitz & Stegun 7.1.26, |error| <= 1.5e-7:
-// measured against fp64 over [-12, 12] the result is within 3.4e-7 absolute, the fp32 evaluation of
-// 0.5 x (1 + erff(x / sqrt 2)) within 4.5e-7; it costs a third of erff's instructions (the epilogue is issue-bound).
-__device__ __forceinline__ float gelu_erf(float x) {
-  const float u = fabsf(x) * 0.70710678118654752f;
-  const float t = __fdividef(1.f, fmaf(0.3275911f, u, 1.f));
-  float poly = fmaf(1.061405429f, t, -1.453152027f);
-  poly = fmaf(poly, t, 1.421413741f);
-  poly = fmaf(poly, t, -0.284496736f);
-  poly = fmaf(poly, t, 0.254829592f);
-  const float q = 0.5f * poly * t * ex2f(-1.4426950408889634f * u * u);  // 0.5 (1 - erf(u))
-  return x >= 0.f ? fmaf(-x, q, x) : x * q;
-}
 __device__ __forceinline__ float ex2f(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
+}
+// erf-GELU (exact GELU, not the tanh form) as  gelu(x) = max(x, 0) - |x| q(|x|),  q(a) = Phi(-a) =
+// 0.5 erfc(a / sqrt 2) = 2^P(a)  with P a degree-7 polynomial fitted (weighted minimax over a in [0, 6], weight a q(a):
+// the error of gelu itself) to log2(0.5 erfc(a / sqrt 2)); beyond a = 6, q < 1e-9 and a is clamped.  Against fp64 the
+// fp32 Horner evaluation is within 7e-8 absolute over [-8, 8] (Abramowitz & Stegun 7.1.26, used before: 2.1e-7, and a
+// reciprocal more).  One MUFU and 8 FMAs per element; the coefficients below are those of P(-n) for n = -|x|.
+constexpr float GELU_A = 6.0f;
+constexpr float GELU_C0 = -1.0f, GELU_C1 = 1.151126929e+00f, GELU_C2 = -4.590439269e-01f, GELU_C3 = 5.294857004e-02f,
+                GELU_C4 = 7.670789278e-03f, GELU_C5 = 5.757889713e-04f, GELU_C6 = -1.279755249e-05f,
+                GELU_C7 = -4.278683871e-06f;
+__device__ __forceinline__ float gelu_erf(float x) {
+  const float nax = -fabsf(x), n = fmaxf(nax, -GELU_A);
+  float pl = fmaf(GELU_C7, n, GELU_C6);
+  pl = fmaf(pl, n, GELU_C5);
+  pl = fmaf(pl, n, GELU_C4);
+  pl = fmaf(pl, n, GELU_C3);
+  pl = fmaf(pl, n, GELU_C2);
+  pl = fmaf(pl, n, GELU_C1);
+  pl = fmaf(pl, n, GELU_C0);
+  return fmaf(nax, ex2f(pl), fmaxf(x, 0.f));
+}
+
+// Two fp32 lanes per instruction (fma.rn.f32x2, sm_100): the epilogue and softmax loops of k_tail_tc are bound by
+// the FMA pipe's issue rate, which a packed instruction uses once for two elements.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) {
+  f32x2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void upk2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+  f32x2 d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+  f32x2 d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+  f32x2 d;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+// gelu of two values, same arithmetic as gelu_erf (bit-identical results)
+__device__ __forceinline__ f32x2 gelu_erf2(f32x2 x) {
+  float x0, x1;
+  upk2(x, x0, x1);
+  const float na0 = -fabsf(x0), na1 = -fabsf(x1);
+  const f32x2 n = pk2(fmaxf(na0, -GELU_A), fmaxf(na1, -GELU_A));
+  f32x2 pl = fma2(pk2(GELU_C7, GELU_C7), n, pk2(GELU_C6, GELU_C6));
+  pl = fma2(pl, n, pk2(GELU_C5, GELU_C5));
+  pl = fma2(pl, n, pk2(GELU_C4, GELU_C4));
+  pl = fma2(pl, n, pk2(GELU_C3, GELU_C3));
+  pl = fma2(pl, n, pk2(GELU_C2, GELU_C2));
+  pl = fma2(pl, n, pk2(GELU_C1, GELU_C1));
+  pl = fma2(pl, n, pk2(GELU_C0, GELU_C0));
+  float p0, p1;
+  upk2(pl, p0, p1);
+  return fma2(pk2(na0, na1), pk2(ex2f(p0), ex2f(p1)), pk2(fmaxf(x0, 0.f), fmaxf(x1, 0.f)));
 }
 
 // ---- k_residual_mma: CTA = R_CWARPS consumer warps (one 16-candidate tile each) + 1 producer / MMA-issuer warp.

@@ -464,18 +464,28 @@ __global__ __launch_bounds__(RT_TAIL_THREADS, 1) void k_tail_tc(const TailParams
     // hid = acc + b1' + rule w_r -> erf-GELU -> fc2 dot; the two halves of a row are added through shared memory
     auto epilogue = [&](int tile, float rule) {
       const int tok = tile * RT_M + m;
-      float z = 0.f;
+      f32x2 z2 = pk2(0.f, 0.f);
+      const f32x2 rule2 = pk2(rule, rule);
 #pragma unroll 1
       for (int c0 = 0; c0 < 128; c0 += 16) {
         float v[16];
         tmem_ld16(tmem + ((uint32_t)(qd * 32) << 16) + (uint32_t)(256 + nh * 128 + c0), v);
         tmem_ld_wait();
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
+        for (int j = 0; j < 16; j += 4) {  // two hidden units per packed instruction; weights as 16-byte broadcasts
           const int n = nh * 128 + c0 + j;
-          z = fmaf(ep_w2[n], gelu_erf(v[j] + fmaf(rule, ep_wr[n], ep_b1[n])), z);
+          const float4 wr = *reinterpret_cast<const float4*>(&ep_wr[n]);
+          const float4 b1 = *reinterpret_cast<const float4*>(&ep_b1[n]);
+          const float4 w2 = *reinterpret_cast<const float4*>(&ep_w2[n]);
+          const f32x2 ha = fma2(rule2, pk2(wr.x, wr.y), add2(pk2(v[j], v[j + 1]), pk2(b1.x, b1.y)));
+          const f32x2 hb = fma2(rule2, pk2(wr.z, wr.w), add2(pk2(v[j + 2], v[j + 3]), pk2(b1.z, b1.w)));
+          z2 = fma2(pk2(w2.x, w2.y), gelu_erf2(ha), z2);
+          z2 = fma2(pk2(w2.z, w2.w), gelu_erf2(hb), z2);
         }
       }
+      float z, zb;
+      upk2(z2, z, zb);
+      z += zb;
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
       __syncwarp();
       if (lane == 0) mbar_arrive(tmem_free);
@@ -540,18 +550,33 @@ __global__ __launch_bounds__(RT_TAIL_THREADS, 1) void k_tail_tc(const TailParams
           for (int c0 = 0; c0 < RT_NXMAX; c0 += 16)
             if (c0 < NXP) tmem_ld16(tmem + ((uint32_t)(qd * 32) << 16) + (uint32_t)(h * NXP + c0), &x[c0]);
           tmem_ld_wait();
+          // two columns per packed fp32 instruction; s_r, s_b as 16-byte broadcasts
+          const f32x2 rule2 = pk2(rule, rule);
           float mx = -CUDART_INF_F;
 #pragma unroll
-          for (int c = 0; c < RT_NXMAX; ++c)
+          for (int c = 0; c < RT_NXMAX; c += 4)
             if (c < NXP) {
-              x[c] = fmaf(rule, sv_r[h * NXP + c], x[c]) + sv_b[h * NXP + c];
-              mx = fmaxf(mx, x[c]);
+              const float4 sr = *reinterpret_cast<const float4*>(&sv_r[h * NXP + c]);
+              const float4 sb = *reinterpret_cast<const float4*>(&sv_b[h * NXP + c]);
+              upk2(fma2(rule2, pk2(sr.x, sr.y), add2(pk2(x[c], x[c + 1]), pk2(sb.x, sb.y))), x[c], x[c + 1]);
+              upk2(fma2(rule2, pk2(sr.z, sr.w), add2(pk2(x[c + 2], x[c + 3]), pk2(sb.z, sb.w))), x[c + 2], x[c + 3]);
+              mx = fmaxf(fmaxf(mx, fmaxf(x[c], x[c + 1])), fmaxf(x[c + 2], x[c + 3]));
             }
-          float l = 0.f;
+          const f32x2 nmx2 = pk2(-mx, -mx);
+          f32x2 l2 = pk2(0.f, 0.f);
 #pragma unroll
-          for (int c = 0; c < RT_NXMAX; ++c)
-            if (c < NXP) { x[c] = ex2f(x[c] - mx); l += x[c]; }
+          for (int c = 0; c < RT_NXMAX; c += 2)
+            if (c < NXP) {
+              float d0, d1;
+              upk2(add2(pk2(x[c], x[c + 1]), nmx2), d0, d1);
+              x[c] = ex2f(d0); x[c + 1] = ex2f(d1);
+              l2 = add2(l2, pk2(x[c], x[c + 1]));
+            }
+          float l, lb;
+          upk2(l2, l, lb);
+          l += lb;
           const float inv = 1.f / l;
+          const f32x2 inv2 = pk2(inv, inv), m1 = pk2(-1.f, -1.f);
           if (hp == 1 && hh == 0) mbar_wait(ak_free, par);  // heads 2, 3 overwrite the kbar rows
           unsigned char* base = (h < 2 ? p01 + h * HR : region0 + (h - 2) * HR) + (m >> 3) * (16 * NXP) + (m & 7) * 16;
 #pragma unroll
@@ -559,7 +584,14 @@ __global__ __launch_bounds__(RT_TAIL_THREADS, 1) void k_tail_tc(const TailParams
             if (g * 8 < NXP) {
               uint32_t hi[4], lo[4];
 #pragma unroll
-              for (int e = 0; e < 4; ++e) split_bf16(x[g * 8 + 2 * e] * inv, x[g * 8 + 2 * e + 1] * inv, hi[e], lo[e]);
+              for (int e = 0; e < 4; ++e) {  // split_bf16 of the normalised pair, the subtraction packed
+                const f32x2 pn = mul2(pk2(x[g * 8 + 2 * e], x[g * 8 + 2 * e + 1]), inv2);
+                float a, b;
+                upk2(pn, a, b);
+                hi[e] = pack_bf16_rn(a, b);
+                upk2(fma2(pk2(bf16lo(hi[e]), bf16hi(hi[e])), m1, pn), a, b);
+                lo[e] = pack_bf16_rn(a, b);
+              }
               *reinterpret_cast<uint4*>(base + g * 128) = make_uint4(hi[0], hi[1], hi[2], hi[3]);
               *reinterpret_cast<uint4*>(base + g * 128 + HR / 2) = make_uint4(lo[0], lo[1], lo[2], lo[3]);
             }
