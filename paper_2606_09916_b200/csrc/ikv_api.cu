@@ -1,5 +1,6 @@
 // ikv_api.cu -- C-ABI of libikv (include/ikv.h): host-side session/scratch manager and kernel launches.
 // Everything on the hot path runs in the kernels of score.cuh / residual.cuh / select.cuh / decode.cuh.
+#include <cuda.h>
 #include <limits.h>
 #include <math.h>
 #include <stdio.h>
@@ -117,7 +118,9 @@ struct ikv_ctx : Scratch {
   std::string static_scratch_err;           // why it could not be resolved
 
   bool pf_attr_done[2][9] = {};
-  bool pt_attr_done[2][9] = {};
+  bool pt_attr_done[2][2][9] = {};
+  CUtensorMap tm_k, tm_v;    // the pools as 2-D tensors [L n_slots H_kv][D], box 64 x 1, SWIZZLE_128B (TMA gather4)
+  bool tm_ok = false;
   int prefill_tiled = 1;     // IKV_TUNE_PREFILL_TILED: 0 = ikv_prefill_attn row by row through the decode kernels
   // multi-row scorer on tcgen05 (score_rows_tc.cuh)
   int rows_tc = 1;           // IKV_TUNE_ROWS_TC
@@ -950,15 +953,15 @@ ikv_status launch_prefill(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaStr
   LAUNCH_CHECK(c);
   return IKV_OK;
 }
-template <int D, int G>
+template <int D, int G, bool TG>
 ikv_status launch_prefill_tc(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaStream_t st) {
-  auto fn = k_prefill_tc<D, G>;
-  if (!c->pt_attr_done[D == 128][G]) {
-    CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pt_smem<D>()));
-    c->pt_attr_done[D == 128][G] = true;
+  auto fn = k_prefill_tc<D, G, TG>;
+  if (!c->pt_attr_done[TG][D == 128][G]) {
+    CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pt_smem<D, TG>()));
+    c->pt_attr_done[TG][D == 128][G] = true;
   }
   constexpr int BR = 128 / G;
-  fn<<<dim3(p.n_split, p.Hkv, (p.n_q + BR - 1) / BR), PT_THREADS, pt_smem<D>(), st>>>(p);
+  fn<<<dim3(p.n_split, p.Hkv, (p.n_q + BR - 1) / BR), TG ? PT_THREADS_TG : PT_THREADS, pt_smem<D, TG>(), st>>>(p, c->tm_k, c->tm_v);
   LAUNCH_CHECK(c);
   k_prefill_merge<D><<<dim3(p.Hkv * G, p.n_q), D, 0, st>>>(p.part_o, p.part_ml, p.n_split, out);
   LAUNCH_CHECK(c);
@@ -966,12 +969,20 @@ ikv_status launch_prefill_tc(ikv_ctx* c, const PrefillParams& p, bf16* out, cuda
 }
 template <int D>
 ikv_status dispatch_prefill(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaStream_t st) {
-  if (c->prefill_tiled == 1) {   // tcgen05 where 128 / G rows x G heads make a 128-row tile
+  if (c->prefill_tiled == 1 && c->tm_ok) {   // tcgen05 where 128 / G rows x G heads make a 128-row tile; TMA gather4
     switch (c->G) {
-      case 1: return launch_prefill_tc<D, 1>(c, p, out, st);
-      case 2: return launch_prefill_tc<D, 2>(c, p, out, st);
-      case 4: return launch_prefill_tc<D, 4>(c, p, out, st);
-      case 8: return launch_prefill_tc<D, 8>(c, p, out, st);
+      case 1: return launch_prefill_tc<D, 1, true>(c, p, out, st);
+      case 2: return launch_prefill_tc<D, 2, true>(c, p, out, st);
+      case 4: return launch_prefill_tc<D, 4, true>(c, p, out, st);
+      case 8: return launch_prefill_tc<D, 8, true>(c, p, out, st);
+    }
+  }
+  if (c->prefill_tiled == 1 || c->prefill_tiled == 3) {   // the same with cp.async producers (no tensor map)
+    switch (c->G) {
+      case 1: return launch_prefill_tc<D, 1, false>(c, p, out, st);
+      case 2: return launch_prefill_tc<D, 2, false>(c, p, out, st);
+      case 4: return launch_prefill_tc<D, 4, false>(c, p, out, st);
+      case 8: return launch_prefill_tc<D, 8, false>(c, p, out, st);
     }
   }
   switch (c->G) {
@@ -1009,13 +1020,14 @@ ikv_status prefill_tiled(ikv_ctx* c, int layer, const ikv_request& r, int q_pos0
   p.k_layer = (const bf16*)c->cfg.k_pool + (int64_t)layer * c->layer_stride;
   p.v_layer = (const bf16*)c->cfg.v_pool + (int64_t)layer * c->layer_stride;
   p.Hkv = Hkv; p.dead = c->cfg.dead_slot; p.S = r.slot_map; p.live_slots = s->live_slots;
+  p.row0 = (int64_t)layer * c->cfg.n_slots * Hkv;
   p.n_live = s->d_n_live; p.n_cached = s->live_ub; p.covered = s->covered;
   p.scale_log2 = sm_scale * 1.4426950408889634f;
   for (int g0 = 0; g0 < n_q; g0 += 1024) {
     const int ng = std::min(1024, n_q - g0);
     p.q_pos0 = q_pos0 + g0; p.n_q = ng;
     p.q = q + (size_t)g0 * Hq * D;
-    const bool tc = c->prefill_tiled == 1 && c->G != 5;
+    const bool tc = (c->prefill_tiled == 1 || c->prefill_tiled == 3) && c->G != 5;
     const int br = tc ? 128 / c->G : PF_BR;
     const int rbs = (ng + br - 1) / br;
     const int tiles = (p.n_cached + (p.q_pos0 + ng - p.covered) + PF_TOK - 1) / PF_TOK;   // upper bound
@@ -1206,6 +1218,29 @@ ikv_status ikv_create(const ikv_config* cfg, ikv_ctx** out) {
     const cudaError_t e = cudaGetSymbolAddress(&sp, g_static_scratch);
     if (e == cudaSuccess) c->static_scratch = (unsigned char*)sp;
     else c->static_scratch_err = cudaGetErrorString(e);
+    cudaGetLastError();
+  }
+  if (cfg->kv_dtype == IKV_BF16 && (cfg->head_dim == 64 || cfg->head_dim == 128)) {
+    // tensor maps of the pools for the TMA gather4 producers of k_prefill_tc; without them the cp.async producers run
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    EncodeFn enc = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    const int64_t rows = (int64_t)cfg->n_layers * cfg->n_slots * cfg->n_kv_heads;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", (void**)&enc, cudaEnableDefault, &qr) == cudaSuccess && enc &&
+        qr == cudaDriverEntryPointSuccess && rows < INT_MAX && ((uintptr_t)cfg->k_pool & 15) == 0 &&
+        ((uintptr_t)cfg->v_pool & 15) == 0) {
+      const cuuint64_t gdim[2] = {(cuuint64_t)cfg->head_dim, (cuuint64_t)rows}, gstr[1] = {(cuuint64_t)cfg->head_dim * 2};
+      const cuuint32_t box[2] = {64, 1}, estr[2] = {1, 1};
+      const CUresult rk = enc(&c->tm_k, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, cfg->k_pool, gdim, gstr, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      const CUresult rv = enc(&c->tm_v, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, cfg->v_pool, gdim, gstr, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+      c->tm_ok = rk == CUDA_SUCCESS && rv == CUDA_SUCCESS;
+    }
     cudaGetLastError();
   }
   *out = c;

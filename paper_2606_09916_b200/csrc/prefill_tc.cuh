@@ -12,24 +12,49 @@
 //                        maximum (moved, with a rescale of the row's O and l, only when a tile's maximum exceeds it by
 //                        more than 2^8), P as bf16 into the canonical A operand [128 x 64].
 // Partials (reference m, l, O) per (row, head, split) as in prefill_mma.cuh; k_prefill_merge combines them.
+//
+// TG = true (the pool is covered by a tensor map, ikv_create): the producers do not touch the data.  Sixteen lanes of each
+// of the four producer warps issue one TMA tile::gather4 each per tile (four rows of 128 bytes per instruction, the row =
+// (layer, slot, KV head) of the pool seen as a 2-D tensor [rows][D]; dead items get an out-of-range row: zero fill) with
+// SWIZZLE_128B, which lands K as the K-major and V as the MN-major 128-byte-swizzled operand of tcgen05.mma: no
+// transposition pass, no staging buffer (its memory holds a second P buffer).  A gather4 costs its issuing warp ~75
+// cycles whatever the lane count, so the issue is spread over the warps: 64 KB-pieces of 256 bytes arrive at 19-27 B per
+// cycle per SM against 12-15 for cp.async or 256-byte bulk copies (micro-benchmark).
 #pragma once
+#include <cuda.h>
 #include "prefill_mma.cuh"
 
 namespace ikv {
 
 constexpr int PT_TOK = 64;            // items per tile
 constexpr int PT_THREADS = 9 * 32;    // 4 softmax warps, 4 producer warps, MMA warp
+constexpr int PT_PW_TG = 8;           // producer warps of the tensor-map path (64 / PT_PW_TG issuing lanes each)
+constexpr int PT_THREADS_TG = (5 + PT_PW_TG) * 32;
 constexpr int PT_NB = 4;               // K / V^T buffers: the gathers run three tiles ahead of the MMAs
+constexpr int PT_NB_TG = 4;            // the same on the tensor-map path (no staging buffers)
 constexpr int PT_PB = 1;               // P buffers (shared memory: 4 K / V^T buffers leave room for one)
 constexpr float PT_GROW = 8.f;        // log2 units a tile's maximum may exceed the reference before it moves
 
 template <int D>
 __host__ __device__ constexpr int pt_vst() { return D * 2 + 16; }   // staged V row stride (conflict-free ldmatrix)
-template <int D>
+template <int D, bool TG = false>
 __host__ __device__ constexpr int pt_smem() {
-  // Q | K[3] | V^T[3] | V staging[2] | P[2] | minrow[3][64] | barriers
-  return 128 * D * 2 + PT_NB * (PT_TOK * D * 2 + D * PT_TOK * 2) + 2 * PT_TOK * pt_vst<D>() + PT_PB * 128 * PT_TOK * 2 +
-         PT_NB * PT_TOK * 4 + 256;
+  // Q | K[NB] | V^T[NB] | V staging[2] (cp.async path) | P[1 or 2] | minrow[NB][64] | barriers
+  return 128 * D * 2 + (TG ? PT_NB_TG : PT_NB) * (PT_TOK * D * 2 + D * PT_TOK * 2 + PT_TOK * 4) +
+         (TG ? 0 : 2 * PT_TOK * pt_vst<D>()) + (TG ? 2 : PT_PB) * 128 * PT_TOK * 2 + 256;
+}
+// shared-memory matrix descriptors of the 128-byte-swizzled operands the tensor map writes ([rows][128 B], 8-row atoms of
+// 1 KB): K-major (start address advanced by 32 B per 16 k) and MN-major (64 contiguous n per atom, the next 64 at `lbo`)
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+  return (uint64_t)((saddr >> 4) & 0x3fff) | ((uint64_t)((lbo >> 4) & 0x3fff) << 16) |
+         ((uint64_t)((sbo >> 4) & 0x3fff) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+}
+__device__ __forceinline__ void tma_gather4(uint32_t dst, const CUtensorMap* tm, uint64_t* bar, int col, int r0, int r1, int r2,
+                                            int r3) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];" ::"r"(dst),
+      "l"(tm), "r"(smem_u32(bar)), "r"(col), "r"(r0), "r"(r1), "r"(r2), "r"(r3)
+      : "memory");
 }
 // canonical K-major (no swizzle) offset of the 16-byte entry (row n, k-group k8) of an operand with kdim elements of K
 __host__ __device__ __forceinline__ int pt_entry(int n, int k8, int kdim) { return (n >> 3) * (kdim / 8) * 128 + k8 * 128 + (n & 7) * 16; }
@@ -44,9 +69,13 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const float* v) {
       : "memory");
 }
 
-template <int D, int G>
-__global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParams p) {
+template <int D, int G, bool TG>
+__global__ __launch_bounds__(TG ? PT_THREADS_TG : PT_THREADS, 1) void k_prefill_tc(const PrefillParams p, const __grid_constant__ CUtensorMap tmk,
+                                                              const __grid_constant__ CUtensorMap tmv) {
   constexpr int BR = 128 / G;                // chunk rows per CTA
+  constexpr int NPB = TG ? 2 : PT_PB;        // P buffers
+  constexpr int NB = TG ? PT_NB_TG : PT_NB;  // K / V buffers
+  constexpr int NPW = TG ? PT_PW_TG : 4, MMA_WARP = 4 + NPW;
   constexpr int CPR = D / 8;                 // 16-byte chunks per K / V row
   constexpr int VST = pt_vst<D>();
   constexpr int QB = 128 * D * 2, KB = PT_TOK * D * 2, VTB = D * PT_TOK * 2, VSB = PT_TOK * VST, PB = 128 * PT_TOK * 2;
@@ -55,27 +84,27 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
   extern __shared__ __align__(1024) unsigned char pt_smem_raw[];
   unsigned char* q_s = pt_smem_raw;
   unsigned char* k_s = q_s + QB;                 // [3][KB]
-  unsigned char* vt_s = k_s + PT_NB * KB;        // [3][VTB]
-  unsigned char* vst_s = vt_s + PT_NB * VTB;     // [2][VSB]: one per producer group
-  unsigned char* p_s = vst_s + 2 * VSB;          // [2][PB]
-  int* minrow_s = reinterpret_cast<int*>(p_s + PT_PB * PB);   // [3][PT_TOK]
-  uint64_t* bars = reinterpret_cast<uint64_t*>(minrow_s + PT_NB * PT_TOK);
-  uint64_t* kv_full = bars;                 // [PT_NB] operands K, V^T and minrow of a tile are in shared memory (64 threads)
-  uint64_t* kv_free = kv_full + PT_NB;      // [PT_NB] the MMAs that read them have completed
-  uint64_t* s_full = kv_free + PT_NB;       // [2] S accumulator complete
+  unsigned char* vt_s = k_s + NB * KB;        // [3][VTB]
+  unsigned char* vst_s = vt_s + NB * VTB;     // [2][VSB]: one per producer group
+  unsigned char* p_s = vst_s + (TG ? 0 : 2 * VSB);   // [NPB][PB]
+  int* minrow_s = reinterpret_cast<int*>(p_s + NPB * PB);   // [NB][PT_TOK]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(minrow_s + NB * PT_TOK);
+  uint64_t* kv_full = bars;                 // [NB] operands K, V^T and minrow of a tile are in shared memory (64 threads)
+  uint64_t* kv_free = kv_full + NB;      // [NB] the MMAs that read them have completed
+  uint64_t* s_full = kv_free + NB;       // [2] S accumulator complete
   uint64_t* s_free = s_full + 2;            // [2] every softmax thread has read it
-  uint64_t* p_full = s_free + 2;            // [PT_PB] P written (and O rescaled) by every softmax thread
-  uint64_t* p_free = p_full + PT_PB;        // [PT_PB] P V of the buffer's tile complete
-  uint64_t* q_ready = p_free + PT_PB;
+  uint64_t* p_full = s_free + 2;            // [NPB] P written (and O rescaled) by every softmax thread
+  uint64_t* p_free = p_full + NPB;          // [NPB] P V of the buffer's tile complete
+  uint64_t* q_ready = p_free + NPB;
   uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(q_ready + 1);
 
   const int split = blockIdx.x, kvh = blockIdx.y, rb = blockIdx.z;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int Hq = p.Hkv * G;
   if (threadIdx.x == 0) {
-    for (int b = 0; b < PT_NB; ++b) { mbar_init(&kv_full[b], 64); mbar_init(&kv_free[b], 1); }
+    for (int b = 0; b < NB; ++b) { mbar_init(&kv_full[b], 64); mbar_init(&kv_free[b], 1); }
     for (int b = 0; b < 2; ++b) { mbar_init(&s_full[b], 1); mbar_init(&s_free[b], 128); }
-    for (int b = 0; b < PT_PB; ++b) { mbar_init(&p_full[b], 128); mbar_init(&p_free[b], 1); }
+    for (int b = 0; b < NPB; ++b) { mbar_init(&p_full[b], 128); mbar_init(&p_free[b], 1); }
     mbar_init(q_ready, 128);
     mbar_fence_init();
   }
@@ -97,7 +126,44 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
   const int t_end = min((int)(((int64_t)tiles_all * (split + 1)) / p.n_split), (lim + PT_TOK - 1) / PT_TOK);
   const int n_t = max(0, t_end - t_begin);
 
-  if (warp >= 4 && warp < 8) {
+  if (TG && warp >= 4 && warp < MMA_WARP) {
+    // ------------------------------------------------------------------ producers, tensor-map path: lane < LPW of warp
+    // 4 + pw is thread j = LPW pw + lane: it writes minrow of item j and issues gather4 o = pw OPW + lane (lane < OPW)
+    constexpr int HALVES = D / 64, OPS = 2 * HALVES * 16, OPW = OPS / NPW, LPW = PT_TOK / NPW;
+    if (lane < LPW) {
+      const int pw = warp - 4, j = pw * LPW + lane;
+      const int o = pw * OPW + lane, mat = o / (OPS / 2), rem = o % (OPS / 2), quad = rem / HALVES, half = rem % HALVES;
+      const bool op = lane < OPW;
+      auto slot_at = [&](int idx) -> int {
+        return idx < lim ? (idx < n_cached ? p.live_slots[idx] : p.S[p.covered + (idx - n_cached)]) : p.dead;
+      };
+      int sj = p.dead, s4[4] = {p.dead, p.dead, p.dead, p.dead};
+      auto load_slots = [&](int tile) {
+        sj = slot_at(tile * PT_TOK + j);
+        if (op) {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) s4[e] = slot_at(tile * PT_TOK + quad * 4 + e);
+        }
+      };
+      if (n_t > 0) load_slots(t_begin);
+      for (int it = 0; it < n_t; ++it) {
+        const int b = it % NB, tile = t_begin + it;
+        mbar_wait(&kv_free[b], ((uint32_t)(it / NB) & 1u) ^ 1u);   // P V of tile it - NB has completed
+        const int idx = tile * PT_TOK + j;
+        minrow_s[b * PT_TOK + j] = sj == p.dead ? INT_MAX : (idx < n_cached ? INT_MIN : p.covered + (idx - n_cached) - p.q_pos0);
+        if (j == 0) mbar_arrive_expect_tx(&kv_full[b], (uint32_t)(OPS * 512));
+        else mbar_arrive(&kv_full[b]);
+        if (op) {
+          int r[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) r[e] = s4[e] == p.dead ? -1 : (int)(p.row0 + (int64_t)s4[e] * p.Hkv + kvh);
+          const uint32_t dst = smem_u32(mat ? vt_s : k_s) + (uint32_t)(b * KB + half * (PT_TOK * 128) + quad * 512);
+          tma_gather4(dst, mat ? &tmv : &tmk, &kv_full[b], half * 64, r[0], r[1], r[2], r[3]);
+        }
+        if (it + 1 < n_t) load_slots(tile + 1);
+      }
+    }
+  } else if (!TG && warp >= 4 && warp < 8) {
     // ------------------------------------------------------------------ producers: two groups of two warps, group gp
     // takes the tiles it = gp, gp + 2, ...: the gather latency of one group's tile hides under the other group's
     constexpr int CPT = PT_TOK * CPR / 64;      // chunks per thread per matrix
@@ -113,8 +179,8 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
     const uint32_t vd = smem_u32(vst_s) + (uint32_t)(gp * VSB);   // the group's staging buffer
     if (gp < n_t) load_slots(t_begin + gp);
     for (int it = gp; it < n_t; it += 2) {
-      const int b = it % PT_NB, tile = t_begin + it;
-      mbar_wait(&kv_free[b], ((uint32_t)(it / PT_NB) & 1u) ^ 1u);   // P V of tile it - 3 has completed
+      const int b = it % NB, tile = t_begin + it;
+      mbar_wait(&kv_free[b], ((uint32_t)(it / NB) & 1u) ^ 1u);   // P V of tile it - 3 has completed
       const uint32_t kd = smem_u32(k_s) + (uint32_t)(b * KB);
 #pragma unroll
       for (int j = 0; j < CPT; ++j) {
@@ -150,37 +216,53 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
       mbar_arrive(&kv_full[b]);
       bar_sync(2 + gp, 64);   // the staging buffer is free for the group's next tile
     }
-  } else if (warp == 8) {
+  } else if (warp == MMA_WARP) {
     // ------------------------------------------------------------------ MMA issuer (one thread)
     if (lane == 0 && n_t > 0) {
       const uint32_t ibase = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 4) << 24);
       const uint32_t idesc_s = ibase | (((uint32_t)PT_TOK >> 3) << 17), idesc_o = ibase | (((uint32_t)D >> 3) << 17);
       const uint64_t dq = umma_desc(smem_u32(q_s), 128, SBO_D);
       auto issue_s = [&](int it) {
-        const int b = it & 1, kb = it % PT_NB;
-        mbar_wait(&kv_full[kb], (uint32_t)(it / PT_NB) & 1u);
+        const int b = it & 1, kb = it % NB;
+        mbar_wait(&kv_full[kb], (uint32_t)(it / NB) & 1u);
         mbar_wait(&s_free[b], ((uint32_t)(it >> 1) & 1u) ^ 1u);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint64_t dk = umma_desc(smem_u32(k_s) + (uint32_t)(kb * KB), 128, SBO_D);
+        if constexpr (TG) {
+          const uint32_t ka = smem_u32(k_s) + (uint32_t)(kb * KB);
 #pragma unroll
-        for (int ks = 0; ks < D / 16; ++ks)
-          umma_bf16(tmem + (uint32_t)(b * PT_TOK), dq + (uint64_t)(ks * 16), dk + (uint64_t)(ks * 16), idesc_s, ks ? 1u : 0u);
+          for (int ks = 0; ks < D / 16; ++ks)
+            umma_bf16(tmem + (uint32_t)(b * PT_TOK), dq + (uint64_t)(ks * 16),
+                      umma_desc_sw128(ka + (uint32_t)((ks >> 2) * (PT_TOK * 128) + (ks & 3) * 32), 16, 1024), idesc_s, ks ? 1u : 0u);
+        } else {
+          const uint64_t dk = umma_desc(smem_u32(k_s) + (uint32_t)(kb * KB), 128, SBO_D);
+#pragma unroll
+          for (int ks = 0; ks < D / 16; ++ks)
+            umma_bf16(tmem + (uint32_t)(b * PT_TOK), dq + (uint64_t)(ks * 16), dk + (uint64_t)(ks * 16), idesc_s, ks ? 1u : 0u);
+        }
         umma_commit(&s_full[b]);
       };
       mbar_wait(q_ready, 0u);
       issue_s(0);
       for (int it = 0; it < n_t; ++it) {
         if (it + 1 < n_t) issue_s(it + 1);      // S of the next tile runs under this tile's softmax
-        const int pb = it % PT_PB;
-        mbar_wait(&p_full[pb], (uint32_t)(it / PT_PB) & 1u);
+        const int pb = it % NPB;
+        mbar_wait(&p_full[pb], (uint32_t)(it / NPB) & 1u);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         const uint64_t dp = umma_desc(smem_u32(p_s) + (uint32_t)(pb * PB), 128, SBO_T);
-        const uint64_t dv = umma_desc(smem_u32(vt_s) + (uint32_t)((it % PT_NB) * VTB), 128, SBO_T);
+        if constexpr (TG) {   // V [item][64 d] per column half: MN-major B, 16 items (two 8-row atoms) per instruction
+          const uint32_t va = smem_u32(vt_s) + (uint32_t)((it % NB) * VTB);
 #pragma unroll
-        for (int ks = 0; ks < PT_TOK / 16; ++ks)
-          umma_bf16(tmem + O_COL, dp + (uint64_t)(ks * 16), dv + (uint64_t)(ks * 16), idesc_o, (it | ks) ? 1u : 0u);
+          for (int ks = 0; ks < PT_TOK / 16; ++ks)
+            umma_bf16(tmem + O_COL, dp + (uint64_t)(ks * 16), umma_desc_sw128(va + (uint32_t)(ks * 2048), PT_TOK * 128, 1024),
+                      idesc_o | (1u << 16), (it | ks) ? 1u : 0u);
+        } else {
+          const uint64_t dv = umma_desc(smem_u32(vt_s) + (uint32_t)((it % NB) * VTB), 128, SBO_T);
+#pragma unroll
+          for (int ks = 0; ks < PT_TOK / 16; ++ks)
+            umma_bf16(tmem + O_COL, dp + (uint64_t)(ks * 16), dv + (uint64_t)(ks * 16), idesc_o, (it | ks) ? 1u : 0u);
+        }
         umma_commit(&p_free[pb]);
-        umma_commit(&kv_free[it % PT_NB]);
+        umma_commit(&kv_free[it % NB]);
       }
     }
   } else {
@@ -203,8 +285,8 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
     for (int it = 0; it < n_t; ++it) {
       const int b = it & 1;
       const uint32_t par = (uint32_t)(it >> 1) & 1u;
-      const int kb = it % PT_NB;
-      mbar_wait(&kv_full[kb], (uint32_t)(it / PT_NB) & 1u);   // minrow of the tile
+      const int kb = it % NB;
+      mbar_wait(&kv_full[kb], (uint32_t)(it / NB) & 1u);   // minrow of the tile
       mbar_wait(&s_full[b], par);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
       float x[PT_TOK];
@@ -229,7 +311,7 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
         const float m_new = grow ? tmax : m_ref;
         const float corr = (m_new == -CUDART_INF_F) ? 1.f : fast_exp2(m_ref - m_new);   // m_ref = -inf: 0
         if (it > 0) {   // O exists from the first P V on; wait for the previous tile's
-          mbar_wait(&p_free[(it - 1) % PT_PB], (uint32_t)((it - 1) / PT_PB) & 1u);
+          mbar_wait(&p_free[(it - 1) % NPB], (uint32_t)((it - 1) / NPB) & 1u);
           asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
           for (int c0 = 0; c0 < D; c0 += 32) {
@@ -256,8 +338,8 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
         s0 += x[c]; s1 += x[c + 1];
       }
       l += s0 + s1;
-      const int pb = it % PT_PB;
-      mbar_wait(&p_free[pb], ((uint32_t)(it / PT_PB) & 1u) ^ 1u);   // the P V that read this buffer has completed
+      const int pb = it % NPB;
+      mbar_wait(&p_free[pb], ((uint32_t)(it / NPB) & 1u) ^ 1u);   // the P V that read this buffer has completed
       unsigned char* pd = p_s + (size_t)pb * PB;
 #pragma unroll
       for (int k8 = 0; k8 < PT_TOK / 8; ++k8) {
@@ -271,7 +353,7 @@ __global__ __launch_bounds__(PT_THREADS, 1) void k_prefill_tc(const PrefillParam
     }
     // ---- partials of the split (an empty split writes m = -inf, l = 0: the scratch is not cleared)
     if (n_t > 0) {
-      mbar_wait(&p_free[(n_t - 1) % PT_PB], (uint32_t)((n_t - 1) / PT_PB) & 1u);
+      mbar_wait(&p_free[(n_t - 1) % NPB], (uint32_t)((n_t - 1) / NPB) & 1u);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     }
     const int64_t ph = ((int64_t)row * Hq + head) * p.n_split + split;
