@@ -313,13 +313,13 @@ def run_next(rig, hbm_peak):
         ms = timed(lambda: ctx.score_rows([rig.req], rows, wts, rig.scores, st))
         # the bank is a bf16 hi + lo pair: two tensor passes per product; the keys are read twice (statistics, sums)
         flop_ms = 2 * 2 * 2.0 * R * L * Hq * T * D / tensor_peak * 1e3
-        tc = R >= 6
+        tc = R >= 4
         roof = max(hbm_ms, flop_ms)
         res[f"multirow_R{R}"] = {"ms": ms, "roofline_ms": roof, "frac_of_roofline": roof / ms,
                                  "bound": "hbm" if hbm_ms >= flop_ms else "tensor",
                                  "passes_over_the_keys": 2 if tc else R,
-                                 "what": ("ikv_score_rows on tcgen05: one bank of 128 bank rows, two sweeps over the keys"
-                                          if tc else "ikv_score_rows: R passes of the single-row key pass (below 6 rows)")}
+                                 "what": ("ikv_score_rows on tcgen05: one bank of 128 bank rows, two sweeps over the keys (TMA gather4)"
+                                          if tc else "ikv_score_rows: R passes of the single-row key pass (below 4 rows)")}
     rows32 = torch.randn((32, L, Hq, D), generator=gen).to(dev).contiguous()
     res["baseline_streaming"] = {"ms": timed(lambda: ctx.score_baseline([rig.req], ikv.BASE_STREAMING, rig.scores, n_sink=4,
                                                                         stream=st)),

@@ -196,8 +196,8 @@ ikv_status ikv_decode_attn_static(ikv_ctx *ctx, int32_t layer, const ikv_request
  * over the candidates of Eq. 3 and the rows are combined with the HOST weights[n_rows]:
  *   s_j = sum_r weights[r] sum_{l,h} softmax_{i in A}(rows[r,l,h] . K[l, h div G, S[i]] / sqrt(D))_j.
  * n_rows = 1, weights = {1}, rows = M_t is ikv_score(IKV_MODE_MEMORY) bit for bit.  scores as in ikv_score (fillers
- * included).  Below six rows: one pass over the keys per row.  From six rows on (bf16 pools): banks of 128 / G rows as a
- * dense tile on tcgen05, two sweeps over the keys per bank (IKV_TUNE_ROWS_TC).  The first call allocates the bank and
+ * included).  Below four rows: one pass over the keys per row.  From four rows on (bf16 pools; six without the pool's
+ * tensor map): banks of 128 / G rows as a dense tile on tcgen05, two sweeps over the keys per bank (IKV_TUNE_ROWS_TC).  The first call allocates the bank and
  * its partials (cudaMalloc). */
 ikv_status ikv_score_rows(ikv_ctx *ctx, const ikv_request *reqs, int32_t n_req, const float *rows, int32_t n_rows,
                           const float *weights, float *scores, void *stream);
@@ -276,9 +276,11 @@ ikv_status ikv_profile_read(ikv_ctx *ctx, float *out_ms, int32_t *out_n);
 #define IKV_TUNE_LAYER_MAJOR 3 /* 1 (default): layer-major key pass with deferred normalisation (no logits scratch) when
                                   the call fits its on-chip capacity and has at least three 32-token tiles per SM;
                                   2: whenever it fits; 0: always the logits-scratch key pass                      */
-#define IKV_TUNE_ROWS_TC 5 /* 1 (default): ikv_score_rows with six or more rows on a bf16 pool runs banks of 128 / G rows on
-                              tcgen05, two sweeps over the keys per bank; 2: from two rows up; 0: one single-row pass
-                              per row                                                                            */
+#define IKV_TUNE_ROWS_TC 5 /* 1 (default): ikv_score_rows with four or more rows on a bf16 pool runs banks of 128 / G rows
+                              on tcgen05, two sweeps over the keys per bank, the keys fetched by TMA gather4 through the
+                              tensor map of the pool (six or more rows, cp.async gather warps, when ikv_create could
+                              not build the map); 2: from two rows up; 3: as 2 with the cp.async gather warps; 0: one
+                              single-row pass per row                                                            */
 #define IKV_TUNE_PREFILL_TILED 6 /* ikv_prefill_attn on a bf16 pool.  1 (default): tcgen05 kernel (128 / G query rows x G
                                     heads per CTA) for G in {1, 2, 4, 8}, its K/V tiles fetched by TMA gather4 through the
                                     tensor maps ikv_create builds over the pools; the mma.sync tiled kernel for G = 5;

@@ -1063,10 +1063,14 @@ ikv_status score_rows_tc(ikv_ctx* c, const ikv_request& r, const float* rows, in
     c->rows_partials_cap = need;
   }
   if (!c->rows_attr_done) {
-    CU(c, cudaFuncSetAttribute(k_rows_pass<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(128)));
-    CU(c, cudaFuncSetAttribute(k_rows_pass<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(128)));
-    CU(c, cudaFuncSetAttribute(k_rows_pass<64, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(64)));
-    CU(c, cudaFuncSetAttribute(k_rows_pass<64, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(64)));
+    CU(c, cudaFuncSetAttribute(k_rows_pass<128, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(128)));
+    CU(c, cudaFuncSetAttribute(k_rows_pass<128, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(128)));
+    CU(c, cudaFuncSetAttribute(k_rows_pass<64, 1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(64)));
+    CU(c, cudaFuncSetAttribute(k_rows_pass<64, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(64)));
+    CU(c, cudaFuncSetAttribute(k_rows_pass<128, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(128)));
+    CU(c, cudaFuncSetAttribute(k_rows_pass<128, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(128)));
+    CU(c, cudaFuncSetAttribute(k_rows_pass<64, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(64)));
+    CU(c, cudaFuncSetAttribute(k_rows_pass<64, 2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rb_smem(64)));
     c->rows_attr_done = true;
   }
   TRY(launch_partition(c, r, 0, scores, nullptr, st));
@@ -1083,9 +1087,12 @@ ikv_status score_rows_tc(ikv_ctx* c, const ikv_request& r, const float* rows, in
     p.n_cols = nr * G;
     p.accumulate = r0 > 0 ? 1 : 0;
     k_rows_prep<D><<<n_items, 256, 0, st>>>(rows + r0 * row_elems, nr, L, Hkv, G, wts, c->rows_bank);
-    k_rows_pass<D, 1><<<grid, RB_THREADS, rb_smem(D), st>>>(p);
+    const bool tg = c->tm_ok && c->rows_tc != 3;   // keys by TMA gather4 through the pool's tensor map
+    if (tg) k_rows_pass<D, 1, true><<<grid, RB_THREADS, rb_smem(D), st>>>(p, c->tm_k);
+    else k_rows_pass<D, 1, false><<<grid, RB_THREADS, rb_smem(D), st>>>(p, c->tm_k);
     k_rows_lse<D><<<n_items, 1024, 0, st>>>(c->rows_partials, n_slots, c->rows_bank);
-    k_rows_pass<D, 2><<<grid, RB_THREADS, rb_smem(D), st>>>(p);
+    if (tg) k_rows_pass<D, 2, true><<<grid, RB_THREADS, rb_smem(D), st>>>(p, c->tm_k);
+    else k_rows_pass<D, 2, false><<<grid, RB_THREADS, rb_smem(D), st>>>(p, c->tm_k);
     LAUNCH_CHECK(c);
   }
   k_axpy_scatter<<<64, 256, 0, st>>>(c->rule_c, c->cand_pos, c->d_ncand, 1.0f, 1, scores);
@@ -1586,8 +1593,10 @@ ikv_status ikv_score_rows(ikv_ctx* c, const ikv_request* reqs, int32_t n_req, co
   for (int r = 0; r < n_req; ++r) TRY(check_request(c, reqs[r]));
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t row_elems = (int64_t)c->cfg.n_layers * c->cfg.n_q_heads * c->cfg.head_dim;
-  // six rows and up: banks on tcgen05 (two sweeps over the keys cost about six single-row passes); rows_tc = 2 forces it
-  if (c->rows_tc && c->cfg.kv_dtype == IKV_BF16 && (n_rows >= 6 || (c->rows_tc >= 2 && n_rows >= 2))) {
+  // banks on tcgen05 from the row count at which two sweeps over the keys beat single-row passes: four rows with the TMA
+  // gather4 warps (1.13 ms against 0.38 ms per pass on configs[1]), six with cp.async; rows_tc >= 2 forces it from two
+  const int tc_from = (c->tm_ok && c->rows_tc != 3) ? 4 : 6;
+  if (c->rows_tc && c->cfg.kv_dtype == IKV_BF16 && (n_rows >= tc_from || (c->rows_tc >= 2 && n_rows >= 2))) {
     int64_t off = 0;
     for (int r = 0; r < n_req; ++r) {
       if (reqs[r].seq_len > 0)

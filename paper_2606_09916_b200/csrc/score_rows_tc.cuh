@@ -21,6 +21,7 @@
 // accumulator's columns each (the statistics are MUFU-bound: 8 cycles per ex2 warp instruction per SM sub-partition,
 // measured); eight more warps gather the keys.
 #pragma once
+#include <cuda.h>
 #include "residual_tc.cuh"
 #include "score_lm.cuh"
 
@@ -91,6 +92,18 @@ __global__ __launch_bounds__(1024) void k_rows_lse(const float2* __restrict__ pa
   }
 }
 
+// K-major, 128-byte-swizzled operand written by TMA (1 KB atoms of 8 rows), and the gather4 instruction itself
+__device__ __forceinline__ uint64_t rb_desc_sw128(uint32_t saddr) {
+  return (uint64_t)((saddr >> 4) & 0x3fff) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) |
+         ((uint64_t)2 << 61);
+}
+__device__ __forceinline__ void rb_gather4(uint32_t dst, const CUtensorMap* tm, uint64_t* bar, int col, int r0, int r1, int r2, int r3) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile::gather4.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];" ::"r"(dst),
+      "l"(tm), "r"(smem_u32(bar)), "r"(col), "r"(r0), "r"(r1), "r"(r2), "r"(r3)
+      : "memory");
+}
+
 struct RowsPassParams {
   const bf16* k_pool;
   int64_t layer_stride;  // elements
@@ -123,8 +136,8 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // Roles: warps [0, RB_CWARPS) take the statistics from TMEM; then one warp streams the banks, one issues the MMAs and
 // RB_PWARPS warps gather the keys.
 // Sub-item K = (pair of tiles, item, tile t): key buffer K % 3, TMEM buffer K & 1, bank buffer (item count) & 1.
-template <int D, int SWEEP>
-__global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParams p) {
+template <int D, int SWEEP, bool TG>
+__global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParams p, const __grid_constant__ CUtensorMap tmk) {
   constexpr int CH = D / 8;                      // 16-byte chunks of a key row of one head
   constexpr int PART = rb_part(D), ITEM = rb_item(D);
   constexpr int COPY = SWEEP == 1 ? 2 * PART : ITEM;
@@ -150,7 +163,7 @@ __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParam
       mbar_init(&bank_empty[b], SWEEP == 1 ? 1 : CT);
     }
     for (int b = 0; b < RB_TB; ++b) { mbar_init(&mma_done[b], 1); mbar_init(&tmem_free[b], CT); }
-    for (int b = 0; b < RB_KBUF; ++b) { mbar_init(&keys_ready[b], RB_PWARPS * 32); mbar_init(&keys_free[b], 1); }
+    for (int b = 0; b < RB_KBUF; ++b) { mbar_init(&keys_ready[b], TG ? 1 : RB_PWARPS * 32); mbar_init(&keys_free[b], 1); }
     mbar_fence_init();
   }
   if (warp == 0) {  // columns [0, 384): three accumulators; [384, 400): exchange between the column groups (sweep 2)
@@ -192,13 +205,16 @@ __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParam
         if (t == 0) mbar_wait(&bank_full[b], (uint32_t)(j >> 1) & 1u);
         mbar_wait(&tmem_free[buf], ((uint32_t)(K / RB_TB) & 1u) ^ 1u);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint64_t d_keys = umma_desc(keys_u32 + (uint32_t)(kb * KB), 128, SBO);
+        const uint64_t d_keys0 = umma_desc(keys_u32 + (uint32_t)(kb * KB), 128, SBO);
         const uint64_t d_hi = umma_desc(bank_u32 + (uint32_t)(b * ITEM), 128, SBO);
         const uint64_t d_lo = d_hi + (uint64_t)(PART >> 4);
         const uint32_t td = tmem + buf * 128u;
 #pragma unroll
         for (int ks = 0; ks < D / 16; ++ks) {
           const uint64_t o = (uint64_t)((ks * 256) >> 4);
+          // tensor-map gathers: keys as [column half][128 tokens][128 B], 128-byte swizzle, 32 B per 16 k inside an atom
+          const uint64_t d_keys = TG ? rb_desc_sw128(keys_u32 + (uint32_t)(kb * KB + (ks >> 2) * (RB_TOK * 128) + (ks & 3) * 32)) - o
+                                     : d_keys0;
           if (SWEEP == 1) {
             umma_bf16(td, d_hi + o, d_keys + o, idesc, ks ? 1u : 0u);
             umma_bf16(td, d_lo + o, d_keys + o, idesc, 1u);
@@ -211,6 +227,51 @@ __global__ __launch_bounds__(RB_THREADS, 1) void k_rows_pass(const RowsPassParam
         umma_commit(&keys_free[kb]);
         if (SWEEP == 1 && t == 1) umma_commit(&bank_empty[b]);   // arrives when every MMA issued so far has completed
         if (++kb == RB_KBUF) { kb = 0; kph ^= 1u; }
+      }
+    }
+  } else if (TG && warp >= RB_CWARPS + 2) {
+    // ------------------------------------------------------------------ key gather warps, tensor-map path: OPW lanes of
+    // each warp issue one TMA gather4 per sub-item (four tokens x 128 bytes of one column half of the head's keys; the
+    // issue costs a warp ~75 cycles per instruction whatever the lane count, hence eight warps); tokens beyond the
+    // candidates get an out-of-range row (zero fill).  The mbarrier of the buffer counts the bytes.
+    constexpr int HALVES = D / 64, OPS = (RB_TOK / 4) * HALVES, OPW = OPS / RB_PWARPS;
+    const int o = (warp - (RB_CWARPS + 2)) * OPW + lane, quad = o / HALVES, half = o % HALVES;
+    if (lane < OPW) {
+      const uint32_t keys_u32 = smem_u32(keys_s);
+      const int rows_per_layer = (int)(p.layer_stride / D);
+      int rw[2][4];   // slot * H_kv of this lane's four tokens in tile 0 / 1 of the pair; -1: no candidate
+      auto load_slots = [&](int pr) {
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+          const int t0 = ((2 * pr + t) * (int)gridDim.x + (int)blockIdx.x) * RB_TOK;
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int tok = t0 + quad * 4 + e;
+            rw[t][e] = tok < nc ? p.cand_slot[tok] * p.Hkv : -1;
+          }
+        }
+      };
+      int g_l = 0, g_kvh = 0, g_sub = 0, g_pr = 0, kb = 0;
+      uint32_t kph = 0u;
+      if (total > 0) load_slots(0);
+      for (int K = 0; K < total; ++K) {
+        const int t = K & 1;
+        mbar_wait(&keys_free[kb], kph ^ 1u);
+        if (o == 0) mbar_arrive_expect_tx(&keys_ready[kb], (uint32_t)KB);
+        const int base = g_l * rows_per_layer + g_kvh;
+        int r[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const int v = t ? rw[1][e] : rw[0][e];
+          r[e] = v >= 0 ? v + base : -1;
+        }
+        rb_gather4(keys_u32 + (uint32_t)(kb * KB + half * (RB_TOK * 128) + quad * 512), &tmk, &keys_ready[kb], half * 64, r[0], r[1],
+                   r[2], r[3]);
+        if (++kb == RB_KBUF) { kb = 0; kph ^= 1u; }
+        if (t == 1) {
+          if (++g_kvh == p.Hkv) { g_kvh = 0; if (++g_l == p.L) g_l = 0; }
+        }
+        if (++g_sub == n_sub) { g_sub = 0; if (++g_pr < p.n_pairs) load_slots(g_pr); }
       }
     }
   } else if (warp >= RB_CWARPS + 2) {

@@ -55,6 +55,11 @@ def test_multirow_scorer_matches_oracle(ikv, oracle, name, shape, R):
     want = np.where(cls == oracle.FORCED, np.inf, np.where(cls == oracle.DEAD, -np.inf, want))
     mabs, mrel = gc.assert_scores_close(scores.cpu().numpy(), want, f"{name} R={R}")
     print(f"[{name} R={R}] multi-row score max abs err {mabs:.3e} rel {mrel:.3e}")
+    if R >= 4:   # the cp.async gather warps (IKV_TUNE_ROWS_TC = 3) feed the tensor cores the same operands as TMA gather4
+        ctx.tune(ikv.TUNE_ROWS_TC, 3)
+        again = torch.full((s.N,), 3.0, device="cuda")
+        ctx.score_rows([req], rows.cuda().contiguous(), wt, again)
+        assert torch.equal(scores.view(torch.int32), again.view(torch.int32))
 
 
 def test_multirow_tc_several_tile_pairs(ikv, oracle):
@@ -77,6 +82,10 @@ def test_multirow_tc_several_tile_pairs(ikv, oracle):
     want = np.where(cls == oracle.FORCED, np.inf, np.where(cls == oracle.DEAD, -np.inf, want))
     mabs, mrel = gc.assert_scores_close(scores.cpu().numpy(), want, "several pairs")
     print(f"[several pairs] multi-row score max abs err {mabs:.3e} rel {mrel:.3e}")
+    ctx.tune(ikv.TUNE_ROWS_TC, 3)   # cp.async gather warps: bit-identical
+    again = torch.full((s.N,), 3.0, device="cuda")
+    ctx.score_rows([req], rows.cuda().contiguous(), wt, again)
+    assert torch.equal(scores.view(torch.int32), again.view(torch.int32))
     ctx.tune(ikv.TUNE_ROWS_TC, 0)
     ref = torch.empty_like(scores)
     ctx.score_rows([req], rows.cuda().contiguous(), wt, ref)
