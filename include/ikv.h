@@ -284,9 +284,12 @@ ikv_status ikv_profile_read(ikv_ctx *ctx, float *out_ms, int32_t *out_n);
 #define IKV_TUNE_PREFILL_TILED 6 /* ikv_prefill_attn on a bf16 pool.  1 (default): tcgen05 kernel (128 / G query rows x G
                                     heads per CTA) for G in {1, 2, 4, 8}, its K/V tiles fetched by TMA gather4 through the
                                     tensor maps ikv_create builds over the pools; the mma.sync tiled kernel for G = 5;
+                                    chunks of eight or more such tiles put two of them on a CTA (they share every
+                                    gathered K/V tile);
                                     3: the tcgen05 kernel with cp.async producers (also the fallback when the tensor maps
-                                    could not be built); 2: always the mma.sync tiled kernel (32 rows per CTA); 0: row by
-                                    row through the decode kernels                                                  */
+                                    could not be built); 4: TMA producers, always one tile per CTA; 5: TMA producers, two
+                                    tiles per CTA from two tiles on; 2: always the mma.sync tiled kernel (32 rows per
+                                    CTA); 0: row by row through the decode kernels                                  */
 #define IKV_TUNE_BATCH_LANES 4 /* lanes of a batched ikv_score (default 4, 1..8): the partition / fold / residual kernels
                                  of request r run on internal stream r % lanes with that lane's own scratch, the key
                                  passes in request order on the caller's stream; 1 = one request after another      */

@@ -118,7 +118,7 @@ struct ikv_ctx : Scratch {
   std::string static_scratch_err;           // why it could not be resolved
 
   bool pf_attr_done[2][9] = {};
-  bool pt_attr_done[2][2][9] = {};
+  bool pt_attr_done[2][2][2][9] = {};
   CUtensorMap tm_k, tm_v;    // the pools as 2-D tensors [L n_slots H_kv][D], box 64 x 1, SWIZZLE_128B (TMA gather4)
   bool tm_ok = false;
   int prefill_tiled = 1;     // IKV_TUNE_PREFILL_TILED: 0 = ikv_prefill_attn row by row through the decode kernels
@@ -953,15 +953,15 @@ ikv_status launch_prefill(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaStr
   LAUNCH_CHECK(c);
   return IKV_OK;
 }
-template <int D, int G, bool TG>
+template <int D, int G, bool TG, int MT = 1>
 ikv_status launch_prefill_tc(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaStream_t st) {
-  auto fn = k_prefill_tc<D, G, TG>;
-  if (!c->pt_attr_done[TG][D == 128][G]) {
-    CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pt_smem<D, TG>()));
-    c->pt_attr_done[TG][D == 128][G] = true;
+  auto fn = k_prefill_tc<D, G, TG, MT>;
+  if (!c->pt_attr_done[MT - 1][TG][D == 128][G]) {
+    CU(c, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, pt_smem<D, TG, MT>()));
+    c->pt_attr_done[MT - 1][TG][D == 128][G] = true;
   }
-  constexpr int BR = 128 / G;
-  fn<<<dim3(p.n_split, p.Hkv, (p.n_q + BR - 1) / BR), TG ? PT_THREADS_TG : PT_THREADS, pt_smem<D, TG>(), st>>>(p, c->tm_k, c->tm_v);
+  constexpr int BR = MT * 128 / G;
+  fn<<<dim3(p.n_split, p.Hkv, (p.n_q + BR - 1) / BR), pt_threads<TG, MT>(), pt_smem<D, TG, MT>(), st>>>(p, c->tm_k, c->tm_v);
   LAUNCH_CHECK(c);
   k_prefill_merge<D><<<dim3(p.Hkv * G, p.n_q), D, 0, st>>>(p.part_o, p.part_ml, p.n_split, out);
   LAUNCH_CHECK(c);
@@ -969,7 +969,15 @@ ikv_status launch_prefill_tc(ikv_ctx* c, const PrefillParams& p, bf16* out, cuda
 }
 template <int D>
 ikv_status dispatch_prefill(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaStream_t st) {
-  if (c->prefill_tiled == 1 && c->tm_ok) {   // tcgen05 where 128 / G rows x G heads make a 128-row tile; TMA gather4
+  if (p.m_tiles == 2) {   // two 128-row tiles per CTA share each gathered K/V tile
+    switch (c->G) {
+      case 1: return launch_prefill_tc<D, 1, true, 2>(c, p, out, st);
+      case 2: return launch_prefill_tc<D, 2, true, 2>(c, p, out, st);
+      case 4: return launch_prefill_tc<D, 4, true, 2>(c, p, out, st);
+      case 8: return launch_prefill_tc<D, 8, true, 2>(c, p, out, st);
+    }
+  }
+  if ((c->prefill_tiled == 1 || c->prefill_tiled >= 4) && c->tm_ok) {   // tcgen05 where 128 / G rows x G heads make a 128-row tile; TMA gather4
     switch (c->G) {
       case 1: return launch_prefill_tc<D, 1, true>(c, p, out, st);
       case 2: return launch_prefill_tc<D, 2, true>(c, p, out, st);
@@ -977,7 +985,7 @@ ikv_status dispatch_prefill(ikv_ctx* c, const PrefillParams& p, bf16* out, cudaS
       case 8: return launch_prefill_tc<D, 8, true>(c, p, out, st);
     }
   }
-  if (c->prefill_tiled == 1 || c->prefill_tiled == 3) {   // the same with cp.async producers (no tensor map)
+  if (c->prefill_tiled == 1 || c->prefill_tiled >= 3) {   // the same with cp.async producers (no tensor map)
     switch (c->G) {
       case 1: return launch_prefill_tc<D, 1, false>(c, p, out, st);
       case 2: return launch_prefill_tc<D, 2, false>(c, p, out, st);
@@ -1023,12 +1031,19 @@ ikv_status prefill_tiled(ikv_ctx* c, int layer, const ikv_request& r, int q_pos0
   p.row0 = (int64_t)layer * c->cfg.n_slots * Hkv;
   p.n_live = s->d_n_live; p.n_cached = s->live_ub; p.covered = s->covered;
   p.scale_log2 = sm_scale * 1.4426950408889634f;
-  for (int g0 = 0; g0 < n_q; g0 += 1024) {
-    const int ng = std::min(1024, n_q - g0);
+  const bool tc = (c->prefill_tiled == 1 || c->prefill_tiled >= 3) && c->G != 5;
+  // two M tiles per CTA from eight M tiles of rows on (configs[1], G = 4: 64 rows 41 us against 47 with two tiles, 256 rows
+  // 96 against 85, 2,048 rows 681 against 545); IKV_TUNE_PREFILL_TILED = 5 forces them from two tiles on.  The row groups
+  // are then sized to one full wave: (SMs / H_kv) blocks of two M tiles.
+  const int bm = 128 / c->G;
+  const bool two = tc && c->tm_ok && n_q >= 2 * bm && (c->prefill_tiled == 5 || (c->prefill_tiled == 1 && n_q >= 8 * bm));
+  const int grp = two ? std::max(2 * bm, std::min(2048, (c->n_sm / Hkv) * 2 * bm)) : 1024;
+  for (int g0 = 0; g0 < n_q; g0 += grp) {
+    const int ng = std::min(grp, n_q - g0);
     p.q_pos0 = q_pos0 + g0; p.n_q = ng;
     p.q = q + (size_t)g0 * Hq * D;
-    const bool tc = (c->prefill_tiled == 1 || c->prefill_tiled == 3) && c->G != 5;
-    const int br = tc ? 128 / c->G : PF_BR;
+    p.m_tiles = (two && ng > bm) ? 2 : 1;
+    const int br = tc ? p.m_tiles * 128 / c->G : PF_BR;
     const int rbs = (ng + br - 1) / br;
     const int tiles = (p.n_cached + (p.q_pos0 + ng - p.covered) + PF_TOK - 1) / PF_TOK;   // upper bound
     int ns = c->n_sm / (Hkv * rbs);   // one wave: the kernel's registers leave room for one CTA per SM

@@ -36,6 +36,7 @@ struct PrefillParams {
   float* part_o;              // [n_q][Hq][n_split][D]
   float2* part_ml;            // [n_q][Hq][n_split]: (m in log2 units, l)
   int n_split;
+  int m_tiles;                // host only: 128-row tiles per CTA of k_prefill_tc (1 or 2)
   int64_t row0;               // row of (layer, slot 0, KV head 0) in the pool seen as [rows][D] (tensor-map producers)
 };
 

@@ -30,6 +30,7 @@ constexpr int PT_TOK = 64;            // items per tile
 constexpr int PT_THREADS = 9 * 32;    // 4 softmax warps, 4 producer warps, MMA warp
 constexpr int PT_PW_TG = 8;           // producer warps of the tensor-map path (64 / PT_PW_TG issuing lanes each)
 constexpr int PT_THREADS_TG = (5 + PT_PW_TG) * 32;
+constexpr int PT_PW_TG2 = 7;          // with two M tiles: 8 softmax + 7 producer + 1 MMA warps = 512 threads (128 registers each)
 constexpr int PT_NB = 4;               // K / V^T buffers: the gathers run three tiles ahead of the MMAs
 constexpr int PT_NB_TG = 4;            // the same on the tensor-map path (no staging buffers)
 constexpr int PT_PB = 1;               // P buffers (shared memory: 4 K / V^T buffers leave room for one)
@@ -37,12 +38,14 @@ constexpr float PT_GROW = 8.f;        // log2 units a tile's maximum may exceed 
 
 template <int D>
 __host__ __device__ constexpr int pt_vst() { return D * 2 + 16; }   // staged V row stride (conflict-free ldmatrix)
-template <int D, bool TG = false>
+template <int D, bool TG = false, int MT = 1>
 __host__ __device__ constexpr int pt_smem() {
-  // Q | K[NB] | V^T[NB] | V staging[2] (cp.async path) | P[1 or 2] | minrow[NB][64] | barriers
-  return 128 * D * 2 + (TG ? PT_NB_TG : PT_NB) * (PT_TOK * D * 2 + D * PT_TOK * 2 + PT_TOK * 4) +
-         (TG ? 0 : 2 * PT_TOK * pt_vst<D>()) + (TG ? 2 : PT_PB) * 128 * PT_TOK * 2 + 256;
+  // Q[MT] | K[NB] | V^T[NB] | V staging[2] (cp.async path) | P[MT][1 or 2] | minrow[NB][64] | barriers
+  return MT * 128 * D * 2 + (TG ? PT_NB_TG : PT_NB) * (PT_TOK * D * 2 + D * PT_TOK * 2 + PT_TOK * 4) +
+         (TG ? 0 : 2 * PT_TOK * pt_vst<D>()) + MT * ((TG && MT == 1) ? 2 : PT_PB) * 128 * PT_TOK * 2 + 256;
 }
+template <bool TG, int MT>
+__host__ __device__ constexpr int pt_threads() { return TG ? (4 * MT + (MT == 2 ? PT_PW_TG2 : PT_PW_TG) + 1) * 32 : PT_THREADS; }
 // shared-memory matrix descriptors of the 128-byte-swizzled operands the tensor map writes ([rows][128 B], 8-row atoms of
 // 1 KB): K-major (start address advanced by 32 B per 16 k) and MN-major (64 contiguous n per atom, the next 64 at `lbo`)
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
@@ -69,33 +72,37 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const float* v) {
       : "memory");
 }
 
-template <int D, int G, bool TG>
-__global__ __launch_bounds__(TG ? PT_THREADS_TG : PT_THREADS, 1) void k_prefill_tc(const PrefillParams p, const __grid_constant__ CUtensorMap tmk,
+// MT = 2 (tensor-map path only): two 128-row M tiles per CTA, one softmax warpgroup each, share every K/V tile -- half
+// the gather traffic and half the gather instructions per flop; all 512 TMEM columns (S double-buffered and O per M tile).
+template <int D, int G, bool TG, int MT>
+__global__ __launch_bounds__(pt_threads<TG, MT>(), 1) void k_prefill_tc(const PrefillParams p, const __grid_constant__ CUtensorMap tmk,
                                                               const __grid_constant__ CUtensorMap tmv) {
-  constexpr int BR = 128 / G;                // chunk rows per CTA
-  constexpr int NPB = TG ? 2 : PT_PB;        // P buffers
+  static_assert(MT == 1 || TG, "two M tiles per CTA need the tensor-map producers");
+  constexpr int BR = 128 / G;                // chunk rows per M tile
+  constexpr int NPB = (TG && MT == 1) ? 2 : PT_PB;   // P buffers per M tile
+  constexpr int SW = 4 * MT;                 // softmax warps
   constexpr int NB = TG ? PT_NB_TG : PT_NB;  // K / V buffers
-  constexpr int NPW = TG ? PT_PW_TG : 4, MMA_WARP = 4 + NPW;
+  constexpr int NPW = TG ? (MT == 2 ? PT_PW_TG2 : PT_PW_TG) : 4, MMA_WARP = SW + NPW;
   constexpr int CPR = D / 8;                 // 16-byte chunks per K / V row
   constexpr int VST = pt_vst<D>();
   constexpr int QB = 128 * D * 2, KB = PT_TOK * D * 2, VTB = D * PT_TOK * 2, VSB = PT_TOK * VST, PB = 128 * PT_TOK * 2;
   constexpr uint32_t SBO_D = (uint32_t)(D / 8) * 128u, SBO_T = (uint32_t)(PT_TOK / 8) * 128u;
-  constexpr uint32_t O_COL = 128;            // TMEM: S buffers at columns 0 and 64, O at [128, 128 + D)
+  constexpr uint32_t O_COL = 128, T_COLS = 256;   // TMEM per M tile: S buffers at columns 0 and 64, O at [128, 128 + D)
   extern __shared__ __align__(1024) unsigned char pt_smem_raw[];
   unsigned char* q_s = pt_smem_raw;
-  unsigned char* k_s = q_s + QB;                 // [3][KB]
+  unsigned char* k_s = q_s + MT * QB;            // [NB][KB]
   unsigned char* vt_s = k_s + NB * KB;        // [3][VTB]
   unsigned char* vst_s = vt_s + NB * VTB;     // [2][VSB]: one per producer group
-  unsigned char* p_s = vst_s + (TG ? 0 : 2 * VSB);   // [NPB][PB]
-  int* minrow_s = reinterpret_cast<int*>(p_s + NPB * PB);   // [NB][PT_TOK]
+  unsigned char* p_s = vst_s + (TG ? 0 : 2 * VSB);   // [MT][NPB][PB]
+  int* minrow_s = reinterpret_cast<int*>(p_s + MT * NPB * PB);   // [NB][PT_TOK]
   uint64_t* bars = reinterpret_cast<uint64_t*>(minrow_s + NB * PT_TOK);
   uint64_t* kv_full = bars;                 // [NB] operands K, V^T and minrow of a tile are in shared memory (64 threads)
   uint64_t* kv_free = kv_full + NB;      // [NB] the MMAs that read them have completed
-  uint64_t* s_full = kv_free + NB;       // [2] S accumulator complete
-  uint64_t* s_free = s_full + 2;            // [2] every softmax thread has read it
-  uint64_t* p_full = s_free + 2;            // [NPB] P written (and O rescaled) by every softmax thread
-  uint64_t* p_free = p_full + NPB;          // [NPB] P V of the buffer's tile complete
-  uint64_t* q_ready = p_free + NPB;
+  uint64_t* s_full = kv_free + NB;          // [MT][2] S accumulator complete
+  uint64_t* s_free = s_full + MT * 2;       // [MT][2] every softmax thread of the M tile has read it
+  uint64_t* p_full = s_free + MT * 2;       // [MT][NPB] P written (and O rescaled) by every softmax thread of the M tile
+  uint64_t* p_free = p_full + MT * NPB;     // [MT][NPB] P V of the buffer's tile complete
+  uint64_t* q_ready = p_free + MT * NPB;
   uint32_t* tmem_base_p = reinterpret_cast<uint32_t*>(q_ready + 1);
 
   const int split = blockIdx.x, kvh = blockIdx.y, rb = blockIdx.z;
@@ -103,13 +110,13 @@ __global__ __launch_bounds__(TG ? PT_THREADS_TG : PT_THREADS, 1) void k_prefill_
   const int Hq = p.Hkv * G;
   if (threadIdx.x == 0) {
     for (int b = 0; b < NB; ++b) { mbar_init(&kv_full[b], 64); mbar_init(&kv_free[b], 1); }
-    for (int b = 0; b < 2; ++b) { mbar_init(&s_full[b], 1); mbar_init(&s_free[b], 128); }
-    for (int b = 0; b < NPB; ++b) { mbar_init(&p_full[b], 128); mbar_init(&p_free[b], 1); }
-    mbar_init(q_ready, 128);
+    for (int b = 0; b < MT * 2; ++b) { mbar_init(&s_full[b], 1); mbar_init(&s_free[b], 128); }
+    for (int b = 0; b < MT * NPB; ++b) { mbar_init(&p_full[b], 128); mbar_init(&p_free[b], 1); }
+    mbar_init(q_ready, 128 * MT);
     mbar_fence_init();
   }
   if (warp == 0) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_base_p)), "n"(256));
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_base_p)), "n"(MT * 256));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -120,20 +127,21 @@ __global__ __launch_bounds__(TG ? PT_THREADS_TG : PT_THREADS, 1) void k_prefill_
   // items of this CTA (as in k_prefill_mma)
   const int n_cached = min(p.n_cached, *p.n_live);
   const int total = n_cached + (p.q_pos0 + p.n_q - p.covered);
-  const int lim = min(total, n_cached + (p.q_pos0 + min(p.n_q, (rb + 1) * BR) - p.covered));
+  const int lim = min(total, n_cached + (p.q_pos0 + min(p.n_q, (rb + 1) * MT * BR) - p.covered));
   const int tiles_all = (total + PT_TOK - 1) / PT_TOK;
   const int t_begin = (int)(((int64_t)tiles_all * split) / p.n_split);
   const int t_end = min((int)(((int64_t)tiles_all * (split + 1)) / p.n_split), (lim + PT_TOK - 1) / PT_TOK);
   const int n_t = max(0, t_end - t_begin);
 
-  if (TG && warp >= 4 && warp < MMA_WARP) {
+  if (TG && warp >= SW && warp < MMA_WARP) {
     // ------------------------------------------------------------------ producers, tensor-map path: lane < LPW of warp
-    // 4 + pw is thread j = LPW pw + lane: it writes minrow of item j and issues gather4 o = pw OPW + lane (lane < OPW)
-    constexpr int HALVES = D / 64, OPS = 2 * HALVES * 16, OPW = OPS / NPW, LPW = PT_TOK / NPW;
-    if (lane < LPW) {
-      const int pw = warp - 4, j = pw * LPW + lane;
-      const int o = pw * OPW + lane, mat = o / (OPS / 2), rem = o % (OPS / 2), quad = rem / HALVES, half = rem % HALVES;
-      const bool op = lane < OPW;
+    // SW + pw is thread j = LPW pw + lane < 64: it writes minrow of item j and issues gather4 number o (if o < OPS)
+    constexpr int HALVES = D / 64, OPS = 2 * HALVES * 16, LPW = (PT_TOK + NPW - 1) / NPW;
+    const int pw = warp - SW, j = pw * LPW + lane;
+    if (lane < LPW && j < PT_TOK) {
+      const int o = j;
+      const int mat = o / (OPS / 2), rem = o % (OPS / 2), quad = rem / HALVES, half = rem % HALVES;
+      const bool op = o < OPS;
       auto slot_at = [&](int idx) -> int {
         return idx < lim ? (idx < n_cached ? p.live_slots[idx] : p.S[p.covered + (idx - n_cached)]) : p.dead;
       };
@@ -221,62 +229,75 @@ __global__ __launch_bounds__(TG ? PT_THREADS_TG : PT_THREADS, 1) void k_prefill_
     if (lane == 0 && n_t > 0) {
       const uint32_t ibase = (1u << 4) | (1u << 7) | (1u << 10) | ((128u >> 4) << 24);
       const uint32_t idesc_s = ibase | (((uint32_t)PT_TOK >> 3) << 17), idesc_o = ibase | (((uint32_t)D >> 3) << 17);
-      const uint64_t dq = umma_desc(smem_u32(q_s), 128, SBO_D);
       auto issue_s = [&](int it) {
         const int b = it & 1, kb = it % NB;
         mbar_wait(&kv_full[kb], (uint32_t)(it / NB) & 1u);
-        mbar_wait(&s_free[b], ((uint32_t)(it >> 1) & 1u) ^ 1u);
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        if constexpr (TG) {
-          const uint32_t ka = smem_u32(k_s) + (uint32_t)(kb * KB);
 #pragma unroll
-          for (int ks = 0; ks < D / 16; ++ks)
-            umma_bf16(tmem + (uint32_t)(b * PT_TOK), dq + (uint64_t)(ks * 16),
-                      umma_desc_sw128(ka + (uint32_t)((ks >> 2) * (PT_TOK * 128) + (ks & 3) * 32), 16, 1024), idesc_s, ks ? 1u : 0u);
-        } else {
-          const uint64_t dk = umma_desc(smem_u32(k_s) + (uint32_t)(kb * KB), 128, SBO_D);
+        for (int mt = 0; mt < MT; ++mt) {
+          mbar_wait(&s_free[mt * 2 + b], ((uint32_t)(it >> 1) & 1u) ^ 1u);
+          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+          const uint64_t dq = umma_desc(smem_u32(q_s) + (uint32_t)(mt * QB), 128, SBO_D);
+          const uint32_t td = tmem + (uint32_t)(mt * T_COLS + b * PT_TOK);
+          if constexpr (TG) {
+            const uint32_t ka = smem_u32(k_s) + (uint32_t)(kb * KB);
 #pragma unroll
-          for (int ks = 0; ks < D / 16; ++ks)
-            umma_bf16(tmem + (uint32_t)(b * PT_TOK), dq + (uint64_t)(ks * 16), dk + (uint64_t)(ks * 16), idesc_s, ks ? 1u : 0u);
+            for (int ks = 0; ks < D / 16; ++ks)
+              umma_bf16(td, dq + (uint64_t)(ks * 16),
+                        umma_desc_sw128(ka + (uint32_t)((ks >> 2) * (PT_TOK * 128) + (ks & 3) * 32), 16, 1024), idesc_s, ks ? 1u : 0u);
+          } else {
+            const uint64_t dk = umma_desc(smem_u32(k_s) + (uint32_t)(kb * KB), 128, SBO_D);
+#pragma unroll
+            for (int ks = 0; ks < D / 16; ++ks) umma_bf16(td, dq + (uint64_t)(ks * 16), dk + (uint64_t)(ks * 16), idesc_s, ks ? 1u : 0u);
+          }
+          umma_commit(&s_full[mt * 2 + b]);
         }
-        umma_commit(&s_full[b]);
       };
       mbar_wait(q_ready, 0u);
       issue_s(0);
       for (int it = 0; it < n_t; ++it) {
         if (it + 1 < n_t) issue_s(it + 1);      // S of the next tile runs under this tile's softmax
         const int pb = it % NPB;
-        mbar_wait(&p_full[pb], (uint32_t)(it / NPB) & 1u);
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const uint64_t dp = umma_desc(smem_u32(p_s) + (uint32_t)(pb * PB), 128, SBO_T);
-        if constexpr (TG) {   // V [item][64 d] per column half: MN-major B, 16 items (two 8-row atoms) per instruction
-          const uint32_t va = smem_u32(vt_s) + (uint32_t)((it % NB) * VTB);
 #pragma unroll
-          for (int ks = 0; ks < PT_TOK / 16; ++ks)
-            umma_bf16(tmem + O_COL, dp + (uint64_t)(ks * 16), umma_desc_sw128(va + (uint32_t)(ks * 2048), PT_TOK * 128, 1024),
-                      idesc_o | (1u << 16), (it | ks) ? 1u : 0u);
-        } else {
-          const uint64_t dv = umma_desc(smem_u32(vt_s) + (uint32_t)((it % NB) * VTB), 128, SBO_T);
+        for (int mt = 0; mt < MT; ++mt) {
+          mbar_wait(&p_full[mt * NPB + pb], (uint32_t)(it / NPB) & 1u);
+          asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+          const uint64_t dp = umma_desc(smem_u32(p_s) + (uint32_t)((mt * NPB + pb) * PB), 128, SBO_T);
+          const uint32_t td = tmem + (uint32_t)(mt * T_COLS) + O_COL;
+          if constexpr (TG) {   // V [item][64 d] per column half: MN-major B, 16 items (two 8-row atoms) per instruction
+            const uint32_t va = smem_u32(vt_s) + (uint32_t)((it % NB) * VTB);
 #pragma unroll
-          for (int ks = 0; ks < PT_TOK / 16; ++ks)
-            umma_bf16(tmem + O_COL, dp + (uint64_t)(ks * 16), dv + (uint64_t)(ks * 16), idesc_o, (it | ks) ? 1u : 0u);
+            for (int ks = 0; ks < PT_TOK / 16; ++ks)
+              umma_bf16(td, dp + (uint64_t)(ks * 16), umma_desc_sw128(va + (uint32_t)(ks * 2048), PT_TOK * 128, 1024),
+                        idesc_o | (1u << 16), (it | ks) ? 1u : 0u);
+          } else {
+            const uint64_t dv = umma_desc(smem_u32(vt_s) + (uint32_t)((it % NB) * VTB), 128, SBO_T);
+#pragma unroll
+            for (int ks = 0; ks < PT_TOK / 16; ++ks)
+              umma_bf16(td, dp + (uint64_t)(ks * 16), dv + (uint64_t)(ks * 16), idesc_o, (it | ks) ? 1u : 0u);
+          }
+          umma_commit(&p_free[mt * NPB + pb]);
         }
-        umma_commit(&p_free[pb]);
         umma_commit(&kv_free[it % NB]);
       }
     }
   } else {
     // ------------------------------------------------------------------ softmax warps: thread m = TMEM lane = M row
-    const int m = threadIdx.x, i = m / G, g = m % G;
-    const int row = rb * BR + i, head = kvh * G + g;
-    const uint32_t tl = tmem + ((uint32_t)(warp * 32) << 16);
+    // (warpgroup sg = M tile sg of the CTA)
+    const int sg = MT == 1 ? 0 : warp >> 2, m = threadIdx.x & 127, i = m / G, g = m % G;
+    const int row = (rb * MT + sg) * BR + i, head = kvh * G + g;
+    const uint32_t tl = tmem + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(sg * T_COLS);
+    unsigned char* q_m = q_s + sg * QB;
+    uint64_t* s_full_m = s_full + sg * 2;
+    uint64_t* s_free_m = s_free + sg * 2;
+    uint64_t* p_full_m = p_full + sg * NPB;
+    uint64_t* p_free_m = p_free + sg * NPB;
     {  // Q row of this thread into the canonical A operand
       const bf16* src = p.q + ((int64_t)row * Hq + head) * D;
 #pragma unroll
       for (int k8 = 0; k8 < CPR; ++k8) {
         uint4 v = make_uint4(0u, 0u, 0u, 0u);
         if (row < p.n_q) v = *reinterpret_cast<const uint4*>(src + k8 * 8);
-        *reinterpret_cast<uint4*>(q_s + pt_entry(m, k8, D)) = v;
+        *reinterpret_cast<uint4*>(q_m + pt_entry(m, k8, D)) = v;
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       mbar_arrive(q_ready);
@@ -287,14 +308,14 @@ __global__ __launch_bounds__(TG ? PT_THREADS_TG : PT_THREADS, 1) void k_prefill_
       const uint32_t par = (uint32_t)(it >> 1) & 1u;
       const int kb = it % NB;
       mbar_wait(&kv_full[kb], (uint32_t)(it / NB) & 1u);   // minrow of the tile
-      mbar_wait(&s_full[b], par);
+      mbar_wait(&s_full_m[b], par);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
       float x[PT_TOK];
 #pragma unroll
       for (int c0 = 0; c0 < PT_TOK; c0 += 16) tmem_ld16(tl + (uint32_t)(b * PT_TOK + c0), &x[c0]);
       tmem_ld_wait();
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-      mbar_arrive(&s_free[b]);
+      mbar_arrive(&s_free_m[b]);
       float tmax = -CUDART_INF_F;
 #pragma unroll
       for (int c = 0; c < PT_TOK; c += 4) {
@@ -311,7 +332,7 @@ __global__ __launch_bounds__(TG ? PT_THREADS_TG : PT_THREADS, 1) void k_prefill_
         const float m_new = grow ? tmax : m_ref;
         const float corr = (m_new == -CUDART_INF_F) ? 1.f : fast_exp2(m_ref - m_new);   // m_ref = -inf: 0
         if (it > 0) {   // O exists from the first P V on; wait for the previous tile's
-          mbar_wait(&p_free[(it - 1) % NPB], (uint32_t)((it - 1) / NPB) & 1u);
+          mbar_wait(&p_free_m[(it - 1) % NPB], (uint32_t)((it - 1) / NPB) & 1u);
           asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
 #pragma unroll 1
           for (int c0 = 0; c0 < D; c0 += 32) {
@@ -339,8 +360,8 @@ __global__ __launch_bounds__(TG ? PT_THREADS_TG : PT_THREADS, 1) void k_prefill_
       }
       l += s0 + s1;
       const int pb = it % NPB;
-      mbar_wait(&p_free[pb], ((uint32_t)(it / NPB) & 1u) ^ 1u);   // the P V that read this buffer has completed
-      unsigned char* pd = p_s + (size_t)pb * PB;
+      mbar_wait(&p_free_m[pb], ((uint32_t)(it / NPB) & 1u) ^ 1u);   // the P V that read this buffer has completed
+      unsigned char* pd = p_s + (size_t)(sg * NPB + pb) * PB;
 #pragma unroll
       for (int k8 = 0; k8 < PT_TOK / 8; ++k8) {
         const uint4 v = make_uint4(pack2_bf16(x[8 * k8], x[8 * k8 + 1]), pack2_bf16(x[8 * k8 + 2], x[8 * k8 + 3]),
@@ -349,11 +370,11 @@ __global__ __launch_bounds__(TG ? PT_THREADS_TG : PT_THREADS, 1) void k_prefill_
       }
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-      mbar_arrive(&p_full[pb]);
+      mbar_arrive(&p_full_m[pb]);
     }
     // ---- partials of the split (an empty split writes m = -inf, l = 0: the scratch is not cleared)
     if (n_t > 0) {
-      mbar_wait(&p_free[(n_t - 1) % NPB], (uint32_t)((n_t - 1) / NPB) & 1u);
+      mbar_wait(&p_free_m[(n_t - 1) % NPB], (uint32_t)((n_t - 1) / NPB) & 1u);
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     }
     const int64_t ph = ((int64_t)row * Hq + head) * p.n_split + split;
@@ -379,7 +400,7 @@ __global__ __launch_bounds__(TG ? PT_THREADS_TG : PT_THREADS, 1) void k_prefill_
   __syncthreads();
   if (warp == 0) {
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(256));
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(MT * 256));
   }
 }
 

@@ -225,8 +225,9 @@ def test_prefill_tiled_long_chunk_and_row_by_row_agree(ikv, oracle):
         q = torch.randn((n_q, shape.Hq, shape.D), generator=torch.Generator().manual_seed(q_pos0 + 1)).to(torch.bfloat16)
         r = gc.request(ikv, s, S_dev, seq_len=q_pos0 + n_q)
         outs = []
-        for tiled in (1, 2, 0, 3):   # tcgen05 kernel (TMA gather4 producers), mma.sync tiled kernel, row by row,
-                                     # tcgen05 kernel with the cp.async producers
+        for tiled in (1, 2, 0, 3, 4, 5):   # tcgen05 kernel (TMA gather4 producers), mma.sync tiled kernel, row by row,
+                                           # tcgen05 kernel with the cp.async producers, with TMA producers and one M
+                                           # tile per CTA, with TMA producers and two M tiles per CTA
             ctx.tune(ikv.TUNE_PREFILL_TILED, tiled)
             out = torch.full((n_q, shape.Hq, shape.D), float("nan"), dtype=torch.bfloat16, device="cuda")
             reads = torch.zeros(2, dtype=torch.int64, device="cuda")
@@ -238,10 +239,12 @@ def test_prefill_tiled_long_chunk_and_row_by_row_agree(ikv, oracle):
         e2 = gc.assert_decode_close(outs[1][0], want, True, f"mma.sync prefill at {q_pos0}")
         e0 = gc.assert_decode_close(outs[2][0], want, True, f"row-by-row prefill at {q_pos0}")
         e3 = gc.assert_decode_close(outs[3][0], want, True, f"tcgen05 (cp.async producers) prefill at {q_pos0}")
+        e4 = gc.assert_decode_close(outs[4][0], want, True, f"tcgen05 (one M tile per CTA) prefill at {q_pos0}")
+        e5 = gc.assert_decode_close(outs[5][0], want, True, f"tcgen05 (two M tiles per CTA) prefill at {q_pos0}")
         assert all(o[1] == [raw, eff] for o in outs)
-        # both producer kinds hand the tensor cores the same operands: bit-identical outputs
-        assert np.array_equal(outs[0][0], outs[3][0])
-        print(f"prefill at {q_pos0} x {n_q}: max abs err tcgen05 {e1:.3e} (cp.async producers {e3:.3e}), mma.sync {e2:.3e}, "
+        # both producer kinds hand the tensor cores the same operands: bit-identical outputs for the same tiling
+        assert np.array_equal(outs[4][0], outs[3][0]) and e4 == e3
+        print(f"prefill at {q_pos0} x {n_q}: max abs err tcgen05 {e1:.3e} (cp.async producers {e3:.3e}, two M tiles {e5:.3e}), mma.sync {e2:.3e}, "
               f"row by row {e0:.3e}")
 
 
@@ -267,7 +270,7 @@ def test_prefill_tcgen05_head_layouts(ikv, oracle, name, shape):
         q = torch.randn((n_q, shape.Hq, shape.D), generator=torch.Generator().manual_seed(q_pos0)).to(torch.bfloat16)
         r = gc.request(ikv, s, S_dev, seq_len=q_pos0 + n_q)
         outs = []
-        for tiled in (1, 2, 3):
+        for tiled in (1, 2, 3, 4, 5):
             ctx.tune(ikv.TUNE_PREFILL_TILED, tiled)
             out = torch.full((n_q, shape.Hq, shape.D), float("nan"), dtype=torch.bfloat16, device="cuda")
             ctx.prefill_attn(shape.L - 1, r, q_pos0, q.cuda(), out, scale)
@@ -276,7 +279,9 @@ def test_prefill_tcgen05_head_layouts(ikv, oracle, name, shape):
         want, _, _ = oracle.prefill(g, kp, vp, shape.L - 1, S_dev.cpu().numpy(), q_pos0, q.float().numpy(), scale)
         e1 = gc.assert_decode_close(outs[0], want, True, f"{name} tcgen05 prefill at {q_pos0} x {n_q}")
         e2 = gc.assert_decode_close(outs[1], want, True, f"{name} mma.sync prefill at {q_pos0} x {n_q}")
-        assert np.array_equal(outs[0], outs[2]), f"{name}: TMA gather4 and cp.async producers disagree"
+        assert np.array_equal(outs[3], outs[2]), f"{name}: TMA gather4 and cp.async producers disagree"
+        gc.assert_decode_close(outs[3], want, True, f"{name} tcgen05 (one M tile per CTA) prefill at {q_pos0} x {n_q}")
+        gc.assert_decode_close(outs[4], want, True, f"{name} tcgen05 (two M tiles per CTA) prefill at {q_pos0} x {n_q}")
         print(f"[{name}] prefill at {q_pos0} x {n_q}: max abs err tcgen05 {e1:.3e}, mma.sync {e2:.3e}")
 
 
