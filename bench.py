@@ -353,8 +353,9 @@ def run_next(rig, hbm_peak):
         res[f"prefill_chunk_{n_q}"] = {"n_q": n_q, "layer_calls": 1, "live_tokens": n_kept, "ms": ms, "roofline_ms": roof,
                                        "bound": "hbm" if hbm_t >= mma_t else "tensor",
                                        "frac_of_roofline": roof / ms, "raw_kv_reads": raw, "effective_kv_reads": eff,
-                                       "what": "ikv_prefill_attn on tcgen05 (k_prefill_tc): 128 / G query rows x G heads per CTA "
-                                               "share each gathered K/V tile; counters per PAPER.md:163-175"}
+                                       "what": "ikv_prefill_attn on tcgen05 (k_prefill_tc): K/V tiles by TMA gather4 into swizzled "
+                                               "operands; 128 / G query rows x G heads per M tile, two M tiles per CTA from "
+                                               "eight tiles of rows on; counters per PAPER.md:163-175"}
     return res
 
 
