@@ -1,25 +1,26 @@
 // prefill_tc.cuh -- NEXT-2 on tcgen05: the causal chunk attention of prefill_mma.cuh with both contractions on the 5th-gen
 // tensor cores, for G in {1, 2, 4, 8} (128 / G query rows x G heads of one KV head = one 128-row tile).
 //
-// CTA = (split of the items, KV head, block of BR = 128 / G rows).  M row m = i G + g: chunk row i, query head kvh G + g.
-// Per tile of 64 items:
-//   producers (2 x 2 warps, alternating tiles) gather the K rows of the head with cp.async straight into the canonical K-major operand
-//                        [64 items x D], the V rows into a row-major staging buffer, then transpose V with
-//                        ldmatrix.trans into the canonical operand V^T [D x 64 items] (P V needs items as K);
+// CTA = (split of the items, KV head, block of MT x BR rows, BR = 128 / G).  M row m = i G + g: chunk row i, query head
+// kvh G + g.  Per tile of 64 items:
+//   producers            TG = true (default; the pools are covered by the tensor maps ikv_create builds): they do not
+//                        touch the data.  Every 64-item tile is fetched by 64 TMA tile::gather4 instructions (four rows of
+//                        128 bytes each; the row = (layer, slot, KV head) of the pool seen as a 2-D tensor [rows][D]; dead
+//                        items get an out-of-range row: zero fill) with SWIZZLE_128B, which lands K as the K-major and
+//                        V as the MN-major 128-byte-swizzled operand of tcgen05.mma: no transposition pass, no staging.
+//                        A gather4 costs its issuing warp ~75 cycles whatever the lane count, so the issue is spread:
+//                        eight warps x eight lanes (seven warps with two M tiles).  Per SM, 32 KB of random 256-byte
+//                        pieces arrive in 1,190-1,730 cycles against 2,150-2,400 for cp.async or 256-byte bulk copies.
+//                        TG = false (no tensor map): 2 x 2 warps, alternating tiles, gather the K rows with cp.async
+//                        straight into the canonical no-swizzle K-major operand [64 items x D], the V rows into a
+//                        row-major staging buffer, then transpose V with ldmatrix.trans into the canonical operand
+//                        V^T [D x 64 items] (P V needs items as K);
 //   MMA thread           S = Q K^T  (D/16 tcgen05.mma M128 N64 K16, double-buffered in TMEM), then O += P V
-//                        (4 tcgen05.mma M128 N=D K16) once P is written;
-//   softmax (4 warps)    thread = M row: tcgen05.ld of its 64 logits, causal / dead mask, exp2 against a LAZY reference
-//                        maximum (moved, with a rescale of the row's O and l, only when a tile's maximum exceeds it by
+//                        (4 tcgen05.mma M128 N=D K16) once P is written; with MT = 2 for both M tiles on each K/V tile;
+//   softmax (4 warps     thread = M row: tcgen05.ld of its 64 logits, causal / dead mask, exp2 against a LAZY reference
+//   per M tile)          maximum (moved, with a rescale of the row's O and l, only when a tile's maximum exceeds it by
 //                        more than 2^8), P as bf16 into the canonical A operand [128 x 64].
 // Partials (reference m, l, O) per (row, head, split) as in prefill_mma.cuh; k_prefill_merge combines them.
-//
-// TG = true (the pool is covered by a tensor map, ikv_create): the producers do not touch the data.  Sixteen lanes of each
-// of the four producer warps issue one TMA tile::gather4 each per tile (four rows of 128 bytes per instruction, the row =
-// (layer, slot, KV head) of the pool seen as a 2-D tensor [rows][D]; dead items get an out-of-range row: zero fill) with
-// SWIZZLE_128B, which lands K as the K-major and V as the MN-major 128-byte-swizzled operand of tcgen05.mma: no
-// transposition pass, no staging buffer (its memory holds a second P buffer).  A gather4 costs its issuing warp ~75
-// cycles whatever the lane count, so the issue is spread over the warps: 64 KB-pieces of 256 bytes arrive at 19-27 B per
-// cycle per SM against 12-15 for cp.async or 256-byte bulk copies (micro-benchmark).
 #pragma once
 #include <cuda.h>
 #include "prefill_mma.cuh"
@@ -91,8 +92,8 @@ __global__ __launch_bounds__(pt_threads<TG, MT>(), 1) void k_prefill_tc(const Pr
   extern __shared__ __align__(1024) unsigned char pt_smem_raw[];
   unsigned char* q_s = pt_smem_raw;
   unsigned char* k_s = q_s + MT * QB;            // [NB][KB]
-  unsigned char* vt_s = k_s + NB * KB;        // [3][VTB]
-  unsigned char* vst_s = vt_s + NB * VTB;     // [2][VSB]: one per producer group
+  unsigned char* vt_s = k_s + NB * KB;           // [NB][VTB]: V^T (cp.async path) or V [half][item][128 B] (tensor map)
+  unsigned char* vst_s = vt_s + NB * VTB;        // [2][VSB]: one per producer group (cp.async path only)
   unsigned char* p_s = vst_s + (TG ? 0 : 2 * VSB);   // [MT][NPB][PB]
   int* minrow_s = reinterpret_cast<int*>(p_s + MT * NPB * PB);   // [NB][PT_TOK]
   uint64_t* bars = reinterpret_cast<uint64_t*>(minrow_s + NB * PT_TOK);
