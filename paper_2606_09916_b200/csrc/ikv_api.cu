@@ -961,8 +961,11 @@ ikv_status launch_prefill_tc(ikv_ctx* c, const PrefillParams& p, bf16* out, cuda
     c->pt_attr_done[MT - 1][TG][D == 128][G] = true;
   }
   constexpr int BR = MT * 128 / G;
-  fn<<<dim3(p.n_split, p.Hkv, (p.n_q + BR - 1) / BR), pt_threads<TG, MT>(), pt_smem<D, TG, MT>(), st>>>(p, c->tm_k, c->tm_v);
+  PrefillParams pk = p;
+  pk.out_direct = p.n_split == 1 ? out : nullptr;   // a single split writes the output itself
+  fn<<<dim3(p.n_split, p.Hkv, (p.n_q + BR - 1) / BR), pt_threads<TG, MT>(), pt_smem<D, TG, MT>(), st>>>(pk, c->tm_k, c->tm_v);
   LAUNCH_CHECK(c);
+  if (pk.out_direct) return IKV_OK;
   k_prefill_merge<D><<<dim3(p.Hkv * G, p.n_q), D, 0, st>>>(p.part_o, p.part_ml, p.n_split, out);
   LAUNCH_CHECK(c);
   return IKV_OK;
@@ -1029,6 +1032,7 @@ ikv_status prefill_tiled(ikv_ctx* c, int layer, const ikv_request& r, int q_pos0
   p.v_layer = (const bf16*)c->cfg.v_pool + (int64_t)layer * c->layer_stride;
   p.Hkv = Hkv; p.dead = c->cfg.dead_slot; p.S = r.slot_map; p.live_slots = s->live_slots;
   p.row0 = (int64_t)layer * c->cfg.n_slots * Hkv;
+  p.out_direct = nullptr;
   p.n_live = s->d_n_live; p.n_cached = s->live_ub; p.covered = s->covered;
   p.scale_log2 = sm_scale * 1.4426950408889634f;
   const bool tc = (c->prefill_tiled == 1 || c->prefill_tiled >= 3) && c->G != 5;

@@ -37,6 +37,7 @@ struct PrefillParams {
   float2* part_ml;            // [n_q][Hq][n_split]: (m in log2 units, l)
   int n_split;
   int m_tiles;                // host only: 128-row tiles per CTA of k_prefill_tc (1 or 2)
+  bf16* out_direct;           // k_prefill_tc with n_split = 1: the output itself ([n_q][Hq][D]); no partials, no merge
   int64_t row0;               // row of (layer, slot 0, KV head 0) in the pool seen as [rows][D] (tensor-map producers)
 };
 

@@ -379,7 +379,8 @@ __global__ __launch_bounds__(pt_threads<TG, MT>(), 1) void k_prefill_tc(const Pr
       asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     }
     const int64_t ph = ((int64_t)row * Hq + head) * p.n_split + split;
-    if (row < p.n_q) p.part_ml[ph] = make_float2(m_ref, l);
+    const bool direct = p.out_direct != nullptr;   // one split: out = O / l, exactly what k_prefill_merge would compute
+    if (row < p.n_q && !direct) p.part_ml[ph] = make_float2(m_ref, l);
 #pragma unroll 1
     for (int c0 = 0; c0 < D; c0 += 16) {
       float o[16];
@@ -390,7 +391,19 @@ __global__ __launch_bounds__(pt_threads<TG, MT>(), 1) void k_prefill_tc(const Pr
 #pragma unroll
         for (int e = 0; e < 16; ++e) o[e] = 0.f;
       }
-      if (row < p.n_q) {
+      if (direct) {
+        if (row < p.n_q) {
+          uint32_t w[8];
+#pragma unroll
+          for (int e = 0; e < 8; ++e) {
+            const float a = l > 0.f ? o[2 * e] / l : 0.f, b = l > 0.f ? o[2 * e + 1] / l : 0.f;
+            w[e] = (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(a)) | ((uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(b)) << 16);
+          }
+          uint4* po = reinterpret_cast<uint4*>(p.out_direct + ((int64_t)row * Hq + head) * D + c0);
+          po[0] = make_uint4(w[0], w[1], w[2], w[3]);
+          po[1] = make_uint4(w[4], w[5], w[6], w[7]);
+        }
+      } else if (row < p.n_q) {
         float4* po = reinterpret_cast<float4*>(p.part_o + ph * D + c0);
         po[0] = make_float4(o[0], o[1], o[2], o[3]);     po[1] = make_float4(o[4], o[5], o[6], o[7]);
         po[2] = make_float4(o[8], o[9], o[10], o[11]);   po[3] = make_float4(o[12], o[13], o[14], o[15]);

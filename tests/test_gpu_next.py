@@ -285,6 +285,38 @@ def test_prefill_tcgen05_head_layouts(ikv, oracle, name, shape):
         print(f"[{name}] prefill at {q_pos0} x {n_q}: max abs err tcgen05 {e1:.3e}, mma.sync {e2:.3e}")
 
 
+def test_prefill_single_split_writes_the_output_itself(ikv, oracle):
+    """Enough (row block, KV head) pairs to fill the SMs with one split each: k_prefill_tc then normalises and writes the
+    output itself (no partials, no merge launch).  700 rows at 8 KV heads, G = 4: one M tile per CTA (22 blocks), two
+    M tiles per CTA (11 blocks) and the cp.async producers, all against the oracle; ragged last block, dead positions."""
+    shape = wl.ModelShape(1, 32, 8, 128, "bf16")
+    w = wl.small(seed=91, shape=shape, n_tokens=1500, budget=600, decode_tokens=720, kv_dtype="bf16")
+    kp, vp = gc.to_cuda(w)
+    ctx = gc.make_ctx(w)
+    s = w.sessions[0]
+    gc.fold_memory_gpu(ctx, s)
+    g = gc.oracle_geom(oracle, w)
+    full = s.slot_map.clone()
+    rng = np.random.default_rng(17)
+    full[torch.from_numpy(rng.choice(s.N + 700, size=450, replace=False))] = w.dead_slot
+    S_dev = full.cuda()
+    scale = 1.0 / math.sqrt(shape.D)
+    q_pos0, n_q = s.N, 700
+    q = torch.randn((n_q, shape.Hq, shape.D), generator=torch.Generator().manual_seed(5)).to(torch.bfloat16)
+    r = gc.request(ikv, s, S_dev, seq_len=q_pos0 + n_q)
+    want, _, _ = oracle.prefill(g, kp, vp, 0, S_dev.cpu().numpy(), q_pos0, q.float().numpy(), scale)
+    outs = {}
+    for tiled in (1, 4, 3):
+        ctx.tune(ikv.TUNE_PREFILL_TILED, tiled)
+        out = torch.full((n_q, shape.Hq, shape.D), float("nan"), dtype=torch.bfloat16, device="cuda")
+        ctx.prefill_attn(0, r, q_pos0, q.cuda(), out, scale)
+        torch.cuda.synchronize()
+        outs[tiled] = out.float().cpu().numpy()
+        err = gc.assert_decode_close(outs[tiled], want, True, f"single-split prefill, IKV_TUNE_PREFILL_TILED = {tiled}")
+        print(f"single-split prefill (tiled = {tiled}): max abs err {err:.3e}")
+    assert np.array_equal(outs[4], outs[3])
+
+
 @pytest.mark.parametrize("n,pos_rate", [(1, 1.0), (700, 0.05), (33000, 0.004), (5000, 0.0), (40, 0.5)])
 def test_train_loss_matches_oracle(ikv, oracle, n, pos_rate):
     """Eq. 8 and dL/ds (ikv_train_loss) against the fp64 oracle: terms within 1e-5 relative, gradient within
