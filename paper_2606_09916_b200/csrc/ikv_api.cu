@@ -966,8 +966,8 @@ ikv_status launch_prefill_tc(ikv_ctx* c, const PrefillParams& p, bf16* out, cuda
   fn<<<dim3(p.n_split, p.Hkv, (p.n_q + BR - 1) / BR), pt_threads<TG, MT>(), pt_smem<D, TG, MT>(), st>>>(pk, c->tm_k, c->tm_v);
   LAUNCH_CHECK(c);
   if (pk.out_direct) return IKV_OK;
-  k_prefill_merge<D><<<dim3(p.Hkv * G, p.n_q), D, 0, st>>>(p.part_o, p.part_ml, p.n_split, out);
-  LAUNCH_CHECK(c);
+  CU(c, launch_pdl(k_prefill_merge<D>, dim3(p.Hkv * G, p.n_q), dim3(D), 0, st, c->use_pdl, (const float*)p.part_o,
+                   (const float2*)p.part_ml, p.n_split, out));
   return IKV_OK;
 }
 template <int D>

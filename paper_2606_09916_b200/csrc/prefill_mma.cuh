@@ -232,6 +232,7 @@ template <int D>
 __global__ __launch_bounds__(D) void k_prefill_merge(const float* __restrict__ part_o, const float2* __restrict__ part_ml,
                                                      int n_split, bf16* __restrict__ out) {
   const int64_t ph = ((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * n_split;
+  pdl_wait();   // launched programmatically behind the split kernel: its partials are complete from here on
   float m = -CUDART_INF_F;
   for (int s = 0; s < n_split; ++s) {
     const float2 ml = part_ml[ph + s];

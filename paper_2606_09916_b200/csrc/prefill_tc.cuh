@@ -124,6 +124,7 @@ __global__ __launch_bounds__(pt_threads<TG, MT>(), 1) void k_prefill_tc(const Pr
   __syncthreads();
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const uint32_t tmem = *tmem_base_p;
+  pdl_launch_dependents();   // the merge grid may be scheduled now; it waits (griddepcontrol.wait) for this grid to complete
 
   // items of this CTA (as in k_prefill_mma)
   const int n_cached = min(p.n_cached, *p.n_live);
