@@ -104,7 +104,11 @@ typedef struct {
 
 /* ---- lifecycle ------------------------------------------------------------------------------------- */
 /* Validates the config, initialises the dead slot's K/V rows on every layer, allocates the session slab.
- * Synchronises.  *out receives the context. */
+ * Synchronises.  *out receives the context.  For bf16 pools with head_dim 64 or 128 it also encodes two TMA tensor maps
+ * (cuTensorMapEncodeTiled through the runtime's driver entry point; no device memory) that describe k_pool and v_pool as
+ * 2-D tensors [n_layers * n_slots * n_kv_heads][head_dim]: ikv_prefill_attn and ikv_score_rows fetch their tiles through
+ * them (tile::gather4).  If that fails (old driver, more than 2^31 - 1 rows, pools not 16-byte aligned) those calls use
+ * their cp.async producers instead; nothing else changes. */
 ikv_status ikv_create(const ikv_config *cfg, ikv_ctx **out);
 ikv_status ikv_destroy(ikv_ctx *ctx);
 /* ctx == NULL: the reason of the last failed ikv_create on this thread. */
